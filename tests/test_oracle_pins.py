@@ -1,0 +1,529 @@
+"""Pins for the CPU oracle: closed forms, paper values, invariants, brute force.
+
+None of these compares the oracle with itself through the same formula: every expected value is a
+closed form typed here, a value printed in the paper (tests/golden), an independent geometric
+computation, a library routine (scipy.special.wofz) or a second, differently structured
+implementation.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from workloads import make
+from workloads.gen import dirs_2d, dirs_fibonacci, METRIC_RELVAR
+from _util import (fig5_levels, iso_workload, max_rel, path_to_boundary, random_unit_dirs, unit_dirs_2d)
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ------------------------------------------------------------------ P1: homogeneous slab
+@pytest.mark.parametrize("ndim", [2, 3])
+def test_p1_homogeneous_slab_any_level(ndim):
+    """with homogeneous parameters the averaged formulation is equivalent; any ray of
+    length L through uniform chi, S gives I = I0 e^{-chi h L} + S (1 - e^{-chi h L}) whatever the
+    cells and levels crossed."""
+    rng = np.random.default_rng(11)
+    brick = 16 if ndim == 2 else 8
+    dims = (64, 48) if ndim == 2 else (24, 16, 32)
+    chi0, S0, h = 0.037, 1.7, 1.3
+    shape = dims[::-1]
+    probes = rng.uniform(0.01, 0.99, size=(40, ndim)) * np.array(dims)
+    dirs = random_unit_dirs(12, ndim, rng)
+    i0 = rng.uniform(0.0, 3.0, size=(dirs.shape[0], 8))
+    wl = iso_workload(dims, brick, np.full(shape, chi0 * S0), np.full(shape, chi0), probes, dirs, h=h,
+                      max_level=int(math.log2(brick)), i0=i0)
+    M = orc.build_mips(wl)
+    nbr = wl.n_bricks
+    lv = rng.integers(0, int(math.log2(brick)) + 1, size=(1, nbr)).astype(np.int8)   # arbitrary levels
+    A = orc.plain_march(wl)
+    B = orc.hdda_march(wl, M, levels=lv)
+    chi32, eta32 = float(np.float32(chi0)), float(np.float32(chi0 * S0))
+    for p in range(probes.shape[0]):
+        for k in range(dirs.shape[0]):
+            L = path_to_boundary(wl.probe_pos[p], wl.dirs[k], dims)
+            att = math.exp(-chi32 * h * L)
+            want = wl.i0[k, 0] * att + (eta32 / chi32) * (1.0 - att)
+            assert abs(A.I[p, k, 0] - want) <= 3e-6 * abs(want)     # fp32 plane times: ~1e-6 in L
+            assert abs(B.I[p, k, 0] - want) <= 3e-6 * abs(want)
+
+
+def test_p1_table1_average_column():
+    """Table 1: averaged eta = 1.2, chi = 0.8 over a corner-to-corner path sqrt(5)
+    prints 1.25 in the 'Average' column of ray gamma."""
+    rows = {}
+    with open(os.path.join(GOLDEN, "table1.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            name, true, avg = line.split()
+            rows[name] = (float(true), float(avg))
+    eta_avg = (2 + 2 + 0.4 + 0.4) / 4
+    chi_avg = (0.2 + 0.2 + 1.4 + 1.4) / 4
+    got = orc.segment(0.0, eta_avg, chi_avg, math.sqrt(5.0))
+    assert abs(got - 1.2492727) < 5e-7
+    assert round(got, 2) == rows["gamma"][1]
+    # the same through the march: 2x1 block of the averaged medium, ray along the diagonal
+    th = math.atan2(1.0, 2.0)
+    wl = iso_workload((2, 2), 2, np.full((2, 2), eta_avg), np.full((2, 2), chi_avg),
+                      probes=[[np.nextafter(np.float32(2.0), np.float32(0)), np.nextafter(np.float32(1.0), np.float32(0))]],
+                      dirs=unit_dirs_2d([th]))
+    A = orc.plain_march(wl)
+    assert abs(A.I[0, 0, 0] - 1.2492727) < 2e-6
+
+
+# ------------------------------------------------------------------ P2: order of accumulation
+def test_p2_order_dependence_table1_coefficients():
+    """opposed rays through the same voxels differ.  Unit paths through a light
+    (eta 2, chi .2) and a dark (eta .4, chi 1.4) voxel: hand-computed 0.6622625 / 1.9889308."""
+    light = (2.0, 0.2)
+    dark = (0.4, 1.4)
+    I_ld = (light[0] / light[1]) * (1 - math.exp(-light[1]))
+    I_ld = I_ld * math.exp(-dark[1]) + (dark[0] / dark[1]) * (1 - math.exp(-dark[1]))
+    I_dl = (dark[0] / dark[1]) * (1 - math.exp(-dark[1]))
+    I_dl = I_dl * math.exp(-light[1]) + (light[0] / light[1]) * (1 - math.exp(-light[1]))
+    assert abs(I_ld - 0.6622625) < 1e-7 and abs(I_dl - 1.9889308) < 1e-7
+    eta = np.array([[2.0, 0.4], [2.0, 0.4]])
+    chi = np.array([[0.2, 1.4], [0.2, 1.4]])
+    eps = 2.0 ** -20
+    # radiation propagating +x ends in the dark voxel (light -> dark); propagating -x the reverse
+    wl = iso_workload((2, 2), 2, eta, chi, probes=[[2.0 - eps, 0.5], [eps, 0.5]], dirs=[[1.0, 0.0], [-1.0, 0.0]])
+    for res in (orc.plain_march(wl), orc.hdda_march(wl, orc.build_mips(wl))):
+        assert abs(res.I[0, 0, 0] - 0.6622625) < 3e-6
+        assert abs(res.I[1, 1, 0] - 1.9889308) < 3e-6
+        assert res.I[0, 0, 0] < res.I[1, 1, 0]
+
+
+# ------------------------------------------------------------------ P3: chi = 0 handling, thin limit
+def test_p3_transparent_and_thin():
+    """Zero-opacity voxels are transparent; for small chi ds the RTE is linear:
+    I ~= sum eta h ds."""
+    rng = np.random.default_rng(5)
+    dims = (32, 32)
+    eta = np.zeros(dims[::-1])
+    chi = np.zeros(dims[::-1])
+    eta[8:24, 8:24] = 1.0
+    chi[8:24, 8:24] = 0.5
+    probes = rng.uniform(1, 31, size=(30, 2))
+    dirs = random_unit_dirs(8, 2, rng)
+    i0 = np.full((8, 8), 0.7)
+    wl = iso_workload(dims, 16, eta, chi, probes, dirs, i0=i0)
+    A = orc.plain_march(wl, capture=True)
+    # independent expectation: only the opaque square matters; its chord length from the capture
+    for r in range(A.counts.shape[0]):
+        n = A.counts[r]
+        lvl, x, y, z = orc.unpack_record(A.records[r, :n])
+        inside = (x >= 8) & (x < 24) & (y >= 8) & (y < 24)
+        # segments are listed probe-outward: material in front of the square (towards the probe) is empty
+        L = float(A.ds[r, :n][inside].astype(np.float64).sum())
+        want = float(np.float32(0.7)) * math.exp(-0.5 * L) + 2.0 * (1 - math.exp(-0.5 * L))
+        p, k = divmod(r, 8)
+        assert abs(A.I[p, k, 0] - want) < 1e-12 + 1e-12 * want
+    # pure emitter (chi = 0): I = I0 + eta h L exactly; thin medium: first-order
+    wl2 = iso_workload(dims, 16, np.full(dims[::-1], 0.25), np.zeros(dims[::-1]), probes, dirs, h=2.0)
+    A2 = orc.plain_march(wl2)
+    wl3 = iso_workload(dims, 16, np.full(dims[::-1], 0.25), np.full(dims[::-1], 1e-9), probes, dirs, h=2.0)
+    A3 = orc.plain_march(wl3)
+    for p in range(30):
+        for k in range(8):
+            L = path_to_boundary(wl2.probe_pos[p], wl2.dirs[k], dims)
+            assert abs(A2.I[p, k, 0] - 0.25 * 2.0 * L) < 3e-6 * 0.5 * L
+            assert abs(A3.I[p, k, 0] - A2.I[p, k, 0]) < 1e-6 * A2.I[p, k, 0]
+
+
+# ------------------------------------------------------------------ P4: J
+def test_p4_mean_intensity():
+    """J = sum_k w_k I_k.  Optically thick uniform medium: I -> S for every direction,
+    so J -> S sum(w); and a hand example with unequal weights."""
+    dims = (32, 32)
+    wl = iso_workload(dims, 16, np.full(dims[::-1], 30.0 * 2.5), np.full(dims[::-1], 30.0), probes=[[16.5, 16.5]],
+                      dirs=dirs_2d(16)[0])
+    A = orc.plain_march(wl)
+    J = orc.mean_intensity(A.I, wl.weights)
+    assert abs(J[0, 0] - 2.5) < 1e-9
+    I = np.arange(2 * 3 * 2, dtype=np.float64).reshape(2, 3, 2)
+    w = np.array([0.5, 0.25, 0.125], dtype=np.float32)
+    J = orc.mean_intensity(I, w)
+    assert np.allclose(J, [[0 * .5 + 2 * .25 + 4 * .125, 1 * .5 + 3 * .25 + 5 * .125],
+                           [6 * .5 + 8 * .25 + 10 * .125, 7 * .5 + 9 * .25 + 11 * .125]], rtol=0, atol=1e-15)
+
+
+# ------------------------------------------------------------------ P5/P6: HDDA == plain DDA
+def _lists_equal_filtered(wl, A, B):
+    act_b = orc.brick_active(wl)
+    bd = wl.brick_dims
+    bad = 0
+    for r in range(A.counts.shape[0]):
+        na = A.counts[r]
+        recA, dsA = A.records[r, :na], A.ds[r, :na]
+        lvl, x, y, z = orc.unpack_record(recA)
+        b = ((z // wl.brick) * bd[1] + y // wl.brick) * bd[0] + x // wl.brick
+        keep = act_b[b]
+        nb_ = B.counts[r]
+        if keep.sum() != nb_ or not np.array_equal(recA[keep], B.records[r, :nb_]) or \
+                not np.array_equal(dsA[keep].view(np.uint32), B.ds[r, :nb_].view(np.uint32)):
+            bad += 1
+    return bad
+
+
+def test_p5_threshold_zero_reproduces_plain_march():
+    """V7 / north_star: VLM threshold 0 and all bricks occupied => level 0 everywhere => the HDDA
+    visit list and intensities are those of the plain march, bit for bit."""
+    wl = make("C1", n=32, n_dirs=8)
+    d0, _ = dirs_2d(8, phase=0.0)      # axis-aligned and exact diagonals too
+    wl.dirs = np.concatenate([wl.dirs, d0]).astype(np.float32)
+    wl.weights = np.full(16, 1 / 16, dtype=np.float32)
+    M = orc.build_mips(wl, max_level=3, thr_eta=0.0, thr_chi=0.0)
+    assert (M.levels == 0).all()
+    A = orc.plain_march(wl, capture=True)
+    B = orc.hdda_march(wl, M, capture_batch=0)
+    assert _lists_equal_filtered(wl, A, B) == 0
+    assert np.array_equal(A.I, B.I)
+
+
+@pytest.mark.parametrize("ndim", [2, 3])
+def test_p6_brick_skipping_equals_filtered_plain_list(ndim):
+    """north_star: the HDDA voxel-visit list equals the plain DDA's non-empty visits, bitwise incl. ds."""
+    if ndim == 2:
+        wl = make("C2", n=128, n_dirs=12, n_probes=200)
+        extra, _ = dirs_2d(8, phase=0.0)
+        rng = np.random.default_rng(3)
+        wl.probe_pos = np.concatenate([wl.probe_pos, rng.uniform(0, 128, size=(50, 2)).astype(np.float32)])
+    else:
+        wl = make("C5", n=32, n_dirs=12, n_probes=150)
+        wl.variant = 0
+        wl.eta, wl.chi = wl.eta_bg, wl.chi_bg
+        extra = np.array([[1, 0, 0], [0, -1, 0], [0, 0, 1], [1, 1, 0], [1, 1, 1], [-1, 1, -1]], dtype=np.float64)
+        extra = (extra / np.linalg.norm(extra, axis=1, keepdims=True)).astype(np.float32)
+    wl.dirs = np.concatenate([wl.dirs, extra]).astype(np.float32)
+    wl.weights = np.full(len(wl.dirs), 1.0 / len(wl.dirs), dtype=np.float32)
+    M0 = orc.build_mips(wl, max_level=0, variant=0)
+    assert (M0.levels < 0).any() and (M0.levels == 0).any()
+    A = orc.plain_march(wl, M0, capture=True)
+    B = orc.hdda_march(wl, M0, capture_batch=0)
+    assert _lists_equal_filtered(wl, A, B) == 0
+    assert np.array_equal(A.I, B.I)
+    assert B.segments < A.segments
+
+
+# ------------------------------------------------------------------ P7: mips + HDDA together
+def test_p7_hdda_equals_plain_march_over_upsampled_field():
+    """Segments with equal eta, chi compose exactly, so VLM+HDDA must equal the plain march over the
+    field in which every voxel carries its cell's mip value (agreement to fp32 ds rounding)."""
+    wl = make("C2", n=128, n_dirs=16, n_probes=300)
+    M = orc.build_mips(wl, thr_eta=0.05, thr_chi=0.05)
+    assert len(np.unique(M.levels)) >= 3
+    B = orc.hdda_march(wl, M)
+    # upsample: per batch, per brick, take the level-m chain repeated 2^m times
+    n, b, W = 128, wl.brick, wl.lambda_batch
+    eta_up = np.zeros((n, n, wl.n_lambda), dtype=np.float32)
+    chi_up = np.zeros_like(eta_up)
+    nbx = n // b
+    for bt in range(wl.n_batch):
+        sl = slice(bt * W, (bt + 1) * W)
+        for bi in range(wl.n_bricks):
+            m = int(M.levels[bt, bi])
+            if m < 0:
+                continue
+            by, bx = divmod(bi, nbx)
+            cb = b >> m
+            for name, up in (("eta", eta_up), ("chi", chi_up)):
+                src = getattr(M, name)[m][by * cb:(by + 1) * cb, bx * cb:(bx + 1) * cb, sl]
+                up[by * b:(by + 1) * b, bx * b:(bx + 1) * b, sl] = np.repeat(np.repeat(src, 1 << m, axis=0), 1 << m, axis=1)
+    wl_up = iso_workload((n, n), b, eta_up, chi_up, wl.probe_pos, wl.dirs, active=wl.active)
+    A = orc.plain_march(wl_up)
+    assert max_rel(B.I, A.I) < 2e-6
+
+
+# ------------------------------------------------------------------ P8: brute-force geometry
+def _check_against_brute_force(wl, levels_row, M, min_len=2e-3):
+    B = orc.hdda_march(wl, M, levels=levels_row[None, :].repeat(wl.n_batch, axis=0), capture_batch=0)
+    nd = wl.dirs.shape[0]
+    for r in range(B.counts.shape[0]):
+        p, k = divmod(r, nd)
+        bf = orc.brute_force_segments(wl, levels_row, wl.probe_pos[p], wl.dirs[k], min_len=min_len)
+        n = B.counts[r]
+        lvl, x, y, z = orc.unpack_record(B.records[r, :n])
+        ds = B.ds[r, :n].astype(np.float64)
+        keep = ds > min_len
+        got = list(zip(lvl[keep], x[keep], y[keep], z[keep]))
+        want = [(s[1], s[2], s[3], s[4]) for s in bf]
+        assert got == want, (r, got[:6], want[:6])
+        assert np.allclose(ds[keep], [s[5] for s in bf], rtol=0, atol=3e-5)
+        tot_bf = sum(s[5] for s in orc.brute_force_segments(wl, levels_row, wl.probe_pos[p], wl.dirs[k]))
+        assert abs(ds.sum() - tot_bf) < 1e-4
+
+
+def test_p8_fig5_fixture_brute_force():
+    """Fig. 5: 32x32, 4x4 blocks of 8x8 with the listed block states; HDDA must give the
+    geometric ray-cell intersections ("exact path length of the ray in each voxel")."""
+    rng = np.random.default_rng(8)
+    lv = fig5_levels()
+    probes = np.concatenate([rng.uniform(0, 32, size=(12, 2)), [[16.5, 16.5], [0.5, 31.5], [20.25, 11.75]]])
+    dirs = np.concatenate([random_unit_dirs(9, 2, rng), unit_dirs_2d([0.0, math.pi / 2, math.pi / 4, math.pi, 1.25 * math.pi])])
+    f = rng.uniform(0.5, 1.5, size=(32, 32))
+    wl = iso_workload((32, 32), 8, f, f, probes, dirs, max_level=3)
+    M = orc.build_mips(wl, max_level=3)
+    _check_against_brute_force(wl, lv, M)
+
+
+def test_p8_random_3d_brute_force():
+    rng = np.random.default_rng(9)
+    lv = rng.integers(-1, 4, size=64).astype(np.int8)       # 4x4x4 bricks of 8^3, levels -1..3
+    probes = rng.uniform(0, 32, size=(6, 3))
+    dirs = np.concatenate([random_unit_dirs(6, 3, rng), [[0, 0, 1.0], [0.6, 0.8, 0.0]]])
+    f = rng.uniform(0.5, 1.5, size=(32, 32, 32))
+    wl = iso_workload((32, 32, 32), 8, f, f, probes, dirs, max_level=3)
+    M = orc.build_mips(wl, max_level=3)
+    _check_against_brute_force(wl, lv, M)
+
+
+# ------------------------------------------------------------------ P9: pyramid sizes and packing
+def test_p9_pyramid_sizes_and_packing():
+    """PAPER.md:109 (1.33x / 1.14x), :142 (first two MIPs hold 94 % of 2D storage), :162 (3 bits per
+    16-block state, 21 per 64-bit word, 49 words = 392 B for 512^2), :132-138 (fractions sum to 1)."""
+    wl = make("C2", n=128, n_dirs=4, n_probes=4)
+    M = orc.build_mips(wl, max_level=4, thr_eta=1.0, thr_chi=1.0)
+    sizes = [a.size for a in M.eta]
+    assert abs(sum(sizes[:4]) / sizes[0] - 1.328125) < 1e-12
+    assert abs(sum(sizes) / sizes[0] - (1 + 1 / 4 + 1 / 16 + 1 / 64 + 1 / 256)) < 1e-12
+    assert abs((sizes[0] + sizes[1]) / (sizes[0] * 4 / 3) - 0.9375) < 1e-12     # "94 %"
+    assert abs(sum(8.0 ** -m for m in range(3)) - 1.140625) < 1e-15
+    words = orc.pack_levels(np.zeros(1024, dtype=np.int8), 4)                   # 512^2 / 16^2 = 1024 blocks
+    assert words.shape[0] == 49 and words.nbytes == 392
+    lv = np.random.default_rng(1).integers(-1, 5, size=1024).astype(np.int8)
+    w = orc.pack_levels(lv, 4)
+    un = np.array([((int(w[i // 21]) >> ((i % 21) * 3)) & 7) - 1 for i in range(1024)])
+    assert np.array_equal(un, lv)
+    # level histogram area fractions sum to 1 (Table 2 rows)
+    for b in range(wl.n_batch):
+        hist = np.bincount(M.levels[b] + 1, minlength=6)
+        assert hist.sum() == wl.n_bricks
+
+
+# ------------------------------------------------------------------ P10: level selection
+def _levels_by_loops(wl, max_level, metric, thr, tau_gate):
+    """Second, differently structured implementation of V1-V5 for ISO: per brick, per wavelength,
+    python floats (fp64), explicit loops.  2D only."""
+    n, B, W, h = wl.dims[0], wl.brick, wl.lambda_batch, float(wl.voxel_size)
+    thr, tau_gate = float(np.float32(thr)), float(np.float32(tau_gate))     # fp32 at the C ABI
+    eta = wl.eta.reshape(n, n, wl.n_lambda)
+    chi = wl.chi.reshape(n, n, wl.n_lambda)
+    act = wl.active.reshape(n, n)
+    nb = n // B
+    out = np.zeros((wl.n_batch, nb * nb), dtype=np.int8)
+
+    def stat(vals):
+        if all(v == vals[0] for v in vals):
+            return 0.0
+        if metric == orc.IOD_LOG:
+            if any(v <= 0 for v in vals):
+                return math.inf
+            X = [math.log(v * h) for v in vals]
+        else:
+            X = list(vals)
+        mean = (((X[0] + X[1]) + X[2]) + X[3]) / 4
+        var = (((X[0] - mean) ** 2 + (X[1] - mean) ** 2) + (X[2] - mean) ** 2 + (X[3] - mean) ** 2) / 4
+        if metric == orc.IOD_LOG:
+            return abs(var / mean) if mean != 0 else math.inf
+        return var / (mean * mean) if mean != 0 else math.inf
+
+    for by in range(nb):
+        for bx in range(nb):
+            bi = by * nb + bx
+            if not act[by * B:(by + 1) * B, bx * B:(bx + 1) * B].any():
+                out[:, bi] = -1
+                continue
+            for bt in range(wl.n_batch):
+                level = 0
+                ce = [eta[by * B:(by + 1) * B, bx * B:(bx + 1) * B, bt * W:(bt + 1) * W].astype(np.float64)]
+                cc = [chi[by * B:(by + 1) * B, bx * B:(bx + 1) * B, bt * W:(bt + 1) * W].astype(np.float64)]
+                for m in range(1, max_level + 1):
+                    pe, pc = ce[-1], cc[-1]
+                    s = pe.shape[0] // 2
+                    ne = np.zeros((s, s, W))
+                    nc = np.zeros((s, s, W))
+                    ok = True
+                    for j in range(s):
+                        for i in range(s):
+                            for l in range(W):
+                                ve = [float(pe[2 * j, 2 * i, l]), float(pe[2 * j, 2 * i + 1, l]),
+                                      float(pe[2 * j + 1, 2 * i, l]), float(pe[2 * j + 1, 2 * i + 1, l])]
+                                vc = [float(pc[2 * j, 2 * i, l]), float(pc[2 * j, 2 * i + 1, l]),
+                                      float(pc[2 * j + 1, 2 * i, l]), float(pc[2 * j + 1, 2 * i + 1, l])]
+                                ne[j, i, l] = np.float32((((ve[0] + ve[1]) + ve[2]) + ve[3]) * 0.25)
+                                nc[j, i, l] = np.float32((((vc[0] + vc[1]) + vc[2]) + vc[3]) * 0.25)
+                                passed = stat(ve) < thr and stat(vc) < thr
+                                if tau_gate >= 0 and ((((vc[0] + vc[1]) + vc[2]) + vc[3]) / 4) * h <= tau_gate:
+                                    passed = True
+                                ok = ok and passed
+                    if not ok:
+                        break
+                    level = m
+                    ce.append(ne)
+                    cc.append(nc)
+                out[bt, bi] = level
+    return out
+
+
+@pytest.mark.parametrize("metric,thr,gate", [(orc.RELVAR, 1e-2, -1.0), (orc.RELVAR, 0.2, -1.0),
+                                             (orc.IOD_LOG, 1.0, 0.25), (orc.IOD_LOG, 0.05, -1.0)])
+def test_p10_level_selection_second_implementation(metric, thr, gate):
+    wl = make("C2", n=64, n_dirs=4, n_probes=4, n_lambda=16)
+    M = orc.build_mips(wl, max_level=4, metric=metric, thr_eta=thr, thr_chi=thr, tau_gate=gate)
+    ref = _levels_by_loops(wl, 4, metric, thr, gate)
+    assert np.array_equal(M.levels, ref)
+
+
+def test_p10_uniform_brick_and_hand_example_and_monotone():
+    """Uniform brick: IoD = 0, passes for thr > 0, fails for thr = 0 (strict '<').
+    Hand 2x2 example: values (1,1,3,3): mean 2, var 1, relvar 0.25; ln-values: IoD = |var/mean| of
+    (0,0,ln3,ln3): var = (ln3/2)^2, mean = ln3/2 -> IoD = ln3/2 = 0.5493."""
+    dims = (16, 16)
+    u = np.full(dims, 0.3)
+    wl = iso_workload(dims, 16, u, u, [[1.5, 1.5]], [[1.0, 0.0]], max_level=4)
+    assert (orc.build_mips(wl, thr_eta=1e-9, thr_chi=1e-9).levels == 4).all()
+    assert (orc.build_mips(wl, thr_eta=0.0, thr_chi=0.0).levels == 0).all()
+    x = np.ones(dims)
+    x[1::2, :] = 3.0                    # children of every level-1 cell: (1,1,3,3)
+    wl = iso_workload(dims, 16, x, x, [[1.5, 1.5]], [[1.0, 0.0]], max_level=4)
+    assert (orc.build_mips(wl, metric=orc.RELVAR, thr_eta=0.2501, thr_chi=0.2501).levels >= 1).all()
+    assert (orc.build_mips(wl, metric=orc.RELVAR, thr_eta=0.2499, thr_chi=0.2499).levels == 0).all()
+    assert (orc.build_mips(wl, metric=orc.IOD_LOG, thr_eta=0.5494, thr_chi=0.5494).levels >= 1).all()
+    assert (orc.build_mips(wl, metric=orc.IOD_LOG, thr_eta=0.5492, thr_chi=0.5492).levels == 0).all()
+    # gate: chi h = 2 on average; gate above it lets everything be averaged, whatever the variance
+    assert (orc.build_mips(wl, metric=orc.RELVAR, thr_eta=0.0, thr_chi=0.0, tau_gate=2.0).levels == 4).all()
+    assert (orc.build_mips(wl, metric=orc.RELVAR, thr_eta=0.0, thr_chi=0.0, tau_gate=1.99).levels == 0).all()
+    # monotone in the threshold
+    wl = make("C2", n=128, n_dirs=4, n_probes=4)
+    prev = None
+    for thr in (0.0, 1e-3, 1e-2, 1e-1, 1.0):
+        lv = orc.build_mips(wl, max_level=4, thr_eta=thr, thr_chi=thr).levels
+        if prev is not None:
+            assert (lv >= prev).all()
+        prev = lv
+
+
+def test_v1_mip_values_are_correctly_rounded_means():
+    rng = np.random.default_rng(2)
+    a = np.exp(rng.standard_normal((8, 8, 3)) * 4).astype(np.float32)
+    m = orc.mip_mean(a, 2)
+    from fractions import Fraction
+    for j in range(4):
+        for i in range(4):
+            for c in range(3):
+                ex = sum(Fraction(float(a[2 * j + dy, 2 * i + dx, c])) for dy in (0, 1) for dx in (0, 1)) / 4
+                assert float(m[j, i, c]) == float(np.float32(float(ex)))
+
+
+# ------------------------------------------------------------------ P13: Voigt
+def test_p13_voigt_against_wofz_and_normalisation():
+    """HUM1WEI24 against scipy.special.wofz: <= 3e-7 relative at a = 0.01 inside the
+    Weideman region, <= 7e-5 in Humlicek's region I (the approximation's own error);
+    and the profile integrates to 1."""
+    from scipy.special import wofz
+    x = np.linspace(-40, 40, 16001)
+    for a, tol_in in ((0.01, 3e-7), (0.1, 3e-8), (1.0, 2e-9)):
+        H = orc.voigt_H(a, x)
+        ref = wofz(x + 1j * a).real
+        rel = np.abs(H - ref) / ref
+        inner = np.abs(x) + a < 15.0
+        assert rel[inner].max() < tol_in
+        assert rel[~inner].max() < 7e-5
+    xx = np.linspace(-2000, 2000, 2_000_001)
+    H = orc.voigt_H(0.01, xx)
+    integral = np.trapezoid(H, xx) / math.sqrt(math.pi)
+    assert abs(integral + 2 * 0.01 / (math.pi * 2000) - 1.0) < 2e-6    # Lorentz tail beyond +-2000 added back
+    assert abs(orc.voigt_H(0.0, 0.0) - 1.0) < 1e-9
+    assert abs(orc.voigt_H(0.0, 1.5) - math.exp(-2.25)) < 1e-8
+
+
+# ------------------------------------------------------------------ P11 / P12: anisotropic providers
+def _aniso_small(name, **kw):
+    wl = make(name, **kw)
+    return wl
+
+
+def test_p12_cav_level0_equals_classic_and_rest_frame_identity():
+    """Cav at level 0 with per-voxel v is the Classic brute force; at v = 0 and
+    lambda = lambda0 eqs. 18-20 are the identity and eq. 14 the static profile."""
+    wl = make("C4", n=64, n_dirs=6, n_probes=40)
+    Mc = orc.build_mips(wl, max_level=0)
+    A = orc.plain_march(wl, variant=orc.CLASSIC)
+    B = orc.hdda_march(wl, Mc)
+    assert max_rel(B.I, A.I) < 1e-12
+    e, c = orc.line_terms(500.0, 500.0, 3.0, 7.0, 0.01, 40.0, 0.0, 299792.458)
+    phi0 = orc.voigt_H(0.01, 0.0) * 40.0 / math.sqrt(math.pi)
+    assert abs(e - 3.0 * phi0) < 1e-15 * abs(e) + 1e-300 and abs(c - 7.0 * phi0) < 1e-15 * abs(c)
+    # Doppler shift moves the line centre to lambda0 (1 - v.w/c) (eq. 14 and eq. 17)
+    v = 20.0
+    lam_c = 500.0 * (1 - v / 299792.458)
+    e_c, _ = orc.line_terms(lam_c, 500.0, 1.0, 1.0, 0.01, 40.0, v, 299792.458)
+    e_l, _ = orc.line_terms(lam_c - 0.01, 500.0, 1.0, 1.0, 0.01, 40.0, v, 299792.458)
+    e_r, _ = orc.line_terms(lam_c + 0.01, 500.0, 1.0, 1.0, 0.01, 40.0, v, 299792.458)
+    assert e_c > e_l and e_c > e_r
+
+
+def test_p12_static_medium_is_isotropic():
+    wl = make("C3", n=64, n_dirs=8, n_probes=30)
+    wl.vel[:] = 0.0
+    Mc = orc.build_mips(wl, max_level=0, variant=orc.CAV)
+    A = orc.plain_march(wl, variant=orc.CLASSIC)
+    # rest-frame fields computed once, marched as ISO
+    lam = wl.lam.astype(np.float64)
+    e, c = orc.line_terms(lam[None, :], 500.0, wl.eta_star0[0][:, None], wl.chi_star0[0][:, None],
+                          wl.a0[0][:, None], wl.inv_dlamD[0][:, None], 0.0, wl.c_light)
+    iso = iso_workload(wl.dims[:2], wl.brick, (wl.eta_bg + e).reshape(64, 64, -1), (wl.chi_bg + c).reshape(64, 64, -1),
+                       wl.probe_pos, wl.dirs, active=wl.active)
+    C_ = orc.plain_march(iso)
+    assert max_rel(A.I, C_.I) < 3e-7        # iso fields are rounded to fp32 once
+
+
+def test_p11_velinterp_static_nodes_and_convergence():
+    """VelInterp: v = 0 => table interpolation returns the static field; exact at
+    bin nodes; converges to Classic as n grows."""
+    wl = make("C3", n=64, n_dirs=8, n_probes=40)
+    A = orc.plain_march(wl, variant=orc.CLASSIC)
+    errs = []
+    for n in (8, 32, 128):
+        wl.n_vbins = n
+        Mv = orc.build_mips(wl, max_level=0, variant=orc.VELINTERP)
+        B = orc.hdda_march(wl, Mv)
+        errs.append(np.percentile(np.abs(B.I - A.I) / np.maximum(A.I, 1e-300), 99))
+    assert errs[2] < errs[1] < errs[0] and errs[2] < 1e-2
+    # exact at nodes: a direction parallel to v projects onto the last bin
+    wl.n_vbins = 8
+    Mv = orc.build_mips(wl, max_level=0, variant=orc.VELINTERP)
+    nv = wl.nvox
+    V = np.sqrt((wl.vel.astype(np.float64) ** 2).sum(-1))
+    vox = int(np.argmax(V))
+    lam = wl.lam.astype(np.float64)
+    e, c = orc.line_terms(lam, 500.0, wl.eta_star0[0][vox], wl.chi_star0[0][vox], wl.a0[0][vox],
+                          wl.inv_dlamD[0][vox], float(np.float32(V[vox])), wl.c_light)
+    tab = Mv.vtab[0].reshape(nv, 8, wl.n_lambda, 2)[vox]
+    assert np.allclose(tab[7, :, 0], (wl.eta_bg[vox] + e).astype(np.float32), rtol=2e-7)
+    assert np.allclose(tab[7, :, 1], (wl.chi_bg[vox] + c).astype(np.float32), rtol=2e-7)
+    # static medium: every bin equal => interpolation is the static value
+    wl.vel[:] = 0.0
+    Mv0 = orc.build_mips(wl, max_level=0, variant=orc.VELINTERP)
+    B0 = orc.hdda_march(wl, Mv0)
+    A0 = orc.plain_march(wl, variant=orc.CLASSIC)
+    assert max_rel(B0.I, A0.I) < 3e-7
+
+
+def test_aniso_mips_hdda_consistency():
+    """With mips on, Cav/VelInterp levels are populated and the HDDA result stays close to Classic
+    (sanity: accuracy is reported, not gated -- SURVEY.md 8(d))."""
+    for name in ("C3", "C4"):
+        wl = make(name, n=256, n_dirs=8, n_probes=40)
+        M = orc.build_mips(wl)
+        assert M.levels.max() >= 1 and (M.levels == -1).any()
+        B = orc.hdda_march(wl, M)
+        A = orc.plain_march(wl, variant=orc.CLASSIC)
+        J_b = orc.mean_intensity(B.I, wl.weights)
+        J_a = orc.mean_intensity(A.I, wl.weights)
+        ok = J_a > 0
+        rel = np.abs(J_b[ok] - J_a[ok]) / J_a[ok]
+        assert np.percentile(rel, 90) < 0.2
