@@ -1,0 +1,201 @@
+/*
+ * dex.h -- C-ABI boundary of the B200-native long-characteristics formal solver
+ * (hot path of arxiv/paper_2511_08498, "A Simple Ray Acceleration Structure for Non-LTE
+ * Radiative Transfer").  PAPER.md below is /root/reference/PAPER.md; T-/V-rules are the
+ * traversal / level contracts of SURVEY.md section 8(c), restated in DESIGN.md.
+ *
+ * Conventions
+ *   - `d_*` pointers are CALLER-OWNED DEVICE memory (e.g. a torch tensor's data_ptr()),
+ *     `h_*` pointers are caller-owned HOST memory.  The library never frees or retains them
+ *     after the call returns; it copies what it needs into the opaque handles it owns until
+ *     dex_destroy_*.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Work is enqueued
+ *     asynchronously; only dex_build_sparse_grid (reads back the active-brick count),
+ *     dex_*_info / dex_*_get_* and a formal solution with visit capture synchronise.
+ *   - Index space: a level-0 voxel has side 1; its physical side is
+ *     `voxel_size` (the "Delta s" of PAPER.md:130).  Voxel v = (z*Ny + y)*Nx + x.
+ *   - Per-voxel spectra are [nvox][n_lambda] fp32 with lambda fastest; per-line fields are
+ *     [n_lines][nvox]; velocities [nvox][ndim].
+ *   - Every call returns a dex_status; nothing throws or aborts across the ABI.  Argument
+ *     errors are detected before any launch.  dex_last_error() gives a thread-local message.
+ *   - NaN / negative eta, chi are the caller's responsibility.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns DEX_ERR_CUDA.
+ */
+#ifndef DEX_H_
+#define DEX_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DEX_MAX_LINES 4 /* maximum overlapping lines in a wavelength batch */
+
+typedef enum {
+  DEX_OK = 0,
+  DEX_ERR_INVALID_ARG = 1,
+  DEX_ERR_SHAPE = 2,
+  DEX_ERR_UNSUPPORTED = 3,
+  DEX_ERR_OOM = 4,
+  DEX_ERR_CUDA = 5,
+  DEX_ERR_CAPACITY = 6
+} dex_status;
+
+/* Thread-local description of the last failure on this thread; valid until the next call. */
+const char* dex_last_error(void);
+/* Library version string (static storage). */
+const char* dex_version(void);
+
+typedef struct dex_grid dex_grid; /* opaque, library-owned */
+typedef struct dex_mips dex_mips; /* opaque, library-owned */
+
+/* ------------------------------------------------------------------------------------------
+ * Sparse brick grid: the model is split into cubic blocks of side
+ * `brick` (16 in 2D / 8 in 3D typically) which are populated or empty.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct {
+  int ndim;         /* 2 or 3 */
+  int dims[3];      /* Nx, Ny, Nz voxels (Nz ignored in 2D); each a multiple of brick */
+  int brick;        /* power of two, 2..32 */
+  float voxel_size; /* h > 0, physical side of a level-0 voxel */
+} dex_grid_desc;
+
+/* a1. Brick occupancy + compaction.  A brick is active iff any of its voxels has
+ * d_active != 0 (the sparsity map is shared by all wavelengths);
+ * d_active == NULL means all active.  Active bricks get storage slots 0..A-1 in brick-index
+ * order.  Synchronises once to read A back.
+ * Errors: DEX_ERR_INVALID_ARG (NULL desc/out, ndim), DEX_ERR_SHAPE (dims not multiple of
+ * brick, brick not a power of two), DEX_ERR_OOM, DEX_ERR_CUDA. */
+dex_status dex_build_sparse_grid(const dex_grid_desc* desc, const uint8_t* d_active /*[nvox] or NULL*/,
+                                 void* stream, dex_grid** out);
+dex_status dex_grid_info(const dex_grid* grid, int64_t* n_bricks, int64_t* n_active);
+/* Validation: slot per brick, -1 = empty.  Brick b = (bz*NBy + by)*NBx + bx. */
+dex_status dex_grid_get_slots(const dex_grid* grid, int32_t* h_slot /*[n_bricks]*/);
+void dex_destroy_grid(dex_grid* grid);
+
+/* ------------------------------------------------------------------------------------------
+ * MIP pyramid + variance-limited mipmapping
+ * ---------------------------------------------------------------------------------------- */
+typedef enum {
+  DEX_ISO = 0,       /* static medium: fetch eta, chi */
+  DEX_VELINTERP = 1, /* velocity-grid AVLM */
+  DEX_CAV = 2,       /* "Core and Voigt" AVLM */
+  DEX_CLASSIC = 3    /* brute force at every level-0 cell for every direction; no mips */
+} dex_variant;
+
+typedef enum {
+  DEX_METRIC_IOD_LOG = 0, /* eq. 8 on ln(eta h), ln(chi h) + chi h gate */
+  DEX_METRIC_RELVAR = 1   /* Var[x]/Mean[x]^2 of eta, chi (BASELINE.json wording) */
+} dex_metric;
+
+typedef struct {
+  dex_variant variant;
+  int n_lambda;     /* total wavelengths; multiple of lambda_batch */
+  int lambda_batch; /* W: wavelengths per batch sharing one level table (8). Must be 8. */
+  int max_level;    /* 0 <= max_level <= log2(brick) */
+  dex_metric metric;
+  float thr_eta, thr_chi; /* a cell passes iff metric < thr for both (strict) */
+  float tau_gate;         /* always average where mean(chi) h <= tau_gate; < 0 disables */
+  const float* d_lambda;  /* [n_lambda] wavelengths (anisotropic variants; same unit as h_lambda0) */
+  /* ISO */
+  const float* d_eta; /* [nvox][n_lambda] */
+  const float* d_chi;
+  /* anisotropic variants (eqs. 10-20) */
+  const float* d_eta_bg; /* [nvox][n_lambda] isotropic background */
+  const float* d_chi_bg;
+  const float* d_vel; /* [nvox][ndim] bulk velocity, unit of c_light */
+  int n_lines;
+  const float* h_lambda0;   /* [n_lines] rest wavelengths (HOST) */
+  const float* d_eta_star0; /* [n_lines][nvox] eta*_l(lambda0)  (eq. 18) */
+  const float* d_chi_star0; /* [n_lines][nvox] chi*_l(lambda0)  (eq. 19) */
+  const float* d_a0;        /* [n_lines][nvox] damping a(lambda0) (eq. 20) */
+  const float* d_inv_dlamD; /* [n_lines][nvox] 1 / Doppler width */
+  const int8_t* h_active_lines; /* [n_batch][DEX_MAX_LINES] line ids, -1 padded (HOST) */
+  int n_vbins;   /* DEX_VELINTERP: velocity bins per cell, 2..32 */
+  float c_light; /* speed of light in the unit of d_vel */
+} dex_mips_desc;
+
+/* a2-a4. Gather active bricks into brick-major storage, build the box-filter mips of every
+ * chain of the variant (V1: fp64 sum of the 2^D children, one rounding), evaluate the VLM cell
+ * test in fp64 (V2-V6) and select one level per (batch, brick) (V5), packed into 64-bit words
+ * (PAPER.md:162).  Asynchronous on `stream`.
+ * Errors: DEX_ERR_INVALID_ARG (NULL pointers required by the variant), DEX_ERR_SHAPE
+ * (max_level > log2(brick), n_lambda % lambda_batch, n_lines > DEX_MAX_LINES, bad line ids),
+ * DEX_ERR_UNSUPPORTED (lambda_batch != 8, n_vbins out of range), DEX_ERR_OOM, DEX_ERR_CUDA. */
+dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, void* stream, dex_mips** out);
+/* Validation accessors (synchronise). */
+dex_status dex_mips_get_levels(const dex_mips* mips, int8_t* h_level /*[n_batch][n_bricks], -1 empty*/);
+dex_status dex_mips_set_levels(dex_mips* mips, const int8_t* h_level /*same shape; injects a table*/);
+/* Packed block states of one batch: state = level + 1 (0 = empty) in ceil(log2(max_level+2)) bits,
+ * floor(64/bits) bricks per word, no straddling.  *n_words receives the word count; h_words may be
+ * NULL to query it. */
+dex_status dex_mips_get_packed_levels(const dex_mips* mips, int batch, uint64_t* h_words, int64_t* n_words);
+typedef enum {
+  DEX_CHAIN_ETA = 0,      /* ISO eta / background eta:  [cells_m][n_lambda] */
+  DEX_CHAIN_CHI = 1,
+  DEX_CHAIN_VEL = 2,      /* [cells_m][4]: box-filtered vx, vy, vz(0 in 2D), max |v| over the cell */
+  DEX_CHAIN_LINE = 3,     /* [cells_m][n_lines][4]: eta*, chi*, a0, 1/dlamD */
+  DEX_CHAIN_VTAB = 4      /* [cells_m][n_vbins][n_lambda][2] (eta, chi), DEX_VELINTERP */
+} dex_chain;
+/* Canonical dense level-m array of a chain (cells of empty bricks are 0). */
+dex_status dex_mips_get_level_data(const dex_mips* mips, int chain, int level, float* h_dense);
+void dex_destroy_mips(dex_mips* mips);
+
+/* ------------------------------------------------------------------------------------------
+ * Rays: long characteristics from each probe along each quadrature direction to the grid
+ * boundary.  I(p, w) is the intensity arriving at p propagating along w; the
+ * library traces the upwind characteristic x(s) = p - s w (T1).
+ * ---------------------------------------------------------------------------------------- */
+typedef struct {
+  int64_t n_probes;
+  const float* d_probe_pos; /* [n_probes][ndim], index space, inside [0, N) on every axis */
+  int n_dirs;
+  const float* d_dirs;    /* [n_dirs][ndim] unit propagation directions */
+  const float* d_weights; /* [n_dirs] quadrature weights (dex_mean_intensity) */
+  const float* d_i0;      /* [n_dirs][n_lambda] incoming boundary intensity, NULL = 0 */
+} dex_rays;
+
+/* a10. Visit-list capture (validation mode).  Ray r = probe * n_dirs + dir.  Records of ray r
+ * are written at d_records[d_offsets[r] + i] in trace order (probe outward) for the traversal of
+ * batch `batch`; a record is level << 56 | z << 36 | y << 18 | x with (x,y,z) the cell coordinate
+ * at that level (T7).  d_ds (optional) receives the fp32 path lengths.  d_counts[r] always gets the
+ * full count; records beyond the ray's room (d_offsets[r+1] - d_offsets[r], last ray: capacity)
+ * are dropped and the call returns DEX_ERR_CAPACITY after finishing. */
+typedef struct {
+  int64_t* d_counts;        /* [n_rays] */
+  uint64_t* d_records;      /* [capacity] */
+  float* d_ds;              /* [capacity] or NULL */
+  int64_t capacity;
+  const int64_t* d_offsets; /* [n_rays] */
+  int batch;
+} dex_visit_capture;
+
+/* a5-a8. HDDA traversal (Algorithm 1, under the T-rules) + per-segment
+ * I_out = I_in e^{-chi h ds} + eta h ds E(chi h ds), E(t) = (1 - e^{-t})/t, for every wavelength
+ * (eq. 3 with piecewise-constant eta, chi).
+ * d_I: [n_probes][n_dirs][n_lambda] fp32.  d_segment_count: NULL or one int64 counter that is
+ * INCREMENTED by the number of emitted (non-empty, ds > 0) segments over all rays and batches. */
+dex_status dex_formal_solution(const dex_grid* grid, const dex_mips* mips, const dex_rays* rays, float* d_I,
+                               dex_visit_capture* capture /*NULL = off*/, int64_t* d_segment_count,
+                               void* stream);
+
+/* a9. J(p, lambda) = sum_k w_k I(p, k, lambda).  d_I == NULL: trace internally and
+ * reduce in the same kernel (fused; I is never materialised).  d_J: [n_probes][n_lambda] fp32. */
+dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const dex_rays* rays,
+                              const float* d_I /*NULL = fused*/, float* d_J, int64_t* d_segment_count,
+                              void* stream);
+
+/* Number of kernel launches this library has enqueued since load (bench.py's gpu_launches). */
+int64_t dex_launch_count(void);
+/* Device time (ms) and launch count of the march kernels since the last reset, measured with CUDA
+ * events on the launching stream when timing is enabled (bench.py roofline leg).  Synchronises. */
+void dex_march_timing_enable(int on);
+dex_status dex_march_timing_read(double* ms_total, int64_t* n_launches, int reset);
+/* Kernel configuration knob (performance experiments): lanes that share one ray, 1/2/4/8. */
+dex_status dex_set_lanes_per_ray(int lanes);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEX_H_ */

@@ -1,0 +1,446 @@
+// dex_api.cu -- the extern "C" boundary declared in include/dex.h: argument validation, handle
+// ownership, and dispatch to the kernels.  No compute happens on the host.
+#include <math.h>
+#include <string.h>
+
+#include <atomic>
+#include <mutex>
+#include <new>
+#include <vector>
+
+#include "dex_internal.h"
+#include "dex_voigt.cuh"
+
+namespace {
+thread_local std::string g_last_error;
+std::atomic<long long> g_launches{0};
+std::atomic<int> g_lanes_per_ray{8};
+std::atomic<int> g_timing{0};
+std::mutex g_timing_mu;
+struct EvPair { cudaEvent_t a, b; };
+std::vector<EvPair> g_events;
+
+int ilog2_exact(int v) {
+  if (v <= 0 || (v & (v - 1))) return -1;
+  int l = 0;
+  while ((1 << l) < v) ++l;
+  return l;
+}
+
+bool have_device() {
+  int n = 0;
+  cudaError_t e = cudaGetDeviceCount(&n);
+  if (e != cudaSuccess || n <= 0) {
+    cudaGetLastError();
+    dex_set_error("no CUDA device available (this library has no CPU fallback)");
+    return false;
+  }
+  return true;
+}
+
+template <typename T>
+dex_status dmalloc(T** p, size_t count) {
+  *p = nullptr;
+  if (count == 0) count = 1;
+  DEX_CUDA_CHECK(cudaMalloc((void**)p, sizeof(T) * count));
+  return DEX_OK;
+}
+
+void free_mips_memory(dex_mips* m) {
+  cudaFree(m->d_store); cudaFree(m->d_line); cudaFree(m->d_vel); cudaFree(m->d_vtab); cudaFree(m->d_lam);
+  cudaFree(m->d_active_lines); cudaFree(m->d_levels); cudaFree(m->d_packed); cudaFree(m->d_fail);
+}
+
+dex_status check_rays(const dex_grid* grid, const dex_mips* mips, const dex_rays* rays, DexRaysDev* out) {
+  if (!grid || !mips || !rays) { dex_set_error("NULL grid / mips / rays"); return DEX_ERR_INVALID_ARG; }
+  if (mips->grid != grid) { dex_set_error("mips were built for a different grid"); return DEX_ERR_INVALID_ARG; }
+  if (rays->n_probes < 0 || rays->n_dirs < 0) { dex_set_error("negative ray counts"); return DEX_ERR_SHAPE; }
+  if (rays->n_probes > 0 && rays->n_dirs > 0 && (!rays->d_probe_pos || !rays->d_dirs)) {
+    dex_set_error("d_probe_pos / d_dirs is NULL");
+    return DEX_ERR_INVALID_ARG;
+  }
+  out->n_probes = rays->n_probes;
+  out->probe_pos = rays->d_probe_pos;
+  out->n_dirs = rays->n_dirs;
+  out->dirs = rays->d_dirs;
+  out->weights = rays->d_weights;
+  out->i0 = rays->d_i0;
+  return DEX_OK;
+}
+
+struct MarchTimer {
+  cudaStream_t st;
+  bool on;
+  EvPair ev{};
+  explicit MarchTimer(cudaStream_t s) : st(s), on(g_timing.load() != 0) {
+    if (on) {
+      cudaEventCreate(&ev.a);
+      cudaEventCreate(&ev.b);
+      cudaEventRecord(ev.a, st);
+    }
+  }
+  ~MarchTimer() {
+    if (on) {
+      cudaEventRecord(ev.b, st);
+      std::lock_guard<std::mutex> lk(g_timing_mu);
+      g_events.push_back(ev);
+    }
+  }
+};
+}  // namespace
+
+void dex_set_error(const std::string& msg) { g_last_error = msg; }
+void dex_count_launch(int n) { g_launches.fetch_add(n); }
+
+extern "C" {
+
+const char* dex_last_error(void) { return g_last_error.c_str(); }
+const char* dex_version(void) { return "dex-b200 0.1 (sm_100a)"; }
+int64_t dex_launch_count(void) { return (int64_t)g_launches.load(); }
+
+dex_status dex_set_lanes_per_ray(int lanes) {
+  if (lanes != 1 && lanes != 2 && lanes != 4 && lanes != 8) {
+    dex_set_error("lanes per ray must be 1, 2, 4 or 8");
+    return DEX_ERR_INVALID_ARG;
+  }
+  g_lanes_per_ray.store(lanes);
+  return DEX_OK;
+}
+
+void dex_march_timing_enable(int on) { g_timing.store(on ? 1 : 0); }
+
+dex_status dex_march_timing_read(double* ms_total, int64_t* n_launches, int reset) {
+  std::lock_guard<std::mutex> lk(g_timing_mu);
+  double total = 0.0;
+  for (auto& ev : g_events) {
+    DEX_CUDA_CHECK(cudaEventSynchronize(ev.b));
+    float ms = 0.f;
+    DEX_CUDA_CHECK(cudaEventElapsedTime(&ms, ev.a, ev.b));
+    total += (double)ms;
+  }
+  if (ms_total) *ms_total = total;
+  if (n_launches) *n_launches = (int64_t)g_events.size();
+  if (reset) {
+    for (auto& ev : g_events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+    g_events.clear();
+  }
+  return DEX_OK;
+}
+
+// ------------------------------------------------------------------------------------------- grid
+dex_status dex_build_sparse_grid(const dex_grid_desc* desc, const uint8_t* d_active, void* stream, dex_grid** out) {
+  if (!desc || !out) { dex_set_error("NULL desc / out"); return DEX_ERR_INVALID_ARG; }
+  *out = nullptr;
+  if (desc->ndim != 2 && desc->ndim != 3) { dex_set_error("ndim must be 2 or 3"); return DEX_ERR_INVALID_ARG; }
+  const int logB = ilog2_exact(desc->brick);
+  if (logB < 1 || desc->brick > 32) { dex_set_error("brick must be a power of two in 2..32"); return DEX_ERR_SHAPE; }
+  if (!(desc->voxel_size > 0.0f)) { dex_set_error("voxel_size must be > 0"); return DEX_ERR_INVALID_ARG; }
+  int64_t nvox = 1, nbr = 1;
+  for (int a = 0; a < desc->ndim; ++a) {
+    if (desc->dims[a] <= 0 || desc->dims[a] % desc->brick) {
+      dex_set_error("every dimension must be a positive multiple of brick");
+      return DEX_ERR_SHAPE;
+    }
+    if (desc->dims[a] >= (1 << 18)) { dex_set_error("dimension too large (< 2^18)"); return DEX_ERR_SHAPE; }
+    nvox *= desc->dims[a];
+    nbr *= desc->dims[a] / desc->brick;
+  }
+  if (nbr > 2147483647LL / 64) { dex_set_error("too many bricks"); return DEX_ERR_SHAPE; }
+  if (!have_device()) return DEX_ERR_CUDA;
+  dex_grid* g = new (std::nothrow) dex_grid();
+  if (!g) { dex_set_error("host allocation failed"); return DEX_ERR_OOM; }
+  g->desc = *desc;
+  if (desc->ndim == 2) g->desc.dims[2] = 1;
+  g->n_bricks = nbr;
+  g->nvox = nvox;
+  DexGridDev& d = g->dev;
+  d.ndim = desc->ndim;
+  for (int a = 0; a < 3; ++a) {
+    d.dims[a] = (a < desc->ndim) ? desc->dims[a] : 1;
+    d.nb[a] = (a < desc->ndim) ? desc->dims[a] / desc->brick : 1;
+  }
+  d.B = desc->brick;
+  d.logB = logB;
+  d.h = desc->voxel_size;
+  d.n_bricks = (int)nbr;
+  d.n_active = 0;
+  dex_status s = dmalloc(&g->d_slot, (size_t)nbr);
+  if (s == DEX_OK) s = dmalloc(&g->d_active_bricks, (size_t)nbr);
+  if (s == DEX_OK) { d.slot = g->d_slot; s = dex_launch_grid_build(g, d_active, (cudaStream_t)stream); }
+  if (s != DEX_OK) { dex_destroy_grid(g); return s; }
+  *out = g;
+  return DEX_OK;
+}
+
+dex_status dex_grid_info(const dex_grid* grid, int64_t* n_bricks, int64_t* n_active) {
+  if (!grid) { dex_set_error("NULL grid"); return DEX_ERR_INVALID_ARG; }
+  if (n_bricks) *n_bricks = grid->n_bricks;
+  if (n_active) *n_active = grid->n_active;
+  return DEX_OK;
+}
+
+dex_status dex_grid_get_slots(const dex_grid* grid, int32_t* h_slot) {
+  if (!grid || !h_slot) { dex_set_error("NULL grid / h_slot"); return DEX_ERR_INVALID_ARG; }
+  DEX_CUDA_CHECK(cudaDeviceSynchronize());
+  DEX_CUDA_CHECK(cudaMemcpy(h_slot, grid->d_slot, sizeof(int) * (size_t)grid->n_bricks, cudaMemcpyDeviceToHost));
+  return DEX_OK;
+}
+
+void dex_destroy_grid(dex_grid* grid) {
+  if (!grid) return;
+  cudaFree(grid->d_slot);
+  cudaFree(grid->d_active_bricks);
+  delete grid;
+}
+
+// ------------------------------------------------------------------------------------------- mips
+dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, void* stream, dex_mips** out) {
+  if (!grid || !desc || !out) { dex_set_error("NULL grid / desc / out"); return DEX_ERR_INVALID_ARG; }
+  *out = nullptr;
+  const int v = (int)desc->variant;
+  if (v < DEX_ISO || v > DEX_CLASSIC) { dex_set_error("unknown variant"); return DEX_ERR_INVALID_ARG; }
+  if (desc->metric != DEX_METRIC_IOD_LOG && desc->metric != DEX_METRIC_RELVAR) {
+    dex_set_error("unknown metric");
+    return DEX_ERR_INVALID_ARG;
+  }
+  if (desc->lambda_batch != DEX_W) { dex_set_error("lambda_batch must be 8 in this build"); return DEX_ERR_UNSUPPORTED; }
+  if (desc->n_lambda <= 0 || desc->n_lambda % desc->lambda_batch) {
+    dex_set_error("n_lambda must be a positive multiple of lambda_batch");
+    return DEX_ERR_SHAPE;
+  }
+  int max_level = desc->max_level;
+  if (max_level < 0 || max_level > grid->dev.logB || max_level >= DEX_MAXLEV) {
+    dex_set_error("max_level must be in 0..log2(brick)");
+    return DEX_ERR_SHAPE;
+  }
+  if (v == DEX_CLASSIC) max_level = 0;   // brute force at full resolution
+  const int n_batch = desc->n_lambda / desc->lambda_batch;
+  if (v == DEX_ISO) {
+    if (!desc->d_eta || !desc->d_chi) { dex_set_error("ISO needs d_eta and d_chi"); return DEX_ERR_INVALID_ARG; }
+  } else {
+    if (!desc->d_eta_bg || !desc->d_chi_bg || !desc->d_vel || !desc->d_lambda || !desc->h_active_lines) {
+      dex_set_error("anisotropic variants need d_eta_bg, d_chi_bg, d_vel, d_lambda, h_active_lines");
+      return DEX_ERR_INVALID_ARG;
+    }
+    if (desc->n_lines < 0 || desc->n_lines > DEX_MAX_LINES) { dex_set_error("n_lines must be 0..4"); return DEX_ERR_SHAPE; }
+    if (desc->n_lines > 0 && (!desc->h_lambda0 || !desc->d_eta_star0 || !desc->d_chi_star0 || !desc->d_a0 ||
+                              !desc->d_inv_dlamD)) {
+      dex_set_error("line arrays are NULL");
+      return DEX_ERR_INVALID_ARG;
+    }
+    for (int i = 0; i < n_batch * DEX_MAX_LINES; ++i) {
+      const int l = desc->h_active_lines[i];
+      if (l < -1 || l >= desc->n_lines) { dex_set_error("active line id out of range"); return DEX_ERR_SHAPE; }
+    }
+    if (!(desc->c_light > 0.0f)) { dex_set_error("c_light must be > 0"); return DEX_ERR_INVALID_ARG; }
+    if (v == DEX_VELINTERP && (desc->n_vbins < 2 || desc->n_vbins > 32)) {
+      dex_set_error("n_vbins must be in 2..32");
+      return DEX_ERR_UNSUPPORTED;
+    }
+  }
+  if (!have_device()) return DEX_ERR_CUDA;
+  dex_mips* m = new (std::nothrow) dex_mips();
+  if (!m) { dex_set_error("host allocation failed"); return DEX_ERR_OOM; }
+  m->grid = grid;
+  m->variant = v;
+  m->n_lambda = desc->n_lambda;
+  m->n_batch = n_batch;
+  m->max_level = max_level;
+  m->metric = (int)desc->metric;
+  m->thr_eta = desc->thr_eta;
+  m->thr_chi = desc->thr_chi;
+  m->tau_gate = desc->tau_gate;
+  DexMipsDev& d = m->dev;
+  memset(&d, 0, sizeof(d));
+  d.variant = v;
+  d.n_lambda = desc->n_lambda;
+  d.n_batch = n_batch;
+  d.max_level = max_level;
+  int bits = 1;
+  while ((1 << bits) < max_level + 2) ++bits;      // ceil(log2(max_level + 2))
+  d.bits = bits;
+  d.per_word = 64 / bits;
+  d.words_per_batch = (int)((grid->n_bricks + d.per_word - 1) / d.per_word);
+  int cps = 0;
+  for (int lv = 0; lv <= max_level; ++lv) {
+    d.lvloff[lv] = cps;
+    const int n = grid->dev.B >> lv;
+    cps += (grid->dev.ndim == 3) ? n * n * n : n * n;
+  }
+  d.cps = cps;
+  d.n_lines = (v == DEX_ISO) ? 0 : desc->n_lines;
+  d.n_vbins = (v == DEX_VELINTERP) ? desc->n_vbins : 0;
+  d.c_light = (double)desc->c_light;
+  for (int l = 0; l < d.n_lines; ++l) d.lambda0[l] = desc->h_lambda0[l];
+  dex_weideman_coefficients(d.wei_c, &d.wei_L);
+  const size_t A = (size_t)grid->n_active;
+  cudaStream_t st = (cudaStream_t)stream;
+  dex_status s = DEX_OK;
+  m->store_floats = (size_t)n_batch * A * cps * DEX_REC;
+  s = dmalloc(&m->d_store, m->store_floats);
+  if (s == DEX_OK) s = dmalloc(&m->d_levels, (size_t)n_batch * grid->n_bricks);
+  if (s == DEX_OK) s = dmalloc(&m->d_packed, (size_t)n_batch * d.words_per_batch);
+  if (s == DEX_OK) s = dmalloc(&m->d_fail, (size_t)n_batch * A * (max_level + 1));
+  if (s == DEX_OK && v != DEX_ISO) {
+    s = dmalloc(&m->d_vel, A * cps);
+    if (s == DEX_OK) s = dmalloc(&m->d_line, A * cps * (size_t)(d.n_lines > 0 ? d.n_lines : 1));
+    if (s == DEX_OK) s = dmalloc(&m->d_lam, (size_t)desc->n_lambda);
+    if (s == DEX_OK) s = dmalloc(&m->d_active_lines, (size_t)n_batch * DEX_MAX_LINES);
+    if (s == DEX_OK && v == DEX_VELINTERP) {
+      m->vtab_floats = m->store_floats * (size_t)d.n_vbins;
+      s = dmalloc(&m->d_vtab, m->vtab_floats);
+    }
+    if (s == DEX_OK) {
+      cudaError_t e = cudaMemcpyAsync(m->d_lam, desc->d_lambda, sizeof(float) * desc->n_lambda,
+                                      cudaMemcpyDeviceToDevice, st);
+      if (e == cudaSuccess)
+        e = cudaMemcpyAsync(m->d_active_lines, desc->h_active_lines, (size_t)n_batch * DEX_MAX_LINES,
+                            cudaMemcpyHostToDevice, st);
+      if (e != cudaSuccess) { dex_set_error(cudaGetErrorString(e)); s = DEX_ERR_CUDA; }
+    }
+  }
+  if (s == DEX_OK) {
+    d.packed = m->d_packed;
+    d.store = m->d_store;
+    d.line = m->d_line;
+    d.vel = m->d_vel;
+    d.vtab = m->d_vtab;
+    d.lam = m->d_lam;
+    d.active_lines = m->d_active_lines;
+    s = dex_launch_mips_build(m, desc, st);
+  }
+  if (s != DEX_OK) { free_mips_memory(m); delete m; return s; }
+  *out = m;
+  return DEX_OK;
+}
+
+dex_status dex_mips_get_levels(const dex_mips* mips, int8_t* h_level) {
+  if (!mips || !h_level) { dex_set_error("NULL mips / h_level"); return DEX_ERR_INVALID_ARG; }
+  DEX_CUDA_CHECK(cudaDeviceSynchronize());
+  DEX_CUDA_CHECK(cudaMemcpy(h_level, mips->d_levels, (size_t)mips->n_batch * mips->grid->n_bricks, cudaMemcpyDeviceToHost));
+  return DEX_OK;
+}
+
+dex_status dex_mips_set_levels(dex_mips* mips, const int8_t* h_level) {
+  if (!mips || !h_level) { dex_set_error("NULL mips / h_level"); return DEX_ERR_INVALID_ARG; }
+  const size_t n = (size_t)mips->n_batch * mips->grid->n_bricks;
+  std::vector<int32_t> slots((size_t)mips->grid->n_bricks);
+  dex_status s = dex_grid_get_slots(mips->grid, slots.data());
+  if (s != DEX_OK) return s;
+  for (size_t i = 0; i < n; ++i) {
+    const int lv = h_level[i];
+    const bool active = slots[i % (size_t)mips->grid->n_bricks] >= 0;
+    if (lv < -1 || lv > mips->max_level || (active != (lv >= 0))) {
+      dex_set_error("injected level out of range or inconsistent with brick occupancy");
+      return DEX_ERR_SHAPE;
+    }
+  }
+  DEX_CUDA_CHECK(cudaMemcpy(mips->d_levels, h_level, n, cudaMemcpyHostToDevice));
+  s = dex_launch_pack_levels(mips, 0);
+  if (s != DEX_OK) return s;
+  DEX_CUDA_CHECK(cudaDeviceSynchronize());
+  return DEX_OK;
+}
+
+dex_status dex_mips_get_packed_levels(const dex_mips* mips, int batch, uint64_t* h_words, int64_t* n_words) {
+  if (!mips) { dex_set_error("NULL mips"); return DEX_ERR_INVALID_ARG; }
+  if (batch < 0 || batch >= mips->n_batch) { dex_set_error("batch out of range"); return DEX_ERR_SHAPE; }
+  if (n_words) *n_words = mips->dev.words_per_batch;
+  if (h_words) {
+    DEX_CUDA_CHECK(cudaDeviceSynchronize());
+    DEX_CUDA_CHECK(cudaMemcpy(h_words, mips->d_packed + (size_t)batch * mips->dev.words_per_batch,
+                              sizeof(uint64_t) * (size_t)mips->dev.words_per_batch, cudaMemcpyDeviceToHost));
+  }
+  return DEX_OK;
+}
+
+dex_status dex_mips_get_level_data(const dex_mips* mips, int chain, int level, float* h_dense) {
+  if (!mips || !h_dense) { dex_set_error("NULL mips / h_dense"); return DEX_ERR_INVALID_ARG; }
+  if (level < 0 || level > mips->max_level) { dex_set_error("level out of range"); return DEX_ERR_SHAPE; }
+  size_t width = 0;
+  switch (chain) {
+    case DEX_CHAIN_ETA: case DEX_CHAIN_CHI: width = (size_t)mips->n_lambda; break;
+    case DEX_CHAIN_VEL: width = 4; if (mips->variant == DEX_ISO) width = 0; break;
+    case DEX_CHAIN_LINE: width = 4 * (size_t)mips->dev.n_lines; break;
+    case DEX_CHAIN_VTAB: width = (mips->variant == DEX_VELINTERP) ? 2 * (size_t)mips->dev.n_vbins * mips->n_lambda : 0; break;
+    default: dex_set_error("unknown chain"); return DEX_ERR_INVALID_ARG;
+  }
+  if (width == 0) { dex_set_error("chain not present in this variant"); return DEX_ERR_INVALID_ARG; }
+  size_t cells = 1;
+  for (int a = 0; a < mips->grid->dev.ndim; ++a) cells *= (size_t)(mips->grid->dev.dims[a] >> level);
+  float* d_dense = nullptr;
+  DEX_CUDA_CHECK(cudaDeviceSynchronize());
+  dex_status s = dmalloc(&d_dense, cells * width);
+  if (s != DEX_OK) return s;
+  cudaError_t e = cudaMemset(d_dense, 0, sizeof(float) * cells * width);
+  if (e == cudaSuccess) {
+    s = dex_launch_level_data(mips, chain, level, d_dense, 0);
+    if (s == DEX_OK) e = cudaMemcpy(h_dense, d_dense, sizeof(float) * cells * width, cudaMemcpyDeviceToHost);
+  }
+  cudaFree(d_dense);
+  if (s != DEX_OK) return s;
+  DEX_CUDA_CHECK(e);
+  return DEX_OK;
+}
+
+void dex_destroy_mips(dex_mips* mips) {
+  if (!mips) return;
+  free_mips_memory(mips);
+  delete mips;
+}
+
+// ------------------------------------------------------------------------------------------- solve
+dex_status dex_formal_solution(const dex_grid* grid, const dex_mips* mips, const dex_rays* rays, float* d_I,
+                               dex_visit_capture* capture, int64_t* d_segment_count, void* stream) {
+  DexRaysDev R;
+  dex_status s = check_rays(grid, mips, rays, &R);
+  if (s != DEX_OK) return s;
+  if (!d_I && !capture) { dex_set_error("d_I is NULL and no capture requested"); return DEX_ERR_INVALID_ARG; }
+  if (capture) {
+    if (!capture->d_counts || !capture->d_records || !capture->d_offsets || capture->capacity < 0) {
+      dex_set_error("capture buffers are NULL");
+      return DEX_ERR_INVALID_ARG;
+    }
+    if (capture->batch < 0 || capture->batch >= mips->n_batch) { dex_set_error("capture batch out of range"); return DEX_ERR_SHAPE; }
+  }
+  if (!have_device()) return DEX_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (d_I) {
+    MarchTimer tm(st);
+    s = dex_launch_march(grid, mips, R, d_I, false, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), st);
+    if (s != DEX_OK) return s;
+  }
+  if (capture) {
+    int* d_over = nullptr;
+    s = dmalloc(&d_over, 1);
+    if (s != DEX_OK) return s;
+    int h_over = 0;
+    cudaError_t e = cudaMemsetAsync(d_over, 0, sizeof(int), st);
+    if (e == cudaSuccess) {
+      s = dex_launch_capture(grid, mips, R, capture, d_over, st);
+      if (s == DEX_OK) e = cudaMemcpyAsync(&h_over, d_over, sizeof(int), cudaMemcpyDeviceToHost, st);
+      if (s == DEX_OK && e == cudaSuccess) e = cudaStreamSynchronize(st);
+    }
+    cudaFree(d_over);
+    if (s != DEX_OK) return s;
+    DEX_CUDA_CHECK(e);
+    if (h_over) { dex_set_error("visit capture overflow: counts are complete, records truncated"); return DEX_ERR_CAPACITY; }
+  }
+  return DEX_OK;
+}
+
+dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const dex_rays* rays, const float* d_I,
+                              float* d_J, int64_t* d_segment_count, void* stream) {
+  DexRaysDev R;
+  dex_status s = check_rays(grid, mips, rays, &R);
+  if (s != DEX_OK) return s;
+  if (!d_J) { dex_set_error("d_J is NULL"); return DEX_ERR_INVALID_ARG; }
+  if (rays->n_dirs > 0 && !rays->d_weights) { dex_set_error("d_weights is NULL"); return DEX_ERR_INVALID_ARG; }
+  if (!have_device()) return DEX_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (d_I) return dex_launch_reduce_j(R, mips->n_lambda, d_I, d_J, st);
+  MarchTimer tm(st);
+  return dex_launch_march(grid, mips, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), st);
+}
+
+}  // extern "C"

@@ -1,0 +1,61 @@
+// dex_internal.h -- host-side declarations shared by the translation units of libdex.so.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+
+#include "../../include/dex.h"
+#include "dex_device.cuh"
+
+struct dex_grid {
+  dex_grid_desc desc;
+  DexGridDev dev;          // device view (pointers into memory owned by this handle)
+  int* d_slot = nullptr;   // [n_bricks]
+  int* d_active_bricks = nullptr;  // [n_active] slot -> brick
+  int64_t n_bricks = 0, n_active = 0;
+  int64_t nvox = 0;
+};
+
+struct dex_mips {
+  const dex_grid* grid = nullptr;
+  DexMipsDev dev;
+  int variant = 0, n_lambda = 0, n_batch = 0, max_level = 0;
+  int metric = 0;
+  float thr_eta = 0, thr_chi = 0, tau_gate = -1;
+  // owned device memory
+  float* d_store = nullptr;
+  float4* d_line = nullptr;
+  float4* d_vel = nullptr;
+  float* d_vtab = nullptr;
+  float* d_lam = nullptr;
+  signed char* d_active_lines = nullptr;
+  signed char* d_levels = nullptr;           // [n_batch][n_bricks]
+  unsigned long long* d_packed = nullptr;    // [n_batch][words_per_batch]
+  int* d_fail = nullptr;                     // [n_batch][n_active][max_level+1]
+  size_t store_floats = 0, vtab_floats = 0;
+};
+
+void dex_set_error(const std::string& msg);
+void dex_count_launch(int n = 1);
+
+// grid_build.cu
+dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStream_t st);
+// mips_build.cu
+dex_status dex_launch_mips_build(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st);
+dex_status dex_launch_pack_levels(dex_mips* m, cudaStream_t st);
+dex_status dex_launch_level_data(const dex_mips* m, int chain, int level, float* d_dense, cudaStream_t st);
+// march.cu
+dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
+                            unsigned long long* d_seg, int lanes_per_ray, cudaStream_t st);
+dex_status dex_launch_capture(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays,
+                              const dex_visit_capture* cap, int* d_overflow, cudaStream_t st);
+dex_status dex_launch_reduce_j(const DexRaysDev& rays, int n_lambda, const float* d_I, float* d_J, cudaStream_t st);
+
+#define DEX_CUDA_CHECK(expr)                                                                   \
+  do {                                                                                         \
+    cudaError_t _e = (expr);                                                                   \
+    if (_e != cudaSuccess) {                                                                   \
+      dex_set_error(std::string(#expr) + ": " + cudaGetErrorString(_e));                       \
+      return (_e == cudaErrorMemoryAllocation) ? DEX_ERR_OOM : DEX_ERR_CUDA;                   \
+    }                                                                                          \
+  } while (0)

@@ -1,0 +1,91 @@
+// grid_build.cu -- a1: brick occupancy + compaction.
+// A brick is populated iff any of its voxels is active; populated bricks get storage slots 0..A-1 in
+// brick-index order (the offset lookup table of).
+#include "dex_internal.h"
+
+namespace {
+
+// one warp per brick: OR-reduce the brick's voxels
+template <int D>
+__global__ void dex_brick_flags_kernel(const DexGridDev G, const uint8_t* __restrict__ active, int* __restrict__ flag) {
+  const int warp = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+  const int lane = threadIdx.x & 31;
+  if (warp >= G.n_bricks) return;
+  int bx = warp % G.nb[0];
+  int by = (warp / G.nb[0]) % G.nb[1];
+  int bz = (D == 3) ? warp / (G.nb[0] * G.nb[1]) : 0;
+  const int B = G.B;
+  const int nvb = (D == 3) ? B * B * B : B * B;
+  int any = 0;
+  for (int i = lane; i < nvb; i += 32) {
+    const int x = i & (B - 1);
+    const int y = (i >> G.logB) & (B - 1);
+    const int z = (D == 3) ? (i >> (2 * G.logB)) : 0;
+    const size_t v = ((size_t)(bz * B + z) * G.dims[1] + (by * B + y)) * G.dims[0] + (bx * B + x);
+    any |= (int)active[v];
+  }
+  any = __any_sync(0xffffffffu, any != 0);
+  if (lane == 0) flag[warp] = any;
+}
+
+__global__ void dex_fill_int_kernel(int* p, int n, int v) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = v;
+}
+
+// single-block exclusive scan of the flags -> slot table, slot -> brick list, active count
+__global__ void __launch_bounds__(1024)
+dex_scan_slots_kernel(const int* __restrict__ flag, int n, int* __restrict__ slot, int* __restrict__ active_bricks,
+                      int* __restrict__ n_active) {
+  __shared__ int part[1024];
+  const int t = threadIdx.x;
+  const int chunk = (n + 1023) / 1024;
+  const int lo = min(n, t * chunk), hi = min(n, lo + chunk);
+  int cnt = 0;
+  for (int i = lo; i < hi; ++i) cnt += (flag[i] != 0);
+  part[t] = cnt;
+  __syncthreads();
+  for (int off = 1; off < 1024; off <<= 1) {      // Hillis-Steele inclusive scan
+    int v = (t >= off) ? part[t - off] : 0;
+    __syncthreads();
+    part[t] += v;
+    __syncthreads();
+  }
+  int base = part[t] - cnt;
+  for (int i = lo; i < hi; ++i) {
+    if (flag[i] != 0) { slot[i] = base; active_bricks[base] = i; ++base; }
+    else slot[i] = -1;
+  }
+  if (t == 1023) *n_active = part[1023];
+}
+
+}  // namespace
+
+dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStream_t st) {
+  const int nb = (int)g->n_bricks;
+  int* d_flag = nullptr;
+  int* d_count = nullptr;
+  DEX_CUDA_CHECK(cudaMalloc(&d_flag, sizeof(int) * (size_t)nb));
+  DEX_CUDA_CHECK(cudaMalloc(&d_count, sizeof(int)));
+  if (d_active == nullptr) {
+    dex_fill_int_kernel<<<(nb + 255) / 256, 256, 0, st>>>(d_flag, nb, 1);
+  } else {
+    const long long threads = (long long)nb * 32;
+    const unsigned blocks = (unsigned)((threads + 255) / 256);
+    if (g->desc.ndim == 2) dex_brick_flags_kernel<2><<<blocks, 256, 0, st>>>(g->dev, d_active, d_flag);
+    else dex_brick_flags_kernel<3><<<blocks, 256, 0, st>>>(g->dev, d_active, d_flag);
+  }
+  dex_count_launch();
+  dex_scan_slots_kernel<<<1, 1024, 0, st>>>(d_flag, nb, g->d_slot, g->d_active_bricks, d_count);
+  dex_count_launch();
+  int h_count = 0;
+  cudaError_t e = cudaMemcpyAsync(&h_count, d_count, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_flag);
+  cudaFree(d_count);
+  DEX_CUDA_CHECK(e);
+  DEX_CUDA_CHECK(cudaGetLastError());
+  g->n_active = h_count;
+  g->dev.n_active = h_count;
+  return DEX_OK;
+}

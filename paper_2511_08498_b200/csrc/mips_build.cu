@@ -1,0 +1,590 @@
+// mips_build.cu -- a2-a4: brick gather, box-filter mips, VLM cell test, per-brick level selection,
+// packed block states.  Compiled with -fmad=false: the statistics are fp64 and are written in the
+// operation order of DESIGN.md's V-rules so that threshold decisions do not depend on contraction.
+//
+//   V1  level m value = fp64 sum of the 2^D children (x fastest, then y, then z) * 2^-D, rounded once
+//   V2  cell test over the children: RELVAR Var/Mean^2, or IOD_LOG |Var/Mean| of ln(x h) (eq. 8,
+//       PAPER.md:127-130), population variance; pass iff both metrics < thr (strict) or the chi h gate
+//   V5  brick level = largest m whose cells (and those of all lower levels >= 1) all pass for all
+//       wavelengths of the batch
+//   V6  test quantity: ISO the chains themselves; VELINTERP the table at v = 0; CAV the
+//       line sum at the worst-case Doppler shift of eq. 17
+#include "dex_internal.h"
+#include "dex_voigt.cuh"
+
+namespace {
+
+struct BuildCtx {
+  DexGridDev G;
+  DexMipsDev M;
+  const int* active_bricks;   // slot -> brick
+  int metric;
+  double thr_eta, thr_chi, tau_gate, h;
+  int* fail;                  // [n_batch][n_active][max_level+1]
+  float* store;
+  float4* line;
+  float4* vel;
+  float* vtab;
+};
+
+template <int D>
+__device__ __forceinline__ void brick_coords(const DexGridDev& G, int bi, int (&b)[3]) {
+  b[0] = bi % G.nb[0];
+  b[1] = (bi / G.nb[0]) % G.nb[1];
+  b[2] = (D == 3) ? bi / (G.nb[0] * G.nb[1]) : 0;
+}
+
+template <int D>
+__device__ __forceinline__ void cell_coords(int idx, int nbm, int (&c)[3]) {
+  c[0] = idx % nbm;
+  c[1] = (idx / nbm) % nbm;
+  c[2] = (D == 3) ? idx / (nbm * nbm) : 0;
+}
+
+template <int D>
+__device__ __forceinline__ int child_index(const int (&pc)[3], int ch, int nbc) {
+  const int dx = ch & 1, dy = (ch >> 1) & 1, dz = (ch >> 2) & 1;
+  int idx = (2 * pc[1] + dy) * nbc + (2 * pc[0] + dx);
+  if (D == 3) idx += (2 * pc[2] + dz) * nbc * nbc;
+  return idx;
+}
+
+template <int D>
+__device__ __forceinline__ size_t voxel_of(const DexGridDev& G, int bi, int cell0) {
+  int b[3], c[3];
+  brick_coords<D>(G, bi, b);
+  cell_coords<D>(cell0, G.B, c);
+  return ((size_t)(b[2] * G.B + c[2]) * G.dims[1] + (b[1] * G.B + c[1])) * G.dims[0] + (b[0] * G.B + c[0]);
+}
+
+// V2/V4 statistic of NC children values (fp64), mirrors the oracle's operation order
+template <int NC>
+__device__ double cell_metric(const double (&x)[NC], int metric, double h) {
+  bool all_equal = true;
+#pragma unroll
+  for (int i = 1; i < NC; ++i) all_equal = all_equal && (x[i] == x[0]);
+  if (all_equal) return 0.0;
+  double X[NC];
+  if (metric == DEX_METRIC_IOD_LOG) {
+    bool bad = false;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      if (!(x[i] > 0.0)) bad = true;
+      X[i] = log(x[i] * h);
+    }
+    if (bad) return __longlong_as_double(0x7ff0000000000000LL);
+  } else {
+#pragma unroll
+    for (int i = 0; i < NC; ++i) X[i] = x[i];
+  }
+  double s = X[0];
+#pragma unroll
+  for (int i = 1; i < NC; ++i) s = s + X[i];
+  const double mean = s / (double)NC;
+  double d = X[0] - mean;
+  double v = d * d;
+#pragma unroll
+  for (int i = 1; i < NC; ++i) {
+    d = X[i] - mean;
+    v = v + d * d;
+  }
+  const double var = v / (double)NC;
+  double val = (metric == DEX_METRIC_IOD_LOG) ? fabs(var / mean) : var / (mean * mean);
+  if (val != val) val = __longlong_as_double(0x7ff0000000000000LL);
+  return val;
+}
+
+template <int NC>
+__device__ bool cell_passes(const double (&e)[NC], const double (&c)[NC], const BuildCtx& X) {
+  bool ok = (cell_metric<NC>(e, X.metric, X.h) < X.thr_eta) && (cell_metric<NC>(c, X.metric, X.h) < X.thr_chi);
+  if (X.tau_gate >= 0.0) {     // always average where chi ds is small
+    double s = c[0];
+#pragma unroll
+    for (int i = 1; i < NC; ++i) s = s + c[i];
+    if ((s / (double)NC) * X.h <= X.tau_gate) ok = true;
+  }
+  return ok;
+}
+
+// ---- a2: level-0 gather of a spectrum pair into [batch][slot][cell][lambda][eta,chi] -------------
+template <int D>
+__global__ void gather_spec_kernel(const BuildCtx X, const float* __restrict__ eta, const float* __restrict__ chi) {
+  const int cells0 = (D == 3) ? X.G.B * X.G.B * X.G.B : X.G.B * X.G.B;
+  const long long total = (long long)X.M.n_batch * X.G.n_active * cells0 * DEX_W;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int j = (int)(i % DEX_W);
+  long long r = i / DEX_W;
+  const int cell = (int)(r % cells0);
+  r /= cells0;
+  const int slot = (int)(r % X.G.n_active);
+  const int b = (int)(r / X.G.n_active);
+  const size_t v = voxel_of<D>(X.G, X.active_bricks[slot], cell);
+  const size_t src = v * X.M.n_lambda + (size_t)b * DEX_W + j;
+  float2 o;
+  o.x = eta[src];
+  o.y = chi[src];
+  reinterpret_cast<float2*>(X.store)[(((size_t)b * X.G.n_active + slot) * X.M.cps + cell) * DEX_W + j] = o;
+}
+
+// ---- a3: level m from level m-1 for the spectrum pair; STATS = ISO cell test -----------------------
+template <int D, bool STATS>
+__global__ void reduce_spec_kernel(const BuildCtx X, int m) {
+  constexpr int NC = 1 << D;
+  const int nbm = X.G.B >> m, nbc = X.G.B >> (m - 1);
+  const int cells = (D == 3) ? nbm * nbm * nbm : nbm * nbm;
+  const long long total = (long long)X.M.n_batch * X.G.n_active * cells * DEX_W;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int j = (int)(i % DEX_W);
+  long long r = i / DEX_W;
+  const int cell = (int)(r % cells);
+  r /= cells;
+  const int slot = (int)(r % X.G.n_active);
+  const int b = (int)(r / X.G.n_active);
+  int pc[3];
+  cell_coords<D>(cell, nbm, pc);
+  const size_t base = ((size_t)b * X.G.n_active + slot) * X.M.cps;
+  float2* st = reinterpret_cast<float2*>(X.store);
+  double e[NC], c[NC];
+#pragma unroll
+  for (int ch = 0; ch < NC; ++ch) {
+    const float2 v = st[(base + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc)) * DEX_W + j];
+    e[ch] = (double)v.x;
+    c[ch] = (double)v.y;
+  }
+  double se = e[0], sc = c[0];
+#pragma unroll
+  for (int ch = 1; ch < NC; ++ch) { se = se + e[ch]; sc = sc + c[ch]; }
+  float2 o;
+  o.x = (float)(se * (1.0 / NC));
+  o.y = (float)(sc * (1.0 / NC));
+  st[(base + X.M.lvloff[m] + cell) * DEX_W + j] = o;
+  if (STATS) {
+    if (!cell_passes<NC>(e, c, X)) X.fail[((size_t)b * X.G.n_active + slot) * (X.M.max_level + 1) + m] = 1;
+  }
+}
+
+// ---- line parameters and velocity: level 0 gather and box filter ------------------------------------
+template <int D>
+__global__ void gather_aux_kernel(const BuildCtx X, const float* __restrict__ vel, const float* __restrict__ es,
+                                  const float* __restrict__ cs, const float* __restrict__ a0,
+                                  const float* __restrict__ inv, long long nvox) {
+  const int cells0 = (D == 3) ? X.G.B * X.G.B * X.G.B : X.G.B * X.G.B;
+  const long long total = (long long)X.G.n_active * cells0;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int cell = (int)(i % cells0);
+  const int slot = (int)(i / cells0);
+  const size_t v = voxel_of<D>(X.G, X.active_bricks[slot], cell);
+  float4 o;
+  o.x = vel[v * D + 0];
+  o.y = vel[v * D + 1];
+  o.z = (D == 3) ? vel[v * D + D - 1] : 0.0f;
+  double s2 = (double)o.x * (double)o.x + (double)o.y * (double)o.y;
+  if (D == 3) s2 = s2 + (double)o.z * (double)o.z;
+  o.w = (float)sqrt(s2);
+  const size_t dst = (size_t)slot * X.M.cps + cell;
+  X.vel[dst] = o;
+  for (int l = 0; l < X.M.n_lines; ++l) {
+    float4 q;
+    q.x = es[(size_t)l * nvox + v];
+    q.y = cs[(size_t)l * nvox + v];
+    q.z = a0[(size_t)l * nvox + v];
+    q.w = inv[(size_t)l * nvox + v];
+    X.line[dst * X.M.n_lines + l] = q;
+  }
+}
+
+template <int D>
+__global__ void reduce_aux_kernel(const BuildCtx X, int m) {
+  constexpr int NC = 1 << D;
+  const int nbm = X.G.B >> m, nbc = X.G.B >> (m - 1);
+  const int cells = (D == 3) ? nbm * nbm * nbm : nbm * nbm;
+  const long long total = (long long)X.G.n_active * cells;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int cell = (int)(i % cells);
+  const int slot = (int)(i / cells);
+  int pc[3];
+  cell_coords<D>(cell, nbm, pc);
+  const size_t base = (size_t)slot * X.M.cps;
+  double sx = 0, sy = 0, sz = 0;
+  float vm = 0.0f;
+#pragma unroll
+  for (int ch = 0; ch < NC; ++ch) {
+    const float4 v = X.vel[base + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc)];
+    if (ch == 0) { sx = (double)v.x; sy = (double)v.y; sz = (double)v.z; vm = v.w; }
+    else { sx = sx + (double)v.x; sy = sy + (double)v.y; sz = sz + (double)v.z; vm = fmaxf(vm, v.w); }
+  }
+  float4 o;
+  o.x = (float)(sx * (1.0 / NC));
+  o.y = (float)(sy * (1.0 / NC));
+  o.z = (float)(sz * (1.0 / NC));
+  o.w = vm;
+  X.vel[base + X.M.lvloff[m] + cell] = o;
+  for (int l = 0; l < X.M.n_lines; ++l) {
+    double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+#pragma unroll
+    for (int ch = 0; ch < NC; ++ch) {
+      const float4 q = X.line[(base + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc)) * X.M.n_lines + l];
+      if (ch == 0) { s0 = (double)q.x; s1 = (double)q.y; s2 = (double)q.z; s3 = (double)q.w; }
+      else { s0 = s0 + (double)q.x; s1 = s1 + (double)q.y; s2 = s2 + (double)q.z; s3 = s3 + (double)q.w; }
+    }
+    float4 q;
+    q.x = (float)(s0 * (1.0 / NC));
+    q.y = (float)(s1 * (1.0 / NC));
+    q.z = (float)(s2 * (1.0 / NC));
+    q.w = (float)(s3 * (1.0 / NC));
+    X.line[(base + X.M.lvloff[m] + cell) * X.M.n_lines + l] = q;
+  }
+}
+
+// eqs. 10-11 at one cell: background + active lines, each at its own projected velocity vp[q]
+__device__ __forceinline__ void line_sum(const BuildCtx& X, size_t cell, int b, double lam, double bg_e, double bg_c,
+                                         const double* vp, bool vp_per_line, double& e, double& c) {
+  e = bg_e;
+  c = bg_c;
+  for (int q = 0; q < DEX_NLINES; ++q) {
+    const int l = X.M.active_lines[b * DEX_NLINES + q];
+    if (l < 0) continue;
+    const float4 ln = X.line[cell * X.M.n_lines + l];
+    double el, cl;
+    dex_line_terms(X.M.wei_c, X.M.wei_L, lam, (double)X.M.lambda0[l], (double)ln.x, (double)ln.y, (double)ln.z,
+                   (double)ln.w, vp_per_line ? vp[q] : vp[0], X.M.c_light, el, cl);
+    e = e + el;
+    c = c + cl;
+  }
+}
+
+// ---- CAV cell test at level m (children at level m-1, worst-case Doppler shift of eq. 17) -----------
+template <int D>
+__global__ void cav_test_kernel(const BuildCtx X, int m) {
+  constexpr int NC = 1 << D;
+  const int nbm = X.G.B >> m, nbc = X.G.B >> (m - 1);
+  const int cells = (D == 3) ? nbm * nbm * nbm : nbm * nbm;
+  const long long total = (long long)X.M.n_batch * X.G.n_active * cells * DEX_W;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int j = (int)(i % DEX_W);
+  long long r = i / DEX_W;
+  const int cell = (int)(r % cells);
+  r /= cells;
+  const int slot = (int)(r % X.G.n_active);
+  const int b = (int)(r / X.G.n_active);
+  int pc[3];
+  cell_coords<D>(cell, nbm, pc);
+  const double lam = (double)X.M.lam[b * DEX_W + j];
+  const float2* st = reinterpret_cast<const float2*>(X.store);
+  double e[NC], c[NC];
+#pragma unroll
+  for (int ch = 0; ch < NC; ++ch) {
+    const size_t cc = (size_t)slot * X.M.cps + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc);
+    const float2 bg = st[(((size_t)b * X.G.n_active) * X.M.cps + cc) * DEX_W + j];
+    const double Vc = (double)X.vel[cc].w;
+    double vd[DEX_NLINES];
+    for (int q = 0; q < DEX_NLINES; ++q) {
+      const int l = X.M.active_lines[b * DEX_NLINES + q];
+      vd[q] = 0.0;
+      if (l < 0) continue;
+      const double want = X.M.c_light * (1.0 - lam / (double)X.M.lambda0[l]);   // minimises eq. 17
+      vd[q] = fmin(fmax(want, -Vc), Vc);
+    }
+    line_sum(X, cc, b, lam, (double)bg.x, (double)bg.y, vd, true, e[ch], c[ch]);
+  }
+  if (!cell_passes<NC>(e, c, X)) X.fail[((size_t)b * X.G.n_active + slot) * (X.M.max_level + 1) + m] = 1;
+}
+
+// ---- VELINTERP tables ---------------------------------------------------------------------------------
+// level 0: Classic formula on the uniform grid v_k = -V + 2 V k/(n-1), V = |v| of the voxel
+template <int D>
+__global__ void vtab_level0_kernel(const BuildCtx X) {
+  const int cells0 = (D == 3) ? X.G.B * X.G.B * X.G.B : X.G.B * X.G.B;
+  const int n = X.M.n_vbins;
+  const long long total = (long long)X.M.n_batch * X.G.n_active * cells0 * n * DEX_W;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int j = (int)(i % DEX_W);
+  long long r = i / DEX_W;
+  const int k = (int)(r % n);
+  r /= n;
+  const int cell = (int)(r % cells0);
+  r /= cells0;
+  const int slot = (int)(r % X.G.n_active);
+  const int b = (int)(r / X.G.n_active);
+  const size_t cc = (size_t)slot * X.M.cps + cell;
+  const double V = (double)X.vel[cc].w;
+  const double vk = -V + (2.0 * V) * ((double)k / (double)(n - 1));
+  const float2 bg = reinterpret_cast<const float2*>(X.store)[(((size_t)b * X.G.n_active) * X.M.cps + cc) * DEX_W + j];
+  double e, c;
+  line_sum(X, cc, b, (double)X.M.lam[b * DEX_W + j], (double)bg.x, (double)bg.y, &vk, false, e, c);
+  float2 o;
+  o.x = (float)e;
+  o.y = (float)c;
+  reinterpret_cast<float2*>(X.vtab)[((((size_t)b * X.G.n_active) * X.M.cps + cc) * n + k) * DEX_W + j] = o;
+}
+
+// table of one cell interpolated at velocity v on its grid [-V, V], clamped
+__device__ __forceinline__ void vtab_interp(const float2* __restrict__ tab /*[n][W]*/, int n, int j, double V, double v,
+                                            double& e, double& c) {
+  int i0 = 0;
+  double w = 0.0;
+  if (V > 0.0) {
+    double f = (v + V) / (2.0 * V) * (double)(n - 1);
+    f = fmin(fmax(f, 0.0), (double)(n - 1));
+    i0 = min((int)floor(f), n - 2);
+    w = f - (double)i0;
+  }
+  const float2 t0 = tab[(size_t)i0 * DEX_W + j];
+  const float2 t1 = tab[(size_t)(i0 + 1) * DEX_W + j];
+  e = (1.0 - w) * (double)t0.x + w * (double)t1.x;
+  c = (1.0 - w) * (double)t0.y + w * (double)t1.y;
+}
+
+// level m: parent bin = mean over children of the child's table at the parent's bin velocity (R-vel)
+template <int D>
+__global__ void vtab_reduce_kernel(const BuildCtx X, int m) {
+  constexpr int NC = 1 << D;
+  const int nbm = X.G.B >> m, nbc = X.G.B >> (m - 1);
+  const int cells = (D == 3) ? nbm * nbm * nbm : nbm * nbm;
+  const int n = X.M.n_vbins;
+  const long long total = (long long)X.M.n_batch * X.G.n_active * cells * n * DEX_W;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int j = (int)(i % DEX_W);
+  long long r = i / DEX_W;
+  const int k = (int)(r % n);
+  r /= n;
+  const int cell = (int)(r % cells);
+  r /= cells;
+  const int slot = (int)(r % X.G.n_active);
+  const int b = (int)(r / X.G.n_active);
+  int pc[3];
+  cell_coords<D>(cell, nbm, pc);
+  const size_t sbase = (size_t)slot * X.M.cps;
+  const size_t bbase = ((size_t)b * X.G.n_active) * X.M.cps;
+  const double Vp = (double)X.vel[sbase + X.M.lvloff[m] + cell].w;
+  const double vk = -Vp + (2.0 * Vp) * ((double)k / (double)(n - 1));
+  const float2* vt = reinterpret_cast<const float2*>(X.vtab);
+  double se = 0, sc = 0;
+#pragma unroll
+  for (int ch = 0; ch < NC; ++ch) {
+    const size_t cc = sbase + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc);
+    double e, c;
+    vtab_interp(vt + (bbase + cc) * n * DEX_W, n, j, (double)X.vel[cc].w, vk, e, c);
+    if (ch == 0) { se = e; sc = c; } else { se = se + e; sc = sc + c; }
+  }
+  float2 o;
+  o.x = (float)(se * (1.0 / NC));
+  o.y = (float)(sc * (1.0 / NC));
+  reinterpret_cast<float2*>(X.vtab)[((bbase + sbase + X.M.lvloff[m] + cell) * n + k) * DEX_W + j] = o;
+}
+
+// VELINTERP cell test: children = rest-frame (v = 0) value of the level m-1 tables
+template <int D>
+__global__ void vtab_test_kernel(const BuildCtx X, int m) {
+  constexpr int NC = 1 << D;
+  const int nbm = X.G.B >> m, nbc = X.G.B >> (m - 1);
+  const int cells = (D == 3) ? nbm * nbm * nbm : nbm * nbm;
+  const int n = X.M.n_vbins;
+  const long long total = (long long)X.M.n_batch * X.G.n_active * cells * DEX_W;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int j = (int)(i % DEX_W);
+  long long r = i / DEX_W;
+  const int cell = (int)(r % cells);
+  r /= cells;
+  const int slot = (int)(r % X.G.n_active);
+  const int b = (int)(r / X.G.n_active);
+  int pc[3];
+  cell_coords<D>(cell, nbm, pc);
+  const size_t sbase = (size_t)slot * X.M.cps;
+  const size_t bbase = ((size_t)b * X.G.n_active) * X.M.cps;
+  const float2* vt = reinterpret_cast<const float2*>(X.vtab);
+  double e[NC], c[NC];
+#pragma unroll
+  for (int ch = 0; ch < NC; ++ch) {
+    const size_t cc = sbase + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc);
+    vtab_interp(vt + (bbase + cc) * n * DEX_W, n, j, (double)X.vel[cc].w, 0.0, e[ch], c[ch]);
+  }
+  if (!cell_passes<NC>(e, c, X)) X.fail[((size_t)b * X.G.n_active + slot) * (X.M.max_level + 1) + m] = 1;
+}
+
+// ---- a4: level select + pack --------------------------------------------------------------------------
+__global__ void select_levels_kernel(const BuildCtx X, signed char* __restrict__ levels) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long long)X.M.n_batch * X.G.n_bricks) return;
+  const int bi = (int)(i % X.G.n_bricks);
+  const int b = (int)(i / X.G.n_bricks);
+  const int slot = X.G.slot[bi];
+  int lv = -1;
+  if (slot >= 0) {
+    lv = 0;
+    const int* f = X.fail + ((size_t)b * X.G.n_active + slot) * (X.M.max_level + 1);
+    for (int m = 1; m <= X.M.max_level; ++m) {
+      if (f[m]) break;
+      lv = m;
+    }
+  }
+  levels[i] = (signed char)lv;
+}
+
+// state = level + 1 in `bits` bits, floor(64/bits) bricks per 64-bit word
+__global__ void pack_levels_kernel(const signed char* __restrict__ levels, int n_batch, int n_bricks, int bits,
+                                   int per_word, int words, unsigned long long* __restrict__ packed) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long long)n_batch * words) return;
+  const int w = (int)(i % words);
+  const int b = (int)(i / words);
+  unsigned long long word = 0ull;
+  for (int q = 0; q < per_word; ++q) {
+    const int bi = w * per_word + q;
+    if (bi >= n_bricks) break;
+    word |= (unsigned long long)(levels[(size_t)b * n_bricks + bi] + 1) << (q * bits);
+  }
+  packed[i] = word;
+}
+
+// ---- validation export: canonical dense level-m array of a chain ------------------------------------
+template <int D>
+__global__ void level_data_kernel(const BuildCtx X, int chain, int m, int width /*floats per cell*/,
+                                  float* __restrict__ dense) {
+  const int nbm = X.G.B >> m;
+  const int cells = (D == 3) ? nbm * nbm * nbm : nbm * nbm;
+  const long long total = (long long)X.G.n_active * cells * width;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int q = (int)(i % width);
+  long long r = i / width;
+  const int cell = (int)(r % cells);
+  const int slot = (int)(r / cells);
+  int b3[3], pc[3];
+  brick_coords<D>(X.G, X.active_bricks[slot], b3);
+  cell_coords<D>(cell, nbm, pc);
+  const size_t nxm = X.G.dims[0] >> m, nym = X.G.dims[1] >> m;
+  const size_t gc = ((size_t)(b3[2] * nbm + pc[2]) * nym + (b3[1] * nbm + pc[1])) * nxm + (b3[0] * nbm + pc[0]);
+  const size_t cc = (size_t)slot * X.M.cps + X.M.lvloff[m] + cell;
+  float v = 0.0f;
+  if (chain == DEX_CHAIN_ETA || chain == DEX_CHAIN_CHI) {           // width = n_lambda
+    const int b = q / DEX_W, j = q % DEX_W;
+    v = X.store[((((size_t)b * X.G.n_active) * X.M.cps + cc) * DEX_W + j) * 2 + (chain == DEX_CHAIN_CHI)];
+  } else if (chain == DEX_CHAIN_VEL) {                               // width = 4
+    v = reinterpret_cast<const float*>(X.vel)[cc * 4 + q];
+  } else if (chain == DEX_CHAIN_LINE) {                              // width = n_lines * 4
+    v = reinterpret_cast<const float*>(X.line)[cc * X.M.n_lines * 4 + q];
+  } else {                                                           // VTAB: width = n_vbins * n_lambda * 2
+    const int f = q & 1;
+    const int lam = (q >> 1) % X.M.n_lambda;
+    const int k = (q >> 1) / X.M.n_lambda;
+    const int b = lam / DEX_W, j = lam % DEX_W;
+    v = X.vtab[((((((size_t)b * X.G.n_active) * X.M.cps + cc) * X.M.n_vbins + k) * DEX_W) + j) * 2 + f];
+  }
+  dense[gc * width + q] = v;
+}
+
+inline unsigned blocks_for(long long total, int threads) { return (unsigned)((total + threads - 1) / threads); }
+
+BuildCtx make_ctx(const dex_mips* m) {
+  BuildCtx X;
+  X.G = m->grid->dev;
+  X.M = m->dev;
+  X.active_bricks = m->grid->d_active_bricks;
+  X.metric = m->metric;
+  X.thr_eta = (double)m->thr_eta;
+  X.thr_chi = (double)m->thr_chi;
+  X.tau_gate = (double)m->tau_gate;
+  X.h = (double)m->grid->desc.voxel_size;
+  X.fail = m->d_fail;
+  X.store = m->d_store;
+  X.line = m->d_line;
+  X.vel = m->d_vel;
+  X.vtab = m->d_vtab;
+  return X;
+}
+
+template <int D>
+dex_status build_t(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st) {
+  const BuildCtx X = make_ctx(m);
+  const int T = 256;
+  const int B = X.G.B;
+  const long long A = X.G.n_active;
+  const int L = m->max_level;
+  auto cells_at = [&](int lv) { long long n = B >> lv; return (D == 3) ? n * n * n : n * n; };
+  DEX_CUDA_CHECK(cudaMemsetAsync(m->d_fail, 0, sizeof(int) * (size_t)m->n_batch * (size_t)A * (L + 1), st));
+  if (A == 0) return DEX_OK;
+  const bool iso = (m->variant == DEX_ISO);
+  const float* eta = iso ? desc->d_eta : desc->d_eta_bg;
+  const float* chi = iso ? desc->d_chi : desc->d_chi_bg;
+  gather_spec_kernel<D><<<blocks_for((long long)m->n_batch * A * cells_at(0) * DEX_W, T), T, 0, st>>>(X, eta, chi);
+  dex_count_launch();
+  if (!iso) {
+    gather_aux_kernel<D><<<blocks_for(A * cells_at(0), T), T, 0, st>>>(X, desc->d_vel, desc->d_eta_star0, desc->d_chi_star0,
+                                                                  desc->d_a0, desc->d_inv_dlamD, m->grid->nvox);
+    dex_count_launch();
+  }
+  if (m->variant == DEX_VELINTERP) {
+    vtab_level0_kernel<D><<<blocks_for((long long)m->n_batch * A * cells_at(0) * m->dev.n_vbins * DEX_W, T), T, 0, st>>>(X);
+    dex_count_launch();
+  }
+  for (int lv = 1; lv <= L; ++lv) {
+    const long long nspec = (long long)m->n_batch * A * cells_at(lv) * DEX_W;
+    if (iso) reduce_spec_kernel<D, true><<<blocks_for(nspec, T), T, 0, st>>>(X, lv);
+    else reduce_spec_kernel<D, false><<<blocks_for(nspec, T), T, 0, st>>>(X, lv);
+    dex_count_launch();
+    if (!iso) {
+      reduce_aux_kernel<D><<<blocks_for(A * cells_at(lv), T), T, 0, st>>>(X, lv);
+      dex_count_launch();
+    }
+    if (m->variant == DEX_VELINTERP) {
+      vtab_test_kernel<D><<<blocks_for(nspec, T), T, 0, st>>>(X, lv);
+      vtab_reduce_kernel<D><<<blocks_for(nspec * m->dev.n_vbins, T), T, 0, st>>>(X, lv);
+      dex_count_launch(2);
+    } else if (m->variant == DEX_CAV) {
+      cav_test_kernel<D><<<blocks_for(nspec, T), T, 0, st>>>(X, lv);
+      dex_count_launch();
+    }
+  }
+  select_levels_kernel<<<blocks_for((long long)m->n_batch * X.G.n_bricks, T), T, 0, st>>>(X, m->d_levels);
+  dex_count_launch();
+  DEX_CUDA_CHECK(cudaGetLastError());
+  return DEX_OK;
+}
+
+}  // namespace
+
+dex_status dex_launch_mips_build(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st) {
+  dex_status s = (m->grid->desc.ndim == 2) ? build_t<2>(m, desc, st) : build_t<3>(m, desc, st);
+  if (s != DEX_OK) return s;
+  return dex_launch_pack_levels(m, st);
+}
+
+dex_status dex_launch_pack_levels(dex_mips* m, cudaStream_t st) {
+  const long long total = (long long)m->n_batch * m->dev.words_per_batch;
+  pack_levels_kernel<<<blocks_for(total, 256), 256, 0, st>>>(m->d_levels, m->n_batch, (int)m->grid->n_bricks,
+                                                             m->dev.bits, m->dev.per_word, m->dev.words_per_batch,
+                                                             m->d_packed);
+  dex_count_launch();
+  DEX_CUDA_CHECK(cudaGetLastError());
+  return DEX_OK;
+}
+
+dex_status dex_launch_level_data(const dex_mips* m, int chain, int level, float* d_dense, cudaStream_t st) {
+  const BuildCtx X = make_ctx(m);
+  int width = 0;
+  switch (chain) {
+    case DEX_CHAIN_ETA: case DEX_CHAIN_CHI: width = m->n_lambda; break;
+    case DEX_CHAIN_VEL: width = 4; break;
+    case DEX_CHAIN_LINE: width = 4 * m->dev.n_lines; break;
+    case DEX_CHAIN_VTAB: width = 2 * m->dev.n_vbins * m->n_lambda; break;
+  }
+  const int nd = m->grid->desc.ndim;
+  long long nbm = X.G.B >> level;
+  const long long cells = (nd == 3) ? nbm * nbm * nbm : nbm * nbm;
+  const long long total = (long long)X.G.n_active * cells * width;
+  if (total == 0) return DEX_OK;
+  if (nd == 2) level_data_kernel<2><<<blocks_for(total, 256), 256, 0, st>>>(X, chain, level, width, d_dense);
+  else level_data_kernel<3><<<blocks_for(total, 256), 256, 0, st>>>(X, chain, level, width, d_dense);
+  dex_count_launch();
+  DEX_CUDA_CHECK(cudaGetLastError());
+  return DEX_OK;
+}

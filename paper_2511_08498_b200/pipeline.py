@@ -1,0 +1,105 @@
+"""Host <-> device plumbing around the C-ABI calls (no arithmetic of the method lives here).
+
+A `workload` is any object with the attributes of workloads.gen.Workload (numpy arrays on the host).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import Optional
+
+import numpy as np
+import torch
+
+from . import binding as B
+
+_SPEC_FIELDS = ("eta", "chi", "eta_bg", "chi_bg", "vel", "eta_star0", "chi_star0", "a0", "inv_dlamD", "lam")
+_RAY_FIELDS = ("probe_pos", "dirs", "weights", "i0")
+
+
+@dataclass
+class DeviceWorkload:
+    wl: object
+    t: dict = field(default_factory=dict)      # name -> device tensor
+    h2d_bytes: int = 0
+
+
+def pin(wl) -> dict:
+    """Pinned host copies of every array the device needs (for the end-to-end timing leg)."""
+    out = {}
+    for name in _SPEC_FIELDS + _RAY_FIELDS + ("active",):
+        a = getattr(wl, name, None)
+        if a is None:
+            continue
+        t = torch.from_numpy(np.ascontiguousarray(a))
+        out[name] = t.pin_memory() if torch.cuda.is_available() else t
+    return out
+
+
+def upload(wl, device="cuda:0", pinned: Optional[dict] = None, non_blocking=True) -> DeviceWorkload:
+    dw = DeviceWorkload(wl=wl)
+    src = pinned if pinned is not None else {n: torch.from_numpy(np.ascontiguousarray(getattr(wl, n)))
+                                             for n in _SPEC_FIELDS + _RAY_FIELDS + ("active",)
+                                             if getattr(wl, n, None) is not None}
+    for name, t in src.items():
+        dw.t[name] = t.to(device, non_blocking=non_blocking)
+        dw.h2d_bytes += t.numel() * t.element_size()
+    return dw
+
+
+def build_grid(dw: DeviceWorkload, stream=None) -> B.Grid:
+    wl = dw.wl
+    return B.dex_build_sparse_grid(wl.ndim, wl.dims[:wl.ndim], wl.brick, wl.voxel_size, dw.t.get("active"), stream)
+
+
+def build_mips(dw: DeviceWorkload, grid: B.Grid, stream=None, **override) -> B.Mips:
+    wl = dw.wl
+    g = lambda k: override.get(k, getattr(wl, k))
+    t = dw.t
+    return B.dex_build_vlm_mips(
+        grid, g("variant"), wl.n_lambda, wl.lambda_batch, g("max_level"), g("metric"), g("thr_eta"), g("thr_chi"),
+        g("tau_gate"), eta=t.get("eta"), chi=t.get("chi"), lam=t.get("lam"), eta_bg=t.get("eta_bg"),
+        chi_bg=t.get("chi_bg"), vel=t.get("vel"), lambda0=wl.lambda0, eta_star0=t.get("eta_star0"),
+        chi_star0=t.get("chi_star0"), a0=t.get("a0"), inv_dlamD=t.get("inv_dlamD"), active_lines=wl.active_lines,
+        n_vbins=g("n_vbins"), c_light=wl.c_light, stream=stream)
+
+
+def rays(dw: DeviceWorkload) -> B.Rays:
+    t = dw.t
+    return B.Rays(t["probe_pos"], t["dirs"], t.get("weights"), t.get("i0"))
+
+
+def mean_intensity(dw: DeviceWorkload, grid: B.Grid, mips: B.Mips, J: Optional[torch.Tensor] = None,
+                   segment_count: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    r = rays(dw)
+    if J is None:
+        J = torch.empty((r.n_probes, dw.wl.n_lambda), dtype=torch.float32, device=r.probe_pos.device)
+    B.dex_mean_intensity(grid, mips, r, J, None, segment_count, stream)
+    return J
+
+
+def formal_solution(dw: DeviceWorkload, grid: B.Grid, mips: B.Mips, capture_batch: Optional[int] = None,
+                    segment_count: Optional[torch.Tensor] = None, want_I=True, room: Optional[int] = None, stream=None):
+    r = rays(dw)
+    dev = r.probe_pos.device
+    I = torch.empty((r.n_probes, r.n_dirs, dw.wl.n_lambda), dtype=torch.float32, device=dev) if want_I else None
+    cap = None
+    if capture_batch is not None:
+        room = room if room is not None else int(sum(dw.wl.dims[:dw.wl.ndim])) + 16
+        cap = B.VisitCapture(r.n_probes * r.n_dirs, room, capture_batch, dev)
+    B.dex_formal_solution(grid, mips, r, I, cap, segment_count, stream)
+    return I, cap
+
+
+def solve_J_from_host(wl, device="cuda:0", pinned: Optional[dict] = None):
+    """The end-to-end call a user makes with HOST buffers: upload, build grid + mips, fused march to J,
+    read J and the emitted-segment count back.  Returns (J numpy, segments, h2d_bytes, d2h_bytes)."""
+    dw = upload(wl, device, pinned)
+    grid = build_grid(dw)
+    mips = build_mips(dw, grid)
+    seg = torch.zeros(1, dtype=torch.int64, device=device)
+    J = mean_intensity(dw, grid, mips, segment_count=seg)
+    Jh = J.cpu()
+    nseg = int(seg.cpu().item())
+    mips.destroy()
+    grid.destroy()
+    return Jh.numpy(), nseg, dw.h2d_bytes, Jh.numel() * 4 + 8
