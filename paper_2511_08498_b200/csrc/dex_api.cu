@@ -14,7 +14,7 @@
 namespace {
 thread_local std::string g_last_error;
 std::atomic<long long> g_launches{0};
-std::atomic<int> g_lanes_per_ray{8};
+std::atomic<int> g_lanes_per_ray{1};  // measured fastest on B200 (profiles/)
 std::atomic<int> g_timing{0};
 std::mutex g_timing_mu;
 struct EvPair { cudaEvent_t a, b; };
@@ -395,6 +395,7 @@ dex_status dex_formal_solution(const dex_grid* grid, const dex_mips* mips, const
   DexRaysDev R;
   dex_status s = check_rays(grid, mips, rays, &R);
   if (s != DEX_OK) return s;
+  if (rays->n_probes == 0 || rays->n_dirs == 0) return DEX_OK;   // nothing to trace
   if (!d_I && !capture) { dex_set_error("d_I is NULL and no capture requested"); return DEX_ERR_INVALID_ARG; }
   if (capture) {
     if (!capture->d_counts || !capture->d_records || !capture->d_offsets || capture->capacity < 0) {
@@ -434,6 +435,7 @@ dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const 
   DexRaysDev R;
   dex_status s = check_rays(grid, mips, rays, &R);
   if (s != DEX_OK) return s;
+  if (rays->n_probes == 0) return DEX_OK;                          // J has no rows
   if (!d_J) { dex_set_error("d_J is NULL"); return DEX_ERR_INVALID_ARG; }
   if (rays->n_dirs > 0 && !rays->d_weights) { dex_set_error("d_weights is NULL"); return DEX_ERR_INVALID_ARG; }
   if (!have_device()) return DEX_ERR_CUDA;

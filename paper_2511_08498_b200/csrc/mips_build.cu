@@ -511,8 +511,13 @@ dex_status build_t(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st) {
   const int L = m->max_level;
   auto cells_at = [&](int lv) { long long n = B >> lv; return (D == 3) ? n * n * n : n * n; };
   DEX_CUDA_CHECK(cudaMemsetAsync(m->d_fail, 0, sizeof(int) * (size_t)m->n_batch * (size_t)A * (L + 1), st));
-  if (A == 0) return DEX_OK;
   const bool iso = (m->variant == DEX_ISO);
+  if (A == 0) {   // no populated brick: every state is "empty"
+    select_levels_kernel<<<blocks_for((long long)m->n_batch * X.G.n_bricks, T), T, 0, st>>>(X, m->d_levels);
+    dex_count_launch();
+    DEX_CUDA_CHECK(cudaGetLastError());
+    return DEX_OK;
+  }
   const float* eta = iso ? desc->d_eta : desc->d_eta_bg;
   const float* chi = iso ? desc->d_chi : desc->d_chi_bg;
   gather_spec_kernel<D><<<blocks_for((long long)m->n_batch * A * cells_at(0) * DEX_W, T), T, 0, st>>>(X, eta, chi);

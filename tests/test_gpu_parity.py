@@ -1,0 +1,284 @@
+"""GPU parity: the CUDA path behind the C ABI against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): level tables and mip values bit-exact, traversal index lists (and
+their fp32 path lengths) bit-exact, intensities and J within 1e-5 max relative error in fp32.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import oracle as orc           # noqa: E402
+from workloads import make                 # noqa: E402
+from workloads.gen import dirs_2d          # noqa: E402
+from _util import fig5_levels, iso_workload, max_rel, random_unit_dirs, unit_dirs_2d   # noqa: E402
+
+TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def P():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2511_08498_b200 as pkg
+    return pkg
+
+
+def _build(P, wl, **ov):
+    dw = P.pipeline.upload(wl, "cuda:0")
+    grid = P.pipeline.build_grid(dw)
+    mips = P.pipeline.build_mips(dw, grid, **ov)
+    return dw, grid, mips
+
+
+def _check_build(P, wl, M, grid, mips, spectra=True):
+    act = orc.brick_active(wl)
+    slots = grid.slots()
+    assert np.array_equal(slots >= 0, act)
+    assert np.array_equal(np.sort(slots[slots >= 0]), np.arange(int(act.sum())))
+    lv = mips.levels()
+    assert np.array_equal(lv, M.levels), f"level tables differ in {(lv != M.levels).sum()} entries"
+    if spectra:
+        for m in range(M.max_level + 1):
+            for chain, ref in ((P.DEX_CHAIN_ETA, M.eta[m]), (P.DEX_CHAIN_CHI, M.chi[m])):
+                got = mips.level_data(chain, m)
+                mask = _active_cell_mask(wl, act, m)
+                assert np.array_equal(got[mask].view(np.uint32), np.ascontiguousarray(ref)[mask].view(np.uint32))
+    for b in range(wl.n_batch):
+        assert np.array_equal(mips.packed_levels(b), orc.pack_levels(M.levels[b], M.max_level))
+
+
+def _active_cell_mask(wl, act_b, m):
+    cb = wl.brick >> m
+    bd = wl.brick_dims
+    if wl.ndim == 2:
+        a = act_b.reshape(bd[1], bd[0])
+        return np.repeat(np.repeat(a, cb, axis=0), cb, axis=1)
+    a = act_b.reshape(bd[2], bd[1], bd[0])
+    return np.repeat(np.repeat(np.repeat(a, cb, axis=0), cb, axis=1), cb, axis=2)
+
+
+def _check_lists(cap, res, room):
+    counts = cap.counts.cpu().numpy()
+    assert np.array_equal(counts, res.counts)
+    rec = cap.records.cpu().numpy().view(np.uint64).reshape(-1, room)
+    ds = cap.ds.cpu().numpy().reshape(-1, room)
+    for r in range(counts.shape[0]):
+        n = counts[r]
+        assert np.array_equal(rec[r, :n], res.records[r, :n]), f"ray {r}: records differ"
+        assert np.array_equal(ds[r, :n].view(np.uint32), res.ds[r, :n].view(np.uint32)), f"ray {r}: ds differ"
+
+
+def _solve_and_compare(P, wl, M, dw, grid, mips, capture_batches=(0,), lanes=(8, 4, 2, 1), tol=TOL):
+    ref = None
+    for cb in capture_batches:
+        res = orc.hdda_march(wl, M, capture_batch=cb)
+        ref = res
+        I, cap = P.pipeline.formal_solution(dw, grid, mips, capture_batch=cb, want_I=False)
+        _check_lists(cap, res, cap.room)
+    Jref = orc.mean_intensity(ref.I, wl.weights)
+    for lpr in lanes:
+        P.dex_set_lanes_per_ray(lpr)
+        seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+        I, _ = P.pipeline.formal_solution(dw, grid, mips, segment_count=seg)
+        assert int(seg.item()) == ref.segments
+        assert max_rel(I.cpu().numpy(), ref.I) <= tol, f"lanes={lpr}"
+        seg.zero_()
+        J = P.pipeline.mean_intensity(dw, grid, mips, segment_count=seg)
+        assert int(seg.item()) == ref.segments
+        assert max_rel(J.cpu().numpy(), Jref) <= tol
+        J2 = torch.empty_like(J)
+        P.dex_mean_intensity(grid, mips, P.pipeline.rays(dw), J2, I)
+        assert max_rel(J2.cpu().numpy(), Jref) <= tol
+    P.dex_set_lanes_per_ray(1)
+    return ref
+
+
+# ------------------------------------------------------------------------------------------ ISO
+def test_c1_full(P):
+    """configs[0]: 64x64 dense, 8 wavelengths, 16 directions, a probe at every voxel centre."""
+    wl = make("C1")
+    M = orc.build_mips(wl)
+    dw, grid, mips = _build(P, wl)
+    _check_build(P, wl, M, grid, mips)
+    _solve_and_compare(P, wl, M, dw, grid, mips)
+
+
+@pytest.mark.parametrize("metric,thr,gate", [(1, 1e-2, -1.0), (0, 1.0, 0.25), (1, 0.0, -1.0)])
+def test_c2_small_with_mips(P, metric, thr, gate):
+    wl = make("C2", n=256, n_dirs=16, n_probes=1500)
+    d0, _ = dirs_2d(8, phase=0.0)           # axis-aligned and exact diagonals
+    wl.dirs = np.concatenate([wl.dirs, d0]).astype(np.float32)
+    wl.weights = np.full(len(wl.dirs), 1.0 / len(wl.dirs), dtype=np.float32)
+    wl.metric, wl.thr_eta, wl.thr_chi, wl.tau_gate = metric, thr, thr, gate
+    M = orc.build_mips(wl)
+    dw, grid, mips = _build(P, wl)
+    _check_build(P, wl, M, grid, mips)
+    _solve_and_compare(P, wl, M, dw, grid, mips, capture_batches=(0, 1))
+
+
+def test_iso_3d_with_mips(P):
+    wl = make("C5", n=64, n_dirs=12, n_probes=600)
+    wl.variant = 0
+    wl.eta, wl.chi = wl.eta_bg, wl.chi_bg
+    wl.thr_eta = wl.thr_chi = 1.0
+    M = orc.build_mips(wl)
+    assert M.levels.max() >= 2
+    dw, grid, mips = _build(P, wl)
+    _check_build(P, wl, M, grid, mips)
+    _solve_and_compare(P, wl, M, dw, grid, mips)
+
+
+def test_fig5_fixture_injected_levels_and_boundary_intensity(P):
+    """Fig. 5 block states injected through dex_mips_set_levels; nonzero incoming intensity."""
+    rng = np.random.default_rng(8)
+    lv = fig5_levels()
+    probes = np.concatenate([rng.uniform(0, 32, size=(40, 2)), [[16.5, 16.5], [0.5, 31.5], [20.25, 11.75]]])
+    dirs = np.concatenate([random_unit_dirs(9, 2, rng), unit_dirs_2d([0.0, math.pi / 2, math.pi / 4, math.pi, 1.25 * math.pi])])
+    f = rng.uniform(0.05, 1.5, size=(32, 32, 8))
+    act = np.repeat(np.repeat((lv >= 0).reshape(4, 4), 8, axis=0), 8, axis=1)
+    f[~act] = 0.0
+    i0 = rng.uniform(0, 2, size=(dirs.shape[0], 8))
+    wl = iso_workload((32, 32), 8, f * 1.3, f, probes, dirs, active=act.astype(np.uint8), max_level=3, i0=i0)
+    M = orc.build_mips(wl, max_level=3)
+    M.levels = np.ascontiguousarray(lv[None, :])
+    dw, grid, mips = _build(P, wl, max_level=3)
+    mips.set_levels(M.levels)
+    assert np.array_equal(mips.levels(), M.levels)
+    _solve_and_compare(P, wl, M, dw, grid, mips)
+
+
+def test_edge_cases(P):
+    # no probes
+    wl = make("C1", n=32, n_dirs=4)
+    full = wl.probe_pos
+    wl.probe_pos = full[:0]
+    dw, grid, mips = _build(P, wl)
+    J = P.pipeline.mean_intensity(dw, grid, mips)
+    assert J.shape == (0, 8)
+    # ragged probe count (not a multiple of any lane grouping), single direction
+    wl.probe_pos = full[:37]
+    wl.dirs, wl.weights = wl.dirs[:1], wl.weights[:1]
+    M = orc.build_mips(wl)
+    dw, grid, mips = _build(P, wl)
+    _solve_and_compare(P, wl, M, dw, grid, mips)
+    # all bricks empty: every intensity is exactly the (attenuation-free) boundary value
+    wl2 = make("C2", n=64, n_dirs=4, n_probes=50)
+    wl2.active[:] = 0
+    wl2.eta[:] = 0
+    wl2.chi[:] = 0
+    wl2.i0 = np.full((4, wl2.n_lambda), 0.5, dtype=np.float32)
+    dw, grid, mips = _build(P, wl2)
+    assert grid.info()[1] == 0 and (mips.levels() == -1).all()
+    I, cap = P.pipeline.formal_solution(dw, grid, mips, capture_batch=0)
+    assert (cap.counts.cpu().numpy() == 0).all()
+    assert (I.cpu().numpy() == 0.5).all()
+    # capture overflow is reported, counts stay complete
+    wl3 = make("C1", n=32, n_dirs=4, n_probes=10)
+    M3 = orc.build_mips(wl3)
+    res = orc.hdda_march(wl3, M3, capture_batch=0)
+    dw, grid, mips = _build(P, wl3)
+    with pytest.raises(P.DexError) as ei:
+        P.pipeline.formal_solution(dw, grid, mips, capture_batch=0, want_I=False, room=3)
+    assert ei.value.status == P.binding.DEX_ERR_CAPACITY
+    # argument errors
+    with pytest.raises(P.DexError):
+        P.pipeline.build_mips(dw, grid, max_level=5)
+    with pytest.raises(P.DexError):
+        P.dex_build_sparse_grid(2, (64, 60), 16, 1.0)
+
+
+def test_accuracy_regimes(P):
+    """Thin (chi ~ 1e-6) and thick (chi ~ 30) media, long rays: the fp32 recurrence must hold 1e-5."""
+    rng = np.random.default_rng(4)
+    n = 512
+    for scale in (1e-6, 1e-3, 0.3, 30.0):
+        chi = scale * np.exp(rng.standard_normal((n, n, 8)))
+        S = np.exp(0.5 * rng.standard_normal((n, n, 1)))
+        probes = rng.uniform(0, n, size=(256, 2))
+        wl = iso_workload((n, n), 16, chi * S, chi, probes, dirs_2d(8)[0])
+        M = orc.build_mips(wl)
+        dw, grid, mips = _build(P, wl)
+        res = orc.hdda_march(wl, M)
+        for lpr in (8, 1):
+            P.dex_set_lanes_per_ray(lpr)
+            I, _ = P.pipeline.formal_solution(dw, grid, mips)
+            assert max_rel(I.cpu().numpy(), res.I) <= TOL, f"scale={scale}"
+    P.dex_set_lanes_per_ray(1)
+
+
+# ------------------------------------------------------------------------------------------ anisotropic
+def _check_aux(P, wl, M, mips):
+    act = orc.brick_active(wl)
+    for m in range(M.max_level + 1):
+        mask = _active_cell_mask(wl, act, m)
+        vel = mips.level_data(P.DEX_CHAIN_VEL, m)
+        nd = wl.ndim
+        assert np.array_equal(vel[mask][:, :nd].view(np.uint32), np.ascontiguousarray(M.vbar[m])[mask].view(np.uint32))
+        assert np.array_equal(vel[mask][:, 3].view(np.uint32), np.ascontiguousarray(M.vmax[m])[mask].view(np.uint32))
+        line = mips.level_data(P.DEX_CHAIN_LINE, m)
+        for l in range(wl.n_lines):
+            for q, ref in enumerate((M.eta_star, M.chi_star, M.a0, M.inv_dlamD)):
+                assert np.array_equal(line[mask][:, l, q].view(np.uint32),
+                                      np.ascontiguousarray(ref[m][l])[mask].view(np.uint32))
+
+
+@pytest.mark.parametrize("name,n,metric,thr,gate", [("C4", 128, 1, 0.3, -1.0), ("C5", 64, 0, 0.3, 0.02),
+                                                    ("C5", 64, 1, 5.0, -1.0)])
+def test_cav_small(P, name, n, metric, thr, gate):
+    wl = make(name, n=n, n_dirs=8, n_probes=300)
+    wl.metric, wl.thr_eta, wl.thr_chi, wl.tau_gate = metric, thr, thr, gate
+    M = orc.build_mips(wl)
+    assert M.levels.max() >= 2
+    dw, grid, mips = _build(P, wl)
+    _check_build(P, wl, M, grid, mips)
+    _check_aux(P, wl, M, mips)
+    _solve_and_compare(P, wl, M, dw, grid, mips, lanes=(8, 2))
+
+
+def test_classic_equals_plain_march(P):
+    wl = make("C4", n=64, n_dirs=6, n_probes=100)
+    A = orc.plain_march(wl, variant=orc.CLASSIC)
+    dw, grid, mips = _build(P, wl, variant=P.DEX_CLASSIC)
+    assert (mips.levels() <= 0).all()
+    I, _ = P.pipeline.formal_solution(dw, grid, mips)
+    assert max_rel(I.cpu().numpy(), A.I) <= TOL
+
+
+def test_velinterp_small(P):
+    wl = make("C3", n=256, n_dirs=8, n_probes=300)
+    M = orc.build_mips(wl)
+    assert M.levels.max() >= 1
+    dw, grid, mips = _build(P, wl)
+    _check_build(P, wl, M, grid, mips)
+    _check_aux(P, wl, M, mips)
+    act = orc.brick_active(wl)
+    for m in range(M.max_level + 1):
+        mask = _active_cell_mask(wl, act, m)
+        got = mips.level_data(P.DEX_CHAIN_VTAB, m)[mask]
+        ref = M.vtab[m][mask]
+        assert max_rel(got, ref) <= 2e-6
+    _solve_and_compare(P, wl, M, dw, grid, mips, lanes=(8, 2))
+
+
+# ------------------------------------------------------------------------------------------ full size
+def test_c2_full_size_sampled(P):
+    """configs[1] at BASELINE size in the launch configuration bench.py times (fused J over all probes);
+    the oracle computes a seeded sample of probes one by one."""
+    wl = make("C2")
+    M = orc.build_mips(wl)
+    dw, grid, mips = _build(P, wl)
+    _check_build(P, wl, M, grid, mips, spectra=False)
+    seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+    J = P.pipeline.mean_intensity(dw, grid, mips, segment_count=seg).cpu().numpy()
+    rng = np.random.default_rng(77)
+    idx = np.sort(rng.choice(wl.probe_pos.shape[0], size=192, replace=False))
+    res = orc.hdda_march(wl, M, probe_pos=wl.probe_pos[idx])
+    Jref = orc.mean_intensity(res.I, wl.weights)
+    assert max_rel(J[idx], Jref) <= TOL
+    assert int(seg.item()) > 0
+    assert np.isfinite(J).all() and (J >= 0).all()
