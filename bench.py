@@ -44,7 +44,13 @@ def parse():
     ap.add_argument("--n", type=int, default=None, help="override grid side (reduced-size runs)")
     ap.add_argument("--n-dirs", type=int, default=None)
     ap.add_argument("--n-probes", type=int, default=None, help="seeded probe subset (default: every probe)")
+    ap.add_argument("--probe-band", type=float, default=None,
+                    help="keep only the probes of a centred band of this fraction of the slowest axis (contiguous, "
+                         "coherent subset for profiling)")
+    ap.add_argument("--probe-tile", default=None, help="reorder 2D every-voxel probes into WxH tiles, e.g. 8x4")
     ap.add_argument("--lanes", type=int, default=None, help="lanes per ray (1/2/4/8)")
+    ap.add_argument("--flat", type=int, default=None, help="flat_loop tuning knob (0/1)")
+    ap.add_argument("--tile", type=int, default=None, help="tile_probes tuning knob (0/1)")
     ap.add_argument("--cpu-probes", type=int, default=None, help="probes in the oracle (cpu_baseline) sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -210,8 +216,24 @@ def main():
 
     # weak scaling: every rank owns an atmosphere of the same size (its own seed)
     wl = make(args.workload, n=args.n, n_dirs=args.n_dirs, n_probes=args.n_probes, seed=SEEDS[args.workload] + 1000 * rank)
+    if args.probe_band:
+        ax = wl.ndim - 1
+        n_ax = wl.dims[ax]
+        lo, hi = n_ax * (0.5 - args.probe_band / 2), n_ax * (0.5 + args.probe_band / 2)
+        keep = (wl.probe_pos[:, ax] >= lo) & (wl.probe_pos[:, ax] < hi)
+        wl.probe_pos = np.ascontiguousarray(wl.probe_pos[keep])
+    if args.probe_tile and wl.ndim == 2:
+        tw, th = (int(v) for v in args.probe_tile.split("x"))
+        px = np.floor(wl.probe_pos[:, 0]).astype(np.int64)
+        py = np.floor(wl.probe_pos[:, 1]).astype(np.int64)
+        key = ((py // th) * (wl.dims[0] // tw) + (px // tw)) * (tw * th) + (py % th) * tw + (px % tw)
+        wl.probe_pos = np.ascontiguousarray(wl.probe_pos[np.argsort(key, kind="stable")])
     if args.lanes:
         P.dex_set_lanes_per_ray(args.lanes)
+    if args.flat is not None:
+        P.dex_set_tuning("flat_loop", args.flat)
+    if args.tile is not None:
+        P.dex_set_tuning("tile_probes", args.tile)
     W = wl.lambda_batch
     dw = P.pipeline.upload(wl, dev, non_blocking=False)
     n_probes = wl.probe_pos.shape[0]

@@ -26,6 +26,9 @@ def _newer(target, deps):
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    # DEX_NVCC_EXTRA: extra nvcc flags (e.g. -DDEX_MARCH_MINB=7) for tuning experiments; forces a rebuild
+    extra_env = os.environ.get("DEX_NVCC_EXTRA", "").split()
+    force = force or bool(extra_env)
     headers = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))]
     headers.append(os.path.join(os.path.dirname(HERE), "include", "dex.h"))
     objs = []
@@ -34,7 +37,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         o = os.path.join(CSRC, src.replace(".cu", ".o"))
         objs.append(o)
         if force or not _newer(o, [s] + headers):
-            cmd = ["nvcc"] + ARCH + COMMON + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
+            cmd = ["nvcc"] + ARCH + COMMON + extra + extra_env + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
             subprocess.run(cmd, check=True)
     if force or not _newer(LIB, objs):
         subprocess.run(["nvcc"] + ARCH + ["-shared", "-o", LIB] + objs + ["-lcudart"], check=True)

@@ -29,7 +29,7 @@ EXPORTS = (
     "dex_destroy_grid", "dex_build_vlm_mips", "dex_mips_get_levels", "dex_mips_set_levels",
     "dex_mips_get_packed_levels", "dex_mips_get_level_data", "dex_destroy_mips", "dex_formal_solution",
     "dex_mean_intensity", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read",
-    "dex_set_lanes_per_ray",
+    "dex_set_lanes_per_ray", "dex_set_tuning",
 )
 
 
@@ -92,6 +92,7 @@ def _load():
     L.dex_march_timing_enable.restype = None
     L.dex_march_timing_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64), C.c_int]
     L.dex_set_lanes_per_ray.argtypes = [C.c_int]
+    L.dex_set_tuning.argtypes = [C.c_char_p, C.c_int]
     return L
 
 
@@ -131,6 +132,10 @@ def dex_launch_count() -> int:
 
 def dex_set_lanes_per_ray(lanes: int):
     _check(_L.dex_set_lanes_per_ray(int(lanes)))
+
+
+def dex_set_tuning(name: str, value: int):
+    _check(_L.dex_set_tuning(name.encode(), int(value)))
 
 
 def dex_march_timing_enable(on: bool):

@@ -29,7 +29,8 @@ struct DexMipsDev {
   int n_lambda, n_batch;
   int max_level;
   int bits, per_word, words_per_batch;
-  const unsigned long long* packed;  // [n_batch][words_per_batch]
+  const unsigned long long* packed;  // [n_batch][words_per_batch]  PAPER.md:162 packed block states (exported)
+  const int* binfo;                  // [n_batch][n_bricks]  (slot << 4) | (level + 1): what the march reads
   int cps;                           // cells per slot (all levels)
   int lvloff[DEX_MAXLEV];            // first cell of level m inside a slot
   const float* store;                // [n_batch][n_active][cps][DEX_REC]  eta/chi (ISO) or background
@@ -228,4 +229,114 @@ __device__ __forceinline__ int dex_cell_in_slot(const DexGridDev& G, const DexMi
   int idx = ((c[1] & mask) >> m) * nb + ((c[0] & mask) >> m);
   if (D == 3) idx += ((c[2] & mask) >> m) * nb * nb;
   return M.lvloff[m] + idx;
+}
+
+
+// ---------------------------------------------------------------------------------------------------
+// v2 stepping used by the march kernel: same T-rules, fewer instructions.
+//   * size = 1 << sh for cells and for empty bricks alike (sh = level, or log2 B for an empty brick)
+//   * zero-direction axes carry inv = 0, off = +INF, so tplane = fma(k, 0, INF) = +INF without a select
+//   * pm[a] = -1 if d[a] > 0 else 0: exit plane = c[a] + (size & pm[a])
+//   * one 4-byte (slot, level) word per brick instead of the packed word + slot table
+// ---------------------------------------------------------------------------------------------------
+template <int D>
+struct DexRay2 {
+  float o[D], d[D], inv[D], off[D];
+  float tn[D];
+  int c[D], pm[D];
+  int sh;        // log2 of the current cell (or empty-brick) size
+  int cellbase;  // slot * cps + lvloff[level]; < 0 for an empty brick
+  float t;
+};
+
+template <int D>
+__device__ __forceinline__ void dex_planes2(DexRay2<D>& r) {
+  const int size = 1 << r.sh;
+#pragma unroll
+  for (int a = 0; a < D; ++a) r.tn[a] = __fmaf_rn((float)(r.c[a] + (size & r.pm[a])), r.inv[a], r.off[a]);
+}
+
+__device__ __forceinline__ void dex_decode_brick(const DexGridDev& G, const DexMipsDev& M, int info, int& sh, int& cellbase) {
+  const int m = (info & 15) - 1;
+  sh = (m < 0) ? G.logB : m;
+  cellbase = (m < 0) ? -1 : (info >> 4) * M.cps + M.lvloff[m];
+}
+
+template <int D>
+__device__ __forceinline__ bool dex_ray_init2(DexRay2<D>& r, const DexGridDev& G, const DexMipsDev& M,
+                                              const int* __restrict__ binfo, const float* probe, const float* omega) {
+  bool ok = true, any = false;
+  int x[D];
+#pragma unroll
+  for (int a = 0; a < D; ++a) {
+    r.o[a] = probe[a];
+    r.d[a] = -omega[a];
+    r.pm[a] = (r.d[a] > 0.0f) ? -1 : 0;
+    if (r.d[a] != 0.0f) {
+      any = true;
+      r.inv[a] = __fdiv_rn(1.0f, r.d[a]);
+      r.off[a] = __fmul_rn(-r.o[a], r.inv[a]);
+    } else {
+      r.inv[a] = 0.0f;
+      r.off[a] = __int_as_float(0x7f800000);
+    }
+    x[a] = (int)floorf(r.o[a]);
+    ok = ok && (x[a] >= 0) && (x[a] < G.dims[a]);
+  }
+  r.t = 0.0f;
+  r.sh = 0;
+  r.cellbase = -1;
+  if (!(ok && any)) return false;
+  dex_decode_brick(G, M, __ldg(binfo + dex_brick_of<D>(G, x)), r.sh, r.cellbase);
+  const int amask = ~((1 << r.sh) - 1);
+#pragma unroll
+  for (int a = 0; a < D; ++a) r.c[a] = x[a] & amask;
+  dex_planes2<D>(r);
+  return true;
+}
+
+// One HDDA event.  emit / cell / ds describe the cell that was just left (T4).  Returns false when the
+// ray has left the grid.
+template <int D>
+__device__ __forceinline__ bool dex_ray_step2(DexRay2<D>& r, const DexGridDev& G, const DexMipsDev& M,
+                                              const int* __restrict__ binfo, bool& emit, int& cell, float& ds) {
+  int s = 0;
+  float th = r.tn[0];
+  if (r.tn[1] < th) { s = 1; th = r.tn[1]; }
+  if (D == 3) { if (r.tn[D - 1] < th) { s = D - 1; th = r.tn[D - 1]; } }
+  emit = (r.cellbase >= 0) && (th > r.t);
+  ds = __fsub_rn(th, r.t);
+  {
+    const int mask = G.B - 1, lsh = G.logB - r.sh;
+    int idx = (((r.c[1] & mask) >> r.sh) << lsh) + ((r.c[0] & mask) >> r.sh);
+    if (D == 3) idx += ((r.c[D - 1] & mask) >> r.sh) << (2 * lsh);
+    cell = r.cellbase + idx;
+  }
+  r.t = fmaxf(r.t, th);
+  const int size = 1 << r.sh;
+  int cs = r.c[0], pms = r.pm[0], Ns = G.dims[0];
+  if (s == 1) { cs = r.c[1]; pms = r.pm[1]; Ns = G.dims[1]; }
+  if (D == 3) { if (s == D - 1) { cs = r.c[D - 1]; pms = r.pm[D - 1]; Ns = G.dims[D - 1]; } }
+  const int xs = pms ? cs + size : cs - 1;                      // T5
+  if ((unsigned)xs >= (unsigned)Ns) return false;
+  int x[D];
+#pragma unroll
+  for (int a = 0; a < D; ++a) x[a] = (a == s) ? xs : r.c[a];
+  if (((xs ^ cs) >> G.logB) != 0) {
+    // new brick: MipLevel (Alg. 1 l.6-8) and re-initialisation (l.32-39)
+    int sh2, cb2;
+    dex_decode_brick(G, M, __ldg(binfo + dex_brick_of<D>(G, x)), sh2, cb2);
+    if (sh2 < r.sh) {
+#pragma unroll
+      for (int a = 0; a < D; ++a)
+        if (a != s) x[a] = dex_fine_coord(r.o[a], r.d[a], r.inv[a], r.off[a], r.c[a], size, th, a < s);
+    }
+    r.sh = sh2;
+    r.cellbase = cb2;
+  }
+  const int amask = ~((1 << r.sh) - 1);
+#pragma unroll
+  for (int a = 0; a < D; ++a) r.c[a] = x[a] & amask;
+  dex_planes2<D>(r);
+  return true;
 }

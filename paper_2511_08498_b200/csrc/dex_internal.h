@@ -31,6 +31,7 @@ struct dex_mips {
   signed char* d_active_lines = nullptr;
   signed char* d_levels = nullptr;           // [n_batch][n_bricks]
   unsigned long long* d_packed = nullptr;    // [n_batch][words_per_batch]
+  int* d_binfo = nullptr;                    // [n_batch][n_bricks] (slot << 4) | (level + 1)
   int* d_fail = nullptr;                     // [n_batch][n_active][max_level+1]
   size_t store_floats = 0, vtab_floats = 0;
 };
@@ -46,7 +47,7 @@ dex_status dex_launch_pack_levels(dex_mips* m, cudaStream_t st);
 dex_status dex_launch_level_data(const dex_mips* m, int chain, int level, float* d_dense, cudaStream_t st);
 // march.cu
 dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                            unsigned long long* d_seg, int lanes_per_ray, cudaStream_t st);
+                            unsigned long long* d_seg, int lanes_per_ray, bool flat, bool tile, cudaStream_t st);
 dex_status dex_launch_capture(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays,
                               const dex_visit_capture* cap, int* d_overflow, cudaStream_t st);
 dex_status dex_launch_reduce_j(const DexRaysDev& rays, int n_lambda, const float* d_I, float* d_J, cudaStream_t st);

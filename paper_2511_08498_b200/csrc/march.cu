@@ -12,11 +12,24 @@
 
 namespace {
 
-// E(tau) = (1 - exp(-tau)) / tau with expm1-quality for small tau (1 - expf(-tau)
-// loses the 1e-5 budget in the thin regime).  Returns e = exp(-tau) as well.
-__device__ __forceinline__ float dex_E(float tau, float& e) {
-  e = __expf(-tau);
-  // Taylor series of E to degree 6: truncation < 1.6e-9 for tau < 0.25
+__device__ __forceinline__ float dex_ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float dex_rcp(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// I_out = I_in e^{-tau} + eta h ds E(tau), E(tau) = (1 - e^{-tau})/tau, accumulated front to back from
+// the probe outward:  I += T * eta h ds E(tau);  T *= e^{-tau}   (eq. 3 with constant eta, chi;
+// PAPER.md:31-34, :347).  E needs expm1 quality in the thin regime: Taylor series
+// to degree 6 below tau = 0.25 (truncation < 1.6e-9), (1 - e)/tau above.  hl = -hds * log2(e).
+__device__ __forceinline__ void dex_accumulate(float eta, float chi, float hds, float hl, float& I, float& T) {
+  const float tau = chi * hds;
+  const float e = dex_ex2(chi * hl);
   float p = -1.0f / 5040.0f;
   p = fmaf(p, tau, 1.0f / 720.0f);
   p = fmaf(p, tau, -1.0f / 120.0f);
@@ -24,17 +37,9 @@ __device__ __forceinline__ float dex_E(float tau, float& e) {
   p = fmaf(p, tau, -1.0f / 6.0f);
   p = fmaf(p, tau, 0.5f);
   p = fmaf(-p, tau, 1.0f);
-  const float q = __fdividef(1.0f - e, fmaxf(tau, 0.25f));
-  return (tau < 0.25f) ? p : q;
-}
-
-// I_out = I_in e^{-tau} + eta h ds E(tau), accumulated front to back from the probe outward:
-// I += T * eta h ds E(tau);  T *= e^{-tau}     (eq. 3 with constant eta, chi)
-__device__ __forceinline__ void dex_accumulate(float eta, float chi, float hds, float& I, float& T) {
-  const float tau = chi * hds;
-  float e;
-  const float E = dex_E(tau, e);
-  I = fmaf(T, eta * hds * E, I);
+  const float q = (1.0f - e) * dex_rcp(fmaxf(tau, 0.25f));
+  const float E = (tau < 0.25f) ? p : q;
+  I = fmaf(T, (eta * hds) * E, I);
   T *= e;
 }
 
@@ -52,25 +57,96 @@ __device__ __forceinline__ void dex_load_rec(const float* __restrict__ rec, floa
   }
 }
 
-template <int D, int VAR, int LPR, bool FUSE_J>
-__global__ void __launch_bounds__(128)
-dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, float* __restrict__ out,
-                 unsigned long long* __restrict__ seg_count) {
+// eta, chi of one cell for this lane's wavelengths, seen along propagation direction om (a7)
+template <int D, int VAR, int LPT>
+__device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_base, int cell, int sub,
+                                             const float* om, const double* lam, const int* al,
+                                             float (&eta)[LPT], float (&chi)[LPT]) {
+  if (VAR == DEX_ISO) {
+    dex_load_rec<LPT>(M.store + (batch_base + (size_t)cell) * DEX_REC + sub * LPT * 2, eta, chi);
+    return;
+  }
+  // projected velocity of the cell's box-filtered bulk velocity, fp64 (DESIGN.md R-vel)
+  const float4 v4 = __ldg(M.vel + cell);
+  double vproj = __dmul_rn((double)v4.x, (double)om[0]);
+  vproj = __dadd_rn(vproj, __dmul_rn((double)v4.y, (double)om[1]));
+  if (D == 3) vproj = __dadd_rn(vproj, __dmul_rn((double)v4.z, (double)om[D - 1]));
+  if (VAR == DEX_VELINTERP) {
+    // linear interpolation on the cell's uniform velocity grid [-V, V]
+    const int nvb = M.n_vbins;
+    const double V = (double)v4.w;
+    int i0 = 0;
+    float w = 0.0f;
+    if (V > 0.0) {
+      double f = __dmul_rn(__ddiv_rn(__dadd_rn(vproj, V), __dmul_rn(2.0, V)), (double)(nvb - 1));
+      f = fmin(fmax(f, 0.0), (double)(nvb - 1));
+      i0 = min((int)floor(f), nvb - 2);
+      w = (float)(f - (double)i0);
+    }
+    const float* r0 = M.vtab + ((batch_base + (size_t)cell) * nvb + i0) * DEX_REC + sub * LPT * 2;
+    float e1[LPT], c1[LPT];
+    dex_load_rec<LPT>(r0, eta, chi);
+    dex_load_rec<LPT>(r0 + DEX_REC, e1, c1);
+#pragma unroll
+    for (int i = 0; i < LPT; ++i) {
+      eta[i] = fmaf(w, e1[i], (1.0f - w) * eta[i]);
+      chi[i] = fmaf(w, c1[i], (1.0f - w) * chi[i]);
+    }
+    return;
+  }
+  // Core-and-Voigt / Classic: background + sum over the active lines (eqs. 10-11)
+  dex_load_rec<LPT>(M.store + (batch_base + (size_t)cell) * DEX_REC + sub * LPT * 2, eta, chi);
+  double de[LPT], dc[LPT];
+#pragma unroll
+  for (int i = 0; i < LPT; ++i) { de[i] = (double)eta[i]; dc[i] = (double)chi[i]; }
+#pragma unroll
+  for (int q = 0; q < DEX_NLINES; ++q) {
+    const int l = al[q];
+    if (l < 0) continue;
+    const float4 ln = __ldg(M.line + (size_t)cell * M.n_lines + l);
+    const double lam0 = (double)M.lambda0[l];
+#pragma unroll
+    for (int i = 0; i < LPT; ++i) {
+      double el, cl;
+      dex_line_terms(M.wei_c, M.wei_L, lam[i], lam0, (double)ln.x, (double)ln.y, (double)ln.z, (double)ln.w, vproj,
+                     M.c_light, el, cl);
+      de[i] += el;
+      dc[i] += cl;
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < LPT; ++i) { eta[i] = (float)de[i]; chi[i] = (float)dc[i]; }
+}
+
+// Each lane group owns one probe and walks through all its directions as one flattened stream of
+// HDDA events ("while-while"): the inner loop advances the ray -- or finishes it and sets up the next
+// direction -- until a segment has to be integrated; the integrate block then runs with every lane
+// that still has work.  No lane waits for the longest ray of a direction.
+#ifndef DEX_MARCH_THREADS
+#define DEX_MARCH_THREADS 128
+#endif
+#ifndef DEX_MARCH_MINB
+#define DEX_MARCH_MINB 7
+#endif
+
+template <int D, int VAR, int LPR, bool FUSE_J, bool FLAT>
+__global__ void __launch_bounds__(DEX_MARCH_THREADS, DEX_MARCH_MINB)
+dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ perm,
+                 float* __restrict__ out, unsigned long long* __restrict__ seg_count) {
   constexpr int LPT = DEX_W / LPR;
   const int batch = blockIdx.y;
-  const long long gid = ((long long)blockIdx.x * blockDim.x + threadIdx.x) / LPR;
+  const long long slot_id = ((long long)blockIdx.x * blockDim.x + threadIdx.x) / LPR;
+  // probes are handed to lanes in tile order (dex_tile_probes): a warp's probes are spatial neighbours
+  const long long gid = (slot_id < R.n_probes && perm != nullptr) ? (long long)perm[slot_id] : slot_id;
   const int sub = threadIdx.x % LPR;
   const int lam_off = batch * DEX_W + sub * LPT;
   unsigned nseg = 0;
-  if (gid < R.n_probes) {
+  if (slot_id < R.n_probes && R.n_dirs > 0) {
+    const int* __restrict__ binfo = M.binfo + (size_t)batch * G.n_bricks;
+    const size_t batch_base = ((size_t)batch * G.n_active) * M.cps;
     float probe[D];
 #pragma unroll
     for (int a = 0; a < D; ++a) probe[a] = __ldg(R.probe_pos + gid * D + a);
-    float J[LPT];
-#pragma unroll
-    for (int i = 0; i < LPT; ++i) J[i] = 0.0f;
-    const size_t batch_base = ((size_t)batch * G.n_active) * M.cps;
-    // per-thread wavelength constants of the anisotropic variants
     double lam[LPT];
     int al[DEX_NLINES];
     if (VAR == DEX_CAV) {
@@ -79,93 +155,96 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, flo
 #pragma unroll
       for (int q = 0; q < DEX_NLINES; ++q) al[q] = M.active_lines[batch * DEX_NLINES + q];
     }
-    for (int k = 0; k < R.n_dirs; ++k) {
-      float om[D];
+    float J[LPT], I[LPT], T[LPT];
 #pragma unroll
-      for (int a = 0; a < D; ++a) om[a] = __ldg(R.dirs + k * D + a);
-      float I[LPT], T[LPT];
-#pragma unroll
-      for (int i = 0; i < LPT; ++i) { I[i] = 0.0f; T[i] = 1.0f; }
-      DexRay<D> ray;
-      bool alive = dex_ray_init<D>(ray, G, M, batch, probe, om);
-      while (alive) {
-        DexSeg<D> seg;
-        alive = dex_ray_step<D>(ray, G, M, batch, seg);
-        if (seg.emit) {
-          ++nseg;
-          const float hds = G.h * seg.ds;
-          const size_t cell = (size_t)seg.slot * M.cps + dex_cell_in_slot<D>(G, M, seg.m, seg.c);
-          float eta[LPT], chi[LPT];
-          if (VAR == DEX_ISO) {
-            dex_load_rec<LPT>(M.store + (batch_base + cell) * DEX_REC + sub * LPT * 2, eta, chi);
-          } else {
-            // projected velocity of the cell's box-filtered bulk velocity, fp64 (DESIGN.md R-vel)
-            const float4 v4 = __ldg(M.vel + cell);
-            double vproj = __dmul_rn((double)v4.x, (double)om[0]);
-            vproj = __dadd_rn(vproj, __dmul_rn((double)v4.y, (double)om[1]));
-            if (D == 3) vproj = __dadd_rn(vproj, __dmul_rn((double)v4.z, (double)om[D - 1]));
-            if (VAR == DEX_VELINTERP) {
-              // linear interpolation on the cell's uniform velocity grid [-V, V]
-              const int nvb = M.n_vbins;
-              const double V = (double)v4.w;
-              int i0 = 0;
-              float w = 0.0f;
-              if (V > 0.0) {
-                double f = __dmul_rn(__ddiv_rn(__dadd_rn(vproj, V), __dmul_rn(2.0, V)), (double)(nvb - 1));
-                f = fmin(fmax(f, 0.0), (double)(nvb - 1));
-                i0 = min((int)floor(f), nvb - 2);
-                w = (float)(f - (double)i0);
+    for (int i = 0; i < LPT; ++i) { J[i] = 0.0f; I[i] = 0.0f; T[i] = 1.0f; }
+    float om[D];
+    DexRay2<D> ray;
+    if (FLAT) {
+      int k = -1;
+      bool alive = false;
+      for (;;) {
+        bool emit = false;
+        int cell = 0;
+        float ds = 0.0f;
+        while (!emit) {
+          if (!alive) {
+            if (k >= 0) {
+              // ray k is complete: boundary term, then the angular quadrature or the I store
+              if (R.i0 != nullptr) {
+  #pragma unroll
+                for (int i = 0; i < LPT; ++i)
+                  I[i] = fmaf(T[i], __ldg(R.i0 + (size_t)k * M.n_lambda + lam_off + i), I[i]);
               }
-              const float* r0 = M.vtab + ((batch_base + cell) * nvb + i0) * DEX_REC + sub * LPT * 2;
-              float e1[LPT], c1[LPT];
-              dex_load_rec<LPT>(r0, eta, chi);
-              dex_load_rec<LPT>(r0 + DEX_REC, e1, c1);
-#pragma unroll
-              for (int i = 0; i < LPT; ++i) {
-                eta[i] = fmaf(w, e1[i], (1.0f - w) * eta[i]);
-                chi[i] = fmaf(w, c1[i], (1.0f - w) * chi[i]);
+              if (FUSE_J) {
+                const float wk = __ldg(R.weights + k);
+  #pragma unroll
+                for (int i = 0; i < LPT; ++i) J[i] = fmaf(wk, I[i], J[i]);
+              } else {
+                float* dst = out + ((size_t)gid * R.n_dirs + k) * M.n_lambda + lam_off;
+  #pragma unroll
+                for (int i = 0; i < LPT; ++i) dst[i] = I[i];
               }
-            } else {
-              // Core-and-Voigt / Classic: background + sum over the active lines (eqs. 10-11)
-              dex_load_rec<LPT>(M.store + (batch_base + cell) * DEX_REC + sub * LPT * 2, eta, chi);
-              double de[LPT], dc[LPT];
-#pragma unroll
-              for (int i = 0; i < LPT; ++i) { de[i] = (double)eta[i]; dc[i] = (double)chi[i]; }
-#pragma unroll
-              for (int q = 0; q < DEX_NLINES; ++q) {
-                const int l = al[q];
-                if (l < 0) continue;
-                const float4 ln = __ldg(M.line + cell * M.n_lines + l);
-                const double lam0 = (double)M.lambda0[l];
-#pragma unroll
-                for (int i = 0; i < LPT; ++i) {
-                  double el, cl;
-                  dex_line_terms(M.wei_c, M.wei_L, lam[i], lam0, (double)ln.x, (double)ln.y, (double)ln.z,
-                                 (double)ln.w, vproj, M.c_light, el, cl);
-                  de[i] += el;
-                  dc[i] += cl;
-                }
-              }
-#pragma unroll
-              for (int i = 0; i < LPT; ++i) { eta[i] = (float)de[i]; chi[i] = (float)dc[i]; }
             }
+            ++k;
+            if (k >= R.n_dirs) break;
+  #pragma unroll
+            for (int a = 0; a < D; ++a) om[a] = __ldg(R.dirs + k * D + a);
+  #pragma unroll
+            for (int i = 0; i < LPT; ++i) { I[i] = 0.0f; T[i] = 1.0f; }
+            alive = dex_ray_init2<D>(ray, G, M, binfo, probe, om);
+            continue;
           }
-#pragma unroll
-          for (int i = 0; i < LPT; ++i) dex_accumulate(eta[i], chi[i], hds, I[i], T[i]);
+          alive = dex_ray_step2<D>(ray, G, M, binfo, emit, cell, ds);
         }
+        if (!emit) break;
+        ++nseg;
+        const float hds = G.h * ds;
+        const float hl = hds * -1.4426950408889634f;
+        float eta[LPT], chi[LPT];
+        dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, lam, al, eta, chi);
+  #pragma unroll
+        for (int i = 0; i < LPT; ++i) dex_accumulate(eta[i], chi[i], hds, hl, I[i], T[i]);
       }
-      if (R.i0 != nullptr) {
+    } else {
+      // one direction at a time: the lanes of a warp trace the same direction together (coherent
+      // fetches); inside a direction, lanes skip ahead to their next segment before integrating
+      for (int k = 0; k < R.n_dirs; ++k) {
 #pragma unroll
-        for (int i = 0; i < LPT; ++i) I[i] = fmaf(T[i], __ldg(R.i0 + (size_t)k * M.n_lambda + lam_off + i), I[i]);
-      }
-      if (FUSE_J) {
-        const float wk = __ldg(R.weights + k);
+        for (int a = 0; a < D; ++a) om[a] = __ldg(R.dirs + k * D + a);
 #pragma unroll
-        for (int i = 0; i < LPT; ++i) J[i] = fmaf(wk, I[i], J[i]);
-      } else {
-        float* dst = out + ((size_t)gid * R.n_dirs + k) * M.n_lambda + lam_off;
+        for (int i = 0; i < LPT; ++i) { I[i] = 0.0f; T[i] = 1.0f; }
+        bool alive = dex_ray_init2<D>(ray, G, M, binfo, probe, om);
+        while (alive) {
+          bool emit = false;
+          int cell = 0;
+          float ds = 0.0f;
+          do {
+            alive = dex_ray_step2<D>(ray, G, M, binfo, emit, cell, ds);
+          } while (alive && !emit);
+          if (emit) {
+            ++nseg;
+            const float hds = G.h * ds;
+            const float hl = hds * -1.4426950408889634f;
+            float eta[LPT], chi[LPT];
+            dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, lam, al, eta, chi);
 #pragma unroll
-        for (int i = 0; i < LPT; ++i) dst[i] = I[i];
+            for (int i = 0; i < LPT; ++i) dex_accumulate(eta[i], chi[i], hds, hl, I[i], T[i]);
+          }
+        }
+        if (R.i0 != nullptr) {
+#pragma unroll
+          for (int i = 0; i < LPT; ++i) I[i] = fmaf(T[i], __ldg(R.i0 + (size_t)k * M.n_lambda + lam_off + i), I[i]);
+        }
+        if (FUSE_J) {
+          const float wk = __ldg(R.weights + k);
+#pragma unroll
+          for (int i = 0; i < LPT; ++i) J[i] = fmaf(wk, I[i], J[i]);
+        } else {
+          float* dst = out + ((size_t)gid * R.n_dirs + k) * M.n_lambda + lam_off;
+#pragma unroll
+          for (int i = 0; i < LPT; ++i) dst[i] = I[i];
+        }
       }
     }
     if (FUSE_J) {
@@ -181,7 +260,8 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, flo
   }
 }
 
-// a10: traversal only, one thread per ray, for one batch's level table.
+// a10: traversal only, one thread per ray, for one batch's level table -- the same stepping code as
+// the march kernel, so the recorded list is the one the production path integrates over.
 template <int D>
 __global__ void __launch_bounds__(128)
 dex_capture_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, long long* __restrict__ counts,
@@ -195,28 +275,84 @@ dex_capture_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, l
   float probe[D], om[D];
 #pragma unroll
   for (int a = 0; a < D; ++a) { probe[a] = R.probe_pos[p * D + a]; om[a] = R.dirs[k * D + a]; }
+  const int* __restrict__ binfo = M.binfo + (size_t)batch * G.n_bricks;
   const long long begin = offsets[ray_id];
   const long long room = ((ray_id + 1 < n_rays) ? offsets[ray_id + 1] : capacity) - begin;
   long long n = 0;
-  DexRay<D> ray;
-  bool alive = dex_ray_init<D>(ray, G, M, batch, probe, om);
+  DexRay2<D> ray;
+  bool alive = dex_ray_init2<D>(ray, G, M, binfo, probe, om);
   while (alive) {
-    DexSeg<D> seg;
-    alive = dex_ray_step<D>(ray, G, M, batch, seg);
-    if (seg.emit) {
+    int c[D];
+#pragma unroll
+    for (int a = 0; a < D; ++a) c[a] = ray.c[a];
+    const int m = ray.sh;
+    bool emit;
+    int cell;
+    float ds;
+    alive = dex_ray_step2<D>(ray, G, M, binfo, emit, cell, ds);
+    if (emit) {
       if (n < room) {
-        unsigned long long rec = ((unsigned long long)(unsigned)seg.m << 56) |
-                                 (unsigned long long)(unsigned)(seg.c[0] >> seg.m);
-        rec |= (unsigned long long)(unsigned)(seg.c[1] >> seg.m) << 18;
-        if (D == 3) rec |= (unsigned long long)(unsigned)(seg.c[D - 1] >> seg.m) << 36;
+        unsigned long long rec = ((unsigned long long)(unsigned)m << 56) | (unsigned long long)(unsigned)(c[0] >> m);
+        rec |= (unsigned long long)(unsigned)(c[1] >> m) << 18;
+        if (D == 3) rec |= (unsigned long long)(unsigned)(c[D - 1] >> m) << 36;
         records[begin + n] = rec;
-        if (ds_out) ds_out[begin + n] = seg.ds;
+        if (ds_out) ds_out[begin + n] = ds;
       }
       ++n;
     }
   }
   counts[ray_id] = n;
   if (n > room) *overflow = 1;
+}
+
+// ---- probe tiling: counting sort of the probes into compact spatial tiles ------------------------------
+// Lane coherence is what the march lives on (profiles/): 32 probes of a 4x8 (2D) or 4x4x2 (3D) block of
+// the probe lattice trace almost the same cells, 32 probes of one row do not.  The tile edge is scaled by
+// the mean probe spacing, so a regular lattice fills every tile with exactly one warp.
+struct DexTiling {
+  float inv_tile[3];
+  int nt[3];
+  int n_tiles;
+};
+
+template <int D>
+__device__ __forceinline__ int dex_tile_of(const DexTiling& TL, const float* __restrict__ pos) {
+  int t[3] = {0, 0, 0};
+#pragma unroll
+  for (int a = 0; a < D; ++a) t[a] = max(0, min(TL.nt[a] - 1, (int)floorf(pos[a] * TL.inv_tile[a])));
+  return (t[2] * TL.nt[1] + t[1]) * TL.nt[0] + t[0];
+}
+
+template <int D>
+__global__ void dex_tile_count_kernel(const DexTiling TL, long long n, const float* __restrict__ pos, int* __restrict__ count) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) atomicAdd(count + dex_tile_of<D>(TL, pos + i * D), 1);
+}
+
+__global__ void __launch_bounds__(1024) dex_tile_scan_kernel(int* __restrict__ count, int n) {
+  __shared__ int part[1024];
+  const int t = threadIdx.x;
+  const int chunk = (n + 1023) / 1024;
+  const int lo = min(n, t * chunk), hi = min(n, lo + chunk);
+  int sum = 0;
+  for (int i = lo; i < hi; ++i) sum += count[i];
+  part[t] = sum;
+  __syncthreads();
+  for (int off = 1; off < 1024; off <<= 1) {
+    int v = (t >= off) ? part[t - off] : 0;
+    __syncthreads();
+    part[t] += v;
+    __syncthreads();
+  }
+  int base = part[t] - sum;
+  for (int i = lo; i < hi; ++i) { const int c = count[i]; count[i] = base; base += c; }
+}
+
+template <int D>
+__global__ void dex_tile_scatter_kernel(const DexTiling TL, long long n, const float* __restrict__ pos,
+                                        int* __restrict__ cursor, int* __restrict__ perm) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) perm[atomicAdd(cursor + dex_tile_of<D>(TL, pos + i * D), 1)] = (int)i;
 }
 
 // J(p, lambda) = sum_k w_k I(p, k, lambda) from a materialised I: one thread per (probe, lambda);
@@ -234,8 +370,8 @@ __global__ void dex_reduce_j_kernel(long long n_probes, int n_dirs, int n_lambda
 
 template <int D, int VAR, int LPR>
 dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                          unsigned long long* d_seg, cudaStream_t st) {
-  const int threads = 128;
+                          unsigned long long* d_seg, bool flat, const int* perm, cudaStream_t st) {
+  const int threads = DEX_MARCH_THREADS;
   const long long probes_per_block = threads / LPR;
   const long long gx = (rays.n_probes + probes_per_block - 1) / probes_per_block;
   if (gx <= 0) return DEX_OK;
@@ -244,10 +380,14 @@ dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev
     return DEX_ERR_UNSUPPORTED;
   }
   dim3 grid((unsigned)gx, (unsigned)m->n_batch, 1);
-  if (fuse_j)
-    dex_march_kernel<D, VAR, LPR, true><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, d_out, d_seg);
+  if (fuse_j && flat)
+    dex_march_kernel<D, VAR, LPR, true, true><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
+  else if (fuse_j)
+    dex_march_kernel<D, VAR, LPR, true, false><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
+  else if (flat)
+    dex_march_kernel<D, VAR, LPR, false, true><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
   else
-    dex_march_kernel<D, VAR, LPR, false><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, d_out, d_seg);
+    dex_march_kernel<D, VAR, LPR, false, false><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
   dex_count_launch();
   DEX_CUDA_CHECK(cudaGetLastError());
   return DEX_OK;
@@ -255,12 +395,12 @@ dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev
 
 template <int D, int VAR>
 dex_status launch_march_v(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                          unsigned long long* d_seg, int lpr, cudaStream_t st) {
+                          unsigned long long* d_seg, int lpr, bool flat, const int* perm, cudaStream_t st) {
   switch (lpr) {
-    case 8: return launch_march_t<D, VAR, 8>(g, m, rays, d_out, fuse_j, d_seg, st);
-    case 4: return launch_march_t<D, VAR, 4>(g, m, rays, d_out, fuse_j, d_seg, st);
-    case 2: return launch_march_t<D, VAR, 2>(g, m, rays, d_out, fuse_j, d_seg, st);
-    case 1: return launch_march_t<D, VAR, 1>(g, m, rays, d_out, fuse_j, d_seg, st);
+    case 8: return launch_march_t<D, VAR, 8>(g, m, rays, d_out, fuse_j, d_seg, flat, perm, st);
+    case 4: return launch_march_t<D, VAR, 4>(g, m, rays, d_out, fuse_j, d_seg, flat, perm, st);
+    case 2: return launch_march_t<D, VAR, 2>(g, m, rays, d_out, fuse_j, d_seg, flat, perm, st);
+    case 1: return launch_march_t<D, VAR, 1>(g, m, rays, d_out, fuse_j, d_seg, flat, perm, st);
   }
   dex_set_error("lanes per ray must be 1, 2, 4 or 8");
   return DEX_ERR_INVALID_ARG;
@@ -268,12 +408,12 @@ dex_status launch_march_v(const dex_grid* g, const dex_mips* m, const DexRaysDev
 
 template <int D>
 dex_status launch_march_d(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                          unsigned long long* d_seg, int lpr, cudaStream_t st) {
+                          unsigned long long* d_seg, int lpr, bool flat, const int* perm, cudaStream_t st) {
   switch (m->variant) {
-    case DEX_ISO: return launch_march_v<D, DEX_ISO>(g, m, rays, d_out, fuse_j, d_seg, lpr, st);
-    case DEX_VELINTERP: return launch_march_v<D, DEX_VELINTERP>(g, m, rays, d_out, fuse_j, d_seg, lpr, st);
+    case DEX_ISO: return launch_march_v<D, DEX_ISO>(g, m, rays, d_out, fuse_j, d_seg, lpr, flat, perm, st);
+    case DEX_VELINTERP: return launch_march_v<D, DEX_VELINTERP>(g, m, rays, d_out, fuse_j, d_seg, lpr, flat, perm, st);
     case DEX_CAV:
-    case DEX_CLASSIC: return launch_march_v<D, DEX_CAV>(g, m, rays, d_out, fuse_j, d_seg, lpr, st);
+    case DEX_CLASSIC: return launch_march_v<D, DEX_CAV>(g, m, rays, d_out, fuse_j, d_seg, lpr, flat, perm, st);
   }
   dex_set_error("unknown variant");
   return DEX_ERR_INVALID_ARG;
@@ -281,10 +421,53 @@ dex_status launch_march_d(const dex_grid* g, const dex_mips* m, const DexRaysDev
 
 }  // namespace
 
+// perm[i] = probe handled by lane group i.  *d_perm is allocated on the stream (stream-ordered) and must be
+// released with cudaFreeAsync by the caller after the march has been enqueued.
+template <int D>
+static dex_status tile_probes_t(const dex_grid* g, const DexRaysDev& rays, int** d_perm, cudaStream_t st) {
+  *d_perm = nullptr;
+  const long long n = rays.n_probes;
+  if (n < 64 || n > 2147483647LL) return DEX_OK;        // nothing to gain / index range
+  DexTiling TL;
+  double vol = 1.0;
+  for (int a = 0; a < D; ++a) vol *= (double)g->dev.dims[a];
+  const double spacing = fmax(1.0, pow(vol / (double)n, 1.0 / D));   // mean probe spacing in voxels
+  const int shape2[3] = {4, 8, 1}, shape3[3] = {4, 4, 2};
+  long long nt_total = 1;
+  for (int a = 0; a < 3; ++a) {
+    const double edge = spacing * (double)((D == 2) ? shape2[a] : shape3[a]);
+    TL.inv_tile[a] = (float)(1.0 / edge);
+    TL.nt[a] = (a < D) ? (int)ceil((double)g->dev.dims[a] / edge) : 1;
+    nt_total *= TL.nt[a];
+  }
+  if (nt_total > (1LL << 28)) return DEX_OK;
+  TL.n_tiles = (int)nt_total;
+  int* d_count = nullptr;
+  DEX_CUDA_CHECK(cudaMallocAsync((void**)&d_count, sizeof(int) * (size_t)(TL.n_tiles + 1), st));
+  cudaError_t e = cudaMallocAsync((void**)d_perm, sizeof(int) * (size_t)n, st);
+  if (e != cudaSuccess) { cudaFreeAsync(d_count, st); *d_perm = nullptr; DEX_CUDA_CHECK(e); }
+  cudaMemsetAsync(d_count, 0, sizeof(int) * (size_t)(TL.n_tiles + 1), st);
+  const unsigned blocks = (unsigned)((n + 255) / 256);
+  dex_tile_count_kernel<D><<<blocks, 256, 0, st>>>(TL, n, rays.probe_pos, d_count);
+  dex_tile_scan_kernel<<<1, 1024, 0, st>>>(d_count, TL.n_tiles);
+  dex_tile_scatter_kernel<D><<<blocks, 256, 0, st>>>(TL, n, rays.probe_pos, d_count, *d_perm);
+  dex_count_launch(3);
+  cudaFreeAsync(d_count, st);
+  DEX_CUDA_CHECK(cudaGetLastError());
+  return DEX_OK;
+}
+
 dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                            unsigned long long* d_seg, int lanes_per_ray, cudaStream_t st) {
-  if (g->desc.ndim == 2) return launch_march_d<2>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, st);
-  return launch_march_d<3>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, st);
+                            unsigned long long* d_seg, int lanes_per_ray, bool flat, bool tile, cudaStream_t st) {
+  int* d_perm = nullptr;
+  dex_status s = DEX_OK;
+  if (tile) s = (g->desc.ndim == 2) ? tile_probes_t<2>(g, rays, &d_perm, st) : tile_probes_t<3>(g, rays, &d_perm, st);
+  if (s == DEX_OK) {
+    if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, flat, d_perm, st);
+    else s = launch_march_d<3>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, flat, d_perm, st);
+  }
+  if (d_perm) cudaFreeAsync(d_perm, st);
+  return s;
 }
 
 dex_status dex_launch_capture(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays,

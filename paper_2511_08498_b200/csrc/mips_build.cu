@@ -429,9 +429,11 @@ __global__ void select_levels_kernel(const BuildCtx X, signed char* __restrict__
   levels[i] = (signed char)lv;
 }
 
-// state = level + 1 in `bits` bits, floor(64/bits) bricks per 64-bit word
-__global__ void pack_levels_kernel(const signed char* __restrict__ levels, int n_batch, int n_bricks, int bits,
-                                   int per_word, int words, unsigned long long* __restrict__ packed) {
+// state = level + 1 in `bits` bits, floor(64/bits) bricks per 64-bit word.  The same pass
+// writes the march's own table: one 4-byte word (slot << 4) | state per (batch, brick).
+__global__ void pack_levels_kernel(const signed char* __restrict__ levels, const int* __restrict__ slot, int n_batch,
+                                   int n_bricks, int bits, int per_word, int words,
+                                   unsigned long long* __restrict__ packed, int* __restrict__ binfo) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (long long)n_batch * words) return;
   const int w = (int)(i % words);
@@ -440,7 +442,9 @@ __global__ void pack_levels_kernel(const signed char* __restrict__ levels, int n
   for (int q = 0; q < per_word; ++q) {
     const int bi = w * per_word + q;
     if (bi >= n_bricks) break;
-    word |= (unsigned long long)(levels[(size_t)b * n_bricks + bi] + 1) << (q * bits);
+    const int state = levels[(size_t)b * n_bricks + bi] + 1;
+    word |= (unsigned long long)state << (q * bits);
+    binfo[(size_t)b * n_bricks + bi] = (state > 0) ? ((slot[bi] << 4) | state) : 0;
   }
   packed[i] = word;
 }
@@ -565,9 +569,9 @@ dex_status dex_launch_mips_build(dex_mips* m, const dex_mips_desc* desc, cudaStr
 
 dex_status dex_launch_pack_levels(dex_mips* m, cudaStream_t st) {
   const long long total = (long long)m->n_batch * m->dev.words_per_batch;
-  pack_levels_kernel<<<blocks_for(total, 256), 256, 0, st>>>(m->d_levels, m->n_batch, (int)m->grid->n_bricks,
-                                                             m->dev.bits, m->dev.per_word, m->dev.words_per_batch,
-                                                             m->d_packed);
+  pack_levels_kernel<<<blocks_for(total, 256), 256, 0, st>>>(m->d_levels, m->grid->d_slot, m->n_batch,
+                                                             (int)m->grid->n_bricks, m->dev.bits, m->dev.per_word,
+                                                             m->dev.words_per_batch, m->d_packed, m->d_binfo);
   dex_count_launch();
   DEX_CUDA_CHECK(cudaGetLastError());
   return DEX_OK;
