@@ -49,7 +49,6 @@ def parse():
                          "coherent subset for profiling)")
     ap.add_argument("--probe-tile", default=None, help="reorder 2D every-voxel probes into WxH tiles, e.g. 8x4")
     ap.add_argument("--lanes", type=int, default=None, help="lanes per ray (1/2/4/8)")
-    ap.add_argument("--flat", type=int, default=None, help="flat_loop tuning knob (0/1)")
     ap.add_argument("--tile", type=int, default=None, help="tile_probes tuning knob (0/1)")
     ap.add_argument("--cpu-probes", type=int, default=None, help="probes in the oracle (cpu_baseline) sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -230,8 +229,6 @@ def main():
         wl.probe_pos = np.ascontiguousarray(wl.probe_pos[np.argsort(key, kind="stable")])
     if args.lanes:
         P.dex_set_lanes_per_ray(args.lanes)
-    if args.flat is not None:
-        P.dex_set_tuning("flat_loop", args.flat)
     if args.tile is not None:
         P.dex_set_tuning("tile_probes", args.tile)
     W = wl.lambda_batch

@@ -194,10 +194,9 @@ void dex_march_timing_enable(int on);
 dex_status dex_march_timing_read(double* ms_total, int64_t* n_launches, int reset);
 /* Kernel configuration knob (performance experiments): lanes that share one ray, 1/2/4/8. */
 dex_status dex_set_lanes_per_ray(int lanes);
-/* Other kernel-structure knobs for performance experiments (results do not change):
- *   "lanes_per_ray" 1/2/4/8;  "flat_loop" 0/1 (1: a lane moves on to its next direction as soon as its ray
- *   ends instead of waiting for the other lanes of the warp);  "tile_probes" 0/1 (1, default: probes are handed to
- *   warps in compact spatial tiles by an internal counting sort instead of in the caller's order). */
+/* Kernel-structure knobs for performance experiments (results do not change): "lanes_per_ray" 1/2/4/8;
+ * "tile_probes" 0/1 (1, default: probes are handed to warps in compact spatial tiles by an internal counting
+ * sort instead of in the caller's order). */
 dex_status dex_set_tuning(const char* name, int value);
 
 #ifdef __cplusplus

@@ -16,7 +16,6 @@ thread_local std::string g_last_error;
 std::atomic<long long> g_launches{0};
 std::atomic<int> g_lanes_per_ray{1};  // measured fastest on B200 (profiles/)
 std::atomic<int> g_timing{0};
-std::atomic<int> g_flat_loop{0};
 std::atomic<int> g_tile_probes{1};
 std::mutex g_timing_mu;
 struct EvPair { cudaEvent_t a, b; };
@@ -49,7 +48,7 @@ dex_status dmalloc(T** p, size_t count) {
 }
 
 void free_mips_memory(dex_mips* m) {
-  cudaFree(m->d_store); cudaFree(m->d_line); cudaFree(m->d_vel); cudaFree(m->d_vtab); cudaFree(m->d_lam);
+  cudaFree(m->d_store); cudaFree(m->d_mrec); cudaFree(m->d_line); cudaFree(m->d_vel); cudaFree(m->d_vtab); cudaFree(m->d_lam);
   cudaFree(m->d_active_lines); cudaFree(m->d_levels); cudaFree(m->d_packed); cudaFree(m->d_fail); cudaFree(m->d_binfo);
 }
 
@@ -112,7 +111,6 @@ dex_status dex_set_lanes_per_ray(int lanes) {
 dex_status dex_set_tuning(const char* name, int value) {
   if (!name) { dex_set_error("NULL tuning name"); return DEX_ERR_INVALID_ARG; }
   if (!strcmp(name, "lanes_per_ray")) return dex_set_lanes_per_ray(value);
-  if (!strcmp(name, "flat_loop")) { g_flat_loop.store(value ? 1 : 0); return DEX_OK; }
   if (!strcmp(name, "tile_probes")) { g_tile_probes.store(value ? 1 : 0); return DEX_OK; }
   dex_set_error("unknown tuning knob");
   return DEX_ERR_INVALID_ARG;
@@ -289,6 +287,7 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
   dex_status s = DEX_OK;
   m->store_floats = (size_t)n_batch * A * cps * DEX_REC;
   s = dmalloc(&m->d_store, m->store_floats);
+  if (s == DEX_OK && v == DEX_ISO) s = dmalloc(&m->d_mrec, m->store_floats);
   if (s == DEX_OK) s = dmalloc(&m->d_levels, (size_t)n_batch * grid->n_bricks);
   if (s == DEX_OK) s = dmalloc(&m->d_packed, (size_t)n_batch * d.words_per_batch);
   if (s == DEX_OK) s = dmalloc(&m->d_binfo, (size_t)n_batch * grid->n_bricks);
@@ -315,6 +314,7 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
     d.packed = m->d_packed;
     d.binfo = m->d_binfo;
     d.store = m->d_store;
+    d.mrec = m->d_mrec;
     d.line = m->d_line;
     d.vel = m->d_vel;
     d.vtab = m->d_vtab;
@@ -421,7 +421,7 @@ dex_status dex_formal_solution(const dex_grid* grid, const dex_mips* mips, const
   cudaStream_t st = (cudaStream_t)stream;
   if (d_I) {
     MarchTimer tm(st);
-    s = dex_launch_march(grid, mips, R, d_I, false, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), g_flat_loop.load() != 0, g_tile_probes.load() != 0, st);
+    s = dex_launch_march(grid, mips, R, d_I, false, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), g_tile_probes.load() != 0, st);
     if (s != DEX_OK) return s;
   }
   if (capture) {
@@ -455,7 +455,7 @@ dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const 
   cudaStream_t st = (cudaStream_t)stream;
   if (d_I) return dex_launch_reduce_j(R, mips->n_lambda, d_I, d_J, st);
   MarchTimer tm(st);
-  return dex_launch_march(grid, mips, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), g_flat_loop.load() != 0, g_tile_probes.load() != 0, st);
+  return dex_launch_march(grid, mips, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), g_tile_probes.load() != 0, st);
 }
 
 }  // extern "C"

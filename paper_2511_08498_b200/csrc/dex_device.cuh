@@ -9,9 +9,13 @@
 #include <stdint.h>
 
 #define DEX_W 8            // wavelengths per batch
-#define DEX_REC (2 * DEX_W) // floats per cell record: [lambda][eta, chi]
+#define DEX_REC (2 * DEX_W) // floats per cell record: chi[0..W-1] then eta[0..W-1] (pairs of wavelengths feed FFMA2)
 #define DEX_MAXLEV 6
 #define DEX_NLINES 4
+
+// cell record accessors: record r (in units of DEX_REC floats) of a store, wavelength j of the batch
+__host__ __device__ __forceinline__ size_t dex_rec_chi(size_t r, int j) { return r * DEX_REC + j; }
+__host__ __device__ __forceinline__ size_t dex_rec_eta(size_t r, int j) { return r * DEX_REC + DEX_W + j; }
 
 struct DexGridDev {
   int ndim;
@@ -33,7 +37,9 @@ struct DexMipsDev {
   const int* binfo;                  // [n_batch][n_bricks]  (slot << 4) | (level + 1): what the march reads
   int cps;                           // cells per slot (all levels)
   int lvloff[DEX_MAXLEV];            // first cell of level m inside a slot
-  const float* store;                // [n_batch][n_active][cps][DEX_REC]  eta/chi (ISO) or background
+  const float* store;                // [n_batch][n_active][cps][DEX_REC]  chi|eta (ISO) or background
+  const float* mrec;                 // ISO march records, same shape as store: chi'|S with S = eta/chi (see
+                                     // make_march_records_kernel); what the ISO march reads
   const float4* line;                // [n_active][cps][n_lines]  (eta*, chi*, a0, 1/dlamD)
   const float4* vel;                 // [n_active][cps]           (vx, vy, vz, max|v|)
   const float* vtab;                 // [n_batch][n_active][cps][n_vbins][DEX_REC]

@@ -24,6 +24,7 @@ struct dex_mips {
   float thr_eta = 0, thr_chi = 0, tau_gate = -1;
   // owned device memory
   float* d_store = nullptr;
+  float* d_mrec = nullptr;
   float4* d_line = nullptr;
   float4* d_vel = nullptr;
   float* d_vtab = nullptr;
@@ -47,7 +48,7 @@ dex_status dex_launch_pack_levels(dex_mips* m, cudaStream_t st);
 dex_status dex_launch_level_data(const dex_mips* m, int chain, int level, float* d_dense, cudaStream_t st);
 // march.cu
 dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                            unsigned long long* d_seg, int lanes_per_ray, bool flat, bool tile, cudaStream_t st);
+                            unsigned long long* d_seg, int lanes_per_ray, bool tile, cudaStream_t st);
 dex_status dex_launch_capture(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays,
                               const dex_visit_capture* cap, int* d_overflow, cudaStream_t st);
 dex_status dex_launch_reduce_j(const DexRaysDev& rays, int n_lambda, const float* d_I, float* d_J, cudaStream_t st);

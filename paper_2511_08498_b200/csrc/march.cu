@@ -43,16 +43,97 @@ __device__ __forceinline__ void dex_accumulate(float eta, float chi, float hds, 
   T *= e;
 }
 
+// The same for two wavelengths at once with Blackwell's packed fp32 pipe (FFMA2 / FMUL2): the kernel is
+// instruction-issue bound (profiles/), and a packed instruction does two wavelengths per issue slot.
+__device__ __forceinline__ void dex_accumulate2(float2 eta, float2 chi, float2 hds2, float2 hl2, float2& I, float2& T) {
+  const float2 tau = __fmul2_rn(chi, hds2);
+  const float2 y = __fmul2_rn(chi, hl2);
+  float2 e;
+  e.x = dex_ex2(y.x);
+  e.y = dex_ex2(y.y);
+  float2 p = make_float2(-1.0f / 5040.0f, -1.0f / 5040.0f);
+  p = __ffma2_rn(p, tau, make_float2(1.0f / 720.0f, 1.0f / 720.0f));
+  p = __ffma2_rn(p, tau, make_float2(-1.0f / 120.0f, -1.0f / 120.0f));
+  p = __ffma2_rn(p, tau, make_float2(1.0f / 24.0f, 1.0f / 24.0f));
+  p = __ffma2_rn(p, tau, make_float2(-1.0f / 6.0f, -1.0f / 6.0f));
+  p = __ffma2_rn(p, tau, make_float2(0.5f, 0.5f));
+  p = __ffma2_rn(p, make_float2(-tau.x, -tau.y), make_float2(1.0f, 1.0f));
+  float2 r;
+  r.x = dex_rcp(fmaxf(tau.x, 0.25f));
+  r.y = dex_rcp(fmaxf(tau.y, 0.25f));
+  const float2 q = __fmul2_rn(__ffma2_rn(e, make_float2(-1.0f, -1.0f), make_float2(1.0f, 1.0f)), r);
+  float2 E;
+  E.x = (tau.x < 0.25f) ? p.x : q.x;
+  E.y = (tau.y < 0.25f) ? p.y : q.y;
+  I = __ffma2_rn(T, __fmul2_rn(__fmul2_rn(eta, hds2), E), I);
+  T = __fmul2_rn(T, e);
+}
+
+// S-form (ISO march records, S = eta/chi):  I += T * S * omE,  omE = 1 - e^{-tau}; below tau = 0.25 omE is
+// the degree-7 Taylor polynomial tau (1 - tau/2 + ... - tau^6/5040) (truncation < 1.6e-9 relative).
+__device__ __forceinline__ void dex_accumulate_S(float S, float chi, float hds, float hl, float& I, float& T) {
+  const float tau = chi * hds;
+  const float e = dex_ex2(chi * hl);
+  float p = -1.0f / 5040.0f;
+  p = fmaf(p, tau, 1.0f / 720.0f);
+  p = fmaf(p, tau, -1.0f / 120.0f);
+  p = fmaf(p, tau, 1.0f / 24.0f);
+  p = fmaf(p, tau, -1.0f / 6.0f);
+  p = fmaf(p, tau, 0.5f);
+  p = fmaf(-p, tau, 1.0f);
+  const float omE = (tau < 0.25f) ? p * tau : 1.0f - e;
+  I = fmaf(T, S * omE, I);
+  T *= e;
+}
+
 template <int LPT>
-__device__ __forceinline__ void dex_load_rec(const float* __restrict__ rec, float (&eta)[LPT], float (&chi)[LPT]) {
+__device__ __forceinline__ void dex_accumulate_all_S(const float (&S)[LPT], const float (&chi)[LPT], float hds,
+                                                     float (&I)[LPT], float (&T)[LPT]) {
+  const float hl = hds * -1.4426950408889634f;
+#pragma unroll
+  for (int i = 0; i < LPT; ++i) dex_accumulate_S(S[i], chi[i], hds, hl, I[i], T[i]);
+}
+
+template <int LPT>
+__device__ __forceinline__ void dex_accumulate_all(const float (&eta)[LPT], const float (&chi)[LPT], float hds,
+                                                   float (&I)[LPT], float (&T)[LPT]) {
+  const float hl = hds * -1.4426950408889634f;
   if (LPT == 1) {
-    const float2 v = __ldg(reinterpret_cast<const float2*>(rec));
-    eta[0] = v.x; chi[0] = v.y;
+    dex_accumulate(eta[0], chi[0], hds, hl, I[0], T[0]);
   } else {
+    const float2 hds2 = make_float2(hds, hds), hl2 = make_float2(hl, hl);
 #pragma unroll
     for (int i = 0; i < LPT / 2; ++i) {
-      const float4 v = __ldg(reinterpret_cast<const float4*>(rec) + i);
-      eta[2 * i] = v.x; chi[2 * i] = v.y; eta[2 * i + 1] = v.z; chi[2 * i + 1] = v.w;
+      float2 Ii = make_float2(I[2 * i], I[2 * i + 1]), Ti = make_float2(T[2 * i], T[2 * i + 1]);
+      dex_accumulate2(make_float2(eta[2 * i], eta[2 * i + 1]), make_float2(chi[2 * i], chi[2 * i + 1]), hds2, hl2, Ii, Ti);
+      I[2 * i] = Ii.x; I[2 * i + 1] = Ii.y;
+      T[2 * i] = Ti.x; T[2 * i + 1] = Ti.y;
+    }
+  }
+}
+
+// record layout: chi[0..7] then eta[0..7]; this lane owns wavelengths sub*LPT .. sub*LPT+LPT-1
+template <int LPT>
+__device__ __forceinline__ void dex_load_rec(const float* __restrict__ rec, int sub, float (&eta)[LPT], float (&chi)[LPT]) {
+  const float* pc = rec + sub * LPT;
+  const float* pe = rec + DEX_W + sub * LPT;
+  if (LPT == 1) {
+    chi[0] = __ldg(pc);
+    eta[0] = __ldg(pe);
+  } else if (LPT == 2) {
+    const float2 c = __ldg(reinterpret_cast<const float2*>(pc));
+    const float2 e = __ldg(reinterpret_cast<const float2*>(pe));
+    chi[0] = c.x; chi[1] = c.y; eta[0] = e.x; eta[1] = e.y;
+  } else {
+#pragma unroll
+    for (int i = 0; i < LPT / 4; ++i) {
+      const float4 c = __ldg(reinterpret_cast<const float4*>(pc) + i);
+      chi[4 * i] = c.x; chi[4 * i + 1] = c.y; chi[4 * i + 2] = c.z; chi[4 * i + 3] = c.w;
+    }
+#pragma unroll
+    for (int i = 0; i < LPT / 4; ++i) {
+      const float4 e = __ldg(reinterpret_cast<const float4*>(pe) + i);
+      eta[4 * i] = e.x; eta[4 * i + 1] = e.y; eta[4 * i + 2] = e.z; eta[4 * i + 3] = e.w;
     }
   }
 }
@@ -62,8 +143,8 @@ template <int D, int VAR, int LPT>
 __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_base, int cell, int sub,
                                              const float* om, const double* lam, const int* al,
                                              float (&eta)[LPT], float (&chi)[LPT]) {
-  if (VAR == DEX_ISO) {
-    dex_load_rec<LPT>(M.store + (batch_base + (size_t)cell) * DEX_REC + sub * LPT * 2, eta, chi);
+  if (VAR == DEX_ISO) {   // march records: eta[] receives S = eta/chi
+    dex_load_rec<LPT>(M.mrec + (batch_base + (size_t)cell) * DEX_REC, sub, eta, chi);
     return;
   }
   // projected velocity of the cell's box-filtered bulk velocity, fp64 (DESIGN.md R-vel)
@@ -83,10 +164,10 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
       i0 = min((int)floor(f), nvb - 2);
       w = (float)(f - (double)i0);
     }
-    const float* r0 = M.vtab + ((batch_base + (size_t)cell) * nvb + i0) * DEX_REC + sub * LPT * 2;
+    const float* r0 = M.vtab + ((batch_base + (size_t)cell) * nvb + i0) * DEX_REC;
     float e1[LPT], c1[LPT];
-    dex_load_rec<LPT>(r0, eta, chi);
-    dex_load_rec<LPT>(r0 + DEX_REC, e1, c1);
+    dex_load_rec<LPT>(r0, sub, eta, chi);
+    dex_load_rec<LPT>(r0 + DEX_REC, sub, e1, c1);
 #pragma unroll
     for (int i = 0; i < LPT; ++i) {
       eta[i] = fmaf(w, e1[i], (1.0f - w) * eta[i]);
@@ -95,7 +176,7 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
     return;
   }
   // Core-and-Voigt / Classic: background + sum over the active lines (eqs. 10-11)
-  dex_load_rec<LPT>(M.store + (batch_base + (size_t)cell) * DEX_REC + sub * LPT * 2, eta, chi);
+  dex_load_rec<LPT>(M.store + (batch_base + (size_t)cell) * DEX_REC, sub, eta, chi);
   double de[LPT], dc[LPT];
 #pragma unroll
   for (int i = 0; i < LPT; ++i) { de[i] = (double)eta[i]; dc[i] = (double)chi[i]; }
@@ -118,10 +199,9 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
   for (int i = 0; i < LPT; ++i) { eta[i] = (float)de[i]; chi[i] = (float)dc[i]; }
 }
 
-// Each lane group owns one probe and walks through all its directions as one flattened stream of
-// HDDA events ("while-while"): the inner loop advances the ray -- or finishes it and sets up the next
-// direction -- until a segment has to be integrated; the integrate block then runs with every lane
-// that still has work.  No lane waits for the longest ray of a direction.
+// Each lane group owns one probe and loops over the quadrature directions, accumulating J in registers.
+// (A flattened variant in which a lane starts its next direction as soon as its ray ends was measured
+// and rejected: it halves the thread efficiency, profiles/r01_march_experiments.md.)
 #ifndef DEX_MARCH_THREADS
 #define DEX_MARCH_THREADS 128
 #endif
@@ -129,7 +209,7 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
 #define DEX_MARCH_MINB 7
 #endif
 
-template <int D, int VAR, int LPR, bool FUSE_J, bool FLAT>
+template <int D, int VAR, int LPR, bool FUSE_J>
 __global__ void __launch_bounds__(DEX_MARCH_THREADS, DEX_MARCH_MINB)
 dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ perm,
                  float* __restrict__ out, unsigned long long* __restrict__ seg_count) {
@@ -160,53 +240,7 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
     for (int i = 0; i < LPT; ++i) { J[i] = 0.0f; I[i] = 0.0f; T[i] = 1.0f; }
     float om[D];
     DexRay2<D> ray;
-    if (FLAT) {
-      int k = -1;
-      bool alive = false;
-      for (;;) {
-        bool emit = false;
-        int cell = 0;
-        float ds = 0.0f;
-        while (!emit) {
-          if (!alive) {
-            if (k >= 0) {
-              // ray k is complete: boundary term, then the angular quadrature or the I store
-              if (R.i0 != nullptr) {
-  #pragma unroll
-                for (int i = 0; i < LPT; ++i)
-                  I[i] = fmaf(T[i], __ldg(R.i0 + (size_t)k * M.n_lambda + lam_off + i), I[i]);
-              }
-              if (FUSE_J) {
-                const float wk = __ldg(R.weights + k);
-  #pragma unroll
-                for (int i = 0; i < LPT; ++i) J[i] = fmaf(wk, I[i], J[i]);
-              } else {
-                float* dst = out + ((size_t)gid * R.n_dirs + k) * M.n_lambda + lam_off;
-  #pragma unroll
-                for (int i = 0; i < LPT; ++i) dst[i] = I[i];
-              }
-            }
-            ++k;
-            if (k >= R.n_dirs) break;
-  #pragma unroll
-            for (int a = 0; a < D; ++a) om[a] = __ldg(R.dirs + k * D + a);
-  #pragma unroll
-            for (int i = 0; i < LPT; ++i) { I[i] = 0.0f; T[i] = 1.0f; }
-            alive = dex_ray_init2<D>(ray, G, M, binfo, probe, om);
-            continue;
-          }
-          alive = dex_ray_step2<D>(ray, G, M, binfo, emit, cell, ds);
-        }
-        if (!emit) break;
-        ++nseg;
-        const float hds = G.h * ds;
-        const float hl = hds * -1.4426950408889634f;
-        float eta[LPT], chi[LPT];
-        dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, lam, al, eta, chi);
-  #pragma unroll
-        for (int i = 0; i < LPT; ++i) dex_accumulate(eta[i], chi[i], hds, hl, I[i], T[i]);
-      }
-    } else {
+    {
       // one direction at a time: the lanes of a warp trace the same direction together (coherent
       // fetches); inside a direction, lanes skip ahead to their next segment before integrating
       for (int k = 0; k < R.n_dirs; ++k) {
@@ -225,11 +259,10 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
           if (emit) {
             ++nseg;
             const float hds = G.h * ds;
-            const float hl = hds * -1.4426950408889634f;
             float eta[LPT], chi[LPT];
             dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, lam, al, eta, chi);
-#pragma unroll
-            for (int i = 0; i < LPT; ++i) dex_accumulate(eta[i], chi[i], hds, hl, I[i], T[i]);
+            if (VAR == DEX_ISO) dex_accumulate_all_S<LPT>(eta, chi, hds, I, T);
+            else dex_accumulate_all<LPT>(eta, chi, hds, I, T);
           }
         }
         if (R.i0 != nullptr) {
@@ -370,7 +403,7 @@ __global__ void dex_reduce_j_kernel(long long n_probes, int n_dirs, int n_lambda
 
 template <int D, int VAR, int LPR>
 dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                          unsigned long long* d_seg, bool flat, const int* perm, cudaStream_t st) {
+                          unsigned long long* d_seg, const int* perm, cudaStream_t st) {
   const int threads = DEX_MARCH_THREADS;
   const long long probes_per_block = threads / LPR;
   const long long gx = (rays.n_probes + probes_per_block - 1) / probes_per_block;
@@ -380,14 +413,10 @@ dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev
     return DEX_ERR_UNSUPPORTED;
   }
   dim3 grid((unsigned)gx, (unsigned)m->n_batch, 1);
-  if (fuse_j && flat)
-    dex_march_kernel<D, VAR, LPR, true, true><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
-  else if (fuse_j)
-    dex_march_kernel<D, VAR, LPR, true, false><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
-  else if (flat)
-    dex_march_kernel<D, VAR, LPR, false, true><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
+  if (fuse_j)
+    dex_march_kernel<D, VAR, LPR, true><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
   else
-    dex_march_kernel<D, VAR, LPR, false, false><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
+    dex_march_kernel<D, VAR, LPR, false><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
   dex_count_launch();
   DEX_CUDA_CHECK(cudaGetLastError());
   return DEX_OK;
@@ -395,12 +424,12 @@ dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev
 
 template <int D, int VAR>
 dex_status launch_march_v(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                          unsigned long long* d_seg, int lpr, bool flat, const int* perm, cudaStream_t st) {
+                          unsigned long long* d_seg, int lpr, const int* perm, cudaStream_t st) {
   switch (lpr) {
-    case 8: return launch_march_t<D, VAR, 8>(g, m, rays, d_out, fuse_j, d_seg, flat, perm, st);
-    case 4: return launch_march_t<D, VAR, 4>(g, m, rays, d_out, fuse_j, d_seg, flat, perm, st);
-    case 2: return launch_march_t<D, VAR, 2>(g, m, rays, d_out, fuse_j, d_seg, flat, perm, st);
-    case 1: return launch_march_t<D, VAR, 1>(g, m, rays, d_out, fuse_j, d_seg, flat, perm, st);
+    case 8: return launch_march_t<D, VAR, 8>(g, m, rays, d_out, fuse_j, d_seg, perm, st);
+    case 4: return launch_march_t<D, VAR, 4>(g, m, rays, d_out, fuse_j, d_seg, perm, st);
+    case 2: return launch_march_t<D, VAR, 2>(g, m, rays, d_out, fuse_j, d_seg, perm, st);
+    case 1: return launch_march_t<D, VAR, 1>(g, m, rays, d_out, fuse_j, d_seg, perm, st);
   }
   dex_set_error("lanes per ray must be 1, 2, 4 or 8");
   return DEX_ERR_INVALID_ARG;
@@ -408,12 +437,12 @@ dex_status launch_march_v(const dex_grid* g, const dex_mips* m, const DexRaysDev
 
 template <int D>
 dex_status launch_march_d(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                          unsigned long long* d_seg, int lpr, bool flat, const int* perm, cudaStream_t st) {
+                          unsigned long long* d_seg, int lpr, const int* perm, cudaStream_t st) {
   switch (m->variant) {
-    case DEX_ISO: return launch_march_v<D, DEX_ISO>(g, m, rays, d_out, fuse_j, d_seg, lpr, flat, perm, st);
-    case DEX_VELINTERP: return launch_march_v<D, DEX_VELINTERP>(g, m, rays, d_out, fuse_j, d_seg, lpr, flat, perm, st);
+    case DEX_ISO: return launch_march_v<D, DEX_ISO>(g, m, rays, d_out, fuse_j, d_seg, lpr, perm, st);
+    case DEX_VELINTERP: return launch_march_v<D, DEX_VELINTERP>(g, m, rays, d_out, fuse_j, d_seg, lpr, perm, st);
     case DEX_CAV:
-    case DEX_CLASSIC: return launch_march_v<D, DEX_CAV>(g, m, rays, d_out, fuse_j, d_seg, lpr, flat, perm, st);
+    case DEX_CLASSIC: return launch_march_v<D, DEX_CAV>(g, m, rays, d_out, fuse_j, d_seg, lpr, perm, st);
   }
   dex_set_error("unknown variant");
   return DEX_ERR_INVALID_ARG;
@@ -458,13 +487,13 @@ static dex_status tile_probes_t(const dex_grid* g, const DexRaysDev& rays, int**
 }
 
 dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                            unsigned long long* d_seg, int lanes_per_ray, bool flat, bool tile, cudaStream_t st) {
+                            unsigned long long* d_seg, int lanes_per_ray, bool tile, cudaStream_t st) {
   int* d_perm = nullptr;
   dex_status s = DEX_OK;
   if (tile) s = (g->desc.ndim == 2) ? tile_probes_t<2>(g, rays, &d_perm, st) : tile_probes_t<3>(g, rays, &d_perm, st);
   if (s == DEX_OK) {
-    if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, flat, d_perm, st);
-    else s = launch_march_d<3>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, flat, d_perm, st);
+    if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, d_perm, st);
+    else s = launch_march_d<3>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, d_perm, st);
   }
   if (d_perm) cudaFreeAsync(d_perm, st);
   return s;

@@ -121,10 +121,9 @@ __global__ void gather_spec_kernel(const BuildCtx X, const float* __restrict__ e
   const int b = (int)(r / X.G.n_active);
   const size_t v = voxel_of<D>(X.G, X.active_bricks[slot], cell);
   const size_t src = v * X.M.n_lambda + (size_t)b * DEX_W + j;
-  float2 o;
-  o.x = eta[src];
-  o.y = chi[src];
-  reinterpret_cast<float2*>(X.store)[(((size_t)b * X.G.n_active + slot) * X.M.cps + cell) * DEX_W + j] = o;
+  const size_t rec = ((size_t)b * X.G.n_active + slot) * X.M.cps + cell;
+  X.store[dex_rec_eta(rec, j)] = eta[src];
+  X.store[dex_rec_chi(rec, j)] = chi[src];
 }
 
 // ---- a3: level m from level m-1 for the spectrum pair; STATS = ISO cell test -----------------------
@@ -145,24 +144,42 @@ __global__ void reduce_spec_kernel(const BuildCtx X, int m) {
   int pc[3];
   cell_coords<D>(cell, nbm, pc);
   const size_t base = ((size_t)b * X.G.n_active + slot) * X.M.cps;
-  float2* st = reinterpret_cast<float2*>(X.store);
   double e[NC], c[NC];
 #pragma unroll
   for (int ch = 0; ch < NC; ++ch) {
-    const float2 v = st[(base + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc)) * DEX_W + j];
-    e[ch] = (double)v.x;
-    c[ch] = (double)v.y;
+    const size_t rec = base + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc);
+    e[ch] = (double)X.store[dex_rec_eta(rec, j)];
+    c[ch] = (double)X.store[dex_rec_chi(rec, j)];
   }
   double se = e[0], sc = c[0];
 #pragma unroll
   for (int ch = 1; ch < NC; ++ch) { se = se + e[ch]; sc = sc + c[ch]; }
-  float2 o;
-  o.x = (float)(se * (1.0 / NC));
-  o.y = (float)(sc * (1.0 / NC));
-  st[(base + X.M.lvloff[m] + cell) * DEX_W + j] = o;
+  X.store[dex_rec_eta(base + X.M.lvloff[m] + cell, j)] = (float)(se * (1.0 / NC));
+  X.store[dex_rec_chi(base + X.M.lvloff[m] + cell, j)] = (float)(sc * (1.0 / NC));
   if (STATS) {
     if (!cell_passes<NC>(e, c, X)) X.fail[((size_t)b * X.G.n_active + slot) * (X.M.max_level + 1) + m] = 1;
   }
+}
+
+// ---- ISO march records --------------------------------------------------------------------------------
+// The march integrates  I += T * eta h ds E(tau),  E = (1 - e^{-tau})/tau.  With S = eta/chi this is
+// I += T * S * (1 - e^{-tau}), which needs no reciprocal in the inner loop (one MUFU instead of two per
+// wavelength).  Records hold (chi', S) for every level of the pyramid; the pyramid itself keeps (eta, chi)
+// exactly (it is what the VLM test and the validation accessors see).  chi < 2^-100 (including chi = 0, a
+// pure emitter: I_out = I_in + eta h ds) is represented by chi' = 2^-100, S = eta 2^100: then tau' is
+// ~1e-30 h ds, e^{-tau'} = 1 and S tau' = eta h ds, so the E(0) = 1 limit of DESIGN.md is kept.
+__global__ void make_march_records_kernel(const float* __restrict__ store, float* __restrict__ mrec, long long n_rec) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_rec * DEX_W) return;
+  const int j = (int)(i % DEX_W);
+  const size_t r = (size_t)(i / DEX_W);
+  const float eta = store[dex_rec_eta(r, j)], chi = store[dex_rec_chi(r, j)];
+  const float tiny = 7.888609052210118e-31f;   // 2^-100
+  float c = chi, S;
+  if (chi < tiny) { c = tiny; S = eta * 1.2676506002282294e30f; }   // 2^100, exact scaling
+  else S = eta / chi;
+  mrec[dex_rec_chi(r, j)] = c;
+  mrec[dex_rec_eta(r, j)] = S;
 }
 
 // ---- line parameters and velocity: level 0 gather and box filter ------------------------------------
@@ -275,12 +292,12 @@ __global__ void cav_test_kernel(const BuildCtx X, int m) {
   int pc[3];
   cell_coords<D>(cell, nbm, pc);
   const double lam = (double)X.M.lam[b * DEX_W + j];
-  const float2* st = reinterpret_cast<const float2*>(X.store);
   double e[NC], c[NC];
 #pragma unroll
   for (int ch = 0; ch < NC; ++ch) {
     const size_t cc = (size_t)slot * X.M.cps + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc);
-    const float2 bg = st[(((size_t)b * X.G.n_active) * X.M.cps + cc) * DEX_W + j];
+    const size_t rb = ((size_t)b * X.G.n_active) * X.M.cps + cc;
+    const float2 bg = make_float2(X.store[dex_rec_eta(rb, j)], X.store[dex_rec_chi(rb, j)]);
     const double Vc = (double)X.vel[cc].w;
     double vd[DEX_NLINES];
     for (int q = 0; q < DEX_NLINES; ++q) {
@@ -315,17 +332,16 @@ __global__ void vtab_level0_kernel(const BuildCtx X) {
   const size_t cc = (size_t)slot * X.M.cps + cell;
   const double V = (double)X.vel[cc].w;
   const double vk = -V + (2.0 * V) * ((double)k / (double)(n - 1));
-  const float2 bg = reinterpret_cast<const float2*>(X.store)[(((size_t)b * X.G.n_active) * X.M.cps + cc) * DEX_W + j];
+  const size_t rb = ((size_t)b * X.G.n_active) * X.M.cps + cc;
   double e, c;
-  line_sum(X, cc, b, (double)X.M.lam[b * DEX_W + j], (double)bg.x, (double)bg.y, &vk, false, e, c);
-  float2 o;
-  o.x = (float)e;
-  o.y = (float)c;
-  reinterpret_cast<float2*>(X.vtab)[((((size_t)b * X.G.n_active) * X.M.cps + cc) * n + k) * DEX_W + j] = o;
+  line_sum(X, cc, b, (double)X.M.lam[b * DEX_W + j], (double)X.store[dex_rec_eta(rb, j)],
+           (double)X.store[dex_rec_chi(rb, j)], &vk, false, e, c);
+  X.vtab[dex_rec_eta(rb * n + k, j)] = (float)e;
+  X.vtab[dex_rec_chi(rb * n + k, j)] = (float)c;
 }
 
 // table of one cell interpolated at velocity v on its grid [-V, V], clamped
-__device__ __forceinline__ void vtab_interp(const float2* __restrict__ tab /*[n][W]*/, int n, int j, double V, double v,
+__device__ __forceinline__ void vtab_interp(const float* __restrict__ tab /*[n] records*/, int n, int j, double V, double v,
                                             double& e, double& c) {
   int i0 = 0;
   double w = 0.0;
@@ -335,10 +351,8 @@ __device__ __forceinline__ void vtab_interp(const float2* __restrict__ tab /*[n]
     i0 = min((int)floor(f), n - 2);
     w = f - (double)i0;
   }
-  const float2 t0 = tab[(size_t)i0 * DEX_W + j];
-  const float2 t1 = tab[(size_t)(i0 + 1) * DEX_W + j];
-  e = (1.0 - w) * (double)t0.x + w * (double)t1.x;
-  c = (1.0 - w) * (double)t0.y + w * (double)t1.y;
+  e = (1.0 - w) * (double)tab[dex_rec_eta(i0, j)] + w * (double)tab[dex_rec_eta(i0 + 1, j)];
+  c = (1.0 - w) * (double)tab[dex_rec_chi(i0, j)] + w * (double)tab[dex_rec_chi(i0 + 1, j)];
 }
 
 // level m: parent bin = mean over children of the child's table at the parent's bin velocity (R-vel)
@@ -365,19 +379,17 @@ __global__ void vtab_reduce_kernel(const BuildCtx X, int m) {
   const size_t bbase = ((size_t)b * X.G.n_active) * X.M.cps;
   const double Vp = (double)X.vel[sbase + X.M.lvloff[m] + cell].w;
   const double vk = -Vp + (2.0 * Vp) * ((double)k / (double)(n - 1));
-  const float2* vt = reinterpret_cast<const float2*>(X.vtab);
   double se = 0, sc = 0;
 #pragma unroll
   for (int ch = 0; ch < NC; ++ch) {
     const size_t cc = sbase + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc);
     double e, c;
-    vtab_interp(vt + (bbase + cc) * n * DEX_W, n, j, (double)X.vel[cc].w, vk, e, c);
+    vtab_interp(X.vtab + (bbase + cc) * n * DEX_REC, n, j, (double)X.vel[cc].w, vk, e, c);
     if (ch == 0) { se = e; sc = c; } else { se = se + e; sc = sc + c; }
   }
-  float2 o;
-  o.x = (float)(se * (1.0 / NC));
-  o.y = (float)(sc * (1.0 / NC));
-  reinterpret_cast<float2*>(X.vtab)[((bbase + sbase + X.M.lvloff[m] + cell) * n + k) * DEX_W + j] = o;
+  const size_t ro = (bbase + sbase + X.M.lvloff[m] + cell) * n + k;
+  X.vtab[dex_rec_eta(ro, j)] = (float)(se * (1.0 / NC));
+  X.vtab[dex_rec_chi(ro, j)] = (float)(sc * (1.0 / NC));
 }
 
 // VELINTERP cell test: children = rest-frame (v = 0) value of the level m-1 tables
@@ -400,12 +412,11 @@ __global__ void vtab_test_kernel(const BuildCtx X, int m) {
   cell_coords<D>(cell, nbm, pc);
   const size_t sbase = (size_t)slot * X.M.cps;
   const size_t bbase = ((size_t)b * X.G.n_active) * X.M.cps;
-  const float2* vt = reinterpret_cast<const float2*>(X.vtab);
   double e[NC], c[NC];
 #pragma unroll
   for (int ch = 0; ch < NC; ++ch) {
     const size_t cc = sbase + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc);
-    vtab_interp(vt + (bbase + cc) * n * DEX_W, n, j, (double)X.vel[cc].w, 0.0, e[ch], c[ch]);
+    vtab_interp(X.vtab + (bbase + cc) * n * DEX_REC, n, j, (double)X.vel[cc].w, 0.0, e[ch], c[ch]);
   }
   if (!cell_passes<NC>(e, c, X)) X.fail[((size_t)b * X.G.n_active + slot) * (X.M.max_level + 1) + m] = 1;
 }
@@ -471,7 +482,8 @@ __global__ void level_data_kernel(const BuildCtx X, int chain, int m, int width 
   float v = 0.0f;
   if (chain == DEX_CHAIN_ETA || chain == DEX_CHAIN_CHI) {           // width = n_lambda
     const int b = q / DEX_W, j = q % DEX_W;
-    v = X.store[((((size_t)b * X.G.n_active) * X.M.cps + cc) * DEX_W + j) * 2 + (chain == DEX_CHAIN_CHI)];
+    const size_t rec = ((size_t)b * X.G.n_active) * X.M.cps + cc;
+    v = X.store[(chain == DEX_CHAIN_CHI) ? dex_rec_chi(rec, j) : dex_rec_eta(rec, j)];
   } else if (chain == DEX_CHAIN_VEL) {                               // width = 4
     v = reinterpret_cast<const float*>(X.vel)[cc * 4 + q];
   } else if (chain == DEX_CHAIN_LINE) {                              // width = n_lines * 4
@@ -481,7 +493,8 @@ __global__ void level_data_kernel(const BuildCtx X, int chain, int m, int width 
     const int lam = (q >> 1) % X.M.n_lambda;
     const int k = (q >> 1) / X.M.n_lambda;
     const int b = lam / DEX_W, j = lam % DEX_W;
-    v = X.vtab[((((((size_t)b * X.G.n_active) * X.M.cps + cc) * X.M.n_vbins + k) * DEX_W) + j) * 2 + f];
+    const size_t rec = (((size_t)b * X.G.n_active) * X.M.cps + cc) * X.M.n_vbins + k;
+    v = X.vtab[f ? dex_rec_chi(rec, j) : dex_rec_eta(rec, j)];
   }
   dense[gc * width + q] = v;
 }
@@ -552,6 +565,11 @@ dex_status build_t(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st) {
       cav_test_kernel<D><<<blocks_for(nspec, T), T, 0, st>>>(X, lv);
       dex_count_launch();
     }
+  }
+  if (iso) {
+    const long long n_rec = (long long)m->n_batch * A * X.M.cps;
+    make_march_records_kernel<<<blocks_for(n_rec * DEX_W, T), T, 0, st>>>(m->d_store, m->d_mrec, n_rec);
+    dex_count_launch();
   }
   select_levels_kernel<<<blocks_for((long long)m->n_batch * X.G.n_bricks, T), T, 0, st>>>(X, m->d_levels);
   dex_count_launch();

@@ -185,6 +185,17 @@ def test_edge_cases(P):
     with pytest.raises(P.DexError) as ei:
         P.pipeline.formal_solution(dw, grid, mips, capture_batch=0, want_I=False, room=3)
     assert ei.value.status == P.binding.DEX_ERR_CAPACITY
+    # pure emitters (chi = 0, eta > 0: I_out = I_in + eta h ds) next to absorbing and to void cells
+    rng = np.random.default_rng(12)
+    chi = rng.uniform(0.0, 0.3, size=(64, 64, 8))
+    eta = rng.uniform(0.0, 1.0, size=(64, 64, 8))
+    chi[:, 20:40] = 0.0
+    eta[30:50, 30:60] = 0.0
+    chi[5:9, 5:9] = 1e-36           # far below 2^-100: treated as chi = 0 by the march records
+    wl4 = iso_workload((64, 64), 16, eta, chi, rng.uniform(0, 64, size=(200, 2)), dirs_2d(12)[0], h=1.7)
+    M4 = orc.build_mips(wl4)
+    dw, grid, mips = _build(P, wl4)
+    _solve_and_compare(P, wl4, M4, dw, grid, mips, lanes=(1, 8))
     # argument errors
     with pytest.raises(P.DexError):
         P.pipeline.build_mips(dw, grid, max_level=5)
