@@ -324,10 +324,13 @@ def main():
         march_avg_ms = march_ms / max(1, march_n)
         achieved = algo_bytes / (march_avg_ms * 1e-3) / 1e9 if march_avg_ms > 0 else 0.0
         traffic = None
-        tp = os.path.join(ROOT, "profiles", f"traffic_{wl.name}.json")
+        tp = os.path.join(ROOT, "profiles", "traffic.csv")      # ncu dram__bytes_{read,write}.sum per launch
         if os.path.exists(tp):
+            import csv
             with open(tp) as f:
-                traffic = json.load(f).get("dram_bytes_per_launch")
+                for row in csv.DictReader(f):
+                    if row["workload"] == wl.name:
+                        traffic = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
