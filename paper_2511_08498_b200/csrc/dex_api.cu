@@ -283,6 +283,7 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
   for (int l = 0; l < d.n_lines; ++l) d.lambda0[l] = desc->h_lambda0[l];
   dex_weideman_coefficients(d.wei_c, &d.wei_L);
   const size_t A = (size_t)grid->n_active;
+  if ((long long)A * cps >= (1LL << 27)) { dex_set_error("too many pyramid cells per batch (brick word holds 27 bits)"); delete m; return DEX_ERR_SHAPE; }
   cudaStream_t st = (cudaStream_t)stream;
   dex_status s = DEX_OK;
   m->store_floats = (size_t)n_batch * A * cps * DEX_REC;
@@ -315,6 +316,7 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
     d.binfo = m->d_binfo;
     d.store = m->d_store;
     d.mrec = m->d_mrec;
+    d.mplane = m->store_floats / 2;
     d.line = m->d_line;
     d.vel = m->d_vel;
     d.vtab = m->d_vtab;

@@ -34,12 +34,14 @@ struct DexMipsDev {
   int max_level;
   int bits, per_word, words_per_batch;
   const unsigned long long* packed;  // [n_batch][words_per_batch]  PAPER.md:162 packed block states (exported)
-  const int* binfo;                  // [n_batch][n_bricks]  (slot << 4) | (level + 1): what the march reads
+  const int* binfo;                  // [n_batch][n_bricks]  ((slot * cps + lvloff[level]) << 4) | (level + 1), 0 = empty:
+                                     // the one word the march reads per brick crossing
   int cps;                           // cells per slot (all levels)
   int lvloff[DEX_MAXLEV];            // first cell of level m inside a slot
   const float* store;                // [n_batch][n_active][cps][DEX_REC]  chi|eta (ISO) or background
-  const float* mrec;                 // ISO march records, same shape as store: chi'|S with S = eta/chi (see
-                                     // make_march_records_kernel); what the ISO march reads
+  const float* mrec;                 // ISO march records (make_march_records_kernel), what the ISO march reads: two planes
+  size_t mplane;                     // [2][n_batch][n_active][cps][DEX_W], plane 0 chi log2(e), plane 1 S = eta/chi;
+                                     // mplane = floats per plane
   const float4* line;                // [n_active][cps][n_lines]  (eta*, chi*, a0, 1/dlamD)
   const float4* vel;                 // [n_active][cps]           (vx, vy, vz, max|v|)
   const float* vtab;                 // [n_batch][n_active][cps][n_vbins][DEX_REC]
@@ -64,25 +66,6 @@ struct DexRaysDev {
 // ---- exact (uncontracted) fp32 helpers -------------------------------------------------
 __device__ __forceinline__ float dex_tplane(int k, float inv, float off) {
   return __fmaf_rn((float)k, inv, off);  // T2
-}
-
-template <int D>
-struct DexRay {
-  float o[D], d[D], inv[D], off[D];
-  float tn[D];
-  int c[D];
-  int m, size, slot;
-  float t;
-};
-
-__device__ __forceinline__ int dex_brick_level(const DexMipsDev& M, int batch, int bi) {
-  int q, r;
-  if (M.bits == 3) { q = bi / 21; r = bi - q * 21; }
-  else if (M.bits == 2) { q = bi >> 5; r = bi & 31; }
-  else if (M.bits == 1) { q = bi >> 6; r = bi & 63; }
-  else { q = bi / M.per_word; r = bi - q * M.per_word; }
-  unsigned long long w = __ldg(M.packed + (size_t)batch * M.words_per_batch + q);
-  return (int)((w >> (r * M.bits)) & ((1ull << M.bits) - 1ull)) - 1;
 }
 
 // plane (a,k) counts as crossed at the event (s, th) iff tplane < th, or == th and a < s  (T5)
@@ -117,232 +100,168 @@ __device__ __forceinline__ int dex_brick_of(const DexGridDev& G, const int* c) {
   return bi;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// HDDA state (Algorithm 1 under the T-rules), arranged so that a crossing that stays inside a brick --
+// the common event -- costs a handful of instructions:
+//   * kf[a] is the coordinate of the exit plane of axis a, kept as a float (integers below 2^24 are exact),
+//     so the plane time is one fma, tn[a] = fma(kf[a], inv[a], off[a]) (T2), and an in-brick crossing of
+//     axis s is  kf[s] += dk[s];  tn[s] = fma(..);  cell += cstep[s].
+//   * tb = min over axes of the time of the BRICK's exit plane.  th < tb (strictly) proves that the plane
+//     being crossed is not a brick face, so the level cannot change and only axis s moves.  Everything
+//     else (brick faces, ties with a brick face, empty bricks, whole-brick cells) takes the general path,
+//     which rebuilds the state from integer coordinates exactly as T3-T5 prescribe.
+//   * zero-direction axes carry inv = 0, off = +INF, so tn = fma(k, 0, INF) = +INF without a select.
+// ---------------------------------------------------------------------------------------------------
+//   * the origin and direction themselves are not kept in registers: only the T5 re-entry into a finer brick
+//     needs them, and reloads them from the (L1-resident) ray arrays.
 template <int D>
-__device__ __forceinline__ void dex_set_planes(DexRay<D>& r) {
+struct DexRay3 {
+  float inv[D], off[D];
+  float tn[D], kf[D], dk[D];  // dk[a] > 0 iff d[a] > 0
+  int cstep[D];
+  int cell;   // record index (slot * cps + lvloff[level] + position) of the current cell; < 0 in an empty brick
+  int sh;     // log2 of the current cell (or empty-brick) size
+  int info;   // brick word of the current brick: (first record of the brick's level << 4) | (level + 1); 0 = empty
+  float t, tb;
+};
+
+// Form the cell of brick word `info` that contains level-0 coordinate x (T3) and everything derived from it.
+template <int D>
+__device__ __forceinline__ void dex_set_cell(DexRay3<D>& r, const DexGridDev& G, const DexMipsDev& M, int info,
+                                             const int* x) {
+  const int m = (info & 15) - 1;
+  const int sh = (m < 0) ? G.logB : m;
+  const int size = 1 << sh, lsh = G.logB - sh, bmask = G.B - 1;
+  r.info = info;
+  r.sh = sh;
+  int idx = 0;
+  float tb = __int_as_float(0x7f800000);
 #pragma unroll
   for (int a = 0; a < D; ++a) {
-    int kp = (r.d[a] > 0.0f) ? r.c[a] + r.size : r.c[a];
-    r.tn[a] = (r.d[a] != 0.0f) ? dex_tplane(kp, r.inv[a], r.off[a]) : __int_as_float(0x7f800000);
+    const bool pos = r.dk[a] > 0.0f;
+    const int c = x[a] & ~(size - 1);
+    r.kf[a] = (float)(c + (pos ? size : 0));
+    r.tn[a] = __fmaf_rn(r.kf[a], r.inv[a], r.off[a]);
+    r.dk[a] = pos ? (float)size : -(float)size;
+    const int bexit = (x[a] & ~bmask) + (pos ? G.B : 0);
+    tb = fminf(tb, __fmaf_rn((float)bexit, r.inv[a], r.off[a]));
+    idx += ((c & bmask) >> sh) << (a * lsh);
+    r.cstep[a] = pos ? (1 << (a * lsh)) : -(1 << (a * lsh));
   }
+  r.tb = tb;
+  r.cell = (m < 0) ? -1 : (info >> 4) + idx;
 }
 
 // T1/T2/T6: trace from the probe outward, o = probe, d = -omega.  Returns false for a probe outside
 // the grid or a null direction (such a ray has no segments).
 template <int D>
-__device__ __forceinline__ bool dex_ray_init(DexRay<D>& r, const DexGridDev& G, const DexMipsDev& M, int batch,
-                                             const float* probe, const float* omega) {
-  bool ok = true, any = false;
-  int x[D];
-#pragma unroll
-  for (int a = 0; a < D; ++a) {
-    r.o[a] = probe[a];
-    r.d[a] = -omega[a];
-    r.inv[a] = 0.0f;
-    r.off[a] = 0.0f;
-    if (r.d[a] != 0.0f) {
-      any = true;
-      r.inv[a] = __fdiv_rn(1.0f, r.d[a]);
-      r.off[a] = __fmul_rn(-r.o[a], r.inv[a]);
-    }
-    x[a] = (int)floorf(r.o[a]);
-    ok = ok && (x[a] >= 0) && (x[a] < G.dims[a]);
-  }
-  r.t = 0.0f;
-  r.m = -1;
-  r.size = 1;
-  r.slot = -1;
-  if (!(ok && any)) return false;
-  int bi = dex_brick_of<D>(G, x);
-  r.m = dex_brick_level(M, batch, bi);
-  r.slot = __ldg(G.slot + bi);
-  r.size = (r.m < 0) ? G.B : (1 << r.m);
-#pragma unroll
-  for (int a = 0; a < D; ++a) r.c[a] = x[a] & ~(r.size - 1);
-  dex_set_planes<D>(r);
-  return true;
-}
-
-// One HDDA event.  On return: `emit` says whether the cell that was just left contributes a segment
-// (non-empty and th > t, T4); em_m / em_c / em_slot / ds describe it.  Returns false when the ray has
-// left the grid (the segment, if any, is still valid).
-template <int D>
-struct DexSeg {
-  bool emit;
-  int m, slot;
-  int c[D];
-  float ds;
-};
-
-template <int D>
-__device__ __forceinline__ bool dex_ray_step(DexRay<D>& r, const DexGridDev& G, const DexMipsDev& M, int batch,
-                                             DexSeg<D>& seg) {
-  // T4: lowest-index axis attaining the minimum
-  int s = 0;
-  float th = r.tn[0];
-  if (r.tn[1] < th) { s = 1; th = r.tn[1]; }
-  if (D == 3) { if (r.tn[D - 1] < th) { s = D - 1; th = r.tn[D - 1]; } }
-  seg.emit = (r.m >= 0) && (th > r.t);
-  seg.m = r.m;
-  seg.slot = r.slot;
-#pragma unroll
-  for (int a = 0; a < D; ++a) seg.c[a] = r.c[a];
-  seg.ds = __fsub_rn(th, r.t);
-  r.t = fmaxf(r.t, th);
-  // T5: cross the plane
-  float ds_ = 0.f; int cs = 0, Ns = 0;
-#pragma unroll
-  for (int a = 0; a < D; ++a) if (a == s) { ds_ = r.d[a]; cs = r.c[a]; Ns = G.dims[a]; }
-  const bool pos = ds_ > 0.0f;
-  const int xs = pos ? cs + r.size : cs - 1;
-  if (xs < 0 || xs >= Ns) return false;
-  if ((xs >> G.logB) == (cs >> G.logB)) {
-    // same brick: same level; only axis s moves
-    const int ncs = pos ? cs + r.size : cs - r.size;
-#pragma unroll
-    for (int a = 0; a < D; ++a)
-      if (a == s) {
-        r.c[a] = ncs;
-        r.tn[a] = dex_tplane(pos ? ncs + r.size : ncs, r.inv[a], r.off[a]);
-      }
-    return true;
-  }
-  // new brick: look up its level (MipLevel, Alg. 1 l.6-8) and re-initialise (l.32-39)
-  int xb[D];
-#pragma unroll
-  for (int a = 0; a < D; ++a) xb[a] = (a == s) ? xs : r.c[a];
-  const int bi = dex_brick_of<D>(G, xb);
-  const int m2 = dex_brick_level(M, batch, bi);
-  const int size2 = (m2 < 0) ? G.B : (1 << m2);
-  if (size2 < r.size) {
-#pragma unroll
-    for (int a = 0; a < D; ++a)
-      if (a != s) xb[a] = dex_fine_coord(r.o[a], r.d[a], r.inv[a], r.off[a], r.c[a], r.size, th, a < s);
-  }
-#pragma unroll
-  for (int a = 0; a < D; ++a) r.c[a] = xb[a] & ~(size2 - 1);
-  r.m = m2;
-  r.size = size2;
-  r.slot = __ldg(G.slot + bi);
-  dex_set_planes<D>(r);
-  return true;
-}
-
-// index of the cell inside its slot: level offset + row-major position at that level
-template <int D>
-__device__ __forceinline__ int dex_cell_in_slot(const DexGridDev& G, const DexMipsDev& M, int m, const int* c) {
-  const int mask = G.B - 1;
-  const int nb = G.B >> m;
-  int idx = ((c[1] & mask) >> m) * nb + ((c[0] & mask) >> m);
-  if (D == 3) idx += ((c[2] & mask) >> m) * nb * nb;
-  return M.lvloff[m] + idx;
-}
-
-
-// ---------------------------------------------------------------------------------------------------
-// v2 stepping used by the march kernel: same T-rules, fewer instructions.
-//   * size = 1 << sh for cells and for empty bricks alike (sh = level, or log2 B for an empty brick)
-//   * zero-direction axes carry inv = 0, off = +INF, so tplane = fma(k, 0, INF) = +INF without a select
-//   * pm[a] = -1 if d[a] > 0 else 0: exit plane = c[a] + (size & pm[a])
-//   * one 4-byte (slot, level) word per brick instead of the packed word + slot table
-// ---------------------------------------------------------------------------------------------------
-template <int D>
-struct DexRay2 {
-  float o[D], d[D], inv[D], off[D];
-  float tn[D];
-  int c[D], pm[D];
-  int sh;        // log2 of the current cell (or empty-brick) size
-  int cellbase;  // slot * cps + lvloff[level]; < 0 for an empty brick
-  float t;
-};
-
-template <int D>
-__device__ __forceinline__ void dex_planes2(DexRay2<D>& r) {
-  const int size = 1 << r.sh;
-#pragma unroll
-  for (int a = 0; a < D; ++a) r.tn[a] = __fmaf_rn((float)(r.c[a] + (size & r.pm[a])), r.inv[a], r.off[a]);
-}
-
-__device__ __forceinline__ void dex_decode_brick(const DexGridDev& G, const DexMipsDev& M, int info, int& sh, int& cellbase) {
-  const int m = (info & 15) - 1;
-  sh = (m < 0) ? G.logB : m;
-  cellbase = (m < 0) ? -1 : (info >> 4) * M.cps + M.lvloff[m];
-}
-
-template <int D>
-__device__ __forceinline__ bool dex_ray_init2(DexRay2<D>& r, const DexGridDev& G, const DexMipsDev& M,
+__device__ __forceinline__ bool dex_ray_init3(DexRay3<D>& r, const DexGridDev& G, const DexMipsDev& M,
                                               const int* __restrict__ binfo, const float* probe, const float* omega) {
   bool ok = true, any = false;
   int x[D];
 #pragma unroll
   for (int a = 0; a < D; ++a) {
-    r.o[a] = probe[a];
-    r.d[a] = -omega[a];
-    r.pm[a] = (r.d[a] > 0.0f) ? -1 : 0;
-    if (r.d[a] != 0.0f) {
+    const float o = probe[a], d = -omega[a];
+    r.dk[a] = d;              // only its sign is read (dex_set_cell), which then stores +-size
+    if (d != 0.0f) {
       any = true;
-      r.inv[a] = __fdiv_rn(1.0f, r.d[a]);
-      r.off[a] = __fmul_rn(-r.o[a], r.inv[a]);
+      r.inv[a] = __fdiv_rn(1.0f, d);
+      r.off[a] = __fmul_rn(-o, r.inv[a]);
     } else {
       r.inv[a] = 0.0f;
       r.off[a] = __int_as_float(0x7f800000);
     }
-    x[a] = (int)floorf(r.o[a]);
+    x[a] = (int)floorf(o);
     ok = ok && (x[a] >= 0) && (x[a] < G.dims[a]);
   }
   r.t = 0.0f;
-  r.sh = 0;
-  r.cellbase = -1;
   if (!(ok && any)) return false;
-  dex_decode_brick(G, M, __ldg(binfo + dex_brick_of<D>(G, x)), r.sh, r.cellbase);
-  const int amask = ~((1 << r.sh) - 1);
-#pragma unroll
-  for (int a = 0; a < D; ++a) r.c[a] = x[a] & amask;
-  dex_planes2<D>(r);
+  dex_set_cell<D>(r, G, M, __ldg(binfo + dex_brick_of<D>(G, x)), x);
   return true;
 }
 
-// One HDDA event.  emit / cell / ds describe the cell that was just left (T4).  Returns false when the
-// ray has left the grid.
+// level and level-0 low corner of the current cell (visit records, T7)
 template <int D>
-__device__ __forceinline__ bool dex_ray_step2(DexRay2<D>& r, const DexGridDev& G, const DexMipsDev& M,
-                                              const int* __restrict__ binfo, bool& emit, int& cell, float& ds) {
-  int s = 0;
-  float th = r.tn[0];
+__device__ __forceinline__ void dex_ray_cell_coords(const DexRay3<D>& r, int* c) {
+#pragma unroll
+  for (int a = 0; a < D; ++a) c[a] = (int)r.kf[a] - ((r.dk[a] > 0.0f) ? (1 << r.sh) : 0);
+}
+
+// T4: lowest-index axis attaining the minimum exit time
+template <int D>
+__device__ __forceinline__ void dex_ray_next_plane(const DexRay3<D>& r, int& s, float& th) {
+  s = 0;
+  th = r.tn[0];
   if (r.tn[1] < th) { s = 1; th = r.tn[1]; }
   if (D == 3) { if (r.tn[D - 1] < th) { s = D - 1; th = r.tn[D - 1]; } }
-  emit = (r.cellbase >= 0) && (th > r.t);
+}
+
+// First half of an HDDA event: emit / cell / ds describe the cell being left (T4); if the crossing stays inside
+// the brick it is carried out and true is returned.  false: the ray now waits at a brick face (or the grid
+// boundary, or a tie with one) and dex_ray_cross completes the event.
+template <int D>
+__device__ __forceinline__ bool dex_ray_advance(DexRay3<D>& r, bool& emit, int& cell, float& ds) {
+  int s;
+  float th;
+  dex_ray_next_plane<D>(r, s, th);
+  emit = (r.cell >= 0) && (th > r.t);
+  cell = r.cell;
   ds = __fsub_rn(th, r.t);
-  {
-    const int mask = G.B - 1, lsh = G.logB - r.sh;
-    int idx = (((r.c[1] & mask) >> r.sh) << lsh) + ((r.c[0] & mask) >> r.sh);
-    if (D == 3) idx += ((r.c[D - 1] & mask) >> r.sh) << (2 * lsh);
-    cell = r.cellbase + idx;
-  }
   r.t = fmaxf(r.t, th);
-  const int size = 1 << r.sh;
-  int cs = r.c[0], pms = r.pm[0], Ns = G.dims[0];
-  if (s == 1) { cs = r.c[1]; pms = r.pm[1]; Ns = G.dims[1]; }
-  if (D == 3) { if (s == D - 1) { cs = r.c[D - 1]; pms = r.pm[D - 1]; Ns = G.dims[D - 1]; } }
-  const int xs = pms ? cs + size : cs - 1;                      // T5
-  if ((unsigned)xs >= (unsigned)Ns) return false;
-  int x[D];
-#pragma unroll
-  for (int a = 0; a < D; ++a) x[a] = (a == s) ? xs : r.c[a];
-  if (((xs ^ cs) >> G.logB) != 0) {
-    // new brick: MipLevel (Alg. 1 l.6-8) and re-initialisation (l.32-39)
-    int sh2, cb2;
-    dex_decode_brick(G, M, __ldg(binfo + dex_brick_of<D>(G, x)), sh2, cb2);
-    if (sh2 < r.sh) {
-#pragma unroll
-      for (int a = 0; a < D; ++a)
-        if (a != s) x[a] = dex_fine_coord(r.o[a], r.d[a], r.inv[a], r.off[a], r.c[a], size, th, a < s);
+  const bool inside = th < r.tb;
+  if (inside) {
+    if (s == 0) {
+      r.kf[0] = __fadd_rn(r.kf[0], r.dk[0]);
+      r.tn[0] = __fmaf_rn(r.kf[0], r.inv[0], r.off[0]);
+      r.cell += r.cstep[0];
+    } else if (D == 2 || s == 1) {
+      r.kf[1] = __fadd_rn(r.kf[1], r.dk[1]);
+      r.tn[1] = __fmaf_rn(r.kf[1], r.inv[1], r.off[1]);
+      r.cell += r.cstep[1];
+    } else {
+      r.kf[D - 1] = __fadd_rn(r.kf[D - 1], r.dk[D - 1]);
+      r.tn[D - 1] = __fmaf_rn(r.kf[D - 1], r.inv[D - 1], r.off[D - 1]);
+      r.cell += r.cstep[D - 1];
     }
-    r.sh = sh2;
-    r.cellbase = cb2;
   }
-  const int amask = ~((1 << r.sh) - 1);
+  return inside;
+}
+
+// Second half, general crossing (T5) for a ray that dex_ray_advance left waiting: the plane is found again (the
+// exit times have not changed), the level-0 coordinates are rebuilt, the brick looked up (MipLevel, Alg. 1 l.6-8)
+// and the state re-initialised (l.32-39).  Returns false when the ray has left the grid.
+template <int D>
+__device__ __forceinline__ bool dex_ray_cross(DexRay3<D>& r, const DexGridDev& G, const DexMipsDev& M,
+                                              const int* __restrict__ binfo, const float* __restrict__ probe,
+                                              const float* __restrict__ omega) {
+  int s;
+  float th;
+  dex_ray_next_plane<D>(r, s, th);
+  const int size = 1 << r.sh;
+  int c[D];
+  dex_ray_cell_coords<D>(r, c);
+  int cs = c[0], Ns = G.dims[0];
+  bool pos = r.dk[0] > 0.0f;
+  if (s == 1) { cs = c[1]; Ns = G.dims[1]; pos = r.dk[1] > 0.0f; }
+  if (D == 3) { if (s == D - 1) { cs = c[D - 1]; Ns = G.dims[D - 1]; pos = r.dk[D - 1] > 0.0f; } }
+  const int xs = pos ? cs + size : cs - 1;
+  const bool alive = (unsigned)xs < (unsigned)Ns;
+  if (alive) {
+    int x[D];
 #pragma unroll
-  for (int a = 0; a < D; ++a) r.c[a] = x[a] & amask;
-  dex_planes2<D>(r);
-  return true;
+    for (int a = 0; a < D; ++a) x[a] = (a == s) ? xs : c[a];
+    int info = r.info;
+    if (((xs ^ cs) >> G.logB) != 0) {
+      info = __ldg(binfo + dex_brick_of<D>(G, x));
+      const int m2 = (info & 15) - 1;
+      const int sh2 = (m2 < 0) ? G.logB : m2;
+      if (sh2 < r.sh) {
+#pragma unroll
+        for (int a = 0; a < D; ++a)
+          if (a != s) x[a] = dex_fine_coord(__ldg(probe + a), -__ldg(omega + a), r.inv[a], r.off[a], c[a], size, th, a < s);
+      }
+    }
+    dex_set_cell<D>(r, G, M, info, x);
+  }
+  return alive;
 }

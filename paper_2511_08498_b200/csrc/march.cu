@@ -69,29 +69,64 @@ __device__ __forceinline__ void dex_accumulate2(float2 eta, float2 chi, float2 h
   T = __fmul2_rn(T, e);
 }
 
-// S-form (ISO march records, S = eta/chi):  I += T * S * omE,  omE = 1 - e^{-tau}; below tau = 0.25 omE is
-// the degree-7 Taylor polynomial tau (1 - tau/2 + ... - tau^6/5040) (truncation < 1.6e-9 relative).
-__device__ __forceinline__ void dex_accumulate_S(float S, float chi, float hds, float hl, float& I, float& T) {
-  const float tau = chi * hds;
-  const float e = dex_ex2(chi * hl);
-  float p = -1.0f / 5040.0f;
-  p = fmaf(p, tau, 1.0f / 720.0f);
-  p = fmaf(p, tau, -1.0f / 120.0f);
-  p = fmaf(p, tau, 1.0f / 24.0f);
-  p = fmaf(p, tau, -1.0f / 6.0f);
-  p = fmaf(p, tau, 0.5f);
-  p = fmaf(-p, tau, 1.0f);
-  const float omE = (tau < 0.25f) ? p * tau : 1.0f - e;
-  I = fmaf(T, S * omE, I);
+// ISO march records (make_march_records_kernel): plane 0 holds chi2 = chi log2(e), plane 1 holds S = eta/chi.
+//   y = -chi2 h ds  (= -tau log2 e),  e = 2^y = e^-tau,  I += T S (1 - e),  T *= e.
+// 1 - e needs expm1 quality in the thin regime: below tau = 1/8 it is the degree-5 Taylor
+// polynomial of -expm1(y ln 2) in y (truncation < 4.2e-8 relative), above it 1 - ex2(y) (error of ex2.approx
+// relative to 1 - e^-1/8: < 1e-6).  Everything but the two MUFUs and the two selects of a wavelength pair is a
+// packed FFMA2 / FMUL2: the kernel is issue-bound (profiles/), a packed instruction does two wavelengths per slot.
+#define DEX_OME_A1 -0.6931471805599453f      // -ln2
+#define DEX_OME_A2 -0.2402265069591007f      // -ln2^2 / 2
+#define DEX_OME_A3 -0.05550410866482158f     // -ln2^3 / 6
+#define DEX_OME_A4 -0.009618129107628477f    // -ln2^4 / 24
+#define DEX_OME_A5 -0.0013333558146428443f   // -ln2^5 / 120
+#define DEX_OME_YTHR -0.18033688011112042f   // -(1/8) log2(e)
+
+__device__ __forceinline__ void dex_accumulate_S2(float2 S, float2 chi2, float2 nhds2, float2& I, float2& T) {
+  const float2 y = __fmul2_rn(chi2, nhds2);
+  float2 e;
+  e.x = dex_ex2(y.x);
+  e.y = dex_ex2(y.y);
+  float2 p = __ffma2_rn(make_float2(DEX_OME_A5, DEX_OME_A5), y, make_float2(DEX_OME_A4, DEX_OME_A4));
+  p = __ffma2_rn(p, y, make_float2(DEX_OME_A3, DEX_OME_A3));
+  p = __ffma2_rn(p, y, make_float2(DEX_OME_A2, DEX_OME_A2));
+  p = __ffma2_rn(p, y, make_float2(DEX_OME_A1, DEX_OME_A1));
+  p = __fmul2_rn(p, y);
+  if (y.x < DEX_OME_YTHR) p.x = 1.0f - e.x;
+  if (y.y < DEX_OME_YTHR) p.y = 1.0f - e.y;
+  I = __ffma2_rn(T, __fmul2_rn(S, p), I);
+  T = __fmul2_rn(T, e);
+}
+
+__device__ __forceinline__ void dex_accumulate_S1(float S, float chi2, float nhds, float& I, float& T) {
+  const float y = chi2 * nhds;
+  const float e = dex_ex2(y);
+  float p = fmaf(DEX_OME_A5, y, DEX_OME_A4);
+  p = fmaf(p, y, DEX_OME_A3);
+  p = fmaf(p, y, DEX_OME_A2);
+  p = fmaf(p, y, DEX_OME_A1);
+  p *= y;
+  if (y < DEX_OME_YTHR) p = 1.0f - e;
+  I = fmaf(T, S * p, I);
   T *= e;
 }
 
 template <int LPT>
-__device__ __forceinline__ void dex_accumulate_all_S(const float (&S)[LPT], const float (&chi)[LPT], float hds,
+__device__ __forceinline__ void dex_accumulate_all_S(const float (&S)[LPT], const float (&chi2)[LPT], float hds,
                                                      float (&I)[LPT], float (&T)[LPT]) {
-  const float hl = hds * -1.4426950408889634f;
+  const float nhds = -hds;
+  if (LPT == 1) {
+    dex_accumulate_S1(S[0], chi2[0], nhds, I[0], T[0]);
+  } else {
+    const float2 nhds2 = make_float2(nhds, nhds);
 #pragma unroll
-  for (int i = 0; i < LPT; ++i) dex_accumulate_S(S[i], chi[i], hds, hl, I[i], T[i]);
+    for (int i = 0; i < LPT / 2; ++i) {
+      float2 Ii = make_float2(I[2 * i], I[2 * i + 1]), Ti = make_float2(T[2 * i], T[2 * i + 1]);
+      dex_accumulate_S2(make_float2(S[2 * i], S[2 * i + 1]), make_float2(chi2[2 * i], chi2[2 * i + 1]), nhds2, Ii, Ti);
+      I[2 * i] = Ii.x; I[2 * i + 1] = Ii.y;
+      T[2 * i] = Ti.x; T[2 * i + 1] = Ti.y;
+    }
+  }
 }
 
 template <int LPT>
@@ -109,6 +144,24 @@ __device__ __forceinline__ void dex_accumulate_all(const float (&eta)[LPT], cons
       I[2 * i] = Ii.x; I[2 * i + 1] = Ii.y;
       T[2 * i] = Ti.x; T[2 * i + 1] = Ti.y;
     }
+  }
+}
+
+// LPT consecutive floats of a 32-byte plane record: one LDG.E.256 / .128 / .64 / .32
+template <int LPT>
+__device__ __forceinline__ void dex_load_plane(const float* __restrict__ p, float (&v)[LPT]) {
+  if (LPT == 8) {
+    asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[LPT - 4]), "=f"(v[LPT - 3]), "=f"(v[LPT - 2]), "=f"(v[LPT - 1])
+        : "l"(p));
+  } else if (LPT == 4) {
+    const float4 q = __ldg(reinterpret_cast<const float4*>(p));
+    v[0] = q.x; v[1] = q.y; v[LPT - 2] = q.z; v[LPT - 1] = q.w;
+  } else if (LPT == 2) {
+    const float2 q = __ldg(reinterpret_cast<const float2*>(p));
+    v[0] = q.x; v[LPT - 1] = q.y;
+  } else {
+    v[0] = __ldg(p);
   }
 }
 
@@ -141,17 +194,19 @@ __device__ __forceinline__ void dex_load_rec(const float* __restrict__ rec, int 
 // eta, chi of one cell for this lane's wavelengths, seen along propagation direction om (a7)
 template <int D, int VAR, int LPT>
 __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_base, int cell, int sub,
-                                             const float* om, const double* lam, const int* al,
+                                             const float* __restrict__ om, const double* lam, const int* al,
+                                             const float* __restrict__ iso0, const float* __restrict__ iso1,
                                              float (&eta)[LPT], float (&chi)[LPT]) {
-  if (VAR == DEX_ISO) {   // march records: eta[] receives S = eta/chi
-    dex_load_rec<LPT>(M.mrec + (batch_base + (size_t)cell) * DEX_REC, sub, eta, chi);
+  if (VAR == DEX_ISO) {   // march records, two planes of 32-byte rows: chi[] receives chi log2(e), eta[] S = eta/chi
+    dex_load_plane<LPT>(iso0 + (unsigned)cell * DEX_W, chi);
+    dex_load_plane<LPT>(iso1 + (unsigned)cell * DEX_W, eta);
     return;
   }
   // projected velocity of the cell's box-filtered bulk velocity, fp64 (DESIGN.md R-vel)
   const float4 v4 = __ldg(M.vel + cell);
-  double vproj = __dmul_rn((double)v4.x, (double)om[0]);
-  vproj = __dadd_rn(vproj, __dmul_rn((double)v4.y, (double)om[1]));
-  if (D == 3) vproj = __dadd_rn(vproj, __dmul_rn((double)v4.z, (double)om[D - 1]));
+  double vproj = __dmul_rn((double)v4.x, (double)__ldg(om));
+  vproj = __dadd_rn(vproj, __dmul_rn((double)v4.y, (double)__ldg(om + 1)));
+  if (D == 3) vproj = __dadd_rn(vproj, __dmul_rn((double)v4.z, (double)__ldg(om + D - 1)));
   if (VAR == DEX_VELINTERP) {
     // linear interpolation on the cell's uniform velocity grid [-V, V]
     const int nvb = M.n_vbins;
@@ -199,14 +254,22 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
   for (int i = 0; i < LPT; ++i) { eta[i] = (float)de[i]; chi[i] = (float)dc[i]; }
 }
 
-// Each lane group owns one probe and loops over the quadrature directions, accumulating J in registers.
-// (A flattened variant in which a lane starts its next direction as soon as its ray ends was measured
-// and rejected: it halves the thread efficiency, profiles/r01_march_experiments.md.)
+// Each lane group owns one probe and loops over the quadrature directions.
+//
+// Control structure (profiles/r01c-r01e): the loop over HDDA events is warp-synchronous.  Every iteration each live
+// lane leaves one cell (dex_ray_advance: segment, in-brick move) and the emitting lanes integrate together.  A lane
+// whose ray reaches a brick face does NOT take the general crossing at once: it waits (`blocked`) until a quorum of
+// the warp's lanes wait too, or nobody else can move, and then they cross together.  With 29 rays per warp each
+// meeting a face every ~17 steps, crossing at once would run the ~100-instruction general path on 4 lanes in 82 % of
+// the iterations (measured); batched, it runs on >= DEX_CROSS_QUORUM lanes a quarter as often.
 #ifndef DEX_MARCH_THREADS
 #define DEX_MARCH_THREADS 128
 #endif
 #ifndef DEX_MARCH_MINB
 #define DEX_MARCH_MINB 7
+#endif
+#ifndef DEX_CROSS_QUORUM
+#define DEX_CROSS_QUORUM 8
 #endif
 
 template <int D, int VAR, int LPR, bool FUSE_J>
@@ -214,81 +277,95 @@ __global__ void __launch_bounds__(DEX_MARCH_THREADS, DEX_MARCH_MINB)
 dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ perm,
                  float* __restrict__ out, unsigned long long* __restrict__ seg_count) {
   constexpr int LPT = DEX_W / LPR;
+  constexpr unsigned FULL = 0xffffffffu;
+  __shared__ float Jsm[FUSE_J ? LPT * DEX_MARCH_THREADS : 1];
   const int batch = blockIdx.y;
   const long long slot_id = ((long long)blockIdx.x * blockDim.x + threadIdx.x) / LPR;
+  const bool valid = slot_id < R.n_probes;          // lanes past the end stay in the warp-synchronous loops, idle
   // probes are handed to lanes in tile order (dex_tile_probes): a warp's probes are spatial neighbours
-  const long long gid = (slot_id < R.n_probes && perm != nullptr) ? (long long)perm[slot_id] : slot_id;
+  const long long gid = !valid ? 0 : (perm != nullptr ? (long long)perm[slot_id] : slot_id);
   const int sub = threadIdx.x % LPR;
   const int lam_off = batch * DEX_W + sub * LPT;
   unsigned nseg = 0;
-  if (slot_id < R.n_probes && R.n_dirs > 0) {
-    const int* __restrict__ binfo = M.binfo + (size_t)batch * G.n_bricks;
-    const size_t batch_base = ((size_t)batch * G.n_active) * M.cps;
-    float probe[D];
+  const int* __restrict__ binfo = M.binfo + (size_t)batch * G.n_bricks;
+  const size_t batch_base = ((size_t)batch * G.n_active) * M.cps;
+  // this lane's rows of the two ISO record planes (cell 0 of the batch); kept opaque so that the pointers stay in
+  // registers instead of being rebuilt from the kernel parameters at every segment
+  const float* iso0 = M.mrec + batch_base * DEX_W + sub * LPT;
+  const float* iso1 = iso0 + M.mplane;
+  if (VAR == DEX_ISO) asm volatile("" : "+l"(iso0), "+l"(iso1));
+  const float* __restrict__ probe = R.probe_pos + gid * D;
+  double lam[LPT];
+  int al[DEX_NLINES];
+  if (VAR == DEX_CAV) {
 #pragma unroll
-    for (int a = 0; a < D; ++a) probe[a] = __ldg(R.probe_pos + gid * D + a);
-    double lam[LPT];
-    int al[DEX_NLINES];
-    if (VAR == DEX_CAV) {
+    for (int i = 0; i < LPT; ++i) lam[i] = (double)__ldg(M.lam + lam_off + i);
 #pragma unroll
-      for (int i = 0; i < LPT; ++i) lam[i] = (double)__ldg(M.lam + lam_off + i);
+    for (int q = 0; q < DEX_NLINES; ++q) al[q] = M.active_lines[batch * DEX_NLINES + q];
+  }
+  // J is touched once per direction, I and T once per segment: J lives in shared memory ([i][thread], conflict-free)
+  float I[LPT], T[LPT];
+  if (FUSE_J) {
 #pragma unroll
-      for (int q = 0; q < DEX_NLINES; ++q) al[q] = M.active_lines[batch * DEX_NLINES + q];
-    }
-    float J[LPT], I[LPT], T[LPT];
+    for (int i = 0; i < LPT; ++i) Jsm[i * DEX_MARCH_THREADS + threadIdx.x] = 0.0f;
+  }
+  DexRay3<D> ray;
+  // one direction at a time: the lanes of a warp trace the same direction together (coherent fetches)
+  for (int k = 0; k < R.n_dirs; ++k) {
+    const float* __restrict__ om = R.dirs + k * D;
 #pragma unroll
-    for (int i = 0; i < LPT; ++i) { J[i] = 0.0f; I[i] = 0.0f; T[i] = 1.0f; }
-    float om[D];
-    DexRay2<D> ray;
-    {
-      // one direction at a time: the lanes of a warp trace the same direction together (coherent
-      // fetches); inside a direction, lanes skip ahead to their next segment before integrating
-      for (int k = 0; k < R.n_dirs; ++k) {
-#pragma unroll
-        for (int a = 0; a < D; ++a) om[a] = __ldg(R.dirs + k * D + a);
-#pragma unroll
-        for (int i = 0; i < LPT; ++i) { I[i] = 0.0f; T[i] = 1.0f; }
-        bool alive = dex_ray_init2<D>(ray, G, M, binfo, probe, om);
-        while (alive) {
-          bool emit = false;
-          int cell = 0;
-          float ds = 0.0f;
-          do {
-            alive = dex_ray_step2<D>(ray, G, M, binfo, emit, cell, ds);
-          } while (alive && !emit);
-          if (emit) {
-            ++nseg;
-            const float hds = G.h * ds;
-            float eta[LPT], chi[LPT];
-            dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, lam, al, eta, chi);
-            if (VAR == DEX_ISO) dex_accumulate_all_S<LPT>(eta, chi, hds, I, T);
-            else dex_accumulate_all<LPT>(eta, chi, hds, I, T);
-          }
+    for (int i = 0; i < LPT; ++i) { I[i] = 0.0f; T[i] = 1.0f; }
+    bool alive = valid && dex_ray_init3<D>(ray, G, M, binfo, probe, om);
+    bool blocked = false;   // waiting at a brick face for dex_ray_cross (implies alive)
+    for (;;) {
+      const unsigned am = __ballot_sync(FULL, alive);
+      if (am == 0u) break;
+      const unsigned bm = __ballot_sync(FULL, blocked);
+      if (bm == am || __popc(bm) >= DEX_CROSS_QUORUM) {
+        if (blocked) {
+          alive = dex_ray_cross<D>(ray, G, M, binfo, probe, om);
+          blocked = false;
         }
-        if (R.i0 != nullptr) {
-#pragma unroll
-          for (int i = 0; i < LPT; ++i) I[i] = fmaf(T[i], __ldg(R.i0 + (size_t)k * M.n_lambda + lam_off + i), I[i]);
-        }
-        if (FUSE_J) {
-          const float wk = __ldg(R.weights + k);
-#pragma unroll
-          for (int i = 0; i < LPT; ++i) J[i] = fmaf(wk, I[i], J[i]);
-        } else {
-          float* dst = out + ((size_t)gid * R.n_dirs + k) * M.n_lambda + lam_off;
-#pragma unroll
-          for (int i = 0; i < LPT; ++i) dst[i] = I[i];
+      }
+      if (alive && !blocked) {
+        bool emit;
+        int cell;
+        float ds;
+        blocked = !dex_ray_advance<D>(ray, emit, cell, ds);
+        if (emit) {
+          ++nseg;
+          const float hds = G.h * ds;
+          float eta[LPT], chi[LPT];
+          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, lam, al, iso0, iso1, eta, chi);
+          if (VAR == DEX_ISO) dex_accumulate_all_S<LPT>(eta, chi, hds, I, T);
+          else dex_accumulate_all<LPT>(eta, chi, hds, I, T);
         }
       }
     }
-    if (FUSE_J) {
-      float* dst = out + (size_t)gid * M.n_lambda + lam_off;
+    if (valid) {
+      if (R.i0 != nullptr) {
 #pragma unroll
-      for (int i = 0; i < LPT; ++i) dst[i] = J[i];
+        for (int i = 0; i < LPT; ++i) I[i] = fmaf(T[i], __ldg(R.i0 + (size_t)k * M.n_lambda + lam_off + i), I[i]);
+      }
+      if (FUSE_J) {
+        const float wk = __ldg(R.weights + k);
+#pragma unroll
+        for (int i = 0; i < LPT; ++i) Jsm[i * DEX_MARCH_THREADS + threadIdx.x] = fmaf(wk, I[i], Jsm[i * DEX_MARCH_THREADS + threadIdx.x]);
+      } else {
+        float* dst = out + ((size_t)gid * R.n_dirs + k) * M.n_lambda + lam_off;
+#pragma unroll
+        for (int i = 0; i < LPT; ++i) dst[i] = I[i];
+      }
     }
+  }
+  if (FUSE_J && valid) {
+    float* dst = out + (size_t)gid * M.n_lambda + lam_off;
+#pragma unroll
+    for (int i = 0; i < LPT; ++i) dst[i] = Jsm[i * DEX_MARCH_THREADS + threadIdx.x];
   }
   if (seg_count != nullptr) {
     unsigned v = (sub == 0) ? nseg : 0u;
-    v = __reduce_add_sync(0xffffffffu, v);
+    v = __reduce_add_sync(FULL, v);
     if ((threadIdx.x & 31) == 0 && v) atomicAdd(seg_count, (unsigned long long)v);
   }
 }
@@ -305,24 +382,22 @@ dex_capture_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, l
   if (ray_id >= n_rays) return;
   const long long p = ray_id / R.n_dirs;
   const int k = (int)(ray_id - p * R.n_dirs);
-  float probe[D], om[D];
-#pragma unroll
-  for (int a = 0; a < D; ++a) { probe[a] = R.probe_pos[p * D + a]; om[a] = R.dirs[k * D + a]; }
+  const float* __restrict__ probe = R.probe_pos + p * D;
+  const float* __restrict__ om = R.dirs + k * D;
   const int* __restrict__ binfo = M.binfo + (size_t)batch * G.n_bricks;
   const long long begin = offsets[ray_id];
   const long long room = ((ray_id + 1 < n_rays) ? offsets[ray_id + 1] : capacity) - begin;
   long long n = 0;
-  DexRay2<D> ray;
-  bool alive = dex_ray_init2<D>(ray, G, M, binfo, probe, om);
+  DexRay3<D> ray;
+  bool alive = dex_ray_init3<D>(ray, G, M, binfo, probe, om);
   while (alive) {
     int c[D];
-#pragma unroll
-    for (int a = 0; a < D; ++a) c[a] = ray.c[a];
+    dex_ray_cell_coords<D>(ray, c);
     const int m = ray.sh;
     bool emit;
     int cell;
     float ds;
-    alive = dex_ray_step2<D>(ray, G, M, binfo, emit, cell, ds);
+    if (!dex_ray_advance<D>(ray, emit, cell, ds)) alive = dex_ray_cross<D>(ray, G, M, binfo, probe, om);
     if (emit) {
       if (n < room) {
         unsigned long long rec = ((unsigned long long)(unsigned)m << 56) | (unsigned long long)(unsigned)(c[0] >> m);

@@ -164,10 +164,12 @@ __global__ void reduce_spec_kernel(const BuildCtx X, int m) {
 // ---- ISO march records --------------------------------------------------------------------------------
 // The march integrates  I += T * eta h ds E(tau),  E = (1 - e^{-tau})/tau.  With S = eta/chi this is
 // I += T * S * (1 - e^{-tau}), which needs no reciprocal in the inner loop (one MUFU instead of two per
-// wavelength).  Records hold (chi', S) for every level of the pyramid; the pyramid itself keeps (eta, chi)
-// exactly (it is what the VLM test and the validation accessors see).  chi < 2^-100 (including chi = 0, a
-// pure emitter: I_out = I_in + eta h ds) is represented by chi' = 2^-100, S = eta 2^100: then tau' is
-// ~1e-30 h ds, e^{-tau'} = 1 and S tau' = eta h ds, so the E(0) = 1 limit of DESIGN.md is kept.
+// wavelength), and with chi2 = chi log2(e) the exponent is a single product, e^{-tau} = 2^(-chi2 h ds).
+// Records hold (chi2, S) for every level of the pyramid in two planes of 32-byte rows (one LDG.E.256 each; four
+// cells per 128-byte line, so the neighbouring rays of a warp share L1 lines); the pyramid itself keeps (eta, chi)
+// exactly (it is what the VLM test and the validation accessors see).  chi < 2^-100 (including chi = 0, a pure
+// emitter: I_out = I_in + eta h ds) is represented by chi = 2^-100, S = eta 2^100: then tau is ~1e-30 h ds,
+// e^{-tau} = 1 and S (1 - e^{-tau}) = eta h ds to 1e-7, so the E(0) = 1 limit of DESIGN.md is kept.
 __global__ void make_march_records_kernel(const float* __restrict__ store, float* __restrict__ mrec, long long n_rec) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_rec * DEX_W) return;
@@ -178,8 +180,8 @@ __global__ void make_march_records_kernel(const float* __restrict__ store, float
   float c = chi, S;
   if (chi < tiny) { c = tiny; S = eta * 1.2676506002282294e30f; }   // 2^100, exact scaling
   else S = eta / chi;
-  mrec[dex_rec_chi(r, j)] = c;
-  mrec[dex_rec_eta(r, j)] = S;
+  mrec[i] = c * 1.4426950408889634f;
+  mrec[(size_t)n_rec * DEX_W + i] = S;
 }
 
 // ---- line parameters and velocity: level 0 gather and box filter ------------------------------------
@@ -441,9 +443,9 @@ __global__ void select_levels_kernel(const BuildCtx X, signed char* __restrict__
 }
 
 // state = level + 1 in `bits` bits, floor(64/bits) bricks per 64-bit word.  The same pass
-// writes the march's own table: one 4-byte word (slot << 4) | state per (batch, brick).
+// writes the march's own table: one 4-byte word (first record of the brick's level << 4) | state per (batch, brick).
 __global__ void pack_levels_kernel(const signed char* __restrict__ levels, const int* __restrict__ slot, int n_batch,
-                                   int n_bricks, int bits, int per_word, int words,
+                                   int n_bricks, int bits, int per_word, int words, const DexMipsDev M,
                                    unsigned long long* __restrict__ packed, int* __restrict__ binfo) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (long long)n_batch * words) return;
@@ -455,7 +457,7 @@ __global__ void pack_levels_kernel(const signed char* __restrict__ levels, const
     if (bi >= n_bricks) break;
     const int state = levels[(size_t)b * n_bricks + bi] + 1;
     word |= (unsigned long long)state << (q * bits);
-    binfo[(size_t)b * n_bricks + bi] = (state > 0) ? ((slot[bi] << 4) | state) : 0;
+    binfo[(size_t)b * n_bricks + bi] = (state > 0) ? (((slot[bi] * M.cps + M.lvloff[state - 1]) << 4) | state) : 0;
   }
   packed[i] = word;
 }
@@ -589,7 +591,7 @@ dex_status dex_launch_pack_levels(dex_mips* m, cudaStream_t st) {
   const long long total = (long long)m->n_batch * m->dev.words_per_batch;
   pack_levels_kernel<<<blocks_for(total, 256), 256, 0, st>>>(m->d_levels, m->grid->d_slot, m->n_batch,
                                                              (int)m->grid->n_bricks, m->dev.bits, m->dev.per_word,
-                                                             m->dev.words_per_batch, m->d_packed, m->d_binfo);
+                                                             m->dev.words_per_batch, m->dev, m->d_packed, m->d_binfo);
   dex_count_launch();
   DEX_CUDA_CHECK(cudaGetLastError());
   return DEX_OK;
