@@ -266,7 +266,7 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
 #define DEX_MARCH_THREADS 128
 #endif
 #ifndef DEX_MARCH_MINB
-#define DEX_MARCH_MINB 7
+#define DEX_MARCH_MINB 8
 #endif
 #ifndef DEX_CROSS_QUORUM
 #define DEX_CROSS_QUORUM 8
@@ -287,7 +287,8 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   const int sub = threadIdx.x % LPR;
   const int lam_off = batch * DEX_W + sub * LPT;
   unsigned nseg = 0;
-  const int* __restrict__ binfo = M.binfo + (size_t)batch * G.n_bricks;
+  const int* binfo = M.binfo + (size_t)batch * G.n_bricks;
+  asm volatile("" : "+l"(binfo));   // opaque for the same reason as iso0 / iso1 below
   const size_t batch_base = ((size_t)batch * G.n_active) * M.cps;
   // this lane's rows of the two ISO record planes (cell 0 of the batch); kept opaque so that the pointers stay in
   // registers instead of being rebuilt from the kernel parameters at every segment
