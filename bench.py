@@ -214,7 +214,8 @@ def main():
     from workloads.gen import SEEDS
 
     # weak scaling: every rank owns an atmosphere of the same size (its own seed)
-    wl = make(args.workload, n=args.n, n_dirs=args.n_dirs, n_probes=args.n_probes, seed=SEEDS[args.workload] + 1000 * rank)
+    wl = make(args.workload, n=args.n, n_dirs=args.n_dirs, n_probes=args.n_probes,
+              seed=P.shard.rank_seed(SEEDS[args.workload], rank))
     if args.probe_band:
         ax = wl.ndim - 1
         n_ax = wl.dims[ax]
@@ -284,13 +285,7 @@ def main():
     step_ms = [a.elapsed_time(b) for a, b in evs]
     total_ms = float(sum(step_ms))
     segs_total = int(seg.item())
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    s = torch.tensor([float(segs_total)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(s, op=dist.ReduceOp.SUM)
-    max_ms = float(t.item())
-    all_segs = float(s.item())
+    max_ms, all_segs = P.shard.job_totals(total_ms, segs_total, dev)      # max over ranks, sum over ranks
     value = all_segs * W / (max_ms * 1e-3)
 
     # end to end through the public API with HOST (pinned) buffers: H2D + build + march + D2H of J per step
@@ -308,12 +303,8 @@ def main():
             torch.cuda.synchronize()
             e_t += time.perf_counter() - t0
             e_seg += nseg
-        et = torch.tensor([e_t], dtype=torch.float64, device=dev)
-        es = torch.tensor([float(e_seg)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(et, op=dist.ReduceOp.MAX)
-            dist.all_reduce(es, op=dist.ReduceOp.SUM)
-        e2e = {"value": float(es.item()) * W / float(et.item()), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+        e_t_max, e_seg_all = P.shard.job_totals(e_t, e_seg, dev)
+        e2e = {"value": e_seg_all * W / e_t_max, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "steps": n_e2e,
                "timing": "host wall clock around upload(pinned)->build->march->J.cpu(), max over ranks"}
 

@@ -11,4 +11,4 @@ from .binding import (  # noqa: F401
     dex_build_sparse_grid, dex_build_vlm_mips, dex_formal_solution, dex_launch_count, dex_march_timing_enable,
     dex_march_timing_read, dex_mean_intensity, dex_set_lanes_per_ray, dex_set_tuning, dex_version,
 )
-from . import pipeline  # noqa: F401
+from . import pipeline, shard  # noqa: F401
