@@ -191,10 +191,19 @@ __device__ __forceinline__ void dex_load_rec(const float* __restrict__ rec, int 
   }
 }
 
+// Core-and-Voigt: what depends on (wavelength of the batch, active line) only -- eqs. 14, 18-20
+struct DexCavTab {
+  double dlam[DEX_NLINES][DEX_W];    // lambda - lambda0
+  double r2[DEX_NLINES][DEX_W];      // (lambda / lambda0)^2:  a(lambda) = r2 a(lambda0)                 (eq. 20)
+  float scale[DEX_NLINES][DEX_W];    // (lambda0 / lambda) / sqrt(pi): eta*(lambda) phi = eta*0 invD scale H (eqs. 18-19)
+  double lam0_over_c[DEX_NLINES];    // Doppler shift of the line centre per unit projected velocity     (eq. 14)
+  int line[DEX_NLINES];              // active line of slot q or -1
+};
+
 // eta, chi of one cell for this lane's wavelengths, seen along propagation direction om (a7)
 template <int D, int VAR, int LPT>
 __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_base, int cell, int sub,
-                                             const float* __restrict__ om, const double* lam, const int* al,
+                                             const float* __restrict__ om, const DexCavTab& CT,
                                              const float* __restrict__ iso0, const float* __restrict__ iso1,
                                              float (&eta)[LPT], float (&chi)[LPT]) {
   if (VAR == DEX_ISO) {   // march records, two planes of 32-byte rows: chi[] receives chi log2(e), eta[] S = eta/chi
@@ -230,28 +239,27 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
     }
     return;
   }
-  // Core-and-Voigt / Classic: background + sum over the active lines (eqs. 10-11)
+  // Core-and-Voigt / Classic: background + sum over the active lines (eqs. 10-11).  Only H(a, x) needs fp64 (the
+  // Weideman form cancels in the wings); the line sum itself is fp32.  Everything that depends
+  // on (wavelength, line) alone comes from the block's shared table CT (one batch per block).
   dex_load_rec<LPT>(M.store + (batch_base + (size_t)cell) * DEX_REC, sub, eta, chi);
-  double de[LPT], dc[LPT];
-#pragma unroll
-  for (int i = 0; i < LPT; ++i) { de[i] = (double)eta[i]; dc[i] = (double)chi[i]; }
 #pragma unroll
   for (int q = 0; q < DEX_NLINES; ++q) {
-    const int l = al[q];
-    if (l < 0) continue;
+    const int l = CT.line[q];
+    if (l < 0) continue;               // block-uniform
     const float4 ln = __ldg(M.line + (size_t)cell * M.n_lines + l);
-    const double lam0 = (double)M.lambda0[l];
+    const double a0 = (double)ln.z, invD = (double)ln.w;
+    const double shift = vproj * CT.lam0_over_c[q];
+    const float es = ln.x * ln.w, cs = ln.y * ln.w;
 #pragma unroll
     for (int i = 0; i < LPT; ++i) {
-      double el, cl;
-      dex_line_terms(M.wei_c, M.wei_L, lam[i], lam0, (double)ln.x, (double)ln.y, (double)ln.z, (double)ln.w, vproj,
-                     M.c_light, el, cl);
-      de[i] += el;
-      dc[i] += cl;
+      const int j = sub * LPT + i;
+      const double x = (CT.dlam[q][j] + shift) * invD;
+      const float phi = (float)dex_voigt_H_march(M.wei_c, M.wei_L, CT.r2[q][j] * a0, x) * CT.scale[q][j];
+      eta[i] = fmaf(es, phi, eta[i]);
+      chi[i] = fmaf(cs, phi, chi[i]);
     }
   }
-#pragma unroll
-  for (int i = 0; i < LPT; ++i) { eta[i] = (float)de[i]; chi[i] = (float)dc[i]; }
 }
 
 // Each lane group owns one probe and loops over the quadrature directions.
@@ -268,12 +276,23 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
 #ifndef DEX_MARCH_MINB
 #define DEX_MARCH_MINB 8
 #endif
+// resident blocks per SM asked of the compiler per variant: the ISO march fits 64 registers; the velocity tables
+// want two records in flight, and Core-and-Voigt runs 8 independent fp64 Goertzel chains per line
+#ifndef DEX_MINB_VEL
+#define DEX_MINB_VEL 5
+#endif
+#ifndef DEX_MINB_CAV
+#define DEX_MINB_CAV 3
+#endif
+constexpr int dex_march_minb(int var) {
+  return var == DEX_ISO ? DEX_MARCH_MINB : (var == DEX_VELINTERP ? DEX_MINB_VEL : DEX_MINB_CAV);
+}
 #ifndef DEX_CROSS_QUORUM
 #define DEX_CROSS_QUORUM 8
 #endif
 
 template <int D, int VAR, int LPR, bool FUSE_J>
-__global__ void __launch_bounds__(DEX_MARCH_THREADS, DEX_MARCH_MINB)
+__global__ void __launch_bounds__(DEX_MARCH_THREADS, dex_march_minb(VAR))
 dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ perm,
                  float* __restrict__ out, unsigned long long* __restrict__ seg_count) {
   constexpr int LPT = DEX_W / LPR;
@@ -296,13 +315,22 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   const float* iso1 = iso0 + M.mplane;
   if (VAR == DEX_ISO) asm volatile("" : "+l"(iso0), "+l"(iso1));
   const float* __restrict__ probe = R.probe_pos + gid * D;
-  double lam[LPT];
-  int al[DEX_NLINES];
+  __shared__ DexCavTab CT;
   if (VAR == DEX_CAV) {
-#pragma unroll
-    for (int i = 0; i < LPT; ++i) lam[i] = (double)__ldg(M.lam + lam_off + i);
-#pragma unroll
-    for (int q = 0; q < DEX_NLINES; ++q) al[q] = M.active_lines[batch * DEX_NLINES + q];
+    if (threadIdx.x < DEX_NLINES * DEX_W) {
+      const int q = threadIdx.x / DEX_W, j = threadIdx.x % DEX_W;
+      const int l = M.active_lines[batch * DEX_NLINES + q];
+      if (j == 0) CT.line[q] = l;
+      if (l >= 0) {
+        const double lm = (double)__ldg(M.lam + batch * DEX_W + j), l0 = (double)M.lambda0[l];
+        const double r = lm / l0;
+        CT.dlam[q][j] = lm - l0;
+        CT.r2[q][j] = r * r;
+        CT.scale[q][j] = (float)((l0 / lm) * 0.56418958354775628695);
+        if (j == 0) CT.lam0_over_c[q] = l0 / M.c_light;
+      }
+    }
+    __syncthreads();
   }
   // J is touched once per direction, I and T once per segment: J lives in shared memory ([i][thread], conflict-free)
   float I[LPT], T[LPT];
@@ -337,7 +365,7 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
           ++nseg;
           const float hds = G.h * ds;
           float eta[LPT], chi[LPT];
-          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, lam, al, iso0, iso1, eta, chi);
+          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, CT, iso0, iso1, eta, chi);
           if (VAR == DEX_ISO) dex_accumulate_all_S<LPT>(eta, chi, hds, I, T);
           else dex_accumulate_all<LPT>(eta, chi, hds, I, T);
         }
