@@ -186,6 +186,18 @@ dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const 
                               const float* d_I /*NULL = fused*/, float* d_J, int64_t* d_segment_count,
                               void* stream);
 
+/* The whole hot path (a1-a9) from HOST buffers in one call: the end-to-end entry a caller without
+ * device memory of their own uses (bench.py's `e2e` leg).  `h_active` is [nvox] or NULL.  In `host_mips`
+ * and `host_rays` EVERY pointer, including the ones named d_*, is HOST memory here (pinned memory makes the
+ * copies asynchronous; pageable memory works, staged by the driver).  The call uploads the inputs, runs
+ * dex_build_sparse_grid, dex_build_vlm_mips and the fused dex_mean_intensity on `stream`, copies J
+ * ([n_probes][n_lambda]) and the emitted-segment count into h_J / h_segment_count (may be NULL), destroys
+ * its temporaries and returns after the stream has drained.  *h2d_bytes / *d2h_bytes (may be NULL) receive
+ * the bytes copied in each direction.  Errors: as the three calls it chains, plus DEX_ERR_OOM. */
+dex_status dex_mean_intensity_host(const dex_grid_desc* desc, const uint8_t* h_active, const dex_mips_desc* host_mips,
+                                   const dex_rays* host_rays, float* h_J, int64_t* h_segment_count,
+                                   int64_t* h2d_bytes, int64_t* d2h_bytes, void* stream);
+
 /* Number of kernel launches this library has enqueued since load (bench.py's gpu_launches). */
 int64_t dex_launch_count(void);
 /* Device time (ms) and launch count of the march kernels since the last reset, measured with CUDA

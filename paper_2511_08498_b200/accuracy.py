@@ -1,0 +1,115 @@
+"""VLM accuracy report (BASELINE.json north_star: "the accuracy of VLM against the exact full-resolution
+march is reported separately as the 99.9th-percentile relative error in J").
+
+Both sides run on the GPU through the C ABI: the approximate side is the workload's own variant and level
+table (VLM + HDDA); the exact side is the same library at level 0 -- `max_level = 0` for the isotropic
+variant, `DEX_CLASSIC` (per-voxel velocity, brute-force line profile in every cell and direction; the
+paper's ground truth) for the anisotropic ones.  The level-0 / Classic march is itself
+parity-checked against the oracle in tests/test_gpu_parity.py.  The paper's Table 3 quotes the same
+percentiles for level populations; J is what this hot path produces.
+
+  python -m paper_2511_08498_b200.accuracy --workload C2 [--n-probes N] [--metric relvar|iod_log]
+
+Prints one JSON line: percentiles of |J_vlm - J_exact| / J_exact over (probe, wavelength), the level
+histogram per batch (Table-2 style), segment counts and march times of both sides.
+Reported, not gated.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def level_histogram(levels: np.ndarray, max_level: int) -> list:
+    """[n_batch][max_level + 2] brick counts for levels -1, 0, ..., max_level."""
+    return [[int((row == m).sum()) for m in range(-1, max_level + 1)] for row in levels]
+
+
+def percentiles(rel: np.ndarray) -> dict:
+    qs = (50.0, 90.0, 99.0, 99.9)
+    out = {f"p{q:g}": float(np.percentile(rel, q)) for q in qs}
+    out["max"] = float(rel.max()) if rel.size else 0.0
+    return out
+
+
+def run(workload: str, n=None, n_dirs=None, n_probes=None, metric=None, thr=None, gate=None, max_level=None,
+        device="cuda:0") -> dict:
+    import torch
+    from . import binding as B
+    from . import pipeline
+    from workloads import make
+
+    wl = make(workload, n=n, n_dirs=n_dirs, n_probes=n_probes)
+    if metric is not None:
+        wl.metric = {"iod_log": 0, "relvar": 1}[metric]
+    if thr is not None:
+        wl.thr_eta = wl.thr_chi = float(thr)
+    if gate is not None:
+        wl.tau_gate = float(gate)
+    if max_level is not None:
+        wl.max_level = int(max_level)
+    dw = pipeline.upload(wl, device, non_blocking=False)
+    grid = pipeline.build_grid(dw)
+    stream = torch.cuda.current_stream()
+
+    def solve(**override):
+        mips = pipeline.build_mips(dw, grid, **override)
+        seg = torch.zeros(1, dtype=torch.int64, device=device)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        J = pipeline.mean_intensity(dw, grid, mips, segment_count=seg)
+        b.record(stream)
+        torch.cuda.synchronize()
+        lv = mips.levels()
+        mips.destroy()
+        return J.cpu().numpy().astype(np.float64), int(seg.item()), a.elapsed_time(b), lv
+
+    J_vlm, seg_vlm, ms_vlm, lv = solve()
+    if wl.variant == B.DEX_ISO:
+        J_ex, seg_ex, ms_ex, _ = solve(max_level=0)
+        exact = "same variant at max_level 0"
+    else:
+        J_ex, seg_ex, ms_ex, _ = solve(variant=B.DEX_CLASSIC, max_level=0)
+        exact = "DEX_CLASSIC (per-voxel velocity, level 0; PAPER.md:365)"
+    grid.destroy()
+    lit = J_ex > 0.0                       # probes/wavelengths that see no emitting cell have J = 0 on both sides
+    rel = np.abs(J_vlm[lit] - J_ex[lit]) / J_ex[lit]
+    assert (J_vlm[~lit] == 0.0).all()
+    hist = np.asarray(level_histogram(lv, wl.max_level))
+    return {
+        "report": "vlm_accuracy_J", "workload": wl.name, "dims": list(wl.dims[:wl.ndim]), "variant": int(wl.variant),
+        "metric": "relvar" if wl.metric == 1 else "iod_log", "thr": float(wl.thr_eta), "tau_gate": float(wl.tau_gate),
+        "max_level": int(wl.max_level), "n_probes": int(wl.probe_pos.shape[0]), "n_dirs": int(wl.dirs.shape[0]),
+        "n_lambda": int(wl.n_lambda), "exact_side": exact, "rel_err_J": percentiles(rel),
+        "values_compared": int(rel.size), "segments_vlm": seg_vlm, "segments_exact": seg_ex,
+        "segment_ratio": seg_ex / max(1, seg_vlm), "march_ms_vlm": ms_vlm, "march_ms_exact": ms_ex,
+        "level_histogram_levels": list(range(-1, wl.max_level + 1)),
+        "level_histogram_mean_fraction": (hist.mean(axis=0) / hist[0].sum()).round(4).tolist(),
+        "level_histogram_per_batch": hist.tolist(),
+    }
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--n", type=int, default=None)
+    ap.add_argument("--n-dirs", type=int, default=None)
+    ap.add_argument("--n-probes", type=int, default=None)
+    ap.add_argument("--metric", default=None, choices=["relvar", "iod_log"])
+    ap.add_argument("--thr", type=float, default=None)
+    ap.add_argument("--gate", type=float, default=None)
+    ap.add_argument("--max-level", type=int, default=None)
+    a = ap.parse_args()
+    print(json.dumps(run(a.workload, a.n, a.n_dirs, a.n_probes, a.metric, a.thr, a.gate, a.max_level)))
+
+
+if __name__ == "__main__":
+    main()

@@ -28,7 +28,7 @@ EXPORTS = (
     "dex_last_error", "dex_version", "dex_build_sparse_grid", "dex_grid_info", "dex_grid_get_slots",
     "dex_destroy_grid", "dex_build_vlm_mips", "dex_mips_get_levels", "dex_mips_set_levels",
     "dex_mips_get_packed_levels", "dex_mips_get_level_data", "dex_destroy_mips", "dex_formal_solution",
-    "dex_mean_intensity", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read",
+    "dex_mean_intensity", "dex_mean_intensity_host", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read",
     "dex_set_lanes_per_ray", "dex_set_tuning",
 )
 
@@ -88,6 +88,9 @@ def _load():
                                       C.c_void_p, C.c_void_p]
     L.dex_mean_intensity.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_Rays), C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p]
+    L.dex_mean_intensity_host.argtypes = [C.POINTER(_GridDesc), C.c_void_p, C.POINTER(_MipsDesc), C.POINTER(_Rays),
+                                          C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64),
+                                          C.c_void_p]
     L.dex_march_timing_enable.argtypes = [C.c_int]
     L.dex_march_timing_enable.restype = None
     L.dex_march_timing_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64), C.c_int]
@@ -111,6 +114,8 @@ def _ptr(t: Optional[torch.Tensor], dtype=None, cuda=True):
         raise TypeError(f"expected {dtype}, got {t.dtype}")
     if cuda and not t.is_cuda:
         raise TypeError("expected a CUDA tensor")
+    if not cuda and t.is_cuda:
+        raise TypeError("expected a host tensor")
     if not t.is_contiguous():
         raise TypeError("expected a contiguous tensor")
     return t.data_ptr()
@@ -240,16 +245,15 @@ class Mips:
             pass
 
 
-def dex_build_vlm_mips(grid: Grid, variant, n_lambda, lambda_batch, max_level, metric, thr_eta, thr_chi, tau_gate,
-                       eta=None, chi=None, lam=None, eta_bg=None, chi_bg=None, vel=None, lambda0=None,
-                       eta_star0=None, chi_star0=None, a0=None, inv_dlamD=None, active_lines=None, n_vbins=0,
-                       c_light=299792.458, stream=None) -> Mips:
+def _mips_desc(variant, n_lambda, lambda_batch, max_level, metric, thr_eta, thr_chi, tau_gate, eta, chi, lam, eta_bg,
+               chi_bg, vel, lambda0, eta_star0, chi_star0, a0, inv_dlamD, active_lines, n_vbins, c_light, cuda=True):
+    """Fill a dex_mips_desc; returns (desc, n_lines, host arrays that must outlive the call)."""
     d = _MipsDesc()
     d.variant, d.n_lambda, d.lambda_batch, d.max_level, d.metric = int(variant), int(n_lambda), int(lambda_batch), int(max_level), int(metric)
     d.thr_eta, d.thr_chi, d.tau_gate = float(thr_eta), float(thr_chi), float(tau_gate)
     f32 = torch.float32
-    d.d_lambda, d.d_eta, d.d_chi = _ptr(lam, f32), _ptr(eta, f32), _ptr(chi, f32)
-    d.d_eta_bg, d.d_chi_bg, d.d_vel = _ptr(eta_bg, f32), _ptr(chi_bg, f32), _ptr(vel, f32)
+    d.d_lambda, d.d_eta, d.d_chi = _ptr(lam, f32, cuda), _ptr(eta, f32, cuda), _ptr(chi, f32, cuda)
+    d.d_eta_bg, d.d_chi_bg, d.d_vel = _ptr(eta_bg, f32, cuda), _ptr(chi_bg, f32, cuda), _ptr(vel, f32, cuda)
     keep = []
     n_lines = 0
     if lambda0 is not None:
@@ -258,7 +262,8 @@ def dex_build_vlm_mips(grid: Grid, variant, n_lambda, lambda_batch, max_level, m
         n_lines = l0.shape[0]
         d.h_lambda0 = l0.ctypes.data
     d.n_lines = n_lines
-    d.d_eta_star0, d.d_chi_star0, d.d_a0, d.d_inv_dlamD = _ptr(eta_star0, f32), _ptr(chi_star0, f32), _ptr(a0, f32), _ptr(inv_dlamD, f32)
+    d.d_eta_star0, d.d_chi_star0 = _ptr(eta_star0, f32, cuda), _ptr(chi_star0, f32, cuda)
+    d.d_a0, d.d_inv_dlamD = _ptr(a0, f32, cuda), _ptr(inv_dlamD, f32, cuda)
     if active_lines is not None:
         al = np.ascontiguousarray(active_lines, dtype=np.int8)
         if al.shape != (n_lambda // lambda_batch, DEX_MAX_LINES):
@@ -267,8 +272,19 @@ def dex_build_vlm_mips(grid: Grid, variant, n_lambda, lambda_batch, max_level, m
         d.h_active_lines = al.ctypes.data
     d.n_vbins = int(n_vbins)
     d.c_light = float(c_light)
+    return d, n_lines, keep
+
+
+def dex_build_vlm_mips(grid: Grid, variant, n_lambda, lambda_batch, max_level, metric, thr_eta, thr_chi, tau_gate,
+                       eta=None, chi=None, lam=None, eta_bg=None, chi_bg=None, vel=None, lambda0=None,
+                       eta_star0=None, chi_star0=None, a0=None, inv_dlamD=None, active_lines=None, n_vbins=0,
+                       c_light=299792.458, stream=None) -> Mips:
+    d, n_lines, keep = _mips_desc(variant, n_lambda, lambda_batch, max_level, metric, thr_eta, thr_chi, tau_gate, eta,
+                                  chi, lam, eta_bg, chi_bg, vel, lambda0, eta_star0, chi_star0, a0, inv_dlamD,
+                                  active_lines, n_vbins, c_light)
     h = C.c_void_p()
     _check(_L.dex_build_vlm_mips(grid.handle, C.byref(d), _stream(stream), C.byref(h)))
+    del keep
     return Mips(h, grid, n_lambda, lambda_batch, 0 if variant == DEX_CLASSIC else max_level, variant, n_lines, int(n_vbins))
 
 
@@ -278,12 +294,12 @@ class Rays:
         self.probe_pos, self.dirs, self.weights, self.i0 = probe_pos, dirs, weights, i0
         self.n_probes, self.n_dirs = int(probe_pos.shape[0]), int(dirs.shape[0])
 
-    def struct(self):
+    def struct(self, cuda=True):
         r = _Rays()
         f32 = torch.float32
         r.n_probes, r.n_dirs = self.n_probes, self.n_dirs
-        r.d_probe_pos, r.d_dirs = _ptr(self.probe_pos, f32), _ptr(self.dirs, f32)
-        r.d_weights, r.d_i0 = _ptr(self.weights, f32), _ptr(self.i0, f32)
+        r.d_probe_pos, r.d_dirs = _ptr(self.probe_pos, f32, cuda), _ptr(self.dirs, f32, cuda)
+        r.d_weights, r.d_i0 = _ptr(self.weights, f32, cuda), _ptr(self.i0, f32, cuda)
         return r
 
 
@@ -321,3 +337,27 @@ def dex_mean_intensity(grid: Grid, mips: Mips, rays: Rays, J: torch.Tensor, I: O
     r = rays.struct()
     _check(_L.dex_mean_intensity(grid.handle, mips.handle, C.byref(r), _ptr(I, torch.float32), _ptr(J, torch.float32),
                                  _ptr(segment_count, torch.int64), _stream(stream)))
+
+
+def dex_mean_intensity_host(ndim, dims, brick, voxel_size, active: Optional[torch.Tensor], mips_args: dict,
+                            rays: Rays, J: torch.Tensor, stream=None):
+    """include/dex.h dex_mean_intensity_host: the whole hot path from HOST tensors (pinned or pageable) to a host J.
+    `mips_args` holds dex_build_vlm_mips' keyword arguments with host tensors.  Returns (segments, h2d, d2h bytes)."""
+    g = _GridDesc()
+    g.ndim = ndim
+    dd = list(dims) + [1] * (3 - len(dims))
+    for a in range(3):
+        g.dims[a] = int(dd[a])
+    g.brick, g.voxel_size = int(brick), float(voxel_size)
+    a = dict(eta=None, chi=None, lam=None, eta_bg=None, chi_bg=None, vel=None, lambda0=None, eta_star0=None,
+             chi_star0=None, a0=None, inv_dlamD=None, active_lines=None, n_vbins=0, c_light=299792.458)
+    a.update(mips_args)
+    d, _, keep = _mips_desc(cuda=False, **a)
+    r = rays.struct(cuda=False)
+    if J.is_cuda or J.dtype != torch.float32 or not J.is_contiguous() or J.numel() != rays.n_probes * int(a["n_lambda"]):
+        raise TypeError("J must be a contiguous host fp32 tensor [n_probes][n_lambda]")
+    seg, h2d, d2h = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+    _check(_L.dex_mean_intensity_host(C.byref(g), _ptr(active, torch.uint8, False), C.byref(d), C.byref(r), J.data_ptr(),
+                                      C.byref(seg), C.byref(h2d), C.byref(d2h), _stream(stream)))
+    del keep
+    return seg.value, h2d.value, d2h.value

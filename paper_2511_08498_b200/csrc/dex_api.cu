@@ -90,6 +90,51 @@ struct MarchTimer {
 };
 }  // namespace
 
+namespace {
+// device copies of host inputs, released when the call returns
+struct Uploads {
+  cudaStream_t st;
+  std::vector<void*> ptrs;
+  int64_t bytes = 0;
+  dex_status status = DEX_OK;
+  explicit Uploads(cudaStream_t s) : st(s) {}
+  ~Uploads() { for (void* p : ptrs) cudaFree(p); }
+  template <typename T>
+  const T* put(const T* h, size_t count) {
+    if (!h || status != DEX_OK) return nullptr;
+    void* d = nullptr;
+    const size_t nbytes = sizeof(T) * (count ? count : 1);
+    if (cudaMalloc(&d, nbytes) != cudaSuccess) {
+      cudaGetLastError();
+      dex_set_error("device allocation failed while uploading host inputs");
+      status = DEX_ERR_OOM;
+      return nullptr;
+    }
+    ptrs.push_back(d);
+    if (count && cudaMemcpyAsync(d, h, sizeof(T) * count, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+      dex_set_error(cudaGetErrorString(cudaGetLastError()));
+      status = DEX_ERR_CUDA;
+      return nullptr;
+    }
+    bytes += (int64_t)(sizeof(T) * count);
+    return (const T*)d;
+  }
+  template <typename T>
+  T* alloc(size_t count) {
+    if (status != DEX_OK) return nullptr;
+    void* d = nullptr;
+    if (cudaMalloc(&d, sizeof(T) * (count ? count : 1)) != cudaSuccess) {
+      cudaGetLastError();
+      dex_set_error("device allocation failed");
+      status = DEX_ERR_OOM;
+      return nullptr;
+    }
+    ptrs.push_back(d);
+    return (T*)d;
+  }
+};
+}  // namespace
+
 void dex_set_error(const std::string& msg) { g_last_error = msg; }
 void dex_count_launch(int n) { g_launches.fetch_add(n); }
 
@@ -458,6 +503,72 @@ dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const 
   if (d_I) return dex_launch_reduce_j(R, mips->n_lambda, d_I, d_J, st);
   MarchTimer tm(st);
   return dex_launch_march(grid, mips, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), g_tile_probes.load() != 0, st);
+}
+
+// ------------------------------------------------------------------------------------------- host entry
+dex_status dex_mean_intensity_host(const dex_grid_desc* desc, const uint8_t* h_active, const dex_mips_desc* hm,
+                                   const dex_rays* hr, float* h_J, int64_t* h_segment_count, int64_t* h2d_bytes,
+                                   int64_t* d2h_bytes, void* stream) {
+  if (!desc || !hm || !hr || !h_J) { dex_set_error("NULL desc / host_mips / host_rays / h_J"); return DEX_ERR_INVALID_ARG; }
+  if (desc->ndim != 2 && desc->ndim != 3) { dex_set_error("ndim must be 2 or 3"); return DEX_ERR_INVALID_ARG; }
+  if (hm->n_lambda <= 0 || hr->n_probes < 0 || hr->n_dirs < 0 || hm->n_lines < 0 || hm->n_lines > DEX_MAX_LINES) {
+    dex_set_error("bad n_lambda / n_probes / n_dirs / n_lines");
+    return DEX_ERR_SHAPE;
+  }
+  if (!have_device()) return DEX_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  size_t nvox = 1;
+  for (int a = 0; a < desc->ndim; ++a) {
+    if (desc->dims[a] <= 0) { dex_set_error("dims must be positive"); return DEX_ERR_SHAPE; }
+    nvox *= (size_t)desc->dims[a];
+  }
+  const size_t nl = (size_t)hm->n_lambda, D = (size_t)desc->ndim;
+  Uploads up(st);
+  dex_mips_desc dm = *hm;                 // host-side members (h_lambda0, h_active_lines) are used as they are
+  dm.d_lambda = up.put(hm->d_lambda, nl);
+  dm.d_eta = up.put(hm->d_eta, nvox * nl);
+  dm.d_chi = up.put(hm->d_chi, nvox * nl);
+  dm.d_eta_bg = up.put(hm->d_eta_bg, nvox * nl);
+  dm.d_chi_bg = up.put(hm->d_chi_bg, nvox * nl);
+  dm.d_vel = up.put(hm->d_vel, nvox * D);
+  dm.d_eta_star0 = up.put(hm->d_eta_star0, nvox * (size_t)hm->n_lines);
+  dm.d_chi_star0 = up.put(hm->d_chi_star0, nvox * (size_t)hm->n_lines);
+  dm.d_a0 = up.put(hm->d_a0, nvox * (size_t)hm->n_lines);
+  dm.d_inv_dlamD = up.put(hm->d_inv_dlamD, nvox * (size_t)hm->n_lines);
+  const uint8_t* d_active = up.put(h_active, nvox);
+  dex_rays dr = *hr;
+  dr.d_probe_pos = up.put(hr->d_probe_pos, (size_t)hr->n_probes * D);
+  dr.d_dirs = up.put(hr->d_dirs, (size_t)hr->n_dirs * D);
+  dr.d_weights = up.put(hr->d_weights, (size_t)hr->n_dirs);
+  dr.d_i0 = up.put(hr->d_i0, (size_t)hr->n_dirs * nl);
+  float* d_J = up.alloc<float>((size_t)hr->n_probes * nl);
+  int64_t* d_seg = up.alloc<int64_t>(1);
+  if (up.status != DEX_OK) return up.status;
+  dex_grid* grid = nullptr;
+  dex_mips* mips = nullptr;
+  dex_status s = dex_build_sparse_grid(desc, d_active, stream, &grid);
+  if (s == DEX_OK) s = dex_build_vlm_mips(grid, &dm, stream, &mips);
+  cudaError_t e = cudaSuccess;
+  if (s == DEX_OK) e = cudaMemsetAsync(d_seg, 0, sizeof(int64_t), st);
+  if (s == DEX_OK && e == cudaSuccess) s = dex_mean_intensity(grid, mips, &dr, nullptr, d_J, d_seg, stream);
+  int64_t out_bytes = 0;
+  if (s == DEX_OK && e == cudaSuccess && hr->n_probes > 0) {
+    e = cudaMemcpyAsync(h_J, d_J, sizeof(float) * (size_t)hr->n_probes * nl, cudaMemcpyDeviceToHost, st);
+    out_bytes += (int64_t)(sizeof(float) * (size_t)hr->n_probes * nl);
+  }
+  if (s == DEX_OK && e == cudaSuccess && h_segment_count) {
+    e = cudaMemcpyAsync(h_segment_count, d_seg, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+    out_bytes += (int64_t)sizeof(int64_t);
+  }
+  const cudaError_t e2 = cudaStreamSynchronize(st);     // the temporaries below must not be freed under running work
+  dex_destroy_mips(mips);
+  dex_destroy_grid(grid);
+  if (s != DEX_OK) return s;
+  DEX_CUDA_CHECK(e);
+  DEX_CUDA_CHECK(e2);
+  if (h2d_bytes) *h2d_bytes = up.bytes;
+  if (d2h_bytes) *d2h_bytes = out_bytes;
+  return DEX_OK;
 }
 
 }  // extern "C"

@@ -90,16 +90,25 @@ def formal_solution(dw: DeviceWorkload, grid: B.Grid, mips: B.Mips, capture_batc
     return I, cap
 
 
-def solve_J_from_host(wl, device="cuda:0", pinned: Optional[dict] = None):
-    """The end-to-end call a user makes with HOST buffers: upload, build grid + mips, fused march to J,
-    read J and the emitted-segment count back.  Returns (J numpy, segments, h2d_bytes, d2h_bytes)."""
-    dw = upload(wl, device, pinned)
-    grid = build_grid(dw)
-    mips = build_mips(dw, grid)
-    seg = torch.zeros(1, dtype=torch.int64, device=device)
-    J = mean_intensity(dw, grid, mips, segment_count=seg)
-    Jh = J.cpu()
-    nseg = int(seg.cpu().item())
-    mips.destroy()
-    grid.destroy()
-    return Jh.numpy(), nseg, dw.h2d_bytes, Jh.numel() * 4 + 8
+def solve_J_from_host(wl, device="cuda:0", pinned: Optional[dict] = None, J_host: Optional[torch.Tensor] = None):
+    """The end-to-end call a user makes with HOST buffers: one dex_mean_intensity_host call (include/dex.h), which
+    uploads the inputs, builds grid + mips, runs the fused march to J and copies J and the emitted-segment count
+    back.  `pinned` = pin(wl) makes the copies asynchronous.  Returns (J numpy, segments, h2d_bytes, d2h_bytes)."""
+    src = pinned if pinned is not None else {n: torch.from_numpy(np.ascontiguousarray(getattr(wl, n)))
+                                             for n in _SPEC_FIELDS + _RAY_FIELDS + ("active",)
+                                             if getattr(wl, n, None) is not None}
+    r = B.Rays(src["probe_pos"], src["dirs"], src.get("weights"), src.get("i0"))
+    if J_host is None:
+        J_host = torch.empty((r.n_probes, wl.n_lambda), dtype=torch.float32)
+        if torch.cuda.is_available():
+            J_host = J_host.pin_memory()
+    args = dict(variant=wl.variant, n_lambda=wl.n_lambda, lambda_batch=wl.lambda_batch, max_level=wl.max_level,
+                metric=wl.metric, thr_eta=wl.thr_eta, thr_chi=wl.thr_chi, tau_gate=wl.tau_gate, eta=src.get("eta"),
+                chi=src.get("chi"), lam=src.get("lam"), eta_bg=src.get("eta_bg"), chi_bg=src.get("chi_bg"),
+                vel=src.get("vel"), lambda0=wl.lambda0, eta_star0=src.get("eta_star0"), chi_star0=src.get("chi_star0"),
+                a0=src.get("a0"), inv_dlamD=src.get("inv_dlamD"), active_lines=wl.active_lines, n_vbins=wl.n_vbins,
+                c_light=wl.c_light)
+    with torch.cuda.device(device):
+        nseg, h2d, d2h = B.dex_mean_intensity_host(wl.ndim, wl.dims[:wl.ndim], wl.brick, wl.voxel_size, src.get("active"),
+                                                   args, r, J_host)
+    return J_host.numpy(), nseg, h2d, d2h

@@ -293,3 +293,27 @@ def test_c2_full_size_sampled(P):
     assert max_rel(J[idx], Jref) <= TOL
     assert int(seg.item()) > 0
     assert np.isfinite(J).all() and (J >= 0).all()
+
+
+# ------------------------------------------------------------------------------------------ host entry
+@pytest.mark.parametrize("name,kw", [("C2", dict(n=128, n_dirs=8, n_probes=333)), ("C5", dict(n=32, n_dirs=6, n_probes=200)),
+                                     ("C3", dict(n=128, n_dirs=6, n_probes=150))])
+def test_host_entry_matches_device_path(P, name, kw):
+    """dex_mean_intensity_host (HOST buffers in, host J out: bench.py's e2e leg) gives bit for bit the J and the
+    segment count of the three device-pointer calls it chains, with pinned and with pageable inputs."""
+    wl = make(name, **kw)
+    wl.i0 = np.random.default_rng(3).uniform(0, 1, size=(wl.dirs.shape[0], wl.n_lambda)).astype(np.float32)
+    dw, grid, mips = _build(P, wl)
+    seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+    J = P.pipeline.mean_intensity(dw, grid, mips, segment_count=seg).cpu().numpy()
+    for pinned in (P.pipeline.pin(wl), None):
+        Jh, nseg, h2d, d2h = P.pipeline.solve_J_from_host(wl, "cuda:0", pinned)
+        assert nseg == int(seg.item()) and nseg > 0
+        assert np.array_equal(Jh.view(np.uint32), J.view(np.uint32))
+        assert d2h == J.size * 4 + 8 and 0 < h2d <= dw.h2d_bytes
+    # argument errors surface as a status, not a crash
+    with pytest.raises(P.DexError):
+        P.dex_mean_intensity_host(2, (64, 60), 16, 1.0, None, dict(variant=0, n_lambda=8, lambda_batch=8, max_level=0,
+                                  metric=1, thr_eta=0.0, thr_chi=0.0, tau_gate=-1.0,
+                                  eta=torch.zeros(64 * 60 * 8), chi=torch.zeros(64 * 60 * 8)),
+                                  P.Rays(torch.zeros(1, 2), torch.ones(1, 2), torch.ones(1)), torch.zeros(1, 8))
