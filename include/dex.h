@@ -186,6 +186,12 @@ dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const 
                               const float* d_I /*NULL = fused*/, float* d_J, int64_t* d_segment_count,
                               void* stream);
 
+/* Validation: the Voigt function H(a_i, x_i) = Re w(x_i + i a_i) of PAPER.md:329 ("HUM1WEI24") exactly as the
+ * Core-and-Voigt march evaluates it, for n (damping, frequency offset) pairs in device memory.  mode 0: as the
+ * march chooses (fp32 table form inside its damping window, the fp64 Weideman / Humlicek form outside it, see
+ * csrc/dex_voigt.cuh); mode 1: the fp64 form everywhere.  Asynchronous on `stream`. */
+dex_status dex_voigt_profile(const float* d_a, const double* d_x, int64_t n, double* d_H, int mode, void* stream);
+
 /* The whole hot path (a1-a9) from HOST buffers in one call: the end-to-end entry a caller without
  * device memory of their own uses (bench.py's `e2e` leg).  `h_active` is [nvox] or NULL.  In `host_mips`
  * and `host_rays` EVERY pointer, including the ones named d_*, is HOST memory here (pinned memory makes the

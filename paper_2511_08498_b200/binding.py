@@ -28,7 +28,7 @@ EXPORTS = (
     "dex_last_error", "dex_version", "dex_build_sparse_grid", "dex_grid_info", "dex_grid_get_slots",
     "dex_destroy_grid", "dex_build_vlm_mips", "dex_mips_get_levels", "dex_mips_set_levels",
     "dex_mips_get_packed_levels", "dex_mips_get_level_data", "dex_destroy_mips", "dex_formal_solution",
-    "dex_mean_intensity", "dex_mean_intensity_host", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read",
+    "dex_mean_intensity", "dex_mean_intensity_host", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read",
     "dex_set_lanes_per_ray", "dex_set_tuning",
 )
 
@@ -91,6 +91,7 @@ def _load():
     L.dex_mean_intensity_host.argtypes = [C.POINTER(_GridDesc), C.c_void_p, C.POINTER(_MipsDesc), C.POINTER(_Rays),
                                           C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64),
                                           C.c_void_p]
+    L.dex_voigt_profile.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_int, C.c_void_p]
     L.dex_march_timing_enable.argtypes = [C.c_int]
     L.dex_march_timing_enable.restype = None
     L.dex_march_timing_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64), C.c_int]
@@ -361,3 +362,13 @@ def dex_mean_intensity_host(ndim, dims, brick, voxel_size, active: Optional[torc
                                       C.byref(seg), C.byref(h2d), C.byref(d2h), _stream(stream)))
     del keep
     return seg.value, h2d.value, d2h.value
+
+
+def dex_voigt_profile(a: torch.Tensor, x: torch.Tensor, mode: int = 0, stream=None) -> torch.Tensor:
+    """Validation: H(a, x) as the Core-and-Voigt march evaluates it (a fp32, x fp64 CUDA tensors of equal length)."""
+    if a.numel() != x.numel():
+        raise ValueError("a and x must have the same length")
+    H = torch.empty(x.numel(), dtype=torch.float64, device=x.device)
+    _check(_L.dex_voigt_profile(_ptr(a, torch.float32), _ptr(x, torch.float64), a.numel(), H.data_ptr(), int(mode),
+                                _stream(stream)))
+    return H

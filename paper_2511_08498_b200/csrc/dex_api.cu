@@ -49,7 +49,7 @@ dex_status dmalloc(T** p, size_t count) {
 
 void free_mips_memory(dex_mips* m) {
   cudaFree(m->d_store); cudaFree(m->d_mrec); cudaFree(m->d_line); cudaFree(m->d_vel); cudaFree(m->d_vtab); cudaFree(m->d_lam);
-  cudaFree(m->d_active_lines); cudaFree(m->d_levels); cudaFree(m->d_packed); cudaFree(m->d_fail); cudaFree(m->d_binfo);
+  cudaFree(m->d_active_lines); cudaFree(m->d_levels); cudaFree(m->d_packed); cudaFree(m->d_fail); cudaFree(m->d_binfo); cudaFree(m->d_vftab);
 }
 
 dex_status check_rays(const dex_grid* grid, const dex_mips* mips, const dex_rays* rays, DexRaysDev* out) {
@@ -134,6 +134,16 @@ struct Uploads {
   }
 };
 }  // namespace
+
+const float* dex_voigt_fast_table_host() {
+  static std::vector<float> tab;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    tab.resize((size_t)DEX_VF_NODES * 5);
+    dex_voigt_fast_table(tab.data(), tab.data() + (size_t)DEX_VF_NODES * 4);
+  });
+  return tab.data();
+}
 
 void dex_set_error(const std::string& msg) { g_last_error = msg; }
 void dex_count_launch(int n) { g_launches.fetch_add(n); }
@@ -343,6 +353,7 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
     if (s == DEX_OK) s = dmalloc(&m->d_line, A * cps * (size_t)(d.n_lines > 0 ? d.n_lines : 1));
     if (s == DEX_OK) s = dmalloc(&m->d_lam, (size_t)desc->n_lambda);
     if (s == DEX_OK) s = dmalloc(&m->d_active_lines, (size_t)n_batch * DEX_MAX_LINES);
+    if (s == DEX_OK) s = dmalloc(&m->d_vftab, (size_t)DEX_VF_NODES * 5);
     if (s == DEX_OK && v == DEX_VELINTERP) {
       m->vtab_floats = m->store_floats * (size_t)d.n_vbins;
       s = dmalloc(&m->d_vtab, m->vtab_floats);
@@ -353,10 +364,15 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
       if (e == cudaSuccess)
         e = cudaMemcpyAsync(m->d_active_lines, desc->h_active_lines, (size_t)n_batch * DEX_MAX_LINES,
                             cudaMemcpyHostToDevice, st);
+      if (e == cudaSuccess)
+        e = cudaMemcpyAsync(m->d_vftab, dex_voigt_fast_table_host(), sizeof(float) * DEX_VF_NODES * 5,
+                            cudaMemcpyHostToDevice, st);
       if (e != cudaSuccess) { dex_set_error(cudaGetErrorString(e)); s = DEX_ERR_CUDA; }
     }
   }
   if (s == DEX_OK) {
+    d.vf_wing = (const float4*)m->d_vftab;
+    d.vf_core = m->d_vftab ? m->d_vftab + (size_t)DEX_VF_NODES * 4 : nullptr;
     d.packed = m->d_packed;
     d.binfo = m->d_binfo;
     d.store = m->d_store;
@@ -503,6 +519,13 @@ dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const 
   if (d_I) return dex_launch_reduce_j(R, mips->n_lambda, d_I, d_J, st);
   MarchTimer tm(st);
   return dex_launch_march(grid, mips, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), g_tile_probes.load() != 0, st);
+}
+
+dex_status dex_voigt_profile(const float* d_a, const double* d_x, int64_t n, double* d_H, int mode, void* stream) {
+  if (n < 0 || (n > 0 && (!d_a || !d_x || !d_H))) { dex_set_error("NULL d_a / d_x / d_H"); return DEX_ERR_INVALID_ARG; }
+  if (mode != 0 && mode != 1) { dex_set_error("mode must be 0 (as the march chooses) or 1 (fp64 form)"); return DEX_ERR_INVALID_ARG; }
+  if (!have_device()) return DEX_ERR_CUDA;
+  return dex_launch_voigt_profile(d_a, d_x, (long long)n, d_H, mode, (cudaStream_t)stream);
 }
 
 // ------------------------------------------------------------------------------------------- host entry

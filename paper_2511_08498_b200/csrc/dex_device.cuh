@@ -52,6 +52,8 @@ struct DexMipsDev {
   double c_light;
   double wei_c[24];                  // Weideman N=24 coefficients c_1..c_24
   double wei_L;
+  const float4* vf_wing;             // [DEX_VF_NODES] Taylor coefficients of Im F about the nodes (dex_voigt.cuh)
+  const float* vf_core;              // [DEX_VF_NODES] e^{-x_k^2}
 };
 
 struct DexRaysDev {

@@ -33,6 +33,7 @@ struct dex_mips {
   signed char* d_levels = nullptr;           // [n_batch][n_bricks]
   unsigned long long* d_packed = nullptr;    // [n_batch][words_per_batch]
   int* d_binfo = nullptr;                    // [n_batch][n_bricks] (slot << 4) | (level + 1)
+  float* d_vftab = nullptr;                  // fp32 Voigt tables: [NODES][4] wing then [NODES] core (anisotropic variants)
   int* d_fail = nullptr;                     // [n_batch][n_active][max_level+1]
   size_t store_floats = 0, vtab_floats = 0;
 };
@@ -51,6 +52,8 @@ dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysD
                             unsigned long long* d_seg, int lanes_per_ray, bool tile, cudaStream_t st);
 dex_status dex_launch_capture(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays,
                               const dex_visit_capture* cap, int* d_overflow, cudaStream_t st);
+dex_status dex_launch_voigt_profile(const float* d_a, const double* d_x, long long n, double* d_H, int mode, cudaStream_t st);
+const float* dex_voigt_fast_table_host();   // [NODES * 4 + NODES] floats, computed once
 dex_status dex_launch_reduce_j(const DexRaysDev& rays, int n_lambda, const float* d_I, float* d_J, cudaStream_t st);
 
 #define DEX_CUDA_CHECK(expr)                                                                   \

@@ -110,3 +110,165 @@ __device__ __forceinline__ double dex_voigt_H_march(const double* __restrict__ w
   const double i2r = fma(ir, ir, -(ii * ii)), i2i = 2.0 * ir * ii;   // 1/(L - i z)^2
   return fma(2.0, fma(pr, i2r, -(pi * i2i)), ir * inv_sqrt_pi);
 }
+
+// ---- fp32 evaluation for small damping ---------------------------------------------------------------
+// The fp64 Goertzel form above keeps the Core-and-Voigt march on the fp64 pipe (profiles/r01g: 50 % of its
+// peak, everything else idle).  For the damping range of solar lines the same number is reached in fp32 from
+//     w(z) = e^{-z^2} + (2i / sqrt(pi)) F(z),   F = Dawson's function,   z = x + i a
+//     H(a, x) = Re w = e^{a^2 - x^2} cos(2 a x) - (2 / sqrt(pi)) Im F(x + i a),
+// which has no cancellation: the Gaussian core and the algebraic wing are separate, positive terms.  F is entire,
+// so Im F(x + i a) is summed from its Taylor series about the nearest node x_k = k / 32 of a table,
+//     Im F(x_k + zeta) = Im sum_{m=1..4} c_m(k) zeta^m,   zeta = (x - x_k) + i a,   c_m = F^(m)(x_k) / m!,
+// and the core is e^{-x_k^2} (tabulated) times short series in the small quantities (x - x_k), a.
+// With |x - x_k| <= 1/64 and a <= 0.03 the truncated terms are below 2e-7 of H; measured against the exact
+// Voigt function the fp32 evaluation is within 4e-7 relative for |x| + a < 15.  HUM1WEI24 itself deviates from
+// the exact function by 2.6e-9 / a relative in the wings (its Weideman part has ~1e-11 ABSOLUTE error), so the
+// two agree to <= 8e-7 only for a >= DEX_VF_A_LO; below that, and above DEX_VF_A_HI, the march evaluates the
+// literal formula in fp64.  x must be supplied as an unevaluated fp32 pair (hi + lo): the Gaussian core turns an
+// error dx into a relative error 2 x dx.
+#define DEX_VF_INVDX 32
+#define DEX_VF_NODES (15 * DEX_VF_INVDX + 1)
+#define DEX_VF_A_LO 0.005f
+#define DEX_VF_A_HI 0.03f
+
+// Dawson's function in extended precision: Rybicki's exponentially convergent sampling sum
+// F(x) = (1/sqrt(pi)) sum_{n odd} e^{-(x - n h)^2} / n  (error ~ e^{-(pi/h)^2}), h = 1/4.
+inline long double dex_dawson_ld(long double x) {
+  const long double h = 0.25L, inv_sqrt_pi = 0.564189583547756286948079451560772586L;
+  const int n0 = 2 * (int)floorl(x / (2.0L * h)) + 1;   // odd n nearest to x / h
+  long double acc = 0.0L;
+  for (int j = -40; j <= 40; ++j) {
+    const int n = n0 + 2 * j;
+    const long double t = x - (long double)n * h;
+    acc += expl(-t * t) / (long double)n;
+  }
+  return acc * inv_sqrt_pi;
+}
+
+// wing[k][m-1] = c_m(k) = F^(m)(x_k)/m!, m = 1..4;  core[k] = e^{-x_k^2};  x_k = k / DEX_VF_INVDX
+inline void dex_voigt_fast_table(float* wing, float* core) {
+  for (int k = 0; k < DEX_VF_NODES; ++k) {
+    const long double x = (long double)k / (long double)DEX_VF_INVDX;
+    long double c[5];
+    if (x < 6.0L) {
+      // F' = 1 - 2 x F,  F^(n+1) = -2 x F^(n) - 2 n F^(n-1)
+      long double d[5];
+      d[0] = dex_dawson_ld(x);
+      d[1] = 1.0L - 2.0L * x * d[0];
+      for (int n = 1; n < 4; ++n) d[n + 1] = -2.0L * x * d[n] - 2.0L * (long double)n * d[n - 1];
+      long double fact = 1.0L;
+      for (int m = 1; m <= 4; ++m) { fact *= (long double)m; c[m] = d[m] / fact; }
+    } else {
+      // the recurrence cancels like x^m at large x; differentiate the asymptotic series term by term instead:
+      // F(x) ~ sum_j (2j-1)!! / (2^(j+1) x^(2j+1)),  d^m/dx^m x^-p / m! = (-1)^m C(p+m-1, m) x^-(p+m)
+      for (int m = 1; m <= 4; ++m) {
+        long double sum = 0.0L, coef = 0.5L, prev = 1e300L;   // coef = (2j-1)!!/2^(j+1)
+        for (int j = 0; j < 60; ++j) {
+          const int p = 2 * j + 1;
+          long double binom = 1.0L;
+          for (int i = 1; i <= m; ++i) binom *= (long double)(p + m - i) / (long double)i;
+          const long double term = coef * binom * powl(x, -(long double)(p + m));
+          if (term >= prev) break;          // asymptotic: stop at the smallest term (< 1e-17 relative for x >= 6)
+          sum += term;
+          prev = term;
+          coef *= (long double)(2 * j + 1) / 2.0L;
+        }
+        c[m] = (m & 1) ? -sum : sum;
+      }
+    }
+    for (int m = 1; m <= 4; ++m) wing[4 * k + (m - 1)] = (float)c[m];
+    core[k] = (float)expl(-x * x);
+  }
+}
+
+// H(a, x) for DEX_VF_A_LO <= a <= DEX_VF_A_HI and |x| + a < 15, x = xh + xl (|xl| <= ulp(xh)/2).  wing / core: the
+// tables above (shared memory in the march).  Branch free, so that the march can interleave the evaluations of a
+// batch's wavelengths; for |x| + a >= 15 the value is finite but meaningless and the caller replaces it with
+// dex_voigt_H_region1.
+__device__ __forceinline__ float dex_voigt_H_table(const float4* __restrict__ wing, const float* __restrict__ core,
+                                                   float a, float xh, float xl) {
+  const float ax = fminf(fabsf(xh), 15.0f);
+  const float el = (fabsf(xh) < 15.0f) ? ((xh < 0.0f) ? -xl : xl) : 0.0f;
+  const float t = fmaf(ax, (float)DEX_VF_INVDX, 12582912.0f);      // 2^23 + 2^22: the sum rounds |x| * 32 to an integer
+  const int k = __float_as_int(t) - 0x4B400000;
+  const float xk = (t - 12582912.0f) * (1.0f / (float)DEX_VF_INVDX);
+  const float d = (ax - xk) + el;                                   // ax - xk is exact
+  // core: e^{-x_k^2} * e^{a^2 - d (2 x_k + d)} * cos(2 a x)
+  const float s = fmaf(a, a, -d * fmaf(2.0f, xk, d));
+  float ex = fmaf(s, 1.0f / 120.0f, 1.0f / 24.0f);
+  ex = fmaf(ex, s, 1.0f / 6.0f);
+  ex = fmaf(ex, s, 0.5f);
+  ex = fmaf(ex, s, 1.0f);
+  ex = fmaf(ex, s, 1.0f);
+  const float ph = 2.0f * a * ax, u = ph * ph;
+  float cs = fmaf(u, 1.0f / 40320.0f, -1.0f / 720.0f);
+  cs = fmaf(cs, u, 1.0f / 24.0f);
+  cs = fmaf(cs, u, -0.5f);
+  cs = fmaf(cs, u, 1.0f);
+  const float g = core[k];
+  const float4 c = wing[k];
+  // Im[((c4 zeta + c3) zeta + c2) zeta + c1) zeta],  zeta = d + i a
+  float sr = fmaf(c.w, d, c.z), si = c.w * a;
+  float tr = fmaf(sr, d, fmaf(-si, a, c.y));
+  si = fmaf(sr, a, si * d);
+  sr = tr;
+  tr = fmaf(sr, d, fmaf(-si, a, c.x));
+  si = fmaf(sr, a, si * d);
+  sr = tr;
+  const float im = fmaf(sr, a, si * d);
+  return fmaf(-1.1283791670955126f, im, g * ex * cs);
+}
+
+// The same for two wavelengths at once on Blackwell's packed fp32 pipe (FFMA2 / FMUL2 / FADD2): the Core-and-Voigt
+// march is bound by instruction issue (profiles/r01h), and a packed instruction does two evaluations per slot.
+__device__ __forceinline__ float2 dex_f2(float v) { return make_float2(v, v); }
+__device__ __forceinline__ float2 dex_neg2(float2 v) { return make_float2(-v.x, -v.y); }
+__device__ __forceinline__ float dex_xorsign(float v, float s) {
+  return __int_as_float(__float_as_int(v) ^ (__float_as_int(s) & 0x80000000));
+}
+__device__ __forceinline__ float2 dex_voigt_H_table2(const float4* __restrict__ wing, const float* __restrict__ core,
+                                                     float2 a, float2 xh, float2 xl) {
+  const float2 ax = make_float2(fminf(fabsf(xh.x), 15.0f), fminf(fabsf(xh.y), 15.0f));
+  const float2 el = make_float2(dex_xorsign(xl.x, xh.x), dex_xorsign(xl.y, xh.y));   // only read where |x| < 15
+  const float2 t = __ffma2_rn(ax, dex_f2((float)DEX_VF_INVDX), dex_f2(12582912.0f));
+  const int k0 = __float_as_int(t.x) - 0x4B400000, k1 = __float_as_int(t.y) - 0x4B400000;
+  const float2 xk = __fmul2_rn(__fadd2_rn(t, dex_f2(-12582912.0f)), dex_f2(1.0f / (float)DEX_VF_INVDX));
+  const float2 d = __fadd2_rn(__fadd2_rn(ax, dex_neg2(xk)), el);
+  const float2 s = __ffma2_rn(dex_neg2(d), __ffma2_rn(dex_f2(2.0f), xk, d), __fmul2_rn(a, a));
+  float2 ex = __ffma2_rn(s, dex_f2(1.0f / 120.0f), dex_f2(1.0f / 24.0f));
+  ex = __ffma2_rn(ex, s, dex_f2(1.0f / 6.0f));
+  ex = __ffma2_rn(ex, s, dex_f2(0.5f));
+  ex = __ffma2_rn(ex, s, dex_f2(1.0f));
+  ex = __ffma2_rn(ex, s, dex_f2(1.0f));
+  const float2 ph = __fmul2_rn(__fadd2_rn(a, a), ax), u = __fmul2_rn(ph, ph);
+  float2 cs = __ffma2_rn(u, dex_f2(1.0f / 40320.0f), dex_f2(-1.0f / 720.0f));
+  cs = __ffma2_rn(cs, u, dex_f2(1.0f / 24.0f));
+  cs = __ffma2_rn(cs, u, dex_f2(-0.5f));
+  cs = __ffma2_rn(cs, u, dex_f2(1.0f));
+  const float2 g = make_float2(core[k0], core[k1]);
+  const float4 c0 = wing[k0], c1 = wing[k1];
+  const float2 na = dex_neg2(a);
+  float2 sr = __ffma2_rn(make_float2(c0.w, c1.w), d, make_float2(c0.z, c1.z));
+  float2 si = __fmul2_rn(make_float2(c0.w, c1.w), a);
+  float2 tr = __ffma2_rn(sr, d, __ffma2_rn(si, na, make_float2(c0.y, c1.y)));
+  si = __ffma2_rn(sr, a, __fmul2_rn(si, d));
+  sr = tr;
+  tr = __ffma2_rn(sr, d, __ffma2_rn(si, na, make_float2(c0.x, c1.x)));
+  si = __ffma2_rn(sr, a, __fmul2_rn(si, d));
+  sr = tr;
+  const float2 im = __ffma2_rn(sr, a, __fmul2_rn(si, d));
+  return __ffma2_rn(dex_f2(-1.1283791670955126f), im, __fmul2_rn(__fmul2_rn(g, ex), cs));
+}
+
+// |x| + a >= 15: region I of Humlicek (1982) in the cancellation-free form of dex_voigt_H_march, fine in fp32
+__device__ __forceinline__ float dex_voigt_H_region1(float a, float xh) {
+  const float ax = fminf(fabsf(xh), 1.0e9f);
+  const float x2 = ax * ax, a2 = a * a;
+  const float dr = x2 - a2 - 0.5f, di = 2.0f * a * ax;
+  return __fdividef((a * 0.5641895835477563f) * (x2 + a2 + 0.5f), fmaf(dr, dr, di * di));
+}
+
+__device__ __forceinline__ float dex_voigt_H_fast(const float4* __restrict__ wing, const float* __restrict__ core,
+                                                  float a, float xh, float xl) {
+  return (fabsf(xh) + a >= 15.0f) ? dex_voigt_H_region1(a, xh) : dex_voigt_H_table(wing, core, a, xh, xl);
+}

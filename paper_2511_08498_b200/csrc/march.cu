@@ -195,15 +195,26 @@ __device__ __forceinline__ void dex_load_rec(const float* __restrict__ rec, int 
 struct DexCavTab {
   double dlam[DEX_NLINES][DEX_W];    // lambda - lambda0
   double r2[DEX_NLINES][DEX_W];      // (lambda / lambda0)^2:  a(lambda) = r2 a(lambda0)                 (eq. 20)
+  float dlam_h[DEX_NLINES][DEX_W];   // the same two as fp32 (dlam as an unevaluated pair hi + lo) for the fp32 Voigt
+  float dlam_l[DEX_NLINES][DEX_W];
+  float r2f[DEX_NLINES][DEX_W];
+  float r2lo[DEX_NLINES], r2hi[DEX_NLINES];   // min / max of r2f over the batch (slightly widened): damping window test
   float scale[DEX_NLINES][DEX_W];    // (lambda0 / lambda) / sqrt(pi): eta*(lambda) phi = eta*0 invD scale H (eqs. 18-19)
   double lam0_over_c[DEX_NLINES];    // Doppler shift of the line centre per unit projected velocity     (eq. 14)
   int line[DEX_NLINES];              // active line of slot q or -1
 };
 
+// the literal fp64 formula for damping outside the fp32 window: rare, so kept out of line (it would otherwise be
+// inlined 8 x DEX_NLINES times and set the register count of the whole kernel)
+__device__ __noinline__ float dex_voigt_H_outside_window(const double* __restrict__ wc, double L, double a, double x) {
+  return (float)dex_voigt_H_march(wc, L, a, x);
+}
+
 // eta, chi of one cell for this lane's wavelengths, seen along propagation direction om (a7)
 template <int D, int VAR, int LPT>
 __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_base, int cell, int sub,
                                              const float* __restrict__ om, const DexCavTab& CT,
+                                             const float4* __restrict__ vfw, const float* __restrict__ vfc,
                                              const float* __restrict__ iso0, const float* __restrict__ iso1,
                                              float (&eta)[LPT], float (&chi)[LPT]) {
   if (VAR == DEX_ISO) {   // march records, two planes of 32-byte rows: chi[] receives chi log2(e), eta[] S = eta/chi
@@ -243,19 +254,70 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
   // Weideman form cancels in the wings); the line sum itself is fp32.  Everything that depends
   // on (wavelength, line) alone comes from the block's shared table CT (one batch per block).
   dex_load_rec<LPT>(M.store + (batch_base + (size_t)cell) * DEX_REC, sub, eta, chi);
-#pragma unroll
-  for (int q = 0; q < DEX_NLINES; ++q) {
+#pragma unroll 1
+  for (int q = 0; q < DEX_NLINES; ++q) {   // not unrolled: the body is ~500 instructions and would be copied 4 times
     const int l = CT.line[q];
     if (l < 0) continue;               // block-uniform
     const float4 ln = __ldg(M.line + (size_t)cell * M.n_lines + l);
-    const double a0 = (double)ln.z, invD = (double)ln.w;
     const double shift = vproj * CT.lam0_over_c[q];
+    const float sh_h = (float)shift, sh_l = (float)(shift - (double)sh_h);
     const float es = ln.x * ln.w, cs = ln.y * ln.w;
+    float H[LPT];
+    if (ln.z * CT.r2lo[q] >= DEX_VF_A_LO && ln.z * CT.r2hi[q] <= DEX_VF_A_HI) {
+      // fp32 table form for every wavelength of the batch, branch free so that the LPT evaluations interleave
+      bool far = false;
+      float xh[LPT], af[LPT];
+      if (LPT == 1) {
+        const int j = sub;
+        af[0] = CT.r2f[q][j] * ln.z;
+        const float dh = CT.dlam_h[q][j];
+        const float sm = dh + sh_h, bb = sm - dh;
+        const float se = ((dh - (sm - bb)) + (sh_h - bb)) + (CT.dlam_l[q][j] + sh_l);
+        xh[0] = sm * ln.w;
+        const float xl = fmaf(se, ln.w, fmaf(sm, ln.w, -xh[0]));
+        H[0] = dex_voigt_H_table(vfw, vfc, af[0], xh[0], xl);
+        far = fabsf(xh[0]) + af[0] >= 15.0f;
+      } else {
+        // x = (dlam + shift) / dlamD as an fp32 pair: two-sum of the leading parts, two-product with 1/dlamD;
+        // two wavelengths per packed instruction
+        const float2 shh = dex_f2(sh_h), nshh = dex_f2(-sh_h), shl = dex_f2(sh_l), inv2 = dex_f2(ln.w), a02 = dex_f2(ln.z);
+#pragma unroll
+        for (int i = 0; i < LPT / 2; ++i) {
+          const int j = sub * LPT + 2 * i;
+          const float2 a2 = __fmul2_rn(*reinterpret_cast<const float2*>(&CT.r2f[q][j]), a02);
+          const float2 dh = *reinterpret_cast<const float2*>(&CT.dlam_h[q][j]);
+          const float2 dl = *reinterpret_cast<const float2*>(&CT.dlam_l[q][j]);
+          const float2 sm = __fadd2_rn(dh, shh);
+          const float2 bb = __fadd2_rn(sm, dex_neg2(dh));
+          const float2 e1 = __fadd2_rn(dh, dex_neg2(__fadd2_rn(sm, dex_neg2(bb))));
+          const float2 e2 = __fadd2_rn(shh, dex_neg2(bb));
+          const float2 se = __fadd2_rn(__fadd2_rn(e1, e2), __fadd2_rn(dl, shl));
+          const float2 x2 = __fmul2_rn(sm, inv2);
+          const float2 xl = __ffma2_rn(se, inv2, __ffma2_rn(sm, inv2, dex_neg2(x2)));
+          const float2 h2 = dex_voigt_H_table2(vfw, vfc, a2, x2, xl);
+          af[2 * i] = a2.x; af[2 * i + 1] = a2.y;
+          xh[2 * i] = x2.x; xh[2 * i + 1] = x2.y;
+          H[2 * i] = h2.x; H[2 * i + 1] = h2.y;
+          far = far || (fabsf(x2.x) + a2.x >= 15.0f) || (fabsf(x2.y) + a2.y >= 15.0f);
+        }
+        (void)nshh;
+      }
+      if (far) {
+#pragma unroll
+        for (int i = 0; i < LPT; ++i)
+          if (fabsf(xh[i]) + af[i] >= 15.0f) H[i] = dex_voigt_H_region1(af[i], xh[i]);
+      }
+    } else {
+#pragma unroll 1
+      for (int i = 0; i < LPT; ++i) {
+        const int j = sub * LPT + i;
+        const double x = (CT.dlam[q][j] + shift) * (double)ln.w;
+        H[i] = dex_voigt_H_outside_window(M.wei_c, M.wei_L, CT.r2[q][j] * (double)ln.z, x);
+      }
+    }
 #pragma unroll
     for (int i = 0; i < LPT; ++i) {
-      const int j = sub * LPT + i;
-      const double x = (CT.dlam[q][j] + shift) * invD;
-      const float phi = (float)dex_voigt_H_march(M.wei_c, M.wei_L, CT.r2[q][j] * a0, x) * CT.scale[q][j];
+      const float phi = H[i] * CT.scale[q][sub * LPT + i];
       eta[i] = fmaf(es, phi, eta[i]);
       chi[i] = fmaf(cs, phi, chi[i]);
     }
@@ -282,7 +344,7 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
 #define DEX_MINB_VEL 5
 #endif
 #ifndef DEX_MINB_CAV
-#define DEX_MINB_CAV 3
+#define DEX_MINB_CAV 4
 #endif
 constexpr int dex_march_minb(int var) {
   return var == DEX_ISO ? DEX_MARCH_MINB : (var == DEX_VELINTERP ? DEX_MINB_VEL : DEX_MINB_CAV);
@@ -316,7 +378,13 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   if (VAR == DEX_ISO) asm volatile("" : "+l"(iso0), "+l"(iso1));
   const float* __restrict__ probe = R.probe_pos + gid * D;
   __shared__ DexCavTab CT;
+  __shared__ float4 vfw[VAR == DEX_CAV ? DEX_VF_NODES : 1];
+  __shared__ float vfc[VAR == DEX_CAV ? DEX_VF_NODES : 1];
   if (VAR == DEX_CAV) {
+    for (int i = threadIdx.x; i < DEX_VF_NODES; i += DEX_MARCH_THREADS) {
+      vfw[i] = __ldg(M.vf_wing + i);
+      vfc[i] = __ldg(M.vf_core + i);
+    }
     if (threadIdx.x < DEX_NLINES * DEX_W) {
       const int q = threadIdx.x / DEX_W, j = threadIdx.x % DEX_W;
       const int l = M.active_lines[batch * DEX_NLINES + q];
@@ -326,8 +394,21 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
         const double r = lm / l0;
         CT.dlam[q][j] = lm - l0;
         CT.r2[q][j] = r * r;
+        CT.dlam_h[q][j] = (float)(lm - l0);
+        CT.dlam_l[q][j] = (float)((lm - l0) - (double)CT.dlam_h[q][j]);
+        CT.r2f[q][j] = (float)(r * r);
         CT.scale[q][j] = (float)((l0 / lm) * 0.56418958354775628695);
-        if (j == 0) CT.lam0_over_c[q] = l0 / M.c_light;
+        if (j == 0) {
+          CT.lam0_over_c[q] = l0 / M.c_light;
+          double lo = 1e300, hi = 0.0;
+          for (int jj = 0; jj < DEX_W; ++jj) {
+            const double rr = (double)__ldg(M.lam + batch * DEX_W + jj) / l0;
+            lo = fmin(lo, rr * rr);
+            hi = fmax(hi, rr * rr);
+          }
+          CT.r2lo[q] = (float)(lo * (1.0 - 1e-6));
+          CT.r2hi[q] = (float)(hi * (1.0 + 1e-6));
+        }
       }
     }
     __syncthreads();
@@ -365,7 +446,7 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
           ++nseg;
           const float hds = G.h * ds;
           float eta[LPT], chi[LPT];
-          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, CT, iso0, iso1, eta, chi);
+          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, CT, vfw, vfc, iso0, iso1, eta, chi);
           if (VAR == DEX_ISO) dex_accumulate_all_S<LPT>(eta, chi, hds, I, T);
           else dex_accumulate_all<LPT>(eta, chi, hds, I, T);
         }
@@ -505,6 +586,23 @@ __global__ void dex_reduce_j_kernel(long long n_probes, int n_dirs, int n_lambda
   J[i] = acc;
 }
 
+// validation (dex_voigt_profile): the march's own Voigt routines on caller-supplied (a, x)
+struct DexWeideman { double c[DEX_WEI_N]; double L; };
+__global__ void dex_voigt_profile_kernel(const float* __restrict__ a, const double* __restrict__ x, long long n,
+                                         double* __restrict__ H, int mode, const DexWeideman Wc,
+                                         const float4* __restrict__ wing, const float* __restrict__ core) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float af = a[i];
+  const double xd = x[i];
+  if (mode == 0 && af >= DEX_VF_A_LO && af <= DEX_VF_A_HI) {
+    const float xh = (float)xd, xl = (float)(xd - (double)xh);
+    H[i] = (double)dex_voigt_H_fast(wing, core, af, xh, xl);
+  } else {
+    H[i] = dex_voigt_H_march(Wc.c, Wc.L, (double)af, xd);
+  }
+}
+
 template <int D, int VAR, int LPR>
 dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
                           unsigned long long* d_seg, const int* perm, cudaStream_t st) {
@@ -625,6 +723,25 @@ dex_status dex_launch_capture(const dex_grid* g, const dex_mips* m, const DexRay
                                                             cap->batch, d_overflow);
   dex_count_launch();
   DEX_CUDA_CHECK(cudaGetLastError());
+  return DEX_OK;
+}
+
+dex_status dex_launch_voigt_profile(const float* d_a, const double* d_x, long long n, double* d_H, int mode, cudaStream_t st) {
+  if (n <= 0) return DEX_OK;
+  DexWeideman Wc;
+  dex_weideman_coefficients(Wc.c, &Wc.L);
+  float* d_tab = nullptr;
+  DEX_CUDA_CHECK(cudaMallocAsync((void**)&d_tab, sizeof(float) * DEX_VF_NODES * 5, st));
+  cudaError_t e = cudaMemcpyAsync(d_tab, dex_voigt_fast_table_host(), sizeof(float) * DEX_VF_NODES * 5, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) {
+    const long long gx = (n + 255) / 256;
+    dex_voigt_profile_kernel<<<(unsigned)gx, 256, 0, st>>>(d_a, d_x, n, d_H, mode, Wc, (const float4*)d_tab,
+                                                           d_tab + (size_t)DEX_VF_NODES * 4);
+    dex_count_launch();
+    e = cudaGetLastError();
+  }
+  cudaFreeAsync(d_tab, st);
+  DEX_CUDA_CHECK(e);
   return DEX_OK;
 }
 

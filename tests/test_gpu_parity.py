@@ -317,3 +317,24 @@ def test_host_entry_matches_device_path(P, name, kw):
                                   metric=1, thr_eta=0.0, thr_chi=0.0, tau_gate=-1.0,
                                   eta=torch.zeros(64 * 60 * 8), chi=torch.zeros(64 * 60 * 8)),
                                   P.Rays(torch.zeros(1, 2), torch.ones(1, 2), torch.ones(1)), torch.zeros(1, 8))
+
+
+# ------------------------------------------------------------------------------------------ Voigt function
+def test_voigt_profile_against_oracle(P):
+    """H(a, x) as the Core-and-Voigt march evaluates it (dex_voigt_profile) against the oracle's HUM1WEI24
+    (PAPER.md:329): the fp64 form to 1e-9, the fp32 table form (damping window of csrc/dex_voigt.cuh) to 1e-6,
+    across the core, the wings, the region-I switch at |x| + a = 15 and far beyond it."""
+    rng = np.random.default_rng(5)
+    x = np.concatenate([rng.uniform(-15.5, 15.5, 200000), rng.uniform(-4, 4, 100000), [0.0, 14.99, 15.0, -15.0, 40.0, 3e3, -2e5],
+                        np.arange(0, 481) / 32.0, (np.arange(0, 480) + 0.5) / 32.0])
+    for a0 in (1e-4, 4.9e-3, 5e-3, 0.01, 0.02, 0.03, 0.031, 0.3, 2.0):
+        a = np.full(x.shape, a0, dtype=np.float32)
+        ref = orc.voigt_H(a.astype(np.float64), x)
+        ta, tx = torch.from_numpy(a).cuda(), torch.from_numpy(x).cuda()
+        # lanes whose |x| + a lies within rounding of the switch may take the other branch (5e-5 apart there)
+        near = np.abs(np.abs(x) + a0 - 15.0) < 1e-5
+        H64 = P.dex_voigt_profile(ta, tx, mode=1).cpu().numpy()
+        assert max_rel(H64[~near], ref[~near]) <= 1e-9, f"a={a0}"
+        H = P.dex_voigt_profile(ta, tx, mode=0).cpu().numpy()
+        assert max_rel(H[~near], ref[~near]) <= 1e-6, f"a={a0}"
+        assert max_rel(H[near], ref[near]) <= 1e-4
