@@ -214,7 +214,9 @@ dex_status dex_march_timing_read(double* ms_total, int64_t* n_launches, int rese
 dex_status dex_set_lanes_per_ray(int lanes);
 /* Kernel-structure knobs for performance experiments (results do not change): "lanes_per_ray" 1/2/4/8;
  * "tile_probes" 0/1 (1, default: probes are handed to warps in compact spatial tiles by an internal counting
- * sort instead of in the caller's order). */
+ * sort instead of in the caller's order); "voigt_fp32" 0/1 (1, default: the Core-and-Voigt march evaluates H(a, x) in
+ * its fp32 table form inside the damping window of csrc/dex_voigt.cuh; 0: the fp64 form everywhere -- results agree
+ * to ~1e-6). */
 dex_status dex_set_tuning(const char* name, int value);
 
 #ifdef __cplusplus

@@ -17,6 +17,7 @@ std::atomic<long long> g_launches{0};
 std::atomic<int> g_lanes_per_ray{1};  // measured fastest on B200 (profiles/)
 std::atomic<int> g_timing{0};
 std::atomic<int> g_tile_probes{1};
+std::atomic<int> g_voigt_fp32{1};
 std::mutex g_timing_mu;
 struct EvPair { cudaEvent_t a, b; };
 std::vector<EvPair> g_events;
@@ -147,6 +148,7 @@ const float* dex_voigt_fast_table_host() {
 
 void dex_set_error(const std::string& msg) { g_last_error = msg; }
 void dex_count_launch(int n) { g_launches.fetch_add(n); }
+int dex_tuning_voigt_fp32() { return g_voigt_fp32.load(); }
 
 extern "C" {
 
@@ -167,6 +169,7 @@ dex_status dex_set_tuning(const char* name, int value) {
   if (!name) { dex_set_error("NULL tuning name"); return DEX_ERR_INVALID_ARG; }
   if (!strcmp(name, "lanes_per_ray")) return dex_set_lanes_per_ray(value);
   if (!strcmp(name, "tile_probes")) { g_tile_probes.store(value ? 1 : 0); return DEX_OK; }
+  if (!strcmp(name, "voigt_fp32")) { g_voigt_fp32.store(value ? 1 : 0); return DEX_OK; }
   dex_set_error("unknown tuning knob");
   return DEX_ERR_INVALID_ARG;
 }

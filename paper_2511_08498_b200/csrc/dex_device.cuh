@@ -54,6 +54,7 @@ struct DexMipsDev {
   double wei_L;
   const float4* vf_wing;             // [DEX_VF_NODES] Taylor coefficients of Im F about the nodes (dex_voigt.cuh)
   const float* vf_core;              // [DEX_VF_NODES] e^{-x_k^2}
+  int voigt_fp32;                    // 0: fp64 HUM1WEI24 everywhere (tuning knob "voigt_fp32")
 };
 
 struct DexRaysDev {

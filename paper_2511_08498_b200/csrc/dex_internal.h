@@ -40,6 +40,7 @@ struct dex_mips {
 
 void dex_set_error(const std::string& msg);
 void dex_count_launch(int n = 1);
+int dex_tuning_voigt_fp32();
 
 // grid_build.cu
 dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStream_t st);

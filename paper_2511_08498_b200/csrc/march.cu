@@ -37,10 +37,14 @@ __device__ __forceinline__ void dex_accumulate(float eta, float chi, float hds, 
   p = fmaf(p, tau, -1.0f / 6.0f);
   p = fmaf(p, tau, 0.5f);
   p = fmaf(-p, tau, 1.0f);
-  const float q = (1.0f - e) * dex_rcp(fmaxf(tau, 0.25f));
-  const float E = (tau < 0.25f) ? p : q;
+  const float ome = 1.0f - e;
+  const float q = ome * dex_rcp(fmaxf(tau, 0.25f));
+  const bool thin = tau < 0.25f;
+  const float E = thin ? p : q;
   I = fmaf(T, (eta * hds) * E, I);
-  T *= e;
+  // T <- T e^-tau as T - T (1 - e^-tau) with the expm1-quality (1 - e^-tau): in the thin regime the product of a
+  // thousand ex2.approx results (2^-22 each) is what limited long rays to ~1e-5; one rounding per segment now
+  T = fmaf(-T, thin ? tau * p : ome, T);
 }
 
 // The same for two wavelengths at once with Blackwell's packed fp32 pipe (FFMA2 / FMUL2): the kernel is
@@ -61,12 +65,16 @@ __device__ __forceinline__ void dex_accumulate2(float2 eta, float2 chi, float2 h
   float2 r;
   r.x = dex_rcp(fmaxf(tau.x, 0.25f));
   r.y = dex_rcp(fmaxf(tau.y, 0.25f));
-  const float2 q = __fmul2_rn(__ffma2_rn(e, make_float2(-1.0f, -1.0f), make_float2(1.0f, 1.0f)), r);
-  float2 E;
+  const float2 ome = __ffma2_rn(e, make_float2(-1.0f, -1.0f), make_float2(1.0f, 1.0f));
+  const float2 q = __fmul2_rn(ome, r);
+  const float2 tp = __fmul2_rn(tau, p);
+  float2 E, w;
   E.x = (tau.x < 0.25f) ? p.x : q.x;
   E.y = (tau.y < 0.25f) ? p.y : q.y;
+  w.x = (tau.x < 0.25f) ? tp.x : ome.x;
+  w.y = (tau.y < 0.25f) ? tp.y : ome.y;
   I = __ffma2_rn(T, __fmul2_rn(__fmul2_rn(eta, hds2), E), I);
-  T = __fmul2_rn(T, e);
+  T = __ffma2_rn(make_float2(-T.x, -T.y), w, T);      // T - T (1 - e^-tau), see dex_accumulate
 }
 
 // ISO march records (make_march_records_kernel): plane 0 holds chi2 = chi log2(e), plane 1 holds S = eta/chi.
@@ -95,7 +103,7 @@ __device__ __forceinline__ void dex_accumulate_S2(float2 S, float2 chi2, float2 
   if (y.x < DEX_OME_YTHR) p.x = 1.0f - e.x;
   if (y.y < DEX_OME_YTHR) p.y = 1.0f - e.y;
   I = __ffma2_rn(T, __fmul2_rn(S, p), I);
-  T = __fmul2_rn(T, e);
+  T = __ffma2_rn(make_float2(-T.x, -T.y), p, T);      // T - T (1 - e^-tau), see dex_accumulate
 }
 
 __device__ __forceinline__ void dex_accumulate_S1(float S, float chi2, float nhds, float& I, float& T) {
@@ -108,7 +116,7 @@ __device__ __forceinline__ void dex_accumulate_S1(float S, float chi2, float nhd
   p *= y;
   if (y < DEX_OME_YTHR) p = 1.0f - e;
   I = fmaf(T, S * p, I);
-  T *= e;
+  T = fmaf(-T, p, T);
 }
 
 template <int LPT>
@@ -263,7 +271,7 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
     const float sh_h = (float)shift, sh_l = (float)(shift - (double)sh_h);
     const float es = ln.x * ln.w, cs = ln.y * ln.w;
     float H[LPT];
-    if (ln.z * CT.r2lo[q] >= DEX_VF_A_LO && ln.z * CT.r2hi[q] <= DEX_VF_A_HI) {
+    if (M.voigt_fp32 && ln.z * CT.r2lo[q] >= DEX_VF_A_LO && ln.z * CT.r2hi[q] <= DEX_VF_A_HI) {
       // fp32 table form for every wavelength of the batch, branch free so that the LPT evaluations interleave
       bool far = false;
       float xh[LPT], af[LPT];
@@ -349,6 +357,9 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
 constexpr int dex_march_minb(int var) {
   return var == DEX_ISO ? DEX_MARCH_MINB : (var == DEX_VELINTERP ? DEX_MINB_VEL : DEX_MINB_CAV);
 }
+#ifndef DEX_FOLD_EVERY
+#define DEX_FOLD_EVERY 32   // power of two
+#endif
 #ifndef DEX_CROSS_QUORUM
 #define DEX_CROSS_QUORUM 8
 #endif
@@ -414,6 +425,19 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
     __syncthreads();
   }
   // J is touched once per direction, I and T once per segment: J lives in shared memory ([i][thread], conflict-free)
+  // I is accumulated on two levels: I[] (registers) holds the sum over the last <= DEX_FOLD_EVERY iterations of the
+  // warp's loop, Ih[] (shared memory, [i][thread], conflict free) everything before.  With one level, a ray of ~1000
+  // thin segments whose optical depth builds up slowly loses every far contribution below ulp(I)/2: -1.07e-5 relative
+  // on C3's longest rays (measured; the rounding of I alone, everything else held in fp64); with two levels the same
+  // rays are within 1.6e-6.  The fold points depend on the warp's iteration count, i.e. on which rays share a warp;
+  // dex_tile_probes makes that a pure function of the probe array, so results are reproducible bit for bit.
+#ifndef DEX_IH_REGISTERS
+  __shared__ float Ihs[LPT * DEX_MARCH_THREADS];
+#define DEX_IH(i) Ihs[(i) * DEX_MARCH_THREADS + threadIdx.x]
+#else
+  float Ih[LPT];
+#define DEX_IH(i) Ih[i]
+#endif
   float I[LPT], T[LPT];
   if (FUSE_J) {
 #pragma unroll
@@ -424,12 +448,16 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   for (int k = 0; k < R.n_dirs; ++k) {
     const float* __restrict__ om = R.dirs + k * D;
 #pragma unroll
-    for (int i = 0; i < LPT; ++i) { I[i] = 0.0f; T[i] = 1.0f; }
+    for (int i = 0; i < LPT; ++i) { I[i] = 0.0f; DEX_IH(i) = 0.0f; T[i] = 1.0f; }
     bool alive = valid && dex_ray_init3<D>(ray, G, M, binfo, probe, om);
     bool blocked = false;   // waiting at a brick face for dex_ray_cross (implies alive)
-    for (;;) {
+    for (unsigned it = 1;; ++it) {
       const unsigned am = __ballot_sync(FULL, alive);
       if (am == 0u) break;
+      if ((it & (DEX_FOLD_EVERY - 1)) == 0) {   // warp-uniform, so the fold costs < 1 % (a per-ray trigger diverges: +8 %)
+#pragma unroll
+        for (int i = 0; i < LPT; ++i) { DEX_IH(i) += I[i]; I[i] = 0.0f; }
+      }
       const unsigned bm = __ballot_sync(FULL, blocked);
       if (bm == am || __popc(bm) >= DEX_CROSS_QUORUM) {
         if (blocked) {
@@ -453,6 +481,8 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
       }
     }
     if (valid) {
+#pragma unroll
+      for (int i = 0; i < LPT; ++i) I[i] += DEX_IH(i);
       if (R.i0 != nullptr) {
 #pragma unroll
         for (int i = 0; i < LPT; ++i) I[i] = fmaf(T[i], __ldg(R.i0 + (size_t)k * M.n_lambda + lam_off + i), I[i]);
@@ -573,6 +603,24 @@ __global__ void dex_tile_scatter_kernel(const DexTiling TL, long long n, const f
   if (i < n) perm[atomicAdd(cursor + dex_tile_of<D>(TL, pos + i * D), 1)] = (int)i;
 }
 
+// The atomic scatter leaves the members of a tile in arrival order; ranking them by probe index makes perm -- and with
+// it the composition of every warp -- a pure function of the probe array.  One thread per probe counts the members of
+// its tile with a smaller index (tiles hold ~32 probes on a regular lattice; any size is handled, in O(size) reads).
+template <int D>
+__global__ void dex_tile_rank_kernel(const DexTiling TL, long long n, const float* __restrict__ pos,
+                                     const int* __restrict__ cursor, const int* __restrict__ perm_in,
+                                     int* __restrict__ perm_out) {
+  const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  const int p = perm_in[s];
+  const int t = dex_tile_of<D>(TL, pos + (long long)p * D);
+  const int begin = (t == 0) ? 0 : cursor[t - 1];      // after the scatter cursor[t] is the END of tile t
+  const int end = cursor[t];
+  int rank = 0;
+  for (int q = begin; q < end; ++q) rank += (perm_in[q] < p) ? 1 : 0;
+  perm_out[begin + rank] = p;
+}
+
 // J(p, lambda) = sum_k w_k I(p, k, lambda) from a materialised I: one thread per (probe, lambda);
 // consecutive threads read consecutive lambda (coalesced).
 __global__ void dex_reduce_j_kernel(long long n_probes, int n_dirs, int n_lambda, const float* __restrict__ w,
@@ -615,10 +663,12 @@ dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev
     return DEX_ERR_UNSUPPORTED;
   }
   dim3 grid((unsigned)gx, (unsigned)m->n_batch, 1);
+  DexMipsDev md = m->dev;
+  md.voigt_fp32 = dex_tuning_voigt_fp32();
   if (fuse_j)
-    dex_march_kernel<D, VAR, LPR, true><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
+    dex_march_kernel<D, VAR, LPR, true><<<grid, threads, 0, st>>>(g->dev, md, rays, perm, d_out, d_seg);
   else
-    dex_march_kernel<D, VAR, LPR, false><<<grid, threads, 0, st>>>(g->dev, m->dev, rays, perm, d_out, d_seg);
+    dex_march_kernel<D, VAR, LPR, false><<<grid, threads, 0, st>>>(g->dev, md, rays, perm, d_out, d_seg);
   dex_count_launch();
   DEX_CUDA_CHECK(cudaGetLastError());
   return DEX_OK;
@@ -681,8 +731,13 @@ static dex_status tile_probes_t(const dex_grid* g, const DexRaysDev& rays, int**
   const unsigned blocks = (unsigned)((n + 255) / 256);
   dex_tile_count_kernel<D><<<blocks, 256, 0, st>>>(TL, n, rays.probe_pos, d_count);
   dex_tile_scan_kernel<<<1, 1024, 0, st>>>(d_count, TL.n_tiles);
-  dex_tile_scatter_kernel<D><<<blocks, 256, 0, st>>>(TL, n, rays.probe_pos, d_count, *d_perm);
-  dex_count_launch(3);
+  int* d_arrival = nullptr;
+  e = cudaMallocAsync((void**)&d_arrival, sizeof(int) * (size_t)n, st);
+  if (e != cudaSuccess) { cudaFreeAsync(d_count, st); cudaFreeAsync(*d_perm, st); *d_perm = nullptr; DEX_CUDA_CHECK(e); }
+  dex_tile_scatter_kernel<D><<<blocks, 256, 0, st>>>(TL, n, rays.probe_pos, d_count, d_arrival);
+  dex_tile_rank_kernel<D><<<blocks, 256, 0, st>>>(TL, n, rays.probe_pos, d_count, d_arrival, *d_perm);
+  dex_count_launch(4);
+  cudaFreeAsync(d_arrival, st);
   cudaFreeAsync(d_count, st);
   DEX_CUDA_CHECK(cudaGetLastError());
   return DEX_OK;

@@ -89,3 +89,53 @@ def max_rel(a, b):
     with np.errstate(all="ignore"):
         r = np.where(diff == 0.0, 0.0, diff / den)
     return float(np.max(r)) if r.size else 0.0
+
+
+def crop_workload(wl, lo, size):
+    """Sub-grid [lo, lo + size) (voxels, brick aligned, per axis x, y[, z]) of a workload with the same fields and
+    build parameters and no rays.  Mips, cell tests and brick levels are brick-local, so building the crop must give
+    exactly the full grid's result for these bricks: this is how the full-size builds are checked against the oracle
+    without running the (slow, numpy) oracle build over the whole grid."""
+    import copy
+    nd = wl.ndim
+    lo = tuple(int(v) for v in lo) + (0,) * (3 - nd)
+    size = tuple(int(v) for v in size) + (1,) * (3 - nd)
+    assert all(l % wl.brick == 0 and s % wl.brick == 0 for l, s in zip(lo[:nd], size[:nd]))
+    nx, ny, nz = wl.dims
+    sl = (slice(lo[2], lo[2] + size[2]), slice(lo[1], lo[1] + size[1]), slice(lo[0], lo[0] + size[0]))
+
+    def per_voxel(a):            # [nvox][...]
+        if a is None:
+            return None
+        g = a.reshape((nz, ny, nx) + a.shape[1:])[sl]
+        return np.ascontiguousarray(g.reshape((-1,) + a.shape[1:]))
+
+    def per_line(a):             # [n_lines][nvox]
+        if a is None:
+            return None
+        g = a.reshape((a.shape[0], nz, ny, nx))[(slice(None),) + sl]
+        return np.ascontiguousarray(g.reshape(a.shape[0], -1))
+
+    out = copy.copy(wl)
+    out.dims = size
+    out.active = per_voxel(wl.active)
+    for name in ("eta", "chi", "eta_bg", "chi_bg", "vel"):
+        setattr(out, name, per_voxel(getattr(wl, name)))
+    for name in ("eta_star0", "chi_star0", "a0", "inv_dlamD"):
+        setattr(out, name, per_line(getattr(wl, name)))
+    out.probe_pos = np.zeros((0, nd), dtype=np.float32)
+    return out
+
+
+def crop_brick_ids(wl, lo, size):
+    """Brick indices (in the full grid's numbering) of the bricks of the crop, in the crop's own brick order."""
+    nd, b = wl.ndim, wl.brick
+    lo = tuple(int(v) for v in lo) + (0,) * (3 - nd)
+    size = tuple(int(v) for v in size) + (b,) * (3 - nd)
+    bd = wl.brick_dims
+    ids = []
+    for bz in range(lo[2] // b, lo[2] // b + (size[2] // b if nd == 3 else 1)):
+        for by in range(lo[1] // b, (lo[1] + size[1]) // b):
+            for bx in range(lo[0] // b, (lo[0] + size[0]) // b):
+                ids.append((bz * bd[1] + by) * bd[0] + bx)
+    return np.asarray(ids, dtype=np.int64)

@@ -15,7 +15,8 @@ torch = pytest.importorskip("torch")
 from oracle import oracle as orc           # noqa: E402
 from workloads import make                 # noqa: E402
 from workloads.gen import dirs_2d          # noqa: E402
-from _util import fig5_levels, iso_workload, max_rel, random_unit_dirs, unit_dirs_2d   # noqa: E402
+from _util import (crop_brick_ids, crop_workload, fig5_levels, iso_workload, max_rel, random_unit_dirs,   # noqa: E402
+                   unit_dirs_2d)
 
 TOL = 1e-5
 
@@ -338,3 +339,87 @@ def test_voigt_profile_against_oracle(P):
         H = P.dex_voigt_profile(ta, tx, mode=0).cpu().numpy()
         assert max_rel(H[~near], ref[~near]) <= 1e-6, f"a={a0}"
         assert max_rel(H[near], ref[near]) <= 1e-4
+
+
+# ------------------------------------------------------------------------------------------ full size, C3-C5
+def _crops(wl, rng, n_crops, side_bricks):
+    """Seeded brick-aligned boxes that contain active bricks."""
+    b, nd = wl.brick, wl.ndim
+    act = orc.brick_active(wl)
+    bd = wl.brick_dims
+    out = []
+    while len(out) < n_crops:
+        lo_b = [int(rng.integers(0, bd[a] - side_bricks + 1)) for a in range(nd)]
+        lo = [v * b for v in lo_b]
+        size = [side_bricks * b] * nd
+        ids = crop_brick_ids(wl, lo, size)
+        if act[ids].any():
+            out.append((lo, size, ids))
+    return out
+
+
+@pytest.mark.parametrize("name,side", [("C3", 6), ("C4", 6), ("C5", 3)])
+def test_full_size_build_on_crops(P, name, side):
+    """BASELINE-size builds (configs[2..4]): slot table exact over the whole grid; level table, packed words and
+    every mip chain exact against the oracle on seeded crops (the build is brick-local, see crop_workload)."""
+    wl = make(name, n_probes=64)
+    dw, grid, mips = _build(P, wl)
+    act = orc.brick_active(wl)
+    slots = grid.slots()
+    assert np.array_equal(slots >= 0, act)
+    lv = mips.levels()
+    assert ((lv >= 0) == act[None, :]).all()
+    full = {}
+    rng = np.random.default_rng(99)
+    for lo, size, ids in _crops(wl, rng, 3, side):
+        cw = crop_workload(wl, lo, size)
+        Mc = orc.build_mips(cw)
+        assert np.array_equal(lv[:, ids], Mc.levels), f"{name}: levels differ in the crop at {lo}"
+        nd = wl.ndim
+        for m in range(Mc.max_level + 1):
+            sl = tuple(slice(lo[a] >> m, (lo[a] + size[a]) >> m) for a in reversed(range(nd)))
+            mask = _active_cell_mask(cw, orc.brick_active(cw), m)
+            for chain, ref in ((P.DEX_CHAIN_ETA, Mc.eta[m]), (P.DEX_CHAIN_CHI, Mc.chi[m])):
+                if (chain, m) not in full:
+                    full[(chain, m)] = mips.level_data(chain, m)
+                got = full[(chain, m)][sl]
+                assert np.array_equal(got[mask].view(np.uint32), np.ascontiguousarray(ref)[mask].view(np.uint32))
+            if (P.DEX_CHAIN_VEL, m) not in full:
+                full[(P.DEX_CHAIN_VEL, m)] = mips.level_data(P.DEX_CHAIN_VEL, m)
+            vel = full[(P.DEX_CHAIN_VEL, m)][sl]
+            assert np.array_equal(vel[mask][:, :nd].view(np.uint32), np.ascontiguousarray(Mc.vbar[m])[mask].view(np.uint32))
+            assert np.array_equal(vel[mask][:, 3].view(np.uint32), np.ascontiguousarray(Mc.vmax[m])[mask].view(np.uint32))
+    hist = [int((lv == m).sum()) for m in range(-1, wl.max_level + 1)]
+    assert sum(hist) == lv.size          # Table-2 style histogram covers every (batch, brick)
+
+
+@pytest.mark.parametrize("name", ["C3", "C5"])
+def test_full_size_march_sampled(P, name):
+    """BASELINE-size grids (configs[2], configs[4]): (i) Classic (level 0, per-voxel velocity) I and J of seeded probes
+    against the oracle's plain AW87 march over the dense arrays -- needs no oracle mip build; (ii) the fused VLM march
+    over ALL probes (the launch configuration bench.py times) against the materialised-I path on the sampled probes."""
+    wl = make(name)
+    dw, grid, mips = _build(P, wl)
+    all_probes = wl.probe_pos
+    seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+    J_all = P.pipeline.mean_intensity(dw, grid, mips, segment_count=seg).cpu().numpy()
+    assert int(seg.item()) > 0 and np.isfinite(J_all).all() and (J_all >= 0).all()
+    rng = np.random.default_rng(31)
+    idx = np.sort(rng.choice(all_probes.shape[0], size=96, replace=False))
+    wl.probe_pos = np.ascontiguousarray(all_probes[idx])
+    dw.t["probe_pos"] = torch.from_numpy(wl.probe_pos).cuda()
+    P.dex_set_lanes_per_ray(8)
+    I, _ = P.pipeline.formal_solution(dw, grid, mips)
+    P.dex_set_lanes_per_ray(1)
+    J2 = torch.empty((idx.size, wl.n_lambda), dtype=torch.float32, device="cuda:0")
+    P.dex_mean_intensity(grid, mips, P.pipeline.rays(dw), J2, I)
+    assert max_rel(J_all[idx], J2.cpu().numpy().astype(np.float64)) <= 2e-6
+    # (i) exact side at full size against the oracle
+    wl.probe_pos = np.ascontiguousarray(wl.probe_pos[:24])
+    dw.t["probe_pos"] = torch.from_numpy(wl.probe_pos).cuda()
+    A = orc.plain_march(wl, variant=orc.CLASSIC)
+    mc = P.pipeline.build_mips(dw, grid, variant=P.DEX_CLASSIC)
+    Ic, _ = P.pipeline.formal_solution(dw, grid, mc)
+    assert max_rel(Ic.cpu().numpy(), A.I) <= TOL
+    Jc = P.pipeline.mean_intensity(dw, grid, mc).cpu().numpy()
+    assert max_rel(Jc, orc.mean_intensity(A.I, wl.weights)) <= TOL

@@ -139,3 +139,22 @@ def test_two_rank_gloo_probe_sharding(tmp_path):
         assert tots[r][0] == 11.0                       # max over ranks of (10, 11)
         assert tots[r][1] == tots[r][2] == float(res.segments)
     assert tots[0][3] == 0 and tots[0][4] == tots[1][3] and tots[1][4] == 150
+
+
+def test_crop_workload_is_brick_local():
+    """tests/_util.crop_workload (used by the full-size GPU build tests): the oracle build of a brick-aligned crop
+    equals the oracle build of the whole grid restricted to the crop's bricks."""
+    from oracle import oracle as orc
+    from workloads import make
+    from _util import crop_brick_ids, crop_workload
+    for name, n, lo, size in (("C4", 128, (32, 48), (64, 48)), ("C5", 32, (8, 0, 16), (16, 24, 16))):
+        wl = make(name, n=n, n_dirs=4, n_probes=4)
+        wl.thr_eta = wl.thr_chi = 0.3
+        M = orc.build_mips(wl)
+        cw = crop_workload(wl, lo, size)
+        Mc = orc.build_mips(cw)
+        ids = crop_brick_ids(wl, lo, size)
+        assert np.array_equal(M.levels[:, ids], Mc.levels)
+        for m in range(M.max_level + 1):
+            sl = tuple(slice(lo[a] >> m, (lo[a] + size[a]) >> m) for a in reversed(range(wl.ndim)))
+            assert np.array_equal(M.eta[m][sl], Mc.eta[m]) and np.array_equal(M.vmax[m][sl], Mc.vmax[m])
