@@ -210,6 +210,10 @@ int64_t dex_launch_count(void);
  * events on the launching stream when timing is enabled (bench.py roofline leg).  Synchronises. */
 void dex_march_timing_enable(int on);
 dex_status dex_march_timing_read(double* ms_total, int64_t* n_launches, int reset);
+/* Work counter of the Core-and-Voigt / Classic march while timing is enabled: sum over emitted segments of the
+ * number of active lines of the segment's batch, i.e. line-profile evaluations / W (bench.py's ALU roofline leg
+ * multiplies by W and by the flops per evaluation stated in DESIGN.md).  Synchronises. */
+dex_status dex_march_work_read(int64_t* line_segments, int reset);
 /* Kernel configuration knob (performance experiments): lanes that share one ray, 1/2/4/8. */
 dex_status dex_set_lanes_per_ray(int lanes);
 /* Kernel-structure knobs for performance experiments (results do not change): "lanes_per_ray" 1/2/4/8;

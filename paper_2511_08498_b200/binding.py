@@ -28,7 +28,7 @@ EXPORTS = (
     "dex_last_error", "dex_version", "dex_build_sparse_grid", "dex_grid_info", "dex_grid_get_slots",
     "dex_destroy_grid", "dex_build_vlm_mips", "dex_mips_get_levels", "dex_mips_set_levels",
     "dex_mips_get_packed_levels", "dex_mips_get_level_data", "dex_destroy_mips", "dex_formal_solution",
-    "dex_mean_intensity", "dex_mean_intensity_host", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read",
+    "dex_mean_intensity", "dex_mean_intensity_host", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read", "dex_march_work_read",
     "dex_set_lanes_per_ray", "dex_set_tuning",
 )
 
@@ -95,6 +95,7 @@ def _load():
     L.dex_march_timing_enable.argtypes = [C.c_int]
     L.dex_march_timing_enable.restype = None
     L.dex_march_timing_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64), C.c_int]
+    L.dex_march_work_read.argtypes = [C.POINTER(C.c_int64), C.c_int]
     L.dex_set_lanes_per_ray.argtypes = [C.c_int]
     L.dex_set_tuning.argtypes = [C.c_char_p, C.c_int]
     return L
@@ -152,6 +153,12 @@ def dex_march_timing_read(reset=True):
     ms, n = C.c_double(0), C.c_int64(0)
     _check(_L.dex_march_timing_read(C.byref(ms), C.byref(n), 1 if reset else 0))
     return ms.value, n.value
+
+
+def dex_march_work_read(reset=True) -> int:
+    v = C.c_int64(0)
+    _check(_L.dex_march_work_read(C.byref(v), 1 if reset else 0))
+    return v.value
 
 
 class Grid:

@@ -21,6 +21,7 @@ std::atomic<int> g_voigt_fp32{1};
 std::mutex g_timing_mu;
 struct EvPair { cudaEvent_t a, b; };
 std::vector<EvPair> g_events;
+unsigned long long* g_d_line_segs = nullptr;   // device counter of (segment, active line) pairs, timing mode only
 
 int ilog2_exact(int v) {
   if (v <= 0 || (v & (v - 1))) return -1;
@@ -41,16 +42,17 @@ bool have_device() {
 }
 
 template <typename T>
-dex_status dmalloc(T** p, size_t count) {
+dex_status dmalloc(T** p, size_t count, cudaStream_t st) {
   *p = nullptr;
   if (count == 0) count = 1;
-  DEX_CUDA_CHECK(cudaMalloc((void**)p, sizeof(T) * count));
+  DEX_CUDA_CHECK(dex_alloc((void**)p, sizeof(T) * count, st));
   return DEX_OK;
 }
 
 void free_mips_memory(dex_mips* m) {
-  cudaFree(m->d_store); cudaFree(m->d_mrec); cudaFree(m->d_line); cudaFree(m->d_vel); cudaFree(m->d_vtab); cudaFree(m->d_lam);
-  cudaFree(m->d_active_lines); cudaFree(m->d_levels); cudaFree(m->d_packed); cudaFree(m->d_fail); cudaFree(m->d_binfo); cudaFree(m->d_vftab);
+  void* ptrs[] = {m->d_store, m->d_mrec, m->d_line, m->d_vel, m->d_vtab, m->d_lam, m->d_active_lines, m->d_levels,
+                  m->d_packed, m->d_fail, m->d_binfo, m->d_vftab};
+  for (void* q : ptrs) dex_free(q, m->stream);
 }
 
 dex_status check_rays(const dex_grid* grid, const dex_mips* mips, const dex_rays* rays, DexRaysDev* out) {
@@ -99,13 +101,13 @@ struct Uploads {
   int64_t bytes = 0;
   dex_status status = DEX_OK;
   explicit Uploads(cudaStream_t s) : st(s) {}
-  ~Uploads() { for (void* p : ptrs) cudaFree(p); }
+  ~Uploads() { for (void* p : ptrs) dex_free(p, st); }
   template <typename T>
   const T* put(const T* h, size_t count) {
     if (!h || status != DEX_OK) return nullptr;
     void* d = nullptr;
     const size_t nbytes = sizeof(T) * (count ? count : 1);
-    if (cudaMalloc(&d, nbytes) != cudaSuccess) {
+    if (dex_alloc(&d, nbytes, st) != cudaSuccess) {
       cudaGetLastError();
       dex_set_error("device allocation failed while uploading host inputs");
       status = DEX_ERR_OOM;
@@ -124,7 +126,7 @@ struct Uploads {
   T* alloc(size_t count) {
     if (status != DEX_OK) return nullptr;
     void* d = nullptr;
-    if (cudaMalloc(&d, sizeof(T) * (count ? count : 1)) != cudaSuccess) {
+    if (dex_alloc(&d, sizeof(T) * (count ? count : 1), st) != cudaSuccess) {
       cudaGetLastError();
       dex_set_error("device allocation failed");
       status = DEX_ERR_OOM;
@@ -146,9 +148,32 @@ const float* dex_voigt_fast_table_host() {
   return tab.data();
 }
 
+cudaError_t dex_alloc(void** p, size_t bytes, cudaStream_t st) {
+  static std::mutex mu;
+  static bool warm[64] = {false};
+  int dev = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64) {
+    std::lock_guard<std::mutex> lk(mu);
+    if (!warm[dev]) {
+      cudaMemPool_t pool;
+      if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        unsigned long long keep = ~0ULL;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+      }
+      cudaGetLastError();
+      warm[dev] = true;
+    }
+  }
+  return cudaMallocAsync(p, bytes, st);
+}
+void dex_free(void* p, cudaStream_t st) {
+  if (p) cudaFreeAsync(p, st);
+}
+
 void dex_set_error(const std::string& msg) { g_last_error = msg; }
 void dex_count_launch(int n) { g_launches.fetch_add(n); }
 int dex_tuning_voigt_fp32() { return g_voigt_fp32.load(); }
+unsigned long long* dex_line_segment_counter() { return g_timing.load() ? g_d_line_segs : nullptr; }
 
 extern "C" {
 
@@ -174,7 +199,28 @@ dex_status dex_set_tuning(const char* name, int value) {
   return DEX_ERR_INVALID_ARG;
 }
 
-void dex_march_timing_enable(int on) { g_timing.store(on ? 1 : 0); }
+void dex_march_timing_enable(int on) {
+  if (on) {
+    std::lock_guard<std::mutex> lk(g_timing_mu);
+    if (!g_d_line_segs && cudaMalloc((void**)&g_d_line_segs, sizeof(unsigned long long)) == cudaSuccess)
+      cudaMemset(g_d_line_segs, 0, sizeof(unsigned long long));
+    else
+      cudaGetLastError();
+  }
+  g_timing.store(on ? 1 : 0);
+}
+
+dex_status dex_march_work_read(int64_t* line_segments, int reset) {
+  std::lock_guard<std::mutex> lk(g_timing_mu);
+  unsigned long long v = 0;
+  if (g_d_line_segs) {
+    DEX_CUDA_CHECK(cudaDeviceSynchronize());
+    DEX_CUDA_CHECK(cudaMemcpy(&v, g_d_line_segs, sizeof(v), cudaMemcpyDeviceToHost));
+    if (reset) DEX_CUDA_CHECK(cudaMemset(g_d_line_segs, 0, sizeof(v)));
+  }
+  if (line_segments) *line_segments = (int64_t)v;
+  return DEX_OK;
+}
 
 dex_status dex_march_timing_read(double* ms_total, int64_t* n_launches, int reset) {
   std::lock_guard<std::mutex> lk(g_timing_mu);
@@ -231,8 +277,9 @@ dex_status dex_build_sparse_grid(const dex_grid_desc* desc, const uint8_t* d_act
   d.h = desc->voxel_size;
   d.n_bricks = (int)nbr;
   d.n_active = 0;
-  dex_status s = dmalloc(&g->d_slot, (size_t)nbr);
-  if (s == DEX_OK) s = dmalloc(&g->d_active_bricks, (size_t)nbr);
+  g->stream = (cudaStream_t)stream;
+  dex_status s = dmalloc(&g->d_slot, (size_t)nbr, g->stream);
+  if (s == DEX_OK) s = dmalloc(&g->d_active_bricks, (size_t)nbr, g->stream);
   if (s == DEX_OK) { d.slot = g->d_slot; s = dex_launch_grid_build(g, d_active, (cudaStream_t)stream); }
   if (s != DEX_OK) { dex_destroy_grid(g); return s; }
   *out = g;
@@ -255,8 +302,8 @@ dex_status dex_grid_get_slots(const dex_grid* grid, int32_t* h_slot) {
 
 void dex_destroy_grid(dex_grid* grid) {
   if (!grid) return;
-  cudaFree(grid->d_slot);
-  cudaFree(grid->d_active_bricks);
+  dex_free(grid->d_slot, grid->stream);
+  dex_free(grid->d_active_bricks, grid->stream);
   delete grid;
 }
 
@@ -343,23 +390,24 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
   const size_t A = (size_t)grid->n_active;
   if ((long long)A * cps >= (1LL << 27)) { dex_set_error("too many pyramid cells per batch (brick word holds 27 bits)"); delete m; return DEX_ERR_SHAPE; }
   cudaStream_t st = (cudaStream_t)stream;
+  m->stream = st;
   dex_status s = DEX_OK;
   m->store_floats = (size_t)n_batch * A * cps * DEX_REC;
-  s = dmalloc(&m->d_store, m->store_floats);
-  if (s == DEX_OK && v == DEX_ISO) s = dmalloc(&m->d_mrec, m->store_floats);
-  if (s == DEX_OK) s = dmalloc(&m->d_levels, (size_t)n_batch * grid->n_bricks);
-  if (s == DEX_OK) s = dmalloc(&m->d_packed, (size_t)n_batch * d.words_per_batch);
-  if (s == DEX_OK) s = dmalloc(&m->d_binfo, (size_t)n_batch * grid->n_bricks);
-  if (s == DEX_OK) s = dmalloc(&m->d_fail, (size_t)n_batch * A * (max_level + 1));
+  s = dmalloc(&m->d_store, m->store_floats, st);
+  if (s == DEX_OK && v == DEX_ISO) s = dmalloc(&m->d_mrec, m->store_floats, st);
+  if (s == DEX_OK) s = dmalloc(&m->d_levels, (size_t)n_batch * grid->n_bricks, st);
+  if (s == DEX_OK) s = dmalloc(&m->d_packed, (size_t)n_batch * d.words_per_batch, st);
+  if (s == DEX_OK) s = dmalloc(&m->d_binfo, (size_t)n_batch * grid->n_bricks, st);
+  if (s == DEX_OK) s = dmalloc(&m->d_fail, (size_t)n_batch * A * (max_level + 1), st);
   if (s == DEX_OK && v != DEX_ISO) {
-    s = dmalloc(&m->d_vel, A * cps);
-    if (s == DEX_OK) s = dmalloc(&m->d_line, A * cps * (size_t)(d.n_lines > 0 ? d.n_lines : 1));
-    if (s == DEX_OK) s = dmalloc(&m->d_lam, (size_t)desc->n_lambda);
-    if (s == DEX_OK) s = dmalloc(&m->d_active_lines, (size_t)n_batch * DEX_MAX_LINES);
-    if (s == DEX_OK) s = dmalloc(&m->d_vftab, (size_t)DEX_VF_NODES * 5);
+    s = dmalloc(&m->d_vel, A * cps, st);
+    if (s == DEX_OK) s = dmalloc(&m->d_line, A * cps * (size_t)(d.n_lines > 0 ? d.n_lines : 1), st);
+    if (s == DEX_OK) s = dmalloc(&m->d_lam, (size_t)desc->n_lambda, st);
+    if (s == DEX_OK) s = dmalloc(&m->d_active_lines, (size_t)n_batch * DEX_MAX_LINES, st);
+    if (s == DEX_OK) s = dmalloc(&m->d_vftab, (size_t)DEX_VF_NODES * 5, st);
     if (s == DEX_OK && v == DEX_VELINTERP) {
       m->vtab_floats = m->store_floats * (size_t)d.n_vbins;
-      s = dmalloc(&m->d_vtab, m->vtab_floats);
+      s = dmalloc(&m->d_vtab, m->vtab_floats, st);
     }
     if (s == DEX_OK) {
       cudaError_t e = cudaMemcpyAsync(m->d_lam, desc->d_lambda, sizeof(float) * desc->n_lambda,
@@ -449,14 +497,15 @@ dex_status dex_mips_get_level_data(const dex_mips* mips, int chain, int level, f
   for (int a = 0; a < mips->grid->dev.ndim; ++a) cells *= (size_t)(mips->grid->dev.dims[a] >> level);
   float* d_dense = nullptr;
   DEX_CUDA_CHECK(cudaDeviceSynchronize());
-  dex_status s = dmalloc(&d_dense, cells * width);
+  dex_status s = dmalloc(&d_dense, cells * width, (cudaStream_t)0);
   if (s != DEX_OK) return s;
   cudaError_t e = cudaMemset(d_dense, 0, sizeof(float) * cells * width);
   if (e == cudaSuccess) {
     s = dex_launch_level_data(mips, chain, level, d_dense, 0);
     if (s == DEX_OK) e = cudaMemcpy(h_dense, d_dense, sizeof(float) * cells * width, cudaMemcpyDeviceToHost);
   }
-  cudaFree(d_dense);
+  cudaDeviceSynchronize();
+  dex_free(d_dense, (cudaStream_t)0);
   if (s != DEX_OK) return s;
   DEX_CUDA_CHECK(e);
   return DEX_OK;
@@ -492,7 +541,7 @@ dex_status dex_formal_solution(const dex_grid* grid, const dex_mips* mips, const
   }
   if (capture) {
     int* d_over = nullptr;
-    s = dmalloc(&d_over, 1);
+    s = dmalloc(&d_over, 1, st);
     if (s != DEX_OK) return s;
     int h_over = 0;
     cudaError_t e = cudaMemsetAsync(d_over, 0, sizeof(int), st);
@@ -501,7 +550,7 @@ dex_status dex_formal_solution(const dex_grid* grid, const dex_mips* mips, const
       if (s == DEX_OK) e = cudaMemcpyAsync(&h_over, d_over, sizeof(int), cudaMemcpyDeviceToHost, st);
       if (s == DEX_OK && e == cudaSuccess) e = cudaStreamSynchronize(st);
     }
-    cudaFree(d_over);
+    dex_free(d_over, st);
     if (s != DEX_OK) return s;
     DEX_CUDA_CHECK(e);
     if (h_over) { dex_set_error("visit capture overflow: counts are complete, records truncated"); return DEX_ERR_CAPACITY; }

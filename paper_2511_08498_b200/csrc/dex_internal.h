@@ -14,6 +14,7 @@ struct dex_grid {
   int* d_active_bricks = nullptr;  // [n_active] slot -> brick
   int64_t n_bricks = 0, n_active = 0;
   int64_t nvox = 0;
+  cudaStream_t stream = nullptr;   // the stream the handle was built on; its memory is released on it
 };
 
 struct dex_mips {
@@ -36,11 +37,17 @@ struct dex_mips {
   float* d_vftab = nullptr;                  // fp32 Voigt tables: [NODES][4] wing then [NODES] core (anisotropic variants)
   int* d_fail = nullptr;                     // [n_batch][n_active][max_level+1]
   size_t store_floats = 0, vtab_floats = 0;
+  cudaStream_t stream = nullptr;   // the stream the handle was built on; its memory is released on it
 };
 
 void dex_set_error(const std::string& msg);
+// Stream-ordered device memory from the device's default pool (kept warm: release threshold = unlimited), so that a
+// rebuild per iteration does not pay cudaMalloc / cudaFree (page mapping, device-wide synchronisation) every time.
+cudaError_t dex_alloc(void** p, size_t bytes, cudaStream_t st);
+void dex_free(void* p, cudaStream_t st);
 void dex_count_launch(int n = 1);
 int dex_tuning_voigt_fp32();
+unsigned long long* dex_line_segment_counter();   // device counter, NULL unless march timing is enabled
 
 // grid_build.cu
 dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStream_t st);

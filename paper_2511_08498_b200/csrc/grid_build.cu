@@ -65,8 +65,8 @@ dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStrea
   const int nb = (int)g->n_bricks;
   int* d_flag = nullptr;
   int* d_count = nullptr;
-  DEX_CUDA_CHECK(cudaMalloc(&d_flag, sizeof(int) * (size_t)nb));
-  DEX_CUDA_CHECK(cudaMalloc(&d_count, sizeof(int)));
+  DEX_CUDA_CHECK(dex_alloc((void**)&d_flag, sizeof(int) * (size_t)nb, st));
+  DEX_CUDA_CHECK(dex_alloc((void**)&d_count, sizeof(int), st));
   if (d_active == nullptr) {
     dex_fill_int_kernel<<<(nb + 255) / 256, 256, 0, st>>>(d_flag, nb, 1);
   } else {
@@ -81,8 +81,8 @@ dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStrea
   int h_count = 0;
   cudaError_t e = cudaMemcpyAsync(&h_count, d_count, sizeof(int), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cudaFree(d_flag);
-  cudaFree(d_count);
+  dex_free(d_flag, st);
+  dex_free(d_count, st);
   DEX_CUDA_CHECK(e);
   DEX_CUDA_CHECK(cudaGetLastError());
   g->n_active = h_count;

@@ -367,7 +367,8 @@ constexpr int dex_march_minb(int var) {
 template <int D, int VAR, int LPR, bool FUSE_J>
 __global__ void __launch_bounds__(DEX_MARCH_THREADS, dex_march_minb(VAR))
 dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ perm,
-                 float* __restrict__ out, unsigned long long* __restrict__ seg_count) {
+                 float* __restrict__ out, unsigned long long* __restrict__ seg_count,
+                 unsigned long long* __restrict__ line_seg_count) {
   constexpr int LPT = DEX_W / LPR;
   constexpr unsigned FULL = 0xffffffffu;
   __shared__ float Jsm[FUSE_J ? LPT * DEX_MARCH_THREADS : 1];
@@ -507,6 +508,14 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
     unsigned v = (sub == 0) ? nseg : 0u;
     v = __reduce_add_sync(FULL, v);
     if ((threadIdx.x & 31) == 0 && v) atomicAdd(seg_count, (unsigned long long)v);
+  }
+  if (VAR == DEX_CAV && line_seg_count != nullptr) {   // bench.py's ALU roofline: segments x active lines of the batch
+    int nact = 0;
+#pragma unroll
+    for (int q = 0; q < DEX_NLINES; ++q) nact += (CT.line[q] >= 0) ? 1 : 0;
+    unsigned v = (sub == 0) ? nseg : 0u;
+    v = __reduce_add_sync(FULL, v);
+    if ((threadIdx.x & 31) == 0 && v && nact) atomicAdd(line_seg_count, (unsigned long long)v * (unsigned long long)nact);
   }
 }
 
@@ -665,10 +674,11 @@ dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev
   dim3 grid((unsigned)gx, (unsigned)m->n_batch, 1);
   DexMipsDev md = m->dev;
   md.voigt_fp32 = dex_tuning_voigt_fp32();
+  unsigned long long* d_work = dex_line_segment_counter();   // NULL unless march timing is enabled
   if (fuse_j)
-    dex_march_kernel<D, VAR, LPR, true><<<grid, threads, 0, st>>>(g->dev, md, rays, perm, d_out, d_seg);
+    dex_march_kernel<D, VAR, LPR, true><<<grid, threads, 0, st>>>(g->dev, md, rays, perm, d_out, d_seg, d_work);
   else
-    dex_march_kernel<D, VAR, LPR, false><<<grid, threads, 0, st>>>(g->dev, md, rays, perm, d_out, d_seg);
+    dex_march_kernel<D, VAR, LPR, false><<<grid, threads, 0, st>>>(g->dev, md, rays, perm, d_out, d_seg, d_work);
   dex_count_launch();
   DEX_CUDA_CHECK(cudaGetLastError());
   return DEX_OK;
