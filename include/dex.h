@@ -127,6 +127,12 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
 /* Validation accessors (synchronise). */
 dex_status dex_mips_get_levels(const dex_mips* mips, int8_t* h_level /*[n_batch][n_bricks], -1 empty*/);
 dex_status dex_mips_set_levels(dex_mips* mips, const int8_t* h_level /*same shape; injects a table*/);
+/* Near-field MIP cap (the long-characteristics analogue of DexRT's per-cascade maximum MIP level
+ * [0,0,1,2,3,4] over intervals ending at 1.5 * 4^i voxels; T8).  A cell entered at
+ * distance t (index units) from the probe is formed at level min(brick level, #{i : t >= h_cap_t[i]}); thresholds
+ * ascending, n_caps <= 8; n_caps = 0 (the default) removes the cap.  Host-side state of the handle: takes effect for
+ * the marches launched afterwards.  Errors: DEX_ERR_INVALID_ARG, DEX_ERR_SHAPE. */
+dex_status dex_mips_set_level_caps(dex_mips* mips, int n_caps, const float* h_cap_t);
 /* Packed block states of one batch: state = level + 1 (0 = empty) in ceil(log2(max_level+2)) bits,
  * floor(64/bits) bricks per word, no straddling.  *n_words receives the word count; h_words may be
  * NULL to query it. */

@@ -164,6 +164,12 @@ typedef struct {
     int dims[3];
     int brick;
     double h;                    /* physical side of a level-0 voxel */
+    /* Distance-dependent MIP cap, the long-characteristics analogue of DexRT's per-cascade maximum MIP level
+     * [0,0,1,2,3,4] with interval ends 1.5 * 4^i voxels (T8): a cell
+     * entered at distance t from the probe is formed at level min(brick level, #{i : t >= cap_t[i]}).
+     * n_caps = 0: no cap. */
+    int n_caps;
+    float cap_t[8];              /* ascending thresholds, index units */
 } orc_grid;
 
 static inline int64_t cell_index(const orc_grid* g, int m, const int* cc)
@@ -335,6 +341,11 @@ static int hdda(const orc_grid* g, const int8_t* level, const float* probe, cons
     int n = 0;
     for (;;) {
         int m = level[brick_index(g, x)];                       /* MipLevel(coord), Alg. 1 l.6-8 */
+        if (m > 0 && g->n_caps > 0) {                            /* T8: near field at fine resolution */
+            int cap = 0;
+            for (int i = 0; i < g->n_caps; ++i) cap += (t >= g->cap_t[i]) ? 1 : 0;
+            if (cap < m) m = cap;
+        }
         int size = (m < 0) ? g->brick : (1 << m);                /* T3: empty brick skipped whole */
         int c[3], kp[3];
         int s = -1;

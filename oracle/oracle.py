@@ -24,7 +24,8 @@ IOD_LOG, RELVAR = 0, 1
 
 
 class _Grid(C.Structure):
-    _fields_ = [("ndim", C.c_int), ("dims", C.c_int * 3), ("brick", C.c_int), ("h", C.c_double)]
+    _fields_ = [("ndim", C.c_int), ("dims", C.c_int * 3), ("brick", C.c_int), ("h", C.c_double),
+                ("n_caps", C.c_int), ("cap_t", C.c_float * 8)]
 
 
 _PP = C.POINTER(C.c_void_p)
@@ -527,11 +528,25 @@ def plain_march(wl, M: Optional[OracleMips] = None, probe_pos=None, dirs=None, i
     return MarchResult(I=I, segments=int(n), counts=counts, records=records, ds=ds)
 
 
+def level_caps_paper(n_levels=4, first=6.0, factor=4.0):
+    """Distance thresholds of the near-field MIP cap: the long-characteristics analogue of DexRT's per-cascade
+    maximum MIP level [0,0,1,2,3,4] with interval ends 1.5 * 4^i voxels: level <= 0 for t < 6,
+    <= 1 for t < 24, <= 2 for t < 96, <= 3 for t < 384, unrestricted beyond."""
+    return np.asarray([first * factor ** i for i in range(n_levels)], dtype=np.float32)
+
+
 def hdda_march(wl, M: OracleMips, probe_pos=None, dirs=None, i0=None, capture_batch=None, levels=None,
-               n_threads=0) -> MarchResult:
-    """(B) HDDA over the brick/level structure with the VLM mips (Algorithm 1)."""
+               n_threads=0, level_cap_t=None) -> MarchResult:
+    """(B) HDDA over the brick/level structure with the VLM mips (Algorithm 1).
+    level_cap_t: ascending distance thresholds of the near-field MIP cap (T8), None = no cap."""
     keep = []
     g, F = _make_structs(wl, M, keep)
+    if level_cap_t is not None:
+        caps = np.asarray(level_cap_t, dtype=np.float32)
+        assert caps.size <= 8 and (np.diff(caps) >= 0).all()
+        g.n_caps = int(caps.size)
+        for i, v in enumerate(caps):
+            g.cap_t[i] = float(v)
     if F.variant == CLASSIC:
         F.variant = CAV
     pp, dd, ii = _rays(wl, probe_pos, dirs, i0)

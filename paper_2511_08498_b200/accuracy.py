@@ -8,7 +8,7 @@ paper's ground truth) for the anisotropic ones.  The level-0 / Cla
 parity-checked against the oracle in tests/test_gpu_parity.py.  The paper's Table 3 quotes the same
 percentiles for level populations; J is what this hot path produces.
 
-  python -m paper_2511_08498_b200.accuracy --workload C2 [--n-probes N] [--metric relvar|iod_log]
+  python -m paper_2511_08498_b200.accuracy --workload C2 [--n-probes N] [--metric relvar|iod_log] [--caps paper]
 
 Prints one JSON line: percentiles of |J_vlm - J_exact| / J_exact over (probe, wavelength), the level
 histogram per batch (Table-2 style), segment counts and march times of both sides.
@@ -40,8 +40,11 @@ def percentiles(rel: np.ndarray) -> dict:
     return out
 
 
+PAPER_CAPS = (6.0, 24.0, 96.0, 384.0)   # level <= 0, 1, 2, 3 below these distances (voxels): PAPER.md:347-349, T8
+
+
 def run(workload: str, n=None, n_dirs=None, n_probes=None, metric=None, thr=None, gate=None, max_level=None,
-        device="cuda:0") -> dict:
+        caps=None, device="cuda:0") -> dict:
     import torch
     from . import binding as B
     from . import pipeline
@@ -60,8 +63,10 @@ def run(workload: str, n=None, n_dirs=None, n_probes=None, metric=None, thr=None
     grid = pipeline.build_grid(dw)
     stream = torch.cuda.current_stream()
 
-    def solve(**override):
+    def solve(use_caps=False, **override):
         mips = pipeline.build_mips(dw, grid, **override)
+        if use_caps and caps:
+            mips.set_level_caps(caps)
         seg = torch.zeros(1, dtype=torch.int64, device=device)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(stream)
@@ -72,7 +77,7 @@ def run(workload: str, n=None, n_dirs=None, n_probes=None, metric=None, thr=None
         mips.destroy()
         return J.cpu().numpy().astype(np.float64), int(seg.item()), a.elapsed_time(b), lv
 
-    J_vlm, seg_vlm, ms_vlm, lv = solve()
+    J_vlm, seg_vlm, ms_vlm, lv = solve(use_caps=True)
     if wl.variant == B.DEX_ISO:
         J_ex, seg_ex, ms_ex, _ = solve(max_level=0)
         exact = "same variant at max_level 0"
@@ -87,7 +92,7 @@ def run(workload: str, n=None, n_dirs=None, n_probes=None, metric=None, thr=None
     return {
         "report": "vlm_accuracy_J", "workload": wl.name, "dims": list(wl.dims[:wl.ndim]), "variant": int(wl.variant),
         "metric": "relvar" if wl.metric == 1 else "iod_log", "thr": float(wl.thr_eta), "tau_gate": float(wl.tau_gate),
-        "max_level": int(wl.max_level), "n_probes": int(wl.probe_pos.shape[0]), "n_dirs": int(wl.dirs.shape[0]),
+        "max_level": int(wl.max_level), "level_cap_t": list(caps) if caps else [], "n_probes": int(wl.probe_pos.shape[0]), "n_dirs": int(wl.dirs.shape[0]),
         "n_lambda": int(wl.n_lambda), "exact_side": exact, "rel_err_J": percentiles(rel),
         "values_compared": int(rel.size), "segments_vlm": seg_vlm, "segments_exact": seg_ex,
         "segment_ratio": seg_ex / max(1, seg_vlm), "march_ms_vlm": ms_vlm, "march_ms_exact": ms_ex,
@@ -107,8 +112,13 @@ def main():
     ap.add_argument("--thr", type=float, default=None)
     ap.add_argument("--gate", type=float, default=None)
     ap.add_argument("--max-level", type=int, default=None)
+    ap.add_argument("--caps", default=None,
+                    help="near-field MIP cap thresholds: 'paper' (6,24,96,384 voxels) or a comma separated list")
     a = ap.parse_args()
-    print(json.dumps(run(a.workload, a.n, a.n_dirs, a.n_probes, a.metric, a.thr, a.gate, a.max_level)))
+    caps = None
+    if a.caps:
+        caps = PAPER_CAPS if a.caps == "paper" else tuple(float(v) for v in a.caps.split(","))
+    print(json.dumps(run(a.workload, a.n, a.n_dirs, a.n_probes, a.metric, a.thr, a.gate, a.max_level, caps)))
 
 
 if __name__ == "__main__":

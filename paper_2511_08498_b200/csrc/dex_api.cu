@@ -469,6 +469,20 @@ dex_status dex_mips_set_levels(dex_mips* mips, const int8_t* h_level) {
   return DEX_OK;
 }
 
+dex_status dex_mips_set_level_caps(dex_mips* mips, int n_caps, const float* h_cap_t) {
+  if (!mips || (n_caps > 0 && !h_cap_t)) { dex_set_error("NULL mips / h_cap_t"); return DEX_ERR_INVALID_ARG; }
+  if (n_caps < 0 || n_caps > 8) { dex_set_error("n_caps must be 0..8"); return DEX_ERR_SHAPE; }
+  for (int i = 0; i < n_caps; ++i) {
+    if (!(h_cap_t[i] >= 0.0f) || (i > 0 && h_cap_t[i] < h_cap_t[i - 1])) {
+      dex_set_error("cap thresholds must be >= 0 and ascending");
+      return DEX_ERR_INVALID_ARG;
+    }
+  }
+  mips->dev.n_caps = n_caps;
+  for (int i = 0; i < 8; ++i) mips->dev.cap_t[i] = (i < n_caps) ? h_cap_t[i] : 0.0f;
+  return DEX_OK;
+}
+
 dex_status dex_mips_get_packed_levels(const dex_mips* mips, int batch, uint64_t* h_words, int64_t* n_words) {
   if (!mips) { dex_set_error("NULL mips"); return DEX_ERR_INVALID_ARG; }
   if (batch < 0 || batch >= mips->n_batch) { dex_set_error("batch out of range"); return DEX_ERR_SHAPE; }

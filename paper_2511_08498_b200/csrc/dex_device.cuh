@@ -54,6 +54,8 @@ struct DexMipsDev {
   double wei_L;
   const float4* vf_wing;             // [DEX_VF_NODES] Taylor coefficients of Im F about the nodes (dex_voigt.cuh)
   const float* vf_core;              // [DEX_VF_NODES] e^{-x_k^2}
+  int n_caps;                        // near-field MIP cap (T8, dex_mips_set_level_caps): a cell entered at distance t is
+  float cap_t[8];                    // formed at level min(brick level, #{i : t >= cap_t[i]}); n_caps = 0: no cap
   int voigt_fp32;                    // 0: fp64 HUM1WEI24 everywhere (tuning knob "voigt_fp32")
 };
 
@@ -132,7 +134,20 @@ struct DexRay3 {
 template <int D>
 __device__ __forceinline__ void dex_set_cell(DexRay3<D>& r, const DexGridDev& G, const DexMipsDev& M, int info,
                                              const int* x) {
-  const int m = (info & 15) - 1;
+  int m = (info & 15) - 1;
+  int base = info >> 4;
+  float tcap = __int_as_float(0x7f800000);
+  if (m > 0 && M.n_caps > 0) {
+    // T8: the level of this visit is capped by the distance r.t at which the cell is entered; the cell is formed
+    // again when the ray reaches the next threshold (folded into tb, so the in-brick fast step pays nothing)
+    int cap = 0;
+    for (int i = 0; i < M.n_caps; ++i) cap += (r.t >= M.cap_t[i]) ? 1 : 0;
+    if (cap < m) {
+      base += M.lvloff[cap] - M.lvloff[m];
+      m = cap;
+      tcap = M.cap_t[cap];
+    }
+  }
   const int sh = (m < 0) ? G.logB : m;
   const int size = 1 << sh, lsh = G.logB - sh, bmask = G.B - 1;
   r.info = info;
@@ -151,8 +166,8 @@ __device__ __forceinline__ void dex_set_cell(DexRay3<D>& r, const DexGridDev& G,
     idx += ((c & bmask) >> sh) << (a * lsh);
     r.cstep[a] = pos ? (1 << (a * lsh)) : -(1 << (a * lsh));
   }
-  r.tb = tb;
-  r.cell = (m < 0) ? -1 : (info >> 4) + idx;
+  r.tb = fminf(tb, tcap);
+  r.cell = (m < 0) ? -1 : base + idx;
 }
 
 // T1/T2/T6: trace from the probe outward, o = probe, d = -omega.  Returns false for a probe outside
@@ -256,7 +271,12 @@ __device__ __forceinline__ bool dex_ray_cross(DexRay3<D>& r, const DexGridDev& G
     int info = r.info;
     if (((xs ^ cs) >> G.logB) != 0) {
       info = __ldg(binfo + dex_brick_of<D>(G, x));
-      const int m2 = (info & 15) - 1;
+      int m2 = (info & 15) - 1;
+      if (m2 > 0 && M.n_caps > 0) {
+        int cap = 0;
+        for (int i = 0; i < M.n_caps; ++i) cap += (r.t >= M.cap_t[i]) ? 1 : 0;
+        m2 = min(m2, cap);
+      }
       const int sh2 = (m2 < 0) ? G.logB : m2;
       if (sh2 < r.sh) {
 #pragma unroll

@@ -423,3 +423,34 @@ def test_full_size_march_sampled(P, name):
     assert max_rel(Ic.cpu().numpy(), A.I) <= TOL
     Jc = P.pipeline.mean_intensity(dw, grid, mc).cpu().numpy()
     assert max_rel(Jc, orc.mean_intensity(A.I, wl.weights)) <= TOL
+
+
+# ------------------------------------------------------------------------------------------ T8: near-field MIP cap
+@pytest.mark.parametrize("name,kw,thr", [("C2", dict(n=256, n_dirs=12, n_probes=800), 0.05),
+                                         ("C5", dict(n=64, n_dirs=8, n_probes=300), 5.0),
+                                         ("C3", dict(n=256, n_dirs=8, n_probes=200), None)])
+def test_level_cap_parity(P, name, kw, thr):
+    """dex_mips_set_level_caps against the oracle's capped HDDA: visit lists and path lengths bit-exact, I and J within
+    1e-5, for the paper-analogue thresholds (6, 24, 96, 384), a dense set of small thresholds, and the two limits."""
+    wl = make(name, **kw)
+    if thr is not None:
+        wl.thr_eta = wl.thr_chi = thr
+    M = orc.build_mips(wl)
+    assert M.levels.max() >= 2
+    dw, grid, mips = _build(P, wl)
+    base = orc.hdda_march(wl, M, capture_batch=0)
+    for caps in (orc.level_caps_paper(), [2.5, 5.0, 11.0, 40.0], [1e9, 1e9, 1e9, 1e9], []):
+        mips.set_level_caps(caps)
+        ref = orc.hdda_march(wl, M, capture_batch=0, level_cap_t=caps)
+        _, cap = P.pipeline.formal_solution(dw, grid, mips, capture_batch=0, want_I=False)
+        _check_lists(cap, ref, cap.room)
+        seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+        I, _ = P.pipeline.formal_solution(dw, grid, mips, segment_count=seg)
+        assert int(seg.item()) == ref.segments
+        assert max_rel(I.cpu().numpy(), ref.I) <= TOL
+        J = P.pipeline.mean_intensity(dw, grid, mips)
+        assert max_rel(J.cpu().numpy(), orc.mean_intensity(ref.I, wl.weights)) <= TOL
+        if len(caps) == 0:
+            assert ref.segments == base.segments
+    with pytest.raises(P.DexError):
+        mips.set_level_caps([5.0, 2.0])

@@ -527,3 +527,84 @@ def test_aniso_mips_hdda_consistency():
         ok = J_a > 0
         rel = np.abs(J_b[ok] - J_a[ok]) / J_a[ok]
         assert np.percentile(rel, 90) < 0.2
+
+
+# ------------------------------------------------------------------------------------------------
+# T8: near-field MIP cap (PAPER.md:347-349 per-cascade caps [0,0,1,2,3,4])
+# ------------------------------------------------------------------------------------------------
+def _slab(lvl, cc, probe, omega):
+    """fp64 slab-method (entry, exit) distances of the ray through cell `cc` of level `lvl` (independent of any DDA)."""
+    o = np.asarray(probe, dtype=np.float32).astype(np.float64)
+    d = -np.asarray(omega, dtype=np.float32).astype(np.float64)
+    size = float(1 << lvl)
+    t0, t1 = 0.0, np.inf
+    for a in range(len(o)):
+        lo, hi = cc[a] * size, (cc[a] + 1) * size
+        if d[a] != 0.0:
+            ta, tb = (lo - o[a]) / d[a], (hi - o[a]) / d[a]
+            t0 = max(t0, min(ta, tb))
+            t1 = min(t1, max(ta, tb))
+    return t0, t1
+
+
+def test_t8_level_cap_limits_and_geometry():
+    """(i) no thresholds, or thresholds that are all passed at t = 0, change nothing; (ii) thresholds never reached
+    give level 0 everywhere, i.e. bit for bit the march over a level-0 table; (iii) on the Fig. 5 fixture every visited
+    cell has level min(brick level, #{thresholds <= distance at which the visit starts}) with the distances from an
+    independent fp64 slab intersection, and the path lengths still add up to the ray's length inside non-empty bricks;
+    (iv) a homogeneous medium is still exact."""
+    wl = make("C2", n=128, n_dirs=8, n_probes=150)
+    wl.thr_eta = wl.thr_chi = 0.05
+    M = orc.build_mips(wl)
+    assert M.levels.max() >= 2
+    a = orc.hdda_march(wl, M, capture_batch=1)
+    for caps in ([], [0.0, 0.0, 0.0]):
+        b = orc.hdda_march(wl, M, capture_batch=1, level_cap_t=caps)
+        assert np.array_equal(a.records, b.records) and np.array_equal(a.ds.view(np.uint32), b.ds.view(np.uint32))
+        assert np.array_equal(a.I, b.I)
+    M0 = orc.build_mips(wl, max_level=0)
+    z = orc.hdda_march(wl, M0, capture_batch=1)
+    c = orc.hdda_march(wl, M, capture_batch=1, level_cap_t=[1e9, 1e9, 1e9])
+    assert np.array_equal(z.records, c.records) and np.array_equal(z.ds.view(np.uint32), c.ds.view(np.uint32))
+    assert np.array_equal(z.I, c.I)
+    # (iii) Fig. 5 fixture (PAPER.md:148): 32x32, 4x4 blocks of 8x8, levels up to 3
+    rng = np.random.default_rng(21)
+    lv = fig5_levels()
+    lv = np.where(lv >= 0, 3, -1).astype(np.int8)          # every populated block at the coarsest level
+    probes = rng.uniform(0, 32, size=(60, 2))
+    dirs = random_unit_dirs(12, 2, rng)
+    f = np.full((32, 32, 8), 0.3)
+    act = np.repeat(np.repeat((lv >= 0).reshape(4, 4), 8, axis=0), 8, axis=1)
+    f[~act] = 0.0
+    wl5 = iso_workload((32, 32), 8, f * 1.7, f, probes, dirs, active=act.astype(np.uint8), max_level=3)
+    M5 = orc.build_mips(wl5, max_level=3)
+    M5.levels = np.ascontiguousarray(lv[None, :])
+    caps = np.array([3.0, 7.5, 16.0], dtype=np.float32)
+    r = orc.hdda_march(wl5, M5, capture_batch=0, level_cap_t=caps)
+    seen = set()
+    n_dirs = dirs.shape[0]
+    for ray in range(r.counts.shape[0]):
+        p, k = divmod(ray, n_dirs)
+        n = int(r.counts[ray])
+        lvl, x, y, _ = orc.unpack_record(r.records[ray, :n])
+        prev_out = 0.0
+        for i in range(n):
+            # a visit starts where the ray enters the cell, or -- when a threshold was passed inside a coarse cell that
+            # had been crossed as finer cells so far -- where the previous visit ended
+            t_in, t_out = _slab(int(lvl[i]), (int(x[i]), int(y[i])), wl5.probe_pos[p], wl5.dirs[k])
+            te = max(t_in, prev_out)
+            prev_out = t_out
+            if np.min(np.abs(caps.astype(np.float64) - te)) < 1e-3:
+                continue                                     # entry within rounding of a threshold
+            assert int(lvl[i]) == min(3, int((caps <= te).sum())), (ray, i, te, int(lvl[i]))
+            seen.add(int(lvl[i]))
+        tot_bf = sum(s[5] for s in orc.brute_force_segments(wl5, lv, wl5.probe_pos[p], wl5.dirs[k]))
+        assert abs(float(r.ds[ray, :n].astype(np.float64).sum()) - tot_bf) < 2e-4
+    assert seen == {0, 1, 2, 3}
+    # (iv) uniform chi, S: closed form for every ray regardless of the levels used
+    chi0 = float(np.float32(0.3))
+    S0 = float(np.float32(0.3 * 1.7)) / chi0
+    for ray in range(r.counts.shape[0]):
+        n = int(r.counts[ray])
+        L = float(r.ds[ray, :n].astype(np.float64).sum())
+        assert abs(r.I[ray // n_dirs, ray % n_dirs, 0] - S0 * (1.0 - math.exp(-chi0 * L))) < 1e-12
