@@ -127,6 +127,12 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
 /* Validation accessors (synchronise). */
 dex_status dex_mips_get_levels(const dex_mips* mips, int8_t* h_level /*[n_batch][n_bricks], -1 empty*/);
 dex_status dex_mips_set_levels(dex_mips* mips, const int8_t* h_level /*same shape; injects a table*/);
+/* Velocity-bin spacing diagnostic of DEX_VELINTERP mips (the code "warns if the spacing between bins
+ * is greater than two times (configurable) the thermal width of the spectral line").  For every line l:
+ * h_max_ratio[l] = max over the level-0 cells of the active bricks of (2 V / (n_vbins - 1)) / (c dlamD_l / lambda0_l),
+ * V = |v| of the voxel; h_cells_over[l] = number of those cells whose ratio exceeds `factor` (the paper's default: 2).
+ * Both arrays hold n_lines entries.  Synchronises.  Errors: DEX_ERR_INVALID_ARG (NULL, not a VELINTERP handle). */
+dex_status dex_mips_velocity_bin_report(const dex_mips* mips, float factor, float* h_max_ratio, int64_t* h_cells_over);
 /* Near-field MIP cap (the long-characteristics analogue of DexRT's per-cascade maximum MIP level
  * [0,0,1,2,3,4] over intervals ending at 1.5 * 4^i voxels; T8).  A cell entered at
  * distance t (index units) from the probe is formed at level min(brick level, #{i : t >= h_cap_t[i]}); thresholds

@@ -528,6 +528,30 @@ def plain_march(wl, M: Optional[OracleMips] = None, probe_pos=None, dirs=None, i
     return MarchResult(I=I, segments=int(n), counts=counts, records=records, ds=ds)
 
 
+def velocity_bin_report(wl, factor=2.0, n_vbins=None):
+    """bin spacing of the per-voxel velocity grid [-|v|, |v|] against the thermal width of
+    each line, over the voxels of active bricks: (max ratio per line, voxels with ratio > factor per line)."""
+    n = wl.n_vbins if n_vbins is None else n_vbins
+    act = np.repeat(brick_active(wl).reshape(grid_shape_bricks(wl)), wl.brick, axis=-1)
+    for ax in range(wl.ndim - 1):
+        act = np.repeat(act, wl.brick, axis=ax)
+    act = act.reshape(-1)
+    V = np.sqrt((wl.vel.astype(np.float64) ** 2).sum(axis=1)).astype(np.float32).astype(np.float64)
+    spacing = 2.0 * V / float(n - 1)
+    mx, over = [], []
+    for l in range(wl.n_lines):
+        ratio = (spacing * wl.inv_dlamD[l].astype(np.float64) * float(wl.lambda0[l]) / float(np.float32(wl.c_light)))
+        ratio = ratio.astype(np.float32)[act]
+        mx.append(float(ratio.max()) if ratio.size else 0.0)
+        over.append(int((ratio > np.float32(factor)).sum()))
+    return np.asarray(mx, dtype=np.float32), np.asarray(over, dtype=np.int64)
+
+
+def grid_shape_bricks(wl):
+    bd = wl.brick_dims
+    return (bd[1], bd[0]) if wl.ndim == 2 else (bd[2], bd[1], bd[0])
+
+
 def level_caps_paper(n_levels=4, first=6.0, factor=4.0):
     """Distance thresholds of the near-field MIP cap: the long-characteristics analogue of DexRT's per-cascade
     maximum MIP level [0,0,1,2,3,4] with interval ends 1.5 * 4^i voxels: level <= 0 for t < 6,

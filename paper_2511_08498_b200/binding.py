@@ -26,7 +26,7 @@ _STATUS = {0: "DEX_OK", 1: "DEX_ERR_INVALID_ARG", 2: "DEX_ERR_SHAPE", 3: "DEX_ER
 
 EXPORTS = (
     "dex_last_error", "dex_version", "dex_build_sparse_grid", "dex_grid_info", "dex_grid_get_slots",
-    "dex_destroy_grid", "dex_build_vlm_mips", "dex_mips_get_levels", "dex_mips_set_levels", "dex_mips_set_level_caps",
+    "dex_destroy_grid", "dex_build_vlm_mips", "dex_mips_get_levels", "dex_mips_set_levels", "dex_mips_set_level_caps", "dex_mips_velocity_bin_report",
     "dex_mips_get_packed_levels", "dex_mips_get_level_data", "dex_destroy_mips", "dex_formal_solution",
     "dex_mean_intensity", "dex_mean_intensity_host", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read", "dex_march_work_read",
     "dex_set_lanes_per_ray", "dex_set_tuning",
@@ -81,6 +81,7 @@ def _load():
     L.dex_mips_get_levels.argtypes = [C.c_void_p, C.c_void_p]
     L.dex_mips_set_levels.argtypes = [C.c_void_p, C.c_void_p]
     L.dex_mips_set_level_caps.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+    L.dex_mips_velocity_bin_report.argtypes = [C.c_void_p, C.c_float, C.c_void_p, C.c_void_p]
     L.dex_mips_get_packed_levels.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.POINTER(C.c_int64)]
     L.dex_mips_get_level_data.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
     L.dex_destroy_mips.argtypes = [C.c_void_p]
@@ -227,6 +228,13 @@ class Mips:
         """Near-field MIP cap thresholds (ascending distances in voxels; empty / None removes the cap)."""
         t = np.ascontiguousarray([] if cap_t is None else cap_t, dtype=np.float32)
         _check(_L.dex_mips_set_level_caps(self.handle, int(t.size), t.ctypes.data if t.size else None))
+
+    def velocity_bin_report(self, factor: float = 2.0):
+        """PAPER.md:200 diagnostic: (max spacing / thermal width per line, level-0 cells above `factor` per line)."""
+        mx = np.zeros(max(1, self.n_lines), dtype=np.float32)
+        over = np.zeros(max(1, self.n_lines), dtype=np.int64)
+        _check(_L.dex_mips_velocity_bin_report(self.handle, float(factor), mx.ctypes.data, over.ctypes.data))
+        return mx[:self.n_lines], over[:self.n_lines]
 
     def packed_levels(self, batch: int) -> np.ndarray:
         n = C.c_int64(0)

@@ -469,6 +469,37 @@ dex_status dex_mips_set_levels(dex_mips* mips, const int8_t* h_level) {
   return DEX_OK;
 }
 
+dex_status dex_mips_velocity_bin_report(const dex_mips* mips, float factor, float* h_max_ratio, int64_t* h_cells_over) {
+  if (!mips || !h_max_ratio || !h_cells_over) { dex_set_error("NULL mips / outputs"); return DEX_ERR_INVALID_ARG; }
+  if (mips->variant != DEX_VELINTERP) { dex_set_error("the bin-spacing report applies to DEX_VELINTERP mips"); return DEX_ERR_INVALID_ARG; }
+  const int nl = mips->dev.n_lines;
+  for (int l = 0; l < nl; ++l) { h_max_ratio[l] = 0.0f; h_cells_over[l] = 0; }
+  if (nl == 0) return DEX_OK;
+  unsigned* d_max = nullptr;
+  unsigned long long* d_cnt = nullptr;
+  DEX_CUDA_CHECK(cudaDeviceSynchronize());
+  dex_status s = dmalloc(&d_max, (size_t)DEX_MAX_LINES, (cudaStream_t)0);
+  if (s == DEX_OK) s = dmalloc(&d_cnt, (size_t)DEX_MAX_LINES, (cudaStream_t)0);
+  cudaError_t e = cudaSuccess;
+  if (s == DEX_OK) e = cudaMemsetAsync(d_max, 0, sizeof(unsigned) * DEX_MAX_LINES, 0);
+  if (s == DEX_OK && e == cudaSuccess) e = cudaMemsetAsync(d_cnt, 0, sizeof(unsigned long long) * DEX_MAX_LINES, 0);
+  if (s == DEX_OK && e == cudaSuccess) s = dex_launch_vbin_report(mips, factor, d_max, d_cnt, 0);
+  unsigned hmax[DEX_MAX_LINES] = {0};
+  unsigned long long hcnt[DEX_MAX_LINES] = {0};
+  if (s == DEX_OK && e == cudaSuccess) e = cudaMemcpy(hmax, d_max, sizeof(hmax), cudaMemcpyDeviceToHost);
+  if (s == DEX_OK && e == cudaSuccess) e = cudaMemcpy(hcnt, d_cnt, sizeof(hcnt), cudaMemcpyDeviceToHost);
+  cudaDeviceSynchronize();
+  dex_free(d_max, 0);
+  dex_free(d_cnt, 0);
+  if (s != DEX_OK) return s;
+  DEX_CUDA_CHECK(e);
+  for (int l = 0; l < nl; ++l) {
+    memcpy(&h_max_ratio[l], &hmax[l], sizeof(float));
+    h_cells_over[l] = (int64_t)hcnt[l];
+  }
+  return DEX_OK;
+}
+
 dex_status dex_mips_set_level_caps(dex_mips* mips, int n_caps, const float* h_cap_t) {
   if (!mips || (n_caps > 0 && !h_cap_t)) { dex_set_error("NULL mips / h_cap_t"); return DEX_ERR_INVALID_ARG; }
   if (n_caps < 0 || n_caps > 8) { dex_set_error("n_caps must be 0..8"); return DEX_ERR_SHAPE; }

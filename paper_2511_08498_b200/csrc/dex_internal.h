@@ -54,6 +54,7 @@ dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStrea
 // mips_build.cu
 dex_status dex_launch_mips_build(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st);
 dex_status dex_launch_pack_levels(dex_mips* m, cudaStream_t st);
+dex_status dex_launch_vbin_report(const dex_mips* m, float factor, unsigned* d_max, unsigned long long* d_cnt, cudaStream_t st);
 dex_status dex_launch_level_data(const dex_mips* m, int chain, int level, float* d_dense, cudaStream_t st);
 // march.cu
 dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,

@@ -597,6 +597,42 @@ dex_status dex_launch_pack_levels(dex_mips* m, cudaStream_t st) {
   return DEX_OK;
 }
 
+// "warns if the spacing between bins is greater than two times (configurable) the thermal width of the
+// spectral line".  Per line: the largest ratio (bin spacing 2V/(n-1)) / (thermal width c dlamD / lambda0, as a
+// velocity) over the level-0 cells of the active bricks, and the number of cells above `factor`.  out[l] = max ratio
+// (float bits, ratios are >= 0 so the unsigned order is the float order), cnt[l] = cells over.
+__global__ void vbin_report_kernel(const BuildCtx X, int cells0, float factor, unsigned* __restrict__ out,
+                                   unsigned long long* __restrict__ cnt) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long total = (long long)X.G.n_active * cells0;
+  if (i >= total) return;
+  const long long slot = i / cells0;
+  const int c = (int)(i - slot * cells0);
+  const size_t cell = (size_t)slot * X.M.cps + c;        // level 0 starts at lvloff[0] = 0
+  const double V = (double)X.M.vel[cell].w;
+  const double spacing = 2.0 * V / (double)(X.M.n_vbins - 1);
+  for (int l = 0; l < X.M.n_lines; ++l) {
+    const double invD = (double)X.M.line[cell * X.M.n_lines + l].w;
+    const double ratio = spacing * invD * (double)X.M.lambda0[l] / X.M.c_light;
+    const float rf = (float)ratio;
+    atomicMax(out + l, __float_as_uint(rf));
+    if (rf > factor) atomicAdd(cnt + l, 1ULL);
+  }
+}
+
+dex_status dex_launch_vbin_report(const dex_mips* m, float factor, unsigned* d_max, unsigned long long* d_cnt, cudaStream_t st) {
+  const BuildCtx X = make_ctx(m);
+  const int nd = m->grid->desc.ndim;
+  const int B = X.G.B;
+  const int cells0 = (nd == 3) ? B * B * B : B * B;
+  const long long total = (long long)X.G.n_active * cells0;
+  if (total == 0) return DEX_OK;
+  vbin_report_kernel<<<blocks_for(total, 256), 256, 0, st>>>(X, cells0, factor, d_max, d_cnt);
+  dex_count_launch();
+  DEX_CUDA_CHECK(cudaGetLastError());
+  return DEX_OK;
+}
+
 dex_status dex_launch_level_data(const dex_mips* m, int chain, int level, float* d_dense, cudaStream_t st) {
   const BuildCtx X = make_ctx(m);
   int width = 0;

@@ -454,3 +454,18 @@ def test_level_cap_parity(P, name, kw, thr):
             assert ref.segments == base.segments
     with pytest.raises(P.DexError):
         mips.set_level_caps([5.0, 2.0])
+
+
+def test_velocity_bin_report(P):
+    """dex_mips_velocity_bin_report against the oracle: per-line maximum ratio bit-exact, counts exact."""
+    wl = make("C3", n=256, n_dirs=4, n_probes=16)
+    dw, grid, mips = _build(P, wl)
+    for factor in (2.0, 1.0, 0.25):
+        mx, over = mips.velocity_bin_report(factor)
+        rmx, rover = orc.velocity_bin_report(wl, factor)
+        assert np.array_equal(mx.view(np.uint32), rmx.view(np.uint32)) and np.array_equal(over, rover)
+    assert over[0] > 0
+    wl2 = make("C4", n=64, n_dirs=4, n_probes=16)
+    _, _, m2 = _build(P, wl2)
+    with pytest.raises(P.DexError):
+        m2.velocity_bin_report(2.0)

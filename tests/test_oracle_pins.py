@@ -608,3 +608,20 @@ def test_t8_level_cap_limits_and_geometry():
         n = int(r.counts[ray])
         L = float(r.ds[ray, :n].astype(np.float64).sum())
         assert abs(r.I[ray // n_dirs, ray % n_dirs, 0] - S0 * (1.0 - math.exp(-chi0 * L))) < 1e-12
+
+
+def test_c13_velocity_bin_spacing_report_hand_example():
+    """PAPER.md:200 warning criterion on a hand-checkable field: |v| = 30 km/s everywhere, 8 bins -> spacing 60/7 km/s;
+    thermal width c dlamD / lambda0 = 5 km/s in the left half, 3 km/s in the right half -> ratios 12/7 and 20/7:
+    only the right half exceeds the paper's factor 2."""
+    wl = make("C3", n=64, n_dirs=4, n_probes=4)
+    wl.active[:] = 1
+    wl.vel[:, 0], wl.vel[:, 1] = 18.0, 24.0
+    vth = np.where(np.arange(64)[None, :] < 32, 5.0, 3.0) * np.ones((64, 1))
+    wl.inv_dlamD[0] = (wl.c_light / (vth.ravel() * float(wl.lambda0[0]))).astype(np.float32)
+    mx, over = orc.velocity_bin_report(wl, factor=2.0)
+    assert abs(float(mx[0]) - 20.0 / 7.0) < 1e-5 and int(over[0]) == 64 * 32
+    mx, over = orc.velocity_bin_report(wl, factor=1.5)
+    assert int(over[0]) == 64 * 64
+    mx16, over16 = orc.velocity_bin_report(wl, factor=2.0, n_vbins=16)      # twice the bins: nothing to warn about
+    assert abs(float(mx16[0]) - 4.0 / 3.0) < 1e-5 and int(over16[0]) == 0
