@@ -166,6 +166,12 @@ typedef struct {
   const float* d_dirs;    /* [n_dirs][ndim] unit propagation directions */
   const float* d_weights; /* [n_dirs] quadrature weights (dex_mean_intensity) */
   const float* d_i0;      /* [n_dirs][n_lambda] incoming boundary intensity, NULL = 0 */
+  const float* d_sin_incl; /* [n_dirs] or NULL.  2.5D rays (in-plane samples "augmented with a 4 sample
+                            * Gauss-Radau quadrature for different inclinations in y", y homogeneous and free of
+                            * velocity): sin of the angle between direction k and the homogeneous
+                            * out-of-plane axis, in (0, 1].  d_dirs stays the in-plane unit direction and the traversal
+                            * is unchanged; every path length is divided by sin_incl[k] and the projected velocity is
+                            * multiplied by it.  2D grids only (else DEX_ERR_INVALID_ARG); NULL = rays in the plane. */
 } dex_rays;
 
 /* a10. Visit-list capture (validation mode).  Ray r = probe * n_dirs + dir.  Records of ray r

@@ -170,6 +170,12 @@ typedef struct {
      * n_caps = 0: no cap. */
     int n_caps;
     float cap_t[8];              /* ascending thresholds, index units */
+    /* 2.5D rays (in-plane angular samples "augmented with a 4 sample Gauss-Radau quadrature for
+     * different inclinations in y", y homogeneous and without velocity components): direction k
+     * makes the angle theta_k with the homogeneous axis, sin_incl[k] = sin(theta_k).  The traversal is the in-plane
+     * one; every path length is divided by sin(theta) and the in-plane direction that projects the velocity is
+     * multiplied by it.  NULL: rays lie in the plane.  2D grids only. */
+    const float* sin_incl;       /* [n_dirs] or NULL */
 } orc_grid;
 
 static inline int64_t cell_index(const orc_grid* g, int m, const int* cc)
@@ -399,7 +405,7 @@ static int hdda(const orc_grid* g, const int8_t* level, const float* probe, cons
 /* Apply eq. 3 from the boundary to the probe over a collected segment list (north_star
  * recurrence I_out = I_in e^{-chi ds} + S (1 - e^{-chi ds})), for the W wavelengths of batch b. */
 static void integrate_list(const orc_grid* g, const orc_fields* F, const seg_t* segs, int n, int b,
-                           const double* omega, const float* i0_dir, double* I_out)
+                           const double* omega, double sin_incl, const float* i0_dir, double* I_out)
 {
     const int W = F->W;
     double I[ORC_MAX_W], eta[ORC_MAX_W], chi[ORC_MAX_W];
@@ -407,7 +413,7 @@ static void integrate_list(const orc_grid* g, const orc_fields* F, const seg_t* 
     for (int i = n - 1; i >= 0; --i) {
         int64_t cell = cell_index(g, segs[i].level, segs[i].cc);
         provider(g, F, segs[i].level, cell, b, omega, eta, chi);
-        double hds = g->h * (double)segs[i].ds;
+        double hds = g->h * (double)segs[i].ds / sin_incl;        /* 3D path length of the in-plane segment */
         for (int j = 0; j < W; ++j) I[j] = orc_segment(I[j], eta[j], chi[j], hds);
     }
     for (int j = 0; j < W; ++j) I_out[b * W + j] = I[j];
@@ -462,13 +468,14 @@ int64_t orc_plain_march(const orc_grid* g, const orc_fields* F, int64_t n_probes
             for (int k = 0; k < n_dirs; ++k) {
                 const float* om = dirs + (int64_t)k * g->ndim;
                 double omega[3] = {0, 0, 0};
-                for (int a = 0; a < g->ndim; ++a) omega[a] = (double)om[a];
+                const double si = (g->sin_incl && g->ndim == 2) ? (double)g->sin_incl[k] : 1.0;
+                for (int a = 0; a < g->ndim; ++a) omega[a] = (double)om[a] * si;   /* in-plane part of the 3D direction */
                 int n = plain_dda(g, probe_pos + p * g->ndim, om, segs, ms);
                 if (n < 0) { err = 1; n = 0; }
                 int64_t ray = p * n_dirs + k;
                 if (cap) capture_store(cap, ray, segs, n);
                 for (int b = 0; b < nb; ++b)
-                    integrate_list(g, F, segs, n, b, omega, i0 ? i0 + (int64_t)k * F->n_lambda : NULL,
+                    integrate_list(g, F, segs, n, b, omega, si, i0 ? i0 + (int64_t)k * F->n_lambda : NULL,
                                    I + ray * F->n_lambda);
                 total += (int64_t)n * nb;
             }
@@ -500,13 +507,14 @@ int64_t orc_hdda_march(const orc_grid* g, const orc_fields* F, const int8_t* lev
             for (int k = 0; k < n_dirs; ++k) {
                 const float* om = dirs + (int64_t)k * g->ndim;
                 double omega[3] = {0, 0, 0};
-                for (int a = 0; a < g->ndim; ++a) omega[a] = (double)om[a];
+                const double si = (g->sin_incl && g->ndim == 2) ? (double)g->sin_incl[k] : 1.0;
+                for (int a = 0; a < g->ndim; ++a) omega[a] = (double)om[a] * si;   /* in-plane part of the 3D direction */
                 int64_t ray = p * n_dirs + k;
                 for (int b = 0; b < nb; ++b) {
                     int n = hdda(g, levels + (int64_t)b * n_bricks, probe_pos + p * g->ndim, om, segs, ms);
                     if (n < 0) { err = 1; n = 0; }
                     if (cap && cap->batch == b) capture_store(cap, ray, segs, n);
-                    integrate_list(g, F, segs, n, b, omega, i0 ? i0 + (int64_t)k * F->n_lambda : NULL,
+                    integrate_list(g, F, segs, n, b, omega, si, i0 ? i0 + (int64_t)k * F->n_lambda : NULL,
                                    I + ray * F->n_lambda);
                     total += n;
                 }

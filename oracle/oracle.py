@@ -25,7 +25,7 @@ IOD_LOG, RELVAR = 0, 1
 
 class _Grid(C.Structure):
     _fields_ = [("ndim", C.c_int), ("dims", C.c_int * 3), ("brick", C.c_int), ("h", C.c_double),
-                ("n_caps", C.c_int), ("cap_t", C.c_float * 8)]
+                ("n_caps", C.c_int), ("cap_t", C.c_float * 8), ("sin_incl", C.c_void_p)]
 
 
 _PP = C.POINTER(C.c_void_p)
@@ -501,8 +501,19 @@ def _rays(wl, probe_pos, dirs, i0):
     return pp, dd, ii
 
 
+def _set_sin_incl(g, wl, dd, sin_incl, keep):
+    """2.5D rays: per-direction sine of the inclination to the homogeneous axis."""
+    si = getattr(wl, "sin_incl", None) if sin_incl is None else sin_incl
+    if si is None:
+        return
+    si = np.ascontiguousarray(si, dtype=np.float32)
+    assert wl.ndim == 2 and si.shape == (dd.shape[0],) and (si > 0).all() and (si <= 1).all()
+    keep.append(si)
+    g.sin_incl = si.ctypes.data
+
+
 def plain_march(wl, M: Optional[OracleMips] = None, probe_pos=None, dirs=None, i0=None, capture=False,
-                variant=None, n_threads=0) -> MarchResult:
+                variant=None, n_threads=0, sin_incl=None) -> MarchResult:
     """(A) AW87 DDA through every level-0 voxel; provider = fetch (ISO) or Classic."""
     if M is None:
         v = wl.variant if variant is None else variant
@@ -515,6 +526,7 @@ def plain_march(wl, M: Optional[OracleMips] = None, probe_pos=None, dirs=None, i
     if F.variant == CAV:
         F.variant = CLASSIC
     pp, dd, ii = _rays(wl, probe_pos, dirs, i0)
+    _set_sin_incl(g, wl, dd, sin_incl, keep)
     n_rays = pp.shape[0] * dd.shape[0]
     I = np.zeros((pp.shape[0], dd.shape[0], wl.n_lambda), dtype=np.float64)
     cap = counts = records = ds = None
@@ -560,7 +572,7 @@ def level_caps_paper(n_levels=4, first=6.0, factor=4.0):
 
 
 def hdda_march(wl, M: OracleMips, probe_pos=None, dirs=None, i0=None, capture_batch=None, levels=None,
-               n_threads=0, level_cap_t=None) -> MarchResult:
+               n_threads=0, level_cap_t=None, sin_incl=None) -> MarchResult:
     """(B) HDDA over the brick/level structure with the VLM mips (Algorithm 1).
     level_cap_t: ascending distance thresholds of the near-field MIP cap (T8), None = no cap."""
     keep = []
@@ -574,6 +586,7 @@ def hdda_march(wl, M: OracleMips, probe_pos=None, dirs=None, i0=None, capture_ba
     if F.variant == CLASSIC:
         F.variant = CAV
     pp, dd, ii = _rays(wl, probe_pos, dirs, i0)
+    _set_sin_incl(g, wl, dd, sin_incl, keep)
     lv = np.ascontiguousarray(M.levels if levels is None else levels, dtype=np.int8)
     n_rays = pp.shape[0] * dd.shape[0]
     I = np.zeros((pp.shape[0], dd.shape[0], wl.n_lambda), dtype=np.float64)

@@ -69,6 +69,8 @@ dex_status check_rays(const dex_grid* grid, const dex_mips* mips, const dex_rays
   out->dirs = rays->d_dirs;
   out->weights = rays->d_weights;
   out->i0 = rays->d_i0;
+  out->sin_incl = rays->d_sin_incl;
+  if (rays->d_sin_incl && grid->dev.ndim != 2) { dex_set_error("d_sin_incl (2.5D rays) needs a 2D grid"); return DEX_ERR_INVALID_ARG; }
   return DEX_OK;
 }
 
@@ -661,6 +663,7 @@ dex_status dex_mean_intensity_host(const dex_grid_desc* desc, const uint8_t* h_a
   dr.d_dirs = up.put(hr->d_dirs, (size_t)hr->n_dirs * D);
   dr.d_weights = up.put(hr->d_weights, (size_t)hr->n_dirs);
   dr.d_i0 = up.put(hr->d_i0, (size_t)hr->n_dirs * nl);
+  dr.d_sin_incl = up.put(hr->d_sin_incl, (size_t)hr->n_dirs);
   float* d_J = up.alloc<float>((size_t)hr->n_probes * nl);
   int64_t* d_seg = up.alloc<int64_t>(1);
   if (up.status != DEX_OK) return up.status;

@@ -66,6 +66,7 @@ struct DexRaysDev {
   const float* dirs;
   const float* weights;
   const float* i0;
+  const float* sin_incl;   // [n_dirs] or NULL: 2.5D rays
 };
 
 // ---- exact (uncontracted) fp32 helpers -------------------------------------------------

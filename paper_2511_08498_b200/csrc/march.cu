@@ -221,7 +221,7 @@ __device__ __noinline__ float dex_voigt_H_outside_window(const double* __restric
 // eta, chi of one cell for this lane's wavelengths, seen along propagation direction om (a7)
 template <int D, int VAR, int LPT>
 __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_base, int cell, int sub,
-                                             const float* __restrict__ om, const DexCavTab& CT,
+                                             const float* __restrict__ om, float sin_incl, const DexCavTab& CT,
                                              const float4* __restrict__ vfw, const float* __restrict__ vfc,
                                              const float* __restrict__ iso0, const float* __restrict__ iso1,
                                              float (&eta)[LPT], float (&chi)[LPT]) {
@@ -235,6 +235,7 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
   double vproj = __dmul_rn((double)v4.x, (double)__ldg(om));
   vproj = __dadd_rn(vproj, __dmul_rn((double)v4.y, (double)__ldg(om + 1)));
   if (D == 3) vproj = __dadd_rn(vproj, __dmul_rn((double)v4.z, (double)__ldg(om + D - 1)));
+  if (D == 2) vproj = __dmul_rn(vproj, (double)sin_incl);   // 2.5D: in-plane part of the 3D direction (1 for in-plane rays)
   if (VAR == DEX_VELINTERP) {
     // linear interpolation on the cell's uniform velocity grid [-V, V]
     const int nvb = M.n_vbins;
@@ -448,6 +449,9 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   // one direction at a time: the lanes of a warp trace the same direction together (coherent fetches)
   for (int k = 0; k < R.n_dirs; ++k) {
     const float* __restrict__ om = R.dirs + k * D;
+    // 2.5D rays: path lengths are divided by the sine of the inclination to the homogeneous axis (dex.h d_sin_incl)
+    const float sin_incl = (D == 2 && R.sin_incl != nullptr) ? __ldg(R.sin_incl + k) : 1.0f;
+    const float hk = (D == 2 && R.sin_incl != nullptr) ? __fdiv_rn(G.h, sin_incl) : G.h;
 #pragma unroll
     for (int i = 0; i < LPT; ++i) { I[i] = 0.0f; DEX_IH(i) = 0.0f; T[i] = 1.0f; }
     bool alive = valid && dex_ray_init3<D>(ray, G, M, binfo, probe, om);
@@ -473,9 +477,9 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
         blocked = !dex_ray_advance<D>(ray, emit, cell, ds);
         if (emit) {
           ++nseg;
-          const float hds = G.h * ds;
+          const float hds = hk * ds;
           float eta[LPT], chi[LPT];
-          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, CT, vfw, vfc, iso0, iso1, eta, chi);
+          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, sin_incl, CT, vfw, vfc, iso0, iso1, eta, chi);
           if (VAR == DEX_ISO) dex_accumulate_all_S<LPT>(eta, chi, hds, I, T);
           else dex_accumulate_all<LPT>(eta, chi, hds, I, T);
         }

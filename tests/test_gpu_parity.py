@@ -469,3 +469,29 @@ def test_velocity_bin_report(P):
     _, _, m2 = _build(P, wl2)
     with pytest.raises(P.DexError):
         m2.velocity_bin_report(2.0)
+
+
+# ------------------------------------------------------------------------------------------ 2.5D rays (8(f)-2)
+@pytest.mark.parametrize("name,kw", [("C2", dict(n=256, n_probes=600)), ("C4", dict(n=128, n_probes=200)),
+                                     ("C3", dict(n=128, n_probes=150))])
+def test_25d_rays_parity(P, name, kw):
+    """dex_rays.d_sin_incl (PAPER.md:347 Gauss-Radau inclinations) against the oracle for the three providers: visit
+    lists unchanged and bit-exact, I and J within 1e-5; also through the host entry; 3D grids reject it."""
+    from workloads.gen import dirs_25d
+    wl = make(name, n_dirs=4, **kw)
+    if name == "C4":
+        wl.thr_eta = wl.thr_chi = 0.3
+    wl.dirs, wl.weights, wl.sin_incl = dirs_25d(5, 4)
+    M = orc.build_mips(wl)
+    dw, grid, mips = _build(P, wl)
+    ref = _solve_and_compare(P, wl, M, dw, grid, mips, lanes=(1, 4))
+    flat = orc.hdda_march(wl, M, sin_incl=np.ones(20, dtype=np.float32))
+    assert max_rel(ref.I, flat.I) > 1e-3                     # the inclination changes the answer
+    Jh, nseg, _, _ = P.pipeline.solve_J_from_host(wl, "cuda:0")
+    assert nseg == ref.segments
+    assert max_rel(Jh, orc.mean_intensity(ref.I, wl.weights)) <= TOL
+    w3 = make("C5", n=32, n_dirs=4, n_probes=20)
+    w3.sin_incl = np.ones(4, dtype=np.float32)
+    d3, g3, m3 = _build(P, w3)
+    with pytest.raises(P.DexError):
+        P.pipeline.mean_intensity(d3, g3, m3)

@@ -625,3 +625,58 @@ def test_c13_velocity_bin_spacing_report_hand_example():
     assert int(over[0]) == 64 * 64
     mx16, over16 = orc.velocity_bin_report(wl, factor=2.0, n_vbins=16)      # twice the bins: nothing to warn about
     assert abs(float(mx16[0]) - 4.0 / 3.0) < 1e-5 and int(over16[0]) == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# 2.5D rays (PAPER.md:347 Gauss-Radau quadrature in the inclination to the homogeneous axis)
+# ------------------------------------------------------------------------------------------------
+def test_25d_quadrature_and_inclined_rays():
+    """(i) the Gauss-Radau rule has its fixed node at mu = 0, weights summing to 1, and is exact to degree 2n - 2;
+    (ii) sin = 1 changes nothing; (iii) homogeneous medium: I = S (1 - exp(-chi h L / sin)) with L the in-plane length
+    (PAPER.md:65); (iv) an inclined ray equals an in-plane ray through the atmosphere with voxel size h / sin and
+    velocities v sin (Classic march, eq. 14), visit lists unchanged; (v) J of a thick uniform medium is S."""
+    from workloads.gen import dirs_25d, gauss_radau_unit
+    for n in (2, 3, 4, 6):
+        mu, w = gauss_radau_unit(n)
+        assert mu[0] == 0.0 and abs(w.sum() - 1.0) < 1e-14 and (np.diff(mu) > 0).all() and mu[-1] < 1.0
+        for k in range(2 * n - 1):
+            assert abs((w * mu ** k).sum() - 1.0 / (k + 1)) < 1e-13
+        assert abs((w * mu ** (2 * n - 1)).sum() - 1.0 / (2 * n)) > 1e-8
+    # (ii), (iii)
+    rng = np.random.default_rng(3)
+    chi0, S0 = 0.07, 1.3
+    f = np.full((48, 48, 8), chi0)
+    probes = rng.uniform(0, 48, size=(20, 2))
+    dirs, wts, si = dirs_25d(6, 4)
+    wl = iso_workload((48, 48), 16, f * S0, f, probes, dirs, weights=wts, max_level=2, thr=1.0, h=1.5)
+    M = orc.build_mips(wl)
+    a = orc.hdda_march(wl, M, capture_batch=0)
+    b = orc.hdda_march(wl, M, capture_batch=0, sin_incl=np.ones(len(si), dtype=np.float32))
+    assert np.array_equal(a.I, b.I) and np.array_equal(a.records, b.records)
+    c = orc.hdda_march(wl, M, capture_batch=0, sin_incl=si)
+    assert np.array_equal(a.records, c.records) and np.array_equal(a.ds, c.ds)
+    chi32, S32 = float(np.float32(chi0)), float(np.float32(chi0 * S0)) / float(np.float32(chi0))
+    for p in range(probes.shape[0]):
+        for k in range(dirs.shape[0]):
+            L = path_to_boundary(wl.probe_pos[p], wl.dirs[k], (48, 48))
+            want = S32 * (1.0 - math.exp(-chi32 * 1.5 * L / float(si[k])))
+            assert abs(c.I[p, k, 0] - want) < 2e-5 * want          # L from fp64 geometry, ds from fp32 plane times
+    # (iv) Classic march with velocities: inclined == in-plane with h / sin and v sin, one direction at a time
+    wv = make("C4", n=64, n_dirs=3, n_probes=12)
+    s = np.float32(0.59375)                                         # exactly representable
+    A = orc.plain_march(wv, variant=orc.CLASSIC, sin_incl=np.full(3, s, dtype=np.float32), capture=True)
+    import copy
+    w2 = copy.copy(wv)
+    w2.voxel_size = float(np.float64(wv.voxel_size) / np.float64(s))
+    w2.vel = (wv.vel.astype(np.float64) * float(s)).astype(np.float32)
+    Bm = orc.plain_march(w2, variant=orc.CLASSIC, capture=True)
+    assert np.array_equal(A.records, Bm.records)
+    assert max_rel(A.I, Bm.I) < 5e-6                                 # v sin and h / sin are rounded to fp32 in w2
+    plain = orc.plain_march(wv, variant=orc.CLASSIC)
+    assert max_rel(A.I, plain.I) > 1e-2                              # and the inclination does matter
+    # (v) thick uniform medium: J -> S for the full 2.5D quadrature
+    f2 = np.full((32, 32, 8), 5.0)
+    wt = iso_workload((32, 32), 16, f2 * 0.8, f2, [[16.5, 16.5]], dirs, weights=wts)
+    r = orc.plain_march(wt, sin_incl=si)
+    J = orc.mean_intensity(r.I, wt.weights)
+    assert abs(J[0, 0] - 0.8) < 1e-6

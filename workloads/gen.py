@@ -53,6 +53,7 @@ class Workload:
     dirs: np.ndarray = None        # [n_dirs][ndim] fp32
     weights: np.ndarray = None     # [n_dirs] fp32
     i0: Optional[np.ndarray] = None  # [n_dirs][n_lambda] fp32 or None (= 0)
+    sin_incl: Optional[np.ndarray] = None  # [n_dirs] fp32 or None: 2.5D rays, sine of the inclination to the homogeneous axis
     # isotropic fields
     eta: Optional[np.ndarray] = None
     chi: Optional[np.ndarray] = None
@@ -136,6 +137,34 @@ def dirs_2d(n, phase=0.5):
     d = np.stack([np.cos(th), np.sin(th)], axis=1).astype(np.float32)
     w = np.full(n, 1.0 / n, dtype=np.float32)
     return d, w
+
+
+def gauss_radau_unit(n):
+    """n-point Gauss-Radau rule on mu in [0, 1] with the fixed node at mu = 0: returns (mu, w), sum w = 1, exact for
+    polynomials of degree <= 2n - 2.  Interior nodes are the roots of (P_{n-1}(x) + P_n(x)) / (1 + x) on [-1, 1],
+    weights (1 - x) / (n^2 P_{n-1}(x)^2) and 2 / n^2 at x = -1 (computed numerically, not tabulated)."""
+    from numpy.polynomial import legendre as L
+    c = np.zeros(n + 1)
+    c[n - 1] = c[n] = 1.0
+    roots = L.legroots(c)
+    x = np.sort(np.real(roots))
+    x[0] = -1.0
+    pn1 = L.legval(x, np.eye(n)[n - 1])
+    w = (1.0 - x) / (n * n * pn1 * pn1)
+    w[0] = 2.0 / (n * n)
+    return (x + 1.0) / 2.0, w / 2.0
+
+
+def dirs_25d(n_phi, n_incl=4, phase=0.5):
+    """2.5D quadrature of PAPER.md:347: n_phi in-plane azimuths x an n_incl-point Gauss-Radau rule in mu = cos(theta),
+    theta the angle to the homogeneous out-of-plane axis (mu = 0: in-plane rays).  Returns in-plane unit directions
+    [n_phi * n_incl][2], weights (sum 1; the hemisphere mu < 0 mirrors mu > 0) and sin(theta) per direction."""
+    d2, _ = dirs_2d(n_phi, phase=phase)
+    mu, w = gauss_radau_unit(n_incl)
+    dirs = np.repeat(d2, n_incl, axis=0)
+    weights = np.tile(w, n_phi) / float(n_phi)
+    sin_incl = np.tile(np.sqrt(1.0 - mu * mu), n_phi)
+    return (np.ascontiguousarray(dirs, dtype=np.float32), weights.astype(np.float32), sin_incl.astype(np.float32))
 
 
 def dirs_fibonacci(n):
