@@ -206,6 +206,7 @@ struct DexCavTab {
   float dlam_h[DEX_NLINES][DEX_W];   // the same two as fp32 (dlam as an unevaluated pair hi + lo) for the fp32 Voigt
   float dlam_l[DEX_NLINES][DEX_W];
   float r2f[DEX_NLINES][DEX_W];
+  float dlam_min[DEX_NLINES], dlam_max[DEX_NLINES];   // extremes of lambda - lambda0 over the batch (region-I pre-test)
   float r2lo[DEX_NLINES], r2hi[DEX_NLINES];   // min / max of r2f over the batch (slightly widened): damping window test
   float scale[DEX_NLINES][DEX_W];    // (lambda0 / lambda) / sqrt(pi): eta*(lambda) phi = eta*0 invD scale H (eqs. 18-19)
   double lam0_over_c[DEX_NLINES];    // Doppler shift of the line centre per unit projected velocity     (eq. 14)
@@ -307,9 +308,12 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
           af[2 * i] = a2.x; af[2 * i + 1] = a2.y;
           xh[2 * i] = x2.x; xh[2 * i + 1] = x2.y;
           H[2 * i] = h2.x; H[2 * i + 1] = h2.y;
-          far = far || (fabsf(x2.x) + a2.x >= 15.0f) || (fabsf(x2.y) + a2.y >= 15.0f);
         }
         (void)nshh;
+        // can any wavelength of the batch be in region I?  One bound per (segment, line) instead of a test per
+        // evaluation: |x_j| <= max(|dlam_min + shift|, |dlam_max + shift|) / dlamD, a_j <= a0 r2hi (slightly widened)
+        const float xb = fmaxf(fabsf(CT.dlam_min[q] + sh_h), fabsf(CT.dlam_max[q] + sh_h)) * ln.w;
+        far = fmaf(xb, 1.0001f, ln.z * CT.r2hi[q]) >= 14.99f;
       }
       if (far) {
 #pragma unroll
@@ -324,11 +328,21 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
         H[i] = dex_voigt_H_outside_window(M.wei_c, M.wei_L, CT.r2[q][j] * (double)ln.z, x);
       }
     }
+    if (LPT == 1) {
+      const float phi = H[0] * CT.scale[q][sub];
+      eta[0] = fmaf(es, phi, eta[0]);
+      chi[0] = fmaf(cs, phi, chi[0]);
+    } else {
+      const float2 es2 = dex_f2(es), cs2 = dex_f2(cs);
 #pragma unroll
-    for (int i = 0; i < LPT; ++i) {
-      const float phi = H[i] * CT.scale[q][sub * LPT + i];
-      eta[i] = fmaf(es, phi, eta[i]);
-      chi[i] = fmaf(cs, phi, chi[i]);
+      for (int i = 0; i < LPT / 2; ++i) {
+        const float2 sc = *reinterpret_cast<const float2*>(&CT.scale[q][sub * LPT + 2 * i]);
+        const float2 phi = __fmul2_rn(make_float2(H[2 * i], H[2 * i + 1]), sc);
+        const float2 e2 = __ffma2_rn(es2, phi, make_float2(eta[2 * i], eta[2 * i + 1]));
+        const float2 c2 = __ffma2_rn(cs2, phi, make_float2(chi[2 * i], chi[2 * i + 1]));
+        eta[2 * i] = e2.x; eta[2 * i + 1] = e2.y;
+        chi[2 * i] = c2.x; chi[2 * i + 1] = c2.y;
+      }
     }
   }
 }
@@ -413,12 +427,17 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
         CT.scale[q][j] = (float)((l0 / lm) * 0.56418958354775628695);
         if (j == 0) {
           CT.lam0_over_c[q] = l0 / M.c_light;
-          double lo = 1e300, hi = 0.0;
+          double lo = 1e300, hi = 0.0, dmin = 1e300, dmax = -1e300;
           for (int jj = 0; jj < DEX_W; ++jj) {
-            const double rr = (double)__ldg(M.lam + batch * DEX_W + jj) / l0;
+            const double lj = (double)__ldg(M.lam + batch * DEX_W + jj);
+            const double rr = lj / l0;
             lo = fmin(lo, rr * rr);
             hi = fmax(hi, rr * rr);
+            dmin = fmin(dmin, lj - l0);
+            dmax = fmax(dmax, lj - l0);
           }
+          CT.dlam_min[q] = (float)dmin;
+          CT.dlam_max[q] = (float)dmax;
           CT.r2lo[q] = (float)(lo * (1.0 - 1e-6));
           CT.r2hi[q] = (float)(hi * (1.0 + 1e-6));
         }
