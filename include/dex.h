@@ -172,6 +172,12 @@ typedef struct {
                             * out-of-plane axis, in (0, 1].  d_dirs stays the in-plane unit direction and the traversal
                             * is unchanged; every path length is divided by sin_incl[k] and the projected velocity is
                             * multiplied by it.  2D grids only (else DEX_ERR_INVALID_ARG); NULL = rays in the plane. */
+  float t_begin, t_end;    /* Finite radiance interval (DexRT traces HDDA(t1, t2) per cascade: Algorithm 1 l.9, l.22,
+                            * PAPER.md:347; T10): only the part of every ray with
+                            * t_begin <= t <= t_end (index units from the probe) contributes; d_i0 enters at t_end.  The
+                            * traversal still starts at the probe, so cells and plane times are those of the full ray
+                            * and each visit is clipped to the interval.  t_end <= 0 (a zero-initialised struct): to the
+                            * grid boundary.  Requires 0 <= t_begin < t_end otherwise (DEX_ERR_INVALID_ARG). */
 } dex_rays;
 
 /* a10. Visit-list capture (validation mode).  Ray r = probe * n_dirs + dir.  Records of ray r

@@ -176,7 +176,19 @@ typedef struct {
      * one; every path length is divided by sin(theta) and the in-plane direction that projects the velocity is
      * multiplied by it.  NULL: rays lie in the plane.  2D grids only. */
     const float* sin_incl;       /* [n_dirs] or NULL */
+    /* Finite radiance interval (DexRT traces HDDA(t1, t2) per cascade, Algorithm 1 l.9 and PAPER.md:347; SURVEY.md
+     * 8(f)-4; T10): only the part of the ray with t in [t_begin, t_end] (index units, from the probe)
+     * contributes.  The traversal itself is unchanged and starts at the probe, so the cells and plane times are
+     * those of the full ray; each visit [t, t_h] is clipped to the interval.  t_end <= 0: to the boundary. */
+    float t_begin, t_end;
 } orc_grid;
+
+/* T10: clip the visit [t, th] to the interval; returns the clipped length (<= 0: nothing to emit) */
+static inline float clip_visit(const orc_grid* g, float t, float th)
+{
+    if (g->t_end <= 0.0f) return th - t;
+    return fminf(th, g->t_end) - fmaxf(t, g->t_begin);
+}
 
 static inline int64_t cell_index(const orc_grid* g, int m, const int* cc)
 {
@@ -310,14 +322,15 @@ static int plain_dda(const orc_grid* g, const float* probe, const float* omega, 
             float tn = tplane(kp, r.inv[a], r.off[a]);
             if (s < 0 || tn < th) { th = tn; s = a; }         /* T4: lowest-index axis attaining the min */
         }
-        if (th > t) {
+        if (th > t && clip_visit(g, t, th) > 0.0f) {
             if (n >= max_segs) return -1;
             segs[n].level = 0;
             segs[n].cc[0] = x[0]; segs[n].cc[1] = x[1]; segs[n].cc[2] = x[2];
-            segs[n].ds = th - t;
+            segs[n].ds = clip_visit(g, t, th);
             ++n;
         }
         if (th > t) t = th;
+        if (g->t_end > 0.0f && t >= g->t_end) break;           /* T10: the interval ends inside the grid */
         x[s] += (r.d[s] > 0.0f) ? 1 : -1;                      /* T5 with size 1 */
         if (x[s] < 0 || x[s] >= g->dims[s]) break;
     }
@@ -363,14 +376,15 @@ static int hdda(const orc_grid* g, const int8_t* level, const float* probe, cons
             float tn = tplane(kp[a], r.inv[a], r.off[a]);
             if (s < 0 || tn < th) { th = tn; s = a; }
         }
-        if (m >= 0 && th > t) {                                  /* "Integrate RTE over [t, t_h]" l.25-26 */
+        if (m >= 0 && th > t && clip_visit(g, t, th) > 0.0f) {   /* "Integrate RTE over [t, t_h]" l.25-26 */
             if (n >= max_segs) return -1;
             segs[n].level = m;
             segs[n].cc[0] = c[0] >> m; segs[n].cc[1] = c[1] >> m; segs[n].cc[2] = (g->ndim == 3) ? (c[2] >> m) : 0;
-            segs[n].ds = th - t;
+            segs[n].ds = clip_visit(g, t, th);
             ++n;
         }
         if (th > t) t = th;
+        if (g->t_end > 0.0f && t >= g->t_end) break;             /* T10: "while t < t2", Alg. 1 l.22 */
         /* T5: cross plane (s, kp[s]); the other axes take the level-0 coordinate the plain DDA
          * would hold at this event: plane (a,k) counts as crossed iff tplane < t_h, or == t_h
          * and a < s (lower-index axes go first in ties).                                      */

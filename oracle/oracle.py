@@ -25,7 +25,8 @@ IOD_LOG, RELVAR = 0, 1
 
 class _Grid(C.Structure):
     _fields_ = [("ndim", C.c_int), ("dims", C.c_int * 3), ("brick", C.c_int), ("h", C.c_double),
-                ("n_caps", C.c_int), ("cap_t", C.c_float * 8), ("sin_incl", C.c_void_p)]
+                ("n_caps", C.c_int), ("cap_t", C.c_float * 8), ("sin_incl", C.c_void_p),
+                ("t_begin", C.c_float), ("t_end", C.c_float)]
 
 
 _PP = C.POINTER(C.c_void_p)
@@ -501,6 +502,15 @@ def _rays(wl, probe_pos, dirs, i0):
     return pp, dd, ii
 
 
+def _set_interval(g, interval):
+    """Finite radiance interval [t1, t2] in index units from the probe (T10); None = to the boundary."""
+    if interval is None:
+        return
+    t1, t2 = (float(np.float32(v)) for v in interval)
+    assert 0.0 <= t1 < t2
+    g.t_begin, g.t_end = t1, t2
+
+
 def _set_sin_incl(g, wl, dd, sin_incl, keep):
     """2.5D rays: per-direction sine of the inclination to the homogeneous axis."""
     si = getattr(wl, "sin_incl", None) if sin_incl is None else sin_incl
@@ -513,7 +523,7 @@ def _set_sin_incl(g, wl, dd, sin_incl, keep):
 
 
 def plain_march(wl, M: Optional[OracleMips] = None, probe_pos=None, dirs=None, i0=None, capture=False,
-                variant=None, n_threads=0, sin_incl=None) -> MarchResult:
+                variant=None, n_threads=0, sin_incl=None, interval=None) -> MarchResult:
     """(A) AW87 DDA through every level-0 voxel; provider = fetch (ISO) or Classic."""
     if M is None:
         v = wl.variant if variant is None else variant
@@ -527,6 +537,7 @@ def plain_march(wl, M: Optional[OracleMips] = None, probe_pos=None, dirs=None, i
         F.variant = CLASSIC
     pp, dd, ii = _rays(wl, probe_pos, dirs, i0)
     _set_sin_incl(g, wl, dd, sin_incl, keep)
+    _set_interval(g, getattr(wl, "interval", None) if interval is None else interval)
     n_rays = pp.shape[0] * dd.shape[0]
     I = np.zeros((pp.shape[0], dd.shape[0], wl.n_lambda), dtype=np.float64)
     cap = counts = records = ds = None
@@ -572,7 +583,7 @@ def level_caps_paper(n_levels=4, first=6.0, factor=4.0):
 
 
 def hdda_march(wl, M: OracleMips, probe_pos=None, dirs=None, i0=None, capture_batch=None, levels=None,
-               n_threads=0, level_cap_t=None, sin_incl=None) -> MarchResult:
+               n_threads=0, level_cap_t=None, sin_incl=None, interval=None) -> MarchResult:
     """(B) HDDA over the brick/level structure with the VLM mips (Algorithm 1).
     level_cap_t: ascending distance thresholds of the near-field MIP cap (T8), None = no cap."""
     keep = []
@@ -587,6 +598,7 @@ def hdda_march(wl, M: OracleMips, probe_pos=None, dirs=None, i0=None, capture_ba
         F.variant = CAV
     pp, dd, ii = _rays(wl, probe_pos, dirs, i0)
     _set_sin_incl(g, wl, dd, sin_incl, keep)
+    _set_interval(g, getattr(wl, "interval", None) if interval is None else interval)
     lv = np.ascontiguousarray(M.levels if levels is None else levels, dtype=np.int8)
     n_rays = pp.shape[0] * dd.shape[0]
     I = np.zeros((pp.shape[0], dd.shape[0], wl.n_lambda), dtype=np.float64)

@@ -56,7 +56,8 @@ class _MipsDesc(C.Structure):
 
 class _Rays(C.Structure):
     _fields_ = [("n_probes", C.c_int64), ("d_probe_pos", C.c_void_p), ("n_dirs", C.c_int), ("d_dirs", C.c_void_p),
-                ("d_weights", C.c_void_p), ("d_i0", C.c_void_p), ("d_sin_incl", C.c_void_p)]
+                ("d_weights", C.c_void_p), ("d_i0", C.c_void_p), ("d_sin_incl", C.c_void_p),
+                ("t_begin", C.c_float), ("t_end", C.c_float)]
 
 
 class _Capture(C.Structure):
@@ -312,8 +313,9 @@ def dex_build_vlm_mips(grid: Grid, variant, n_lambda, lambda_batch, max_level, m
 
 class Rays:
     def __init__(self, probe_pos: torch.Tensor, dirs: torch.Tensor, weights: Optional[torch.Tensor] = None,
-                 i0: Optional[torch.Tensor] = None, sin_incl: Optional[torch.Tensor] = None):
+                 i0: Optional[torch.Tensor] = None, sin_incl: Optional[torch.Tensor] = None, interval=None):
         self.probe_pos, self.dirs, self.weights, self.i0, self.sin_incl = probe_pos, dirs, weights, i0, sin_incl
+        self.interval = interval            # (t_begin, t_end) in voxels from the probe, None = to the boundary
         self.n_probes, self.n_dirs = int(probe_pos.shape[0]), int(dirs.shape[0])
 
     def struct(self, cuda=True):
@@ -323,6 +325,8 @@ class Rays:
         r.d_probe_pos, r.d_dirs = _ptr(self.probe_pos, f32, cuda), _ptr(self.dirs, f32, cuda)
         r.d_weights, r.d_i0 = _ptr(self.weights, f32, cuda), _ptr(self.i0, f32, cuda)
         r.d_sin_incl = _ptr(self.sin_incl, f32, cuda)
+        if self.interval is not None:
+            r.t_begin, r.t_end = float(self.interval[0]), float(self.interval[1])
         return r
 
 

@@ -70,6 +70,12 @@ dex_status check_rays(const dex_grid* grid, const dex_mips* mips, const dex_rays
   out->weights = rays->d_weights;
   out->i0 = rays->d_i0;
   out->sin_incl = rays->d_sin_incl;
+  out->t_begin = rays->t_begin;
+  out->t_end = rays->t_end;
+  if (rays->t_end > 0.0f && !(rays->t_begin >= 0.0f && rays->t_begin < rays->t_end)) {
+    dex_set_error("radiance interval needs 0 <= t_begin < t_end");
+    return DEX_ERR_INVALID_ARG;
+  }
   if (rays->d_sin_incl && grid->dev.ndim != 2) { dex_set_error("d_sin_incl (2.5D rays) needs a 2D grid"); return DEX_ERR_INVALID_ARG; }
   return DEX_OK;
 }

@@ -67,6 +67,7 @@ struct DexRaysDev {
   const float* weights;
   const float* i0;
   const float* sin_incl;   // [n_dirs] or NULL: 2.5D rays
+  float t_begin, t_end;    // finite radiance interval (T10); t_end <= 0: to the boundary
 };
 
 // ---- exact (uncontracted) fp32 helpers -------------------------------------------------

@@ -379,7 +379,7 @@ constexpr int dex_march_minb(int var) {
 #define DEX_CROSS_QUORUM 8
 #endif
 
-template <int D, int VAR, int LPR, bool FUSE_J>
+template <int D, int VAR, int LPR, bool FUSE_J, bool CLIP>
 __global__ void __launch_bounds__(DEX_MARCH_THREADS, dex_march_minb(VAR))
 dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ perm,
                  float* __restrict__ out, unsigned long long* __restrict__ seg_count,
@@ -493,7 +493,13 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
         bool emit;
         int cell;
         float ds;
+        const float t0 = ray.t;
         blocked = !dex_ray_advance<D>(ray, emit, cell, ds);
+        if (CLIP) {   // T10 (compile time: the full-ray kernels do not pay for it): visit [t0, ray.t] clipped to the interval
+          ds = __fsub_rn(fminf(ray.t, R.t_end), fmaxf(t0, R.t_begin));
+          emit = emit && ds > 0.0f;
+          if (ray.t >= R.t_end) { alive = false; blocked = false; }
+        }
         if (emit) {
           ++nseg;
           const float hds = hk * ds;
@@ -569,7 +575,14 @@ dex_capture_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, l
     bool emit;
     int cell;
     float ds;
-    if (!dex_ray_advance<D>(ray, emit, cell, ds)) alive = dex_ray_cross<D>(ray, G, M, binfo, probe, om);
+    const float t0 = ray.t;
+    const bool inside = dex_ray_advance<D>(ray, emit, cell, ds);
+    if (R.t_end > 0.0f) {
+      ds = __fsub_rn(fminf(ray.t, R.t_end), fmaxf(t0, R.t_begin));
+      emit = emit && ds > 0.0f;
+    }
+    if (R.t_end > 0.0f && ray.t >= R.t_end) alive = false;
+    else if (!inside) alive = dex_ray_cross<D>(ray, G, M, binfo, probe, om);
     if (emit) {
       if (n < room) {
         unsigned long long rec = ((unsigned long long)(unsigned)m << 56) | (unsigned long long)(unsigned)(c[0] >> m);
@@ -683,7 +696,7 @@ __global__ void dex_voigt_profile_kernel(const float* __restrict__ a, const doub
   }
 }
 
-template <int D, int VAR, int LPR>
+template <int D, int VAR, int LPR, bool CLIP = false>
 dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
                           unsigned long long* d_seg, const int* perm, cudaStream_t st) {
   const int threads = DEX_MARCH_THREADS;
@@ -699,9 +712,9 @@ dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev
   md.voigt_fp32 = dex_tuning_voigt_fp32();
   unsigned long long* d_work = dex_line_segment_counter();   // NULL unless march timing is enabled
   if (fuse_j)
-    dex_march_kernel<D, VAR, LPR, true><<<grid, threads, 0, st>>>(g->dev, md, rays, perm, d_out, d_seg, d_work);
+    dex_march_kernel<D, VAR, LPR, true, CLIP><<<grid, threads, 0, st>>>(g->dev, md, rays, perm, d_out, d_seg, d_work);
   else
-    dex_march_kernel<D, VAR, LPR, false><<<grid, threads, 0, st>>>(g->dev, md, rays, perm, d_out, d_seg, d_work);
+    dex_march_kernel<D, VAR, LPR, false, CLIP><<<grid, threads, 0, st>>>(g->dev, md, rays, perm, d_out, d_seg, d_work);
   dex_count_launch();
   DEX_CUDA_CHECK(cudaGetLastError());
   return DEX_OK;
@@ -710,6 +723,9 @@ dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev
 template <int D, int VAR>
 dex_status launch_march_v(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
                           unsigned long long* d_seg, int lpr, const int* perm, cudaStream_t st) {
+  // finite radiance intervals (T10) are compiled for the production mapping only (lanes per ray is a performance knob:
+  // results do not depend on it)
+  if (rays.t_end > 0.0f) return launch_march_t<D, VAR, 1, true>(g, m, rays, d_out, fuse_j, d_seg, perm, st);
   switch (lpr) {
     case 8: return launch_march_t<D, VAR, 8>(g, m, rays, d_out, fuse_j, d_seg, perm, st);
     case 4: return launch_march_t<D, VAR, 4>(g, m, rays, d_out, fuse_j, d_seg, perm, st);

@@ -65,7 +65,8 @@ def build_mips(dw: DeviceWorkload, grid: B.Grid, stream=None, **override) -> B.M
 
 def rays(dw: DeviceWorkload) -> B.Rays:
     t = dw.t
-    return B.Rays(t["probe_pos"], t["dirs"], t.get("weights"), t.get("i0"), t.get("sin_incl"))
+    return B.Rays(t["probe_pos"], t["dirs"], t.get("weights"), t.get("i0"), t.get("sin_incl"),
+                  getattr(dw.wl, "interval", None))
 
 
 def mean_intensity(dw: DeviceWorkload, grid: B.Grid, mips: B.Mips, J: Optional[torch.Tensor] = None,
@@ -97,7 +98,8 @@ def solve_J_from_host(wl, device="cuda:0", pinned: Optional[dict] = None, J_host
     src = pinned if pinned is not None else {n: torch.from_numpy(np.ascontiguousarray(getattr(wl, n)))
                                              for n in _SPEC_FIELDS + _RAY_FIELDS + ("active",)
                                              if getattr(wl, n, None) is not None}
-    r = B.Rays(src["probe_pos"], src["dirs"], src.get("weights"), src.get("i0"), src.get("sin_incl"))
+    r = B.Rays(src["probe_pos"], src["dirs"], src.get("weights"), src.get("i0"), src.get("sin_incl"),
+               getattr(wl, "interval", None))
     if J_host is None:
         J_host = torch.empty((r.n_probes, wl.n_lambda), dtype=torch.float32)
         if torch.cuda.is_available():

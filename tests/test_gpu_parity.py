@@ -495,3 +495,31 @@ def test_25d_rays_parity(P, name, kw):
     d3, g3, m3 = _build(P, w3)
     with pytest.raises(P.DexError):
         P.pipeline.mean_intensity(d3, g3, m3)
+
+
+# ------------------------------------------------------------------------------------------ T10: radiance intervals
+@pytest.mark.parametrize("name,kw,thr", [("C2", dict(n=256, n_dirs=12, n_probes=700), 0.05),
+                                         ("C5", dict(n=64, n_dirs=8, n_probes=300), 5.0)])
+def test_radiance_interval_parity(P, name, kw, thr):
+    """dex_rays.t_begin / t_end (Algorithm 1's HDDA(t1, t2)) against the oracle: clipped visit lists and path lengths
+    bit-exact, I and J within 1e-5, with a boundary intensity entering at t_end and together with the near-field cap."""
+    wl = make(name, **kw)
+    wl.thr_eta = wl.thr_chi = thr
+    wl.i0 = np.random.default_rng(9).uniform(0, 1, size=(wl.dirs.shape[0], wl.n_lambda)).astype(np.float32)
+    M = orc.build_mips(wl)
+    dw, grid, mips = _build(P, wl)
+    for interval, caps in (((0.0, 7.5), None), ((6.0, 24.0), None), ((24.0, 96.0), [6.0, 24.0]), ((3.0, 1.0e9), None)):
+        wl.interval = interval
+        mips.set_level_caps(caps)
+        ref = orc.hdda_march(wl, M, capture_batch=0, level_cap_t=caps)
+        _, cap = P.pipeline.formal_solution(dw, grid, mips, capture_batch=0, want_I=False)
+        _check_lists(cap, ref, cap.room)
+        seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+        I, _ = P.pipeline.formal_solution(dw, grid, mips, segment_count=seg)
+        assert int(seg.item()) == ref.segments
+        assert max_rel(I.cpu().numpy(), ref.I) <= TOL
+        J = P.pipeline.mean_intensity(dw, grid, mips)
+        assert max_rel(J.cpu().numpy(), orc.mean_intensity(ref.I, wl.weights)) <= TOL
+    wl.interval = (5.0, 2.0)
+    with pytest.raises(P.DexError):
+        P.pipeline.mean_intensity(dw, grid, mips)

@@ -680,3 +680,61 @@ def test_25d_quadrature_and_inclined_rays():
     r = orc.plain_march(wt, sin_incl=si)
     J = orc.mean_intensity(r.I, wt.weights)
     assert abs(J[0, 0] - 0.8) < 1e-6
+
+
+# ------------------------------------------------------------------------------------------------
+# T10: finite radiance intervals (Algorithm 1 HDDA(t1, t2))
+# ------------------------------------------------------------------------------------------------
+def test_t10_radiance_intervals_compose():
+    """(i) an interval that covers the ray changes nothing; (ii) the formal solution composes over a split of the
+    ray: I(0, inf) = I(0, t) + T(0, t) I(t, inf), with T(0, t) = e^-tau obtained from the same march with eta = 0 and
+    unit incoming intensity (eq. 3); (iii) the visit list of an interval is a contiguous run of the full list with
+    only its first and last path lengths shortened; (iv) homogeneous medium closed form on [t1, t2]."""
+    wl = make("C2", n=128, n_dirs=8, n_probes=120)
+    wl.thr_eta = wl.thr_chi = 0.05
+    M = orc.build_mips(wl)
+    full = orc.hdda_march(wl, M, capture_batch=0)
+    same = orc.hdda_march(wl, M, capture_batch=0, interval=(0.0, 1.0e9))
+    assert np.array_equal(full.I, same.I) and np.array_equal(full.records, same.records)
+    assert np.array_equal(full.ds.view(np.uint32), same.ds.view(np.uint32))
+    for tsplit in (3.25, 17.3, 61.0):
+        a = orc.hdda_march(wl, M, capture_batch=0, interval=(0.0, tsplit))
+        b = orc.hdda_march(wl, M, capture_batch=0, interval=(tsplit, 1.0e9))
+        import copy
+        w0 = copy.copy(wl)
+        w0.eta = np.zeros_like(wl.eta)
+        M0 = copy.copy(M)
+        M0.wl = w0
+        M0.eta = [np.zeros_like(e) for e in M.eta]
+        one = np.ones((wl.dirs.shape[0], wl.n_lambda), dtype=np.float32)
+        Ta = orc.hdda_march(w0, M0, i0=one, interval=(0.0, tsplit)).I
+        assert (Ta <= 1.0).all() and (Ta > 0.0).all()
+        assert max_rel(a.I + Ta * b.I, full.I) < 1e-12
+        # (iii)
+        for ray in range(full.counts.shape[0]):
+            nf, na, nb = int(full.counts[ray]), int(a.counts[ray]), int(b.counts[ray])
+            assert nf - 0 <= na + nb <= nf + 1                    # the cell that contains tsplit appears in both
+            assert np.array_equal(a.records[ray, :na], full.records[ray, :na])
+            assert np.array_equal(b.records[ray, :nb], full.records[ray, nf - nb:nf])
+            if na > 1:
+                assert np.array_equal(a.ds[ray, :na - 1], full.ds[ray, :na - 1])
+            if nb > 1:
+                assert np.array_equal(b.ds[ray, 1:nb], full.ds[ray, nf - nb + 1:nf])
+            tot = float(a.ds[ray, :na].astype(np.float64).sum() + b.ds[ray, :nb].astype(np.float64).sum())
+            assert abs(tot - float(full.ds[ray, :nf].astype(np.float64).sum())) < 2e-4
+    # (iv)
+    f = np.full((40, 40, 8), 0.11)
+    rng = np.random.default_rng(2)
+    probes = rng.uniform(0, 40, size=(15, 2))
+    wh = iso_workload((40, 40), 8, f * 2.5, f, probes, dirs_2d(7)[0], max_level=2, thr=1.0, h=0.8)
+    Mh = orc.build_mips(wh)
+    t1, t2 = 2.5, 19.0
+    r = orc.hdda_march(wh, Mh, interval=(t1, t2))
+    chi32 = float(np.float32(0.11))
+    S32 = float(np.float32(0.11 * 2.5)) / chi32
+    for p in range(probes.shape[0]):
+        for k in range(7):
+            L = path_to_boundary(wh.probe_pos[p], wh.dirs[k], (40, 40))
+            seg = max(0.0, min(L, t2) - t1)
+            want = S32 * (1.0 - math.exp(-chi32 * 0.8 * seg))
+            assert abs(r.I[p, k, 0] - want) < 2e-5 * max(want, 1e-3)

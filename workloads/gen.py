@@ -54,6 +54,7 @@ class Workload:
     weights: np.ndarray = None     # [n_dirs] fp32
     i0: Optional[np.ndarray] = None  # [n_dirs][n_lambda] fp32 or None (= 0)
     sin_incl: Optional[np.ndarray] = None  # [n_dirs] fp32 or None: 2.5D rays, sine of the inclination to the homogeneous axis
+    interval: Optional[tuple] = None       # (t_begin, t_end) voxels from the probe: finite radiance interval, None = to the boundary
     # isotropic fields
     eta: Optional[np.ndarray] = None
     chi: Optional[np.ndarray] = None
