@@ -57,6 +57,9 @@ def parse():
     ap.add_argument("--lanes", type=int, default=None, help="lanes per ray (1/2/4/8)")
     ap.add_argument("--tile", type=int, default=None, help="tile_probes tuning knob (0/1)")
     ap.add_argument("--cpu-probes", type=int, default=None, help="probes in the oracle (cpu_baseline) sample")
+    ap.add_argument("--pipeline", type=int, default=0,
+                    help="time the per-iteration rebuild pipeline (dex_mean_intensity_pipelined) with this many "
+                         "wavelength batches per stage instead of the whole-spectrum build + march")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -253,8 +256,15 @@ def main():
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()
 
+    class _NoMips:
+        def destroy(self):
+            pass
+
     def step():
         grid = P.pipeline.build_grid(dw)
+        if args.pipeline > 0:              # stage s+1's mips are built while stage s is marched
+            P.pipeline.mean_intensity_pipelined(dw, grid, args.pipeline, J=J, segment_count=seg)
+            return grid, _NoMips()
         mips = P.pipeline.build_mips(dw, grid)
         P.pipeline.mean_intensity(dw, grid, mips, J=J, segment_count=seg)
         return grid, mips
@@ -271,6 +281,7 @@ def main():
         m.destroy(); g.destroy()
 
     clocks = ClockSampler(local)
+    P.dex_pool_high_water(reset=True)
     P.dex_march_timing_read(reset=True)
     P.dex_march_timing_enable(True)
     seg.zero_()
@@ -291,6 +302,7 @@ def main():
     t_wall = time.perf_counter() - t_wall0
     clk = clocks.stop()
     launches = P.dex_launch_count() - launches0
+    pool_high = P.dex_pool_high_water()
     P.dex_march_timing_enable(False)
     march_ms, march_n = P.dex_march_timing_read(reset=True)
     line_segs = P.dex_march_work_read(reset=True)
@@ -366,7 +378,10 @@ def main():
             "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": config_dict(wl, args, {"lanes_per_ray": args.lanes or 1,
-                                             "segments_per_step": segs_total // max(1, args.steps)}),
+                                             "segments_per_step": segs_total // max(1, args.steps),
+                                             "path": (f"rebuild pipeline, {args.pipeline} batch(es) per stage"
+                                                      if args.pipeline > 0 else "whole-spectrum build + march"),
+                                             "library_device_bytes_high_water": int(pool_high)}),
             "clocks": clk,
             "e2e": e2e,
             "gpu_launches": int(launches),

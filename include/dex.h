@@ -114,6 +114,10 @@ typedef struct {
   const int8_t* h_active_lines; /* [n_batch][DEX_MAX_LINES] line ids, -1 padded (HOST) */
   int n_vbins;   /* DEX_VELINTERP: velocity bins per cell, 2..32 */
   float c_light; /* speed of light in the unit of d_vel */
+  int lambda_stride; /* floats between consecutive voxels in d_eta, d_chi, d_eta_bg, d_chi_bg; 0 = n_lambda (dense).
+                      * A larger stride lets a handle be built for a window of a wider spectrum (the stages of
+                      * dex_mean_intensity_pipelined): pass the arrays offset to the window's first wavelength.
+                      * Must be 0 or >= n_lambda (DEX_ERR_SHAPE). */
 } dex_mips_desc;
 
 /* a2-a4. Gather active bricks into brick-major storage, build the box-filter mips of every
@@ -210,6 +214,23 @@ dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const 
                               const float* d_I /*NULL = fused*/, float* d_J, int64_t* d_segment_count,
                               void* stream);
 
+/* Per-iteration rebuild pipeline.  In the paper every iteration recomputes the MIP chains "from
+ * scratch from MIP 0" and configures the refinement "at each wavelength batch": the pyramid of a
+ * batch lives only as long as that batch's formal solution.  This entry does the same for a whole spectrum: the
+ * n_lambda / lambda_batch batches of `desc` are taken in stages of `batches_per_stage` consecutive batches; stage s+1's
+ * pyramid and level table (a2-a4) are built on an internal high-priority stream while stage s's fused march (a5-a9)
+ * runs on `stream`, and a stage's pyramid is released as soon as its march has finished, so at most two stages' mips
+ * are resident (instead of the whole spectrum's).  The probe tiling is computed once.  Results are those of
+ * dex_build_vlm_mips + dex_mean_intensity on the whole spectrum, bit for bit (batches are independent: each has its
+ * own level table).  d_J: [n_probes][n_lambda]; *d_segment_count (may be NULL) is incremented by the
+ * emitted segments of all stages; n_caps / h_cap_t: near-field cap as in dex_mips_set_level_caps (0 / NULL: none);
+ * h_levels (may be NULL): receives the level table [n_batch][n_bricks] (the call then synchronises).  The caller's
+ * input arrays must stay valid until `stream` has drained.  Errors: as the calls it chains; DEX_ERR_INVALID_ARG for
+ * batches_per_stage < 1. */
+dex_status dex_mean_intensity_pipelined(const dex_grid* grid, const dex_mips_desc* desc, const dex_rays* rays,
+                                        int batches_per_stage, int n_caps, const float* h_cap_t, float* d_J,
+                                        int64_t* d_segment_count, int8_t* h_levels, void* stream);
+
 /* Validation: the Voigt function H(a_i, x_i) = Re w(x_i + i a_i) of PAPER.md:329 ("HUM1WEI24") exactly as the
  * Core-and-Voigt march evaluates it, for n (damping, frequency offset) pairs in device memory.  mode 0: as the
  * march chooses (fp32 table form inside its damping window, the fp64 Weideman / Humlicek form outside it, see
@@ -230,6 +251,10 @@ dex_status dex_mean_intensity_host(const dex_grid_desc* desc, const uint8_t* h_a
 
 /* Number of kernel launches this library has enqueued since load (bench.py's gpu_launches). */
 int64_t dex_launch_count(void);
+/* High-water mark (bytes) of the device memory this library's handles and temporaries have held at once since the last
+ * reset (all of it comes from the device's default stream-ordered pool; a caller that uses that pool too is counted
+ * with it).  Synchronises.  bench.py reports it to show what the rebuild pipeline keeps resident. */
+dex_status dex_pool_high_water(int64_t* bytes_in_use_high, int reset);
 /* Device time (ms) and launch count of the march kernels since the last reset, measured with CUDA
  * events on the launching stream when timing is enabled (bench.py roofline leg).  Synchronises. */
 void dex_march_timing_enable(int on);

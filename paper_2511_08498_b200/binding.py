@@ -28,7 +28,7 @@ EXPORTS = (
     "dex_last_error", "dex_version", "dex_build_sparse_grid", "dex_grid_info", "dex_grid_get_slots",
     "dex_destroy_grid", "dex_build_vlm_mips", "dex_mips_get_levels", "dex_mips_set_levels", "dex_mips_set_level_caps", "dex_mips_velocity_bin_report",
     "dex_mips_get_packed_levels", "dex_mips_get_level_data", "dex_destroy_mips", "dex_formal_solution",
-    "dex_mean_intensity", "dex_mean_intensity_host", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read", "dex_march_work_read",
+    "dex_mean_intensity", "dex_mean_intensity_host", "dex_mean_intensity_pipelined", "dex_pool_high_water", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read", "dex_march_work_read",
     "dex_set_lanes_per_ray", "dex_set_tuning",
 )
 
@@ -51,6 +51,7 @@ class _MipsDesc(C.Structure):
         ("d_chi_bg", C.c_void_p), ("d_vel", C.c_void_p), ("n_lines", C.c_int), ("h_lambda0", C.c_void_p),
         ("d_eta_star0", C.c_void_p), ("d_chi_star0", C.c_void_p), ("d_a0", C.c_void_p), ("d_inv_dlamD", C.c_void_p),
         ("h_active_lines", C.c_void_p), ("n_vbins", C.c_int), ("c_light", C.c_float),
+        ("lambda_stride", C.c_int),
     ]
 
 
@@ -94,6 +95,9 @@ def _load():
     L.dex_mean_intensity_host.argtypes = [C.POINTER(_GridDesc), C.c_void_p, C.POINTER(_MipsDesc), C.POINTER(_Rays),
                                           C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64),
                                           C.c_void_p]
+    L.dex_mean_intensity_pipelined.argtypes = [C.c_void_p, C.POINTER(_MipsDesc), C.POINTER(_Rays), C.c_int, C.c_int,
+                                               C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.dex_pool_high_water.argtypes = [C.POINTER(C.c_int64), C.c_int]
     L.dex_voigt_profile.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_int, C.c_void_p]
     L.dex_march_timing_enable.argtypes = [C.c_int]
     L.dex_march_timing_enable.restype = None
@@ -388,6 +392,36 @@ def dex_mean_intensity_host(ndim, dims, brick, voxel_size, active: Optional[torc
                                       C.byref(seg), C.byref(h2d), C.byref(d2h), _stream(stream)))
     del keep
     return seg.value, h2d.value, d2h.value
+
+
+def dex_mean_intensity_pipelined(grid: Grid, mips_args: dict, rays: Rays, J: torch.Tensor, batches_per_stage: int = 1,
+                                 level_caps=None, segment_count: Optional[torch.Tensor] = None, want_levels=False,
+                                 stream=None):
+    """include/dex.h dex_mean_intensity_pipelined: per-stage rebuild of the mips overlapped with the previous stage's
+    march.  `mips_args` holds dex_build_vlm_mips' keyword arguments (device tensors).  Returns the level table
+    [n_batch][n_bricks] when `want_levels`, else None."""
+    a = dict(eta=None, chi=None, lam=None, eta_bg=None, chi_bg=None, vel=None, lambda0=None, eta_star0=None,
+             chi_star0=None, a0=None, inv_dlamD=None, active_lines=None, n_vbins=0, c_light=299792.458)
+    a.update(mips_args)
+    d, _, keep = _mips_desc(**a)
+    r = rays.struct()
+    t = np.ascontiguousarray([] if level_caps is None else level_caps, dtype=np.float32)
+    lv = None
+    if want_levels:
+        nb, _ = grid.info()
+        lv = np.empty((int(a["n_lambda"]) // int(a["lambda_batch"]), nb), dtype=np.int8)
+    _check(_L.dex_mean_intensity_pipelined(grid.handle, C.byref(d), C.byref(r), int(batches_per_stage), int(t.size),
+                                           t.ctypes.data if t.size else None, _ptr(J, torch.float32),
+                                           _ptr(segment_count, torch.int64), lv.ctypes.data if lv is not None else None,
+                                           _stream(stream)))
+    del keep
+    return lv
+
+
+def dex_pool_high_water(reset=False) -> int:
+    v = C.c_int64(0)
+    _check(_L.dex_pool_high_water(C.byref(v), int(bool(reset))))
+    return v.value
 
 
 def dex_voigt_profile(a: torch.Tensor, x: torch.Tensor, mode: int = 0, stream=None) -> torch.Tensor:

@@ -189,6 +189,23 @@ const char* dex_last_error(void) { return g_last_error.c_str(); }
 const char* dex_version(void) { return "dex-b200 0.1 (sm_100a)"; }
 int64_t dex_launch_count(void) { return (int64_t)g_launches.load(); }
 
+dex_status dex_pool_high_water(int64_t* bytes_in_use_high, int reset) {
+  if (!have_device()) return DEX_ERR_CUDA;
+  int dev = 0;
+  DEX_CUDA_CHECK(cudaGetDevice(&dev));
+  cudaMemPool_t pool;
+  DEX_CUDA_CHECK(cudaDeviceGetDefaultMemPool(&pool, dev));
+  DEX_CUDA_CHECK(cudaDeviceSynchronize());
+  unsigned long long v = 0;
+  DEX_CUDA_CHECK(cudaMemPoolGetAttribute(pool, cudaMemPoolAttrUsedMemHigh, &v));
+  if (bytes_in_use_high) *bytes_in_use_high = (int64_t)v;
+  if (reset) {
+    v = 0;
+    DEX_CUDA_CHECK(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrUsedMemHigh, &v));
+  }
+  return DEX_OK;
+}
+
 dex_status dex_set_lanes_per_ray(int lanes) {
   if (lanes != 1 && lanes != 2 && lanes != 4 && lanes != 8) {
     dex_set_error("lanes per ray must be 1, 2, 4 or 8");
@@ -330,6 +347,10 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
     dex_set_error("n_lambda must be a positive multiple of lambda_batch");
     return DEX_ERR_SHAPE;
   }
+  if (desc->lambda_stride != 0 && desc->lambda_stride < desc->n_lambda) {
+    dex_set_error("lambda_stride must be 0 (dense) or >= n_lambda");
+    return DEX_ERR_SHAPE;
+  }
   int max_level = desc->max_level;
   if (max_level < 0 || max_level > grid->dev.logB || max_level >= DEX_MAXLEV) {
     dex_set_error("max_level must be in 0..log2(brick)");
@@ -378,6 +399,9 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
   d.n_lambda = desc->n_lambda;
   d.n_batch = n_batch;
   d.max_level = max_level;
+  d.in_stride = desc->lambda_stride ? desc->lambda_stride : desc->n_lambda;
+  d.io_stride = desc->n_lambda;
+  d.io_base = 0;
   int bits = 1;
   while ((1 << bits) < max_level + 2) ++bits;      // ceil(log2(max_level + 2))
   d.bits = bits;
@@ -624,6 +648,134 @@ dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const 
   if (d_I) return dex_launch_reduce_j(R, mips->n_lambda, d_I, d_J, st);
   MarchTimer tm(st);
   return dex_launch_march(grid, mips, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), g_tile_probes.load() != 0, st);
+}
+
+// ------------------------------------------------------------------------------------------- rebuild pipeline
+dex_status dex_mean_intensity_pipelined(const dex_grid* grid, const dex_mips_desc* desc, const dex_rays* rays,
+                                        int batches_per_stage, int n_caps, const float* h_cap_t, float* d_J,
+                                        int64_t* d_segment_count, int8_t* h_levels, void* stream) {
+  if (!grid || !desc || !rays) { dex_set_error("NULL grid / desc / rays"); return DEX_ERR_INVALID_ARG; }
+  if (batches_per_stage < 1) { dex_set_error("batches_per_stage must be >= 1"); return DEX_ERR_INVALID_ARG; }
+  if (desc->lambda_batch != DEX_W) { dex_set_error("lambda_batch must be 8 in this build"); return DEX_ERR_UNSUPPORTED; }
+  if (desc->n_lambda <= 0 || desc->n_lambda % DEX_W) {
+    dex_set_error("n_lambda must be a positive multiple of lambda_batch");
+    return DEX_ERR_SHAPE;
+  }
+  if (desc->lambda_stride != 0 && desc->lambda_stride < desc->n_lambda) {
+    dex_set_error("lambda_stride must be 0 (dense) or >= n_lambda");
+    return DEX_ERR_SHAPE;
+  }
+  if (rays->n_probes > 0 && !d_J) { dex_set_error("d_J is NULL"); return DEX_ERR_INVALID_ARG; }
+  if (rays->n_probes > 0 && rays->n_dirs > 0 && !rays->d_weights) { dex_set_error("d_weights is NULL"); return DEX_ERR_INVALID_ARG; }
+  if (!have_device()) return DEX_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int n_batch = desc->n_lambda / DEX_W;
+  const int n_stage = (n_batch + batches_per_stage - 1) / batches_per_stage;
+  const int stride = desc->lambda_stride ? desc->lambda_stride : desc->n_lambda;
+  const bool aniso = desc->variant != DEX_ISO;
+
+  // Streams: builds on `sb`, which outranks the marches so that its small kernels take the first SM slots that fall
+  // free; marches alternate between two streams so that stage s+1's blocks fill the SMs that stage s's last wave
+  // leaves idle (a stage of one batch is only ~1.7 waves of blocks on C2: serialised, the tails cost 20 %).
+  int prio_lo = 0, prio_hi = 0;
+  cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+  cudaStream_t sb = nullptr, sm[2] = {nullptr, nullptr};
+  DEX_CUDA_CHECK(cudaStreamCreateWithPriority(&sb, cudaStreamNonBlocking, prio_hi));
+  for (int i = 0; i < 2; ++i) {
+    cudaError_t ce = cudaStreamCreateWithPriority(&sm[i], cudaStreamNonBlocking, prio_lo);
+    if (ce != cudaSuccess) { cudaStreamDestroy(sb); if (i) cudaStreamDestroy(sm[0]); DEX_CUDA_CHECK(ce); }
+  }
+  cudaEvent_t ev_in = nullptr, ev_built[2] = {nullptr, nullptr}, ev_marched[2] = {nullptr, nullptr};
+  cudaEventCreateWithFlags(&ev_in, cudaEventDisableTiming);
+  for (int i = 0; i < 2; ++i) {
+    cudaEventCreateWithFlags(&ev_built[i], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&ev_marched[i], cudaEventDisableTiming);
+  }
+
+  dex_status s = DEX_OK;
+  cudaError_t e = cudaSuccess;
+  int* d_perm = nullptr;
+  if (rays->n_probes > 0 && g_tile_probes.load() != 0) {   // the probe tiling is the same for every stage
+    DexRaysDev R;
+    R.n_probes = rays->n_probes;
+    R.probe_pos = rays->d_probe_pos;
+    if (!rays->d_probe_pos) { dex_set_error("d_probe_pos is NULL"); s = DEX_ERR_INVALID_ARG; }
+    else s = dex_make_probe_tiling(grid, R, &d_perm, st);
+  }
+  cudaEventRecord(ev_in, st);            // the caller's inputs (and the tiling) are ordered on `stream`
+  cudaStreamWaitEvent(sb, ev_in, 0);
+  cudaStreamWaitEvent(sm[0], ev_in, 0);
+  cudaStreamWaitEvent(sm[1], ev_in, 0);
+
+  dex_mips* prev = nullptr;              // stage s-1, released on the build stream once its march has finished
+  int prev_ev = 0;
+  for (int sg = 0; sg < n_stage && s == DEX_OK && e == cudaSuccess; ++sg) {
+    const int b0 = sg * batches_per_stage;
+    const int nb = (b0 + batches_per_stage <= n_batch) ? batches_per_stage : n_batch - b0;
+    const size_t off = (size_t)b0 * DEX_W;
+    dex_mips_desc sub = *desc;
+    sub.n_lambda = nb * DEX_W;
+    sub.lambda_stride = stride;
+    if (desc->d_lambda) sub.d_lambda = desc->d_lambda + off;
+    if (desc->d_eta) sub.d_eta = desc->d_eta + off;
+    if (desc->d_chi) sub.d_chi = desc->d_chi + off;
+    if (desc->d_eta_bg) sub.d_eta_bg = desc->d_eta_bg + off;
+    if (desc->d_chi_bg) sub.d_chi_bg = desc->d_chi_bg + off;
+    if (aniso && desc->h_active_lines) sub.h_active_lines = desc->h_active_lines + (size_t)b0 * DEX_MAX_LINES;
+    dex_mips* cur = nullptr;
+    s = dex_build_vlm_mips(grid, &sub, (void*)sb, &cur);
+    if (s != DEX_OK) break;
+    cur->dev.io_stride = desc->n_lambda;
+    cur->dev.io_base = (int)off;
+    s = dex_mips_set_level_caps(cur, n_caps, h_cap_t);
+    if (s == DEX_OK && h_levels)
+      e = cudaMemcpyAsync(h_levels + (size_t)b0 * grid->n_bricks, cur->d_levels, (size_t)nb * grid->n_bricks,
+                          cudaMemcpyDeviceToHost, sb);
+    cudaEventRecord(ev_built[sg & 1], sb);
+    if (prev) {   // enqueued AFTER this stage's build: stage s-1 is released when its march is done, and the build of
+                  // stage s+1 queues behind that, so at most two stages' pyramids are resident
+      cudaStreamWaitEvent(sb, ev_marched[prev_ev], 0);
+      dex_destroy_mips(prev);
+      prev = nullptr;
+    }
+    cudaStream_t ms = sm[sg & 1];
+    if (s == DEX_OK && e == cudaSuccess && rays->n_probes > 0) {
+      DexRaysDev R;
+      s = check_rays(grid, cur, rays, &R);
+      if (s == DEX_OK) {
+        cudaStreamWaitEvent(ms, ev_built[sg & 1], 0);
+        MarchTimer tm(ms);
+        s = dex_launch_march(grid, cur, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(),
+                             false, ms, d_perm);
+      }
+    }
+    cudaEventRecord(ev_marched[sg & 1], ms);
+    prev = cur;
+    prev_ev = sg & 1;
+  }
+  if (prev) {
+    cudaStreamWaitEvent(sb, ev_marched[prev_ev], 0);
+    dex_destroy_mips(prev);
+  }
+  // join: `stream` waits for both march streams and for the build stream's tail (level copies, releases), so draining
+  // `stream` drains the call
+  for (int i = 0; i < 2; ++i) {
+    cudaEventRecord(ev_built[i], sm[i]);
+    cudaStreamWaitEvent(st, ev_built[i], 0);
+  }
+  cudaEventRecord(ev_in, sb);
+  cudaStreamWaitEvent(st, ev_in, 0);
+  if (d_perm) cudaFreeAsync(d_perm, st);
+  if (h_levels && e == cudaSuccess) e = cudaStreamSynchronize(sb);
+  cudaEventDestroy(ev_in);
+  for (int i = 0; i < 2; ++i) { cudaEventDestroy(ev_built[i]); cudaEventDestroy(ev_marched[i]); }
+  cudaStreamDestroy(sb);                 // deferred by the runtime until the streams' work has completed
+  cudaStreamDestroy(sm[0]);
+  cudaStreamDestroy(sm[1]);
+  if (s != DEX_OK) return s;
+  DEX_CUDA_CHECK(e);
+  DEX_CUDA_CHECK(cudaGetLastError());
+  return DEX_OK;
 }
 
 dex_status dex_voigt_profile(const float* d_a, const double* d_x, int64_t n, double* d_H, int mode, void* stream) {

@@ -57,6 +57,9 @@ struct DexMipsDev {
   int n_caps;                        // near-field MIP cap (T8, dex_mips_set_level_caps): a cell entered at distance t is
   float cap_t[8];                    // formed at level min(brick level, #{i : t >= cap_t[i]}); n_caps = 0: no cap
   int voigt_fp32;                    // 0: fp64 HUM1WEI24 everywhere (tuning knob "voigt_fp32")
+  int in_stride;                     // floats between consecutive voxels of the caller's [nvox][lambda] inputs (build)
+  int io_stride, io_base;            // row length and first column of this handle's wavelengths in I / J / i0: n_lambda and
+                                     // 0 unless the handle is one stage of dex_mean_intensity_pipelined
 };
 
 struct DexRaysDev {

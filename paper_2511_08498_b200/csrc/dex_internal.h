@@ -58,7 +58,11 @@ dex_status dex_launch_vbin_report(const dex_mips* m, float factor, unsigned* d_m
 dex_status dex_launch_level_data(const dex_mips* m, int chain, int level, float* d_dense, cudaStream_t st);
 // march.cu
 dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                            unsigned long long* d_seg, int lanes_per_ray, bool tile, cudaStream_t st);
+                            unsigned long long* d_seg, int lanes_per_ray, bool tile, cudaStream_t st,
+                            const int* perm_in = nullptr);
+// perm[i] = probe handled by lane group i (compact spatial tiles); *d_perm stays NULL when tiling does not apply.
+// Stream-ordered allocation: release with cudaFreeAsync on `st`.
+dex_status dex_make_probe_tiling(const dex_grid* g, const DexRaysDev& rays, int** d_perm, cudaStream_t st);
 dex_status dex_launch_capture(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays,
                               const dex_visit_capture* cap, int* d_overflow, cudaStream_t st);
 dex_status dex_launch_voigt_profile(const float* d_a, const double* d_x, long long n, double* d_H, int mode, cudaStream_t st);

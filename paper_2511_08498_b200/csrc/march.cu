@@ -515,21 +515,21 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
       for (int i = 0; i < LPT; ++i) I[i] += DEX_IH(i);
       if (R.i0 != nullptr) {
 #pragma unroll
-        for (int i = 0; i < LPT; ++i) I[i] = fmaf(T[i], __ldg(R.i0 + (size_t)k * M.n_lambda + lam_off + i), I[i]);
+        for (int i = 0; i < LPT; ++i) I[i] = fmaf(T[i], __ldg(R.i0 + (size_t)k * M.io_stride + M.io_base + lam_off + i), I[i]);
       }
       if (FUSE_J) {
         const float wk = __ldg(R.weights + k);
 #pragma unroll
         for (int i = 0; i < LPT; ++i) Jsm[i * DEX_MARCH_THREADS + threadIdx.x] = fmaf(wk, I[i], Jsm[i * DEX_MARCH_THREADS + threadIdx.x]);
       } else {
-        float* dst = out + ((size_t)gid * R.n_dirs + k) * M.n_lambda + lam_off;
+        float* dst = out + ((size_t)gid * R.n_dirs + k) * M.io_stride + M.io_base + lam_off;
 #pragma unroll
         for (int i = 0; i < LPT; ++i) dst[i] = I[i];
       }
     }
   }
   if (FUSE_J && valid) {
-    float* dst = out + (size_t)gid * M.n_lambda + lam_off;
+    float* dst = out + (size_t)gid * M.io_stride + M.io_base + lam_off;
 #pragma unroll
     for (int i = 0; i < LPT; ++i) dst[i] = Jsm[i * DEX_MARCH_THREADS + threadIdx.x];
   }
@@ -792,14 +792,20 @@ static dex_status tile_probes_t(const dex_grid* g, const DexRaysDev& rays, int**
   return DEX_OK;
 }
 
+dex_status dex_make_probe_tiling(const dex_grid* g, const DexRaysDev& rays, int** d_perm, cudaStream_t st) {
+  return (g->desc.ndim == 2) ? tile_probes_t<2>(g, rays, d_perm, st) : tile_probes_t<3>(g, rays, d_perm, st);
+}
+
 dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
-                            unsigned long long* d_seg, int lanes_per_ray, bool tile, cudaStream_t st) {
+                            unsigned long long* d_seg, int lanes_per_ray, bool tile, cudaStream_t st,
+                            const int* perm_in) {
   int* d_perm = nullptr;
   dex_status s = DEX_OK;
-  if (tile) s = (g->desc.ndim == 2) ? tile_probes_t<2>(g, rays, &d_perm, st) : tile_probes_t<3>(g, rays, &d_perm, st);
+  if (tile && !perm_in) s = dex_make_probe_tiling(g, rays, &d_perm, st);
+  const int* perm = perm_in ? perm_in : d_perm;
   if (s == DEX_OK) {
-    if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, d_perm, st);
-    else s = launch_march_d<3>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, d_perm, st);
+    if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, perm, st);
+    else s = launch_march_d<3>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, perm, st);
   }
   if (d_perm) cudaFreeAsync(d_perm, st);
   return s;

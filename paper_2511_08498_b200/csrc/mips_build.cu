@@ -120,7 +120,7 @@ __global__ void gather_spec_kernel(const BuildCtx X, const float* __restrict__ e
   const int slot = (int)(r % X.G.n_active);
   const int b = (int)(r / X.G.n_active);
   const size_t v = voxel_of<D>(X.G, X.active_bricks[slot], cell);
-  const size_t src = v * X.M.n_lambda + (size_t)b * DEX_W + j;
+  const size_t src = v * (size_t)X.M.in_stride + (size_t)b * DEX_W + j;
   const size_t rec = ((size_t)b * X.G.n_active + slot) * X.M.cps + cell;
   X.store[dex_rec_eta(rec, j)] = eta[src];
   X.store[dex_rec_chi(rec, j)] = chi[src];

@@ -78,6 +78,28 @@ def mean_intensity(dw: DeviceWorkload, grid: B.Grid, mips: B.Mips, J: Optional[t
     return J
 
 
+def _mips_args(wl, t: dict, **override) -> dict:
+    g = lambda k: override.get(k, getattr(wl, k))
+    return dict(variant=g("variant"), n_lambda=wl.n_lambda, lambda_batch=wl.lambda_batch, max_level=g("max_level"),
+                metric=g("metric"), thr_eta=g("thr_eta"), thr_chi=g("thr_chi"), tau_gate=g("tau_gate"), eta=t.get("eta"),
+                chi=t.get("chi"), lam=t.get("lam"), eta_bg=t.get("eta_bg"), chi_bg=t.get("chi_bg"), vel=t.get("vel"),
+                lambda0=wl.lambda0, eta_star0=t.get("eta_star0"), chi_star0=t.get("chi_star0"), a0=t.get("a0"),
+                inv_dlamD=t.get("inv_dlamD"), active_lines=wl.active_lines, n_vbins=g("n_vbins"), c_light=wl.c_light)
+
+
+def mean_intensity_pipelined(dw: DeviceWorkload, grid: B.Grid, batches_per_stage: int = 1, J: Optional[torch.Tensor] = None,
+                             level_caps=None, segment_count: Optional[torch.Tensor] = None, want_levels=False,
+                             stream=None, **override):
+    """Per-iteration rebuild pipeline (include/dex.h dex_mean_intensity_pipelined): mips of stage s+1 are built while
+    stage s is marched; returns (J, level table or None)."""
+    r = rays(dw)
+    if J is None:
+        J = torch.empty((r.n_probes, dw.wl.n_lambda), dtype=torch.float32, device=r.probe_pos.device)
+    lv = B.dex_mean_intensity_pipelined(grid, _mips_args(dw.wl, dw.t, **override), r, J, batches_per_stage, level_caps,
+                                        segment_count, want_levels, stream)
+    return J, lv
+
+
 def formal_solution(dw: DeviceWorkload, grid: B.Grid, mips: B.Mips, capture_batch: Optional[int] = None,
                     segment_count: Optional[torch.Tensor] = None, want_I=True, room: Optional[int] = None, stream=None):
     r = rays(dw)

@@ -523,3 +523,44 @@ def test_radiance_interval_parity(P, name, kw, thr):
     wl.interval = (5.0, 2.0)
     with pytest.raises(P.DexError):
         P.pipeline.mean_intensity(dw, grid, mips)
+
+
+# ------------------------------------------------------------------------------------------ 8(f)-3: rebuild pipeline
+@pytest.mark.parametrize("name,kw,caps", [("C2", dict(n=256, n_dirs=12, n_probes=900), None),
+                                          ("C2", dict(n=128, n_dirs=8, n_probes=300), [6.0, 24.0]),
+                                          ("C3", dict(n=128, n_dirs=8, n_probes=300), None),
+                                          ("C4", dict(n=128, n_dirs=8, n_probes=150), None),
+                                          ("C5", dict(n=64, n_dirs=8, n_probes=300), None)])
+def test_rebuild_pipeline_parity(P, name, kw, caps):
+    """dex_mean_intensity_pipelined (mips of stage s+1 built on a second stream while stage s is marched, two stages
+    resident) against the oracle: level table bit-exact, segment count exact, J within 1e-5; and against the
+    whole-spectrum path of the library, bit for bit, for every stage size including a ragged last stage."""
+    wl = make(name, **kw)
+    wl.i0 = np.random.default_rng(11).uniform(0, 1, size=(wl.dirs.shape[0], wl.n_lambda)).astype(np.float32)
+    M = orc.build_mips(wl)
+    ref = orc.hdda_march(wl, M, level_cap_t=caps)
+    Jref = orc.mean_intensity(ref.I, wl.weights)
+    dw, grid, mips = _build(P, wl)
+    mips.set_level_caps(caps)
+    seg0 = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+    J0 = P.pipeline.mean_intensity(dw, grid, mips, segment_count=seg0)
+    assert int(seg0.item()) == ref.segments
+    for bps in sorted({1, 2, 3, wl.n_batch, wl.n_batch + 5}):
+        seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+        J, lv = P.pipeline.mean_intensity_pipelined(dw, grid, bps, level_caps=caps, segment_count=seg, want_levels=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(lv, M.levels), f"bps={bps}: level tables differ"
+        assert int(seg.item()) == ref.segments
+        assert max_rel(J.cpu().numpy(), Jref) <= TOL
+        assert torch.equal(J, J0), f"bps={bps}: pipelined J differs from the whole-spectrum path"
+    # a new iteration's eta (here: halved) goes through the same call, no handle surviving between the two
+    if name == "C2":
+        dw.t["eta"] = dw.t["eta"] * 0.5
+        wl.eta = (wl.eta * np.float32(0.5)).astype(np.float32)
+        J2, lv2 = P.pipeline.mean_intensity_pipelined(dw, grid, 2, level_caps=caps, want_levels=True)
+        M2 = orc.build_mips(wl)
+        assert np.array_equal(lv2, M2.levels)
+        r2 = orc.hdda_march(wl, M2, level_cap_t=caps)
+        assert max_rel(J2.cpu().numpy(), orc.mean_intensity(r2.I, wl.weights)) <= TOL
+    with pytest.raises(P.DexError):
+        P.pipeline.mean_intensity_pipelined(dw, grid, 0)

@@ -738,3 +738,25 @@ def test_t10_radiance_intervals_compose():
             seg = max(0.0, min(L, t2) - t1)
             want = S32 * (1.0 - math.exp(-chi32 * 0.8 * seg))
             assert abs(r.I[p, k, 0] - want) < 2e-5 * max(want, 1e-3)
+
+
+# ------------------------------------------------------------------------------------------------
+# 8(f)-3: wavelength batches are independent (one level table per batch), which is what lets the
+# rebuild pipeline build and solve the spectrum stage by stage
+# ------------------------------------------------------------------------------------------------
+def test_batches_are_independent_in_the_oracle():
+    import copy
+    wl = make("C2", n=128, n_dirs=6, n_probes=60)
+    M = orc.build_mips(wl)
+    full = orc.hdda_march(wl, M)
+    assert len({M.levels[b].tobytes() for b in range(wl.n_batch)}) > 1      # the batches do differ (core vs wing)
+    for b0, b1 in ((0, 1), (1, 3), (3, 4)):
+        sub = copy.copy(wl)
+        sl = slice(b0 * wl.lambda_batch, b1 * wl.lambda_batch)
+        sub.eta = np.ascontiguousarray(wl.eta[..., sl])
+        sub.chi = np.ascontiguousarray(wl.chi[..., sl])
+        sub.n_lambda = (b1 - b0) * wl.lambda_batch
+        Ms = orc.build_mips(sub)
+        assert np.array_equal(Ms.levels, M.levels[b0:b1])
+        r = orc.hdda_march(sub, Ms)
+        assert np.array_equal(r.I, full.I[..., sl])
