@@ -675,3 +675,77 @@ def brute_force_segments(wl, levels_row, probe, omega, min_len=0.0):
                         out.append((t0, m, cc[0], cc[1], cc[2], t1 - t0))
     out.sort(key=lambda r: r[0])
     return out
+
+
+# --------------------------------------------------------------------------------------
+# Single-direction VLM (T11)
+# --------------------------------------------------------------------------------------
+def direction_fields(wl, omega, sin_incl=None):
+    """Emissivity and opacity of an anisotropic medium as seen along ONE direction omega, at full resolution: the
+    Classic formula (eqs. 10-20: background + sum over the batch's active lines of the Doppler-shifted Voigt profile)
+    with v_proj = v . omega per voxel (times sin_incl for a 2.5D ray, T9), evaluated in fp64 and rounded
+    once to fp32.  These are "a grid of emissivity and opacity given a single direction" to which the plain VLM method
+    applies.  Voxels of unpopulated bricks are 0.  Returns (eta, chi), fp32 [nvox][n_lambda]."""
+    nd, W, nl = wl.ndim, wl.lambda_batch, wl.n_lambda
+    g0 = grid_shape(wl, 0)
+    nL = wl.n_lines
+    es, cs = wl.eta_star0.reshape((nL,) + g0), wl.chi_star0.reshape((nL,) + g0)
+    a0, inv = wl.a0.reshape((nL,) + g0), wl.inv_dlamD.reshape((nL,) + g0)
+    v0 = _to_grid(wl, wl.vel, 0, (nd,))
+    om = np.asarray(omega, dtype=np.float32).astype(np.float64)
+    vproj = np.zeros(g0, dtype=np.float64)
+    for a in range(nd):
+        vproj = vproj + v0[..., a].astype(np.float64) * om[a]
+    if sin_incl is not None:
+        vproj = vproj * float(np.float32(sin_incl))
+    bg_e, bg_c = _to_grid(wl, wl.eta_bg, 0, (nl,)), _to_grid(wl, wl.chi_bg, 0, (nl,))
+    eta = np.zeros(g0 + (nl,), dtype=np.float32)
+    chi = np.zeros(g0 + (nl,), dtype=np.float32)
+    for b in range(wl.n_batch):
+        lines = [int(l) for l in wl.active_lines[b] if l >= 0]
+        idx = np.arange(b * W, (b + 1) * W)
+        ee, cc = _line_sum(wl, idx, lines, es, cs, a0, inv, {l: vproj for l in lines}, bg_e[..., idx], bg_c[..., idx])
+        eta[..., idx] = ee.astype(np.float32)
+        chi[..., idx] = cc.astype(np.float32)
+    # voxels of unpopulated bricks carry nothing (PAPER.md:148)
+    B = wl.brick
+    act_b = brick_active(wl)
+    bd = tuple(s // B for s in g0)
+    vox_act = act_b.reshape(bd)
+    for ax in range(nd):
+        vox_act = np.repeat(vox_act, B, axis=ax)
+    eta[~vox_act] = 0.0
+    chi[~vox_act] = 0.0
+    return eta.reshape(-1, nl), chi.reshape(-1, nl)
+
+
+def single_direction_workload(wl, k):
+    """The static (ISO) workload direction k of an anisotropic workload defines: its direction fields, that one ray
+    direction with its quadrature weight and boundary intensity; thresholds, metric and max_level as wl's."""
+    import copy
+    s = copy.copy(wl)
+    si = getattr(wl, "sin_incl", None)
+    s.eta, s.chi = direction_fields(wl, wl.dirs[k], None if si is None else si[k])
+    s.variant = ISO
+    s.dirs = np.ascontiguousarray(wl.dirs[k:k + 1])
+    s.weights = np.ascontiguousarray(wl.weights[k:k + 1])
+    s.i0 = None if wl.i0 is None else np.ascontiguousarray(wl.i0[k:k + 1])
+    s.sin_incl = None if si is None else np.ascontiguousarray(si[k:k + 1])
+    return s
+
+
+def single_direction_solve(wl, level_cap_t=None, n_threads=0):
+    """for each quadrature direction, VLM on that direction's fields, HDDA march of that direction's
+    rays; J = sum_k w_k I_k.  Returns (J fp64 [n_probes][n_lambda], levels int8
+    [n_dirs][n_batch][n_bricks], emitted segments)."""
+    n_dirs = wl.dirs.shape[0]
+    I = np.zeros((wl.probe_pos.shape[0], n_dirs, wl.n_lambda), dtype=np.float64)
+    levels, segs = [], 0
+    for k in range(n_dirs):
+        s = single_direction_workload(wl, k)
+        M = build_mips(s, variant=ISO)
+        r = hdda_march(s, M, level_cap_t=level_cap_t, n_threads=n_threads)
+        I[:, k, :] = r.I[:, 0, :]
+        levels.append(M.levels)
+        segs += r.segments
+    return mean_intensity(I, wl.weights), np.stack(levels), segs

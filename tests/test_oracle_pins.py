@@ -760,3 +760,69 @@ def test_batches_are_independent_in_the_oracle():
         assert np.array_equal(Ms.levels, M.levels[b0:b1])
         r = orc.hdda_march(sub, Ms)
         assert np.array_equal(r.I, full.I[..., sl])
+
+
+# ------------------------------------------------------------------------------------------------
+# T11: single-direction VLM
+# ------------------------------------------------------------------------------------------------
+def test_t11_direction_fields_and_single_direction_solve():
+    """(i) a direction field value against the textbook formula with scipy's Faddeeva function (not the oracle's
+    HUM1WEI24): eta = eta_bg + (lam0/lam) eta*_0 H(a, x) / (sqrt(pi) dlamD), x from the projected velocity;
+    (ii) v -> -v together with omega -> -omega leaves the fields unchanged, v = 0 makes them direction independent;
+    (iii) with mips off the per-direction static marches reproduce the Classic march (fields rounded to fp32 once);
+    (iv) with mips on, each direction's level table is the ISO table of that direction's fields, differs between
+    directions, and J stays within the VLM error of the exact Classic J."""
+    from scipy.special import wofz
+    wl = make("C4", n=64, n_dirs=6, n_probes=50)
+    nl = wl.n_lambda
+    om = wl.dirs[2]
+    eta, chi = orc.direction_fields(wl, om)
+    act = orc.brick_active(wl)
+    rng = np.random.default_rng(5)
+    vox_ok = np.flatnonzero(wl.active.ravel() != 0)
+    for v in rng.choice(vox_ok, size=40, replace=False):
+        for j in rng.choice(nl, size=6, replace=False):
+            b = j // wl.lambda_batch
+            lam = float(wl.lam[j])
+            vproj = sum(float(wl.vel[v, a]) * float(om[a]) for a in range(wl.ndim))
+            e, c = float(wl.eta_bg[v, j]), float(wl.chi_bg[v, j])
+            for l in [int(q) for q in wl.active_lines[b] if q >= 0]:
+                lam0, inv = float(wl.lambda0[l]), float(wl.inv_dlamD[l][v])
+                x = (lam - lam0 + vproj / wl.c_light * lam0) * inv
+                a = (lam / lam0) ** 2 * float(wl.a0[l][v])
+                phi = wofz(x + 1j * a).real * inv / math.sqrt(math.pi)
+                e += lam0 / lam * float(wl.eta_star0[l][v]) * phi
+                c += lam0 / lam * float(wl.chi_star0[l][v]) * phi
+            # HUM1WEI24's own error is ~1e-11 absolute in H, i.e. up to ~1e-6 relative in the far wings (p13)
+            assert abs(eta[v, j] - e) <= 3e-6 * e and abs(chi[v, j] - c) <= 3e-6 * c
+    # (ii)
+    import copy
+    wm = copy.copy(wl)
+    wm.vel = -wl.vel
+    e2, c2 = orc.direction_fields(wm, -om)
+    assert np.array_equal(e2, eta) and np.array_equal(c2, chi)
+    wz = copy.copy(wl)
+    wz.vel = np.zeros_like(wl.vel)
+    ea, _ = orc.direction_fields(wz, wl.dirs[0])
+    eb, _ = orc.direction_fields(wz, wl.dirs[4])
+    assert np.array_equal(ea, eb)
+    assert not np.array_equal(orc.direction_fields(wl, wl.dirs[0])[0], orc.direction_fields(wl, wl.dirs[4])[0])
+    # (iii)
+    A = orc.plain_march(wl, variant=orc.CLASSIC)
+    JA = orc.mean_intensity(A.I, wl.weights)
+    w0 = copy.copy(wl)
+    w0.max_level = 0
+    J0, lv0, seg0 = orc.single_direction_solve(w0)
+    assert (lv0[:, :, act] == 0).all() and (lv0[:, :, ~act] == -1).all()
+    assert seg0 == orc.hdda_march(wl, orc.build_mips(wl, max_level=0)).segments      # same non-empty visits
+    assert max_rel(J0, JA) < 3e-7
+    # (iv)
+    wv = copy.copy(wl)
+    wv.thr_eta = wv.thr_chi = 0.3
+    J1, lv1, seg1 = orc.single_direction_solve(wv)
+    assert lv1.shape == (wl.dirs.shape[0], wl.n_batch, act.shape[0])
+    assert (lv1 > 0).any() and seg1 < seg0
+    assert any(not np.array_equal(lv1[0], lv1[k]) for k in range(1, lv1.shape[0]))
+    s3 = orc.single_direction_workload(wv, 3)
+    assert np.array_equal(orc.build_mips(s3, variant=orc.ISO).levels, lv1[3])
+    assert np.percentile(np.abs(J1 - JA) / JA, 99) < 0.2
