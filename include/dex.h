@@ -182,6 +182,8 @@ typedef struct {
                             * traversal still starts at the probe, so cells and plane times are those of the full ray
                             * and each visit is clipped to the interval.  t_end <= 0 (a zero-initialised struct): to the
                             * grid boundary.  Requires 0 <= t_begin < t_end otherwise (DEX_ERR_INVALID_ARG). */
+  int accumulate;          /* fused dex_mean_intensity only: d_J += sum_k w_k I_k instead of d_J = ... (0: overwrite).  Lets a
+                            * caller sum solves that use different level structures per direction (single-direction VLM). */
 } dex_rays;
 
 /* a10. Visit-list capture (validation mode).  Ray r = probe * n_dirs + dir.  Records of ray r
@@ -230,6 +232,27 @@ dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const 
 dex_status dex_mean_intensity_pipelined(const dex_grid* grid, const dex_mips_desc* desc, const dex_rays* rays,
                                         int batches_per_stage, int n_caps, const float* h_cap_t, float* d_J,
                                         int64_t* d_segment_count, int8_t* h_levels, void* stream);
+
+/* Single-direction VLM ("the VLM method can be employed to generate the error-limited MIP
+ * structure for a grid of emissivity and opacity given a single direction ... combined with the adaptive grid and ray
+ * acceleration technique"; T11).
+ * dex_direction_fields: eta, chi of the anisotropic medium `desc` describes (the inputs of DEX_CAV / DEX_CLASSIC: backgrounds,
+ * velocity, line arrays, h_active_lines; thresholds and variant ignored) as seen along ONE direction d_omega[ndim] (device):
+ * eqs. 10-20 at full resolution with v_proj = v . omega (times *d_sin_incl if not NULL, a device scalar: 2.5D ray), evaluated
+ * in fp64 (HUM1WEI24) and rounded once.  d_eta, d_chi: dense [nvox][n_lambda] fp32, voxels of empty bricks written as 0;
+ * they are inputs of a DEX_ISO dex_build_vlm_mips.  Asynchronous on `stream` (h_active_lines is copied at the call).
+ * dex_mean_intensity_single_direction: for every quadrature direction k: direction fields, DEX_ISO mips with desc's metric,
+ * thresholds, gate and max_level, fused march of direction k's rays (weight w_k, boundary row i0[k], sin_incl[k], interval),
+ * accumulated into d_J [n_probes][n_lambda] (overwritten, not added to).  *d_segment_count (may be NULL) is incremented by
+ * the emitted segments; h_levels (may be NULL) receives [n_dirs][n_batch][n_bricks] (the call then synchronises).  Holds
+ * two dense [nvox][n_lambda] arrays and one direction's pyramid at a time.
+ * Errors: DEX_ERR_INVALID_ARG (NULL pointers, desc->variant == DEX_ISO: a static medium has no direction dependence),
+ * DEX_ERR_SHAPE, DEX_ERR_OOM, DEX_ERR_CUDA. */
+dex_status dex_direction_fields(const dex_grid* grid, const dex_mips_desc* desc, const float* d_omega,
+                                const float* d_sin_incl, float* d_eta, float* d_chi, void* stream);
+dex_status dex_mean_intensity_single_direction(const dex_grid* grid, const dex_mips_desc* desc, const dex_rays* rays,
+                                               int n_caps, const float* h_cap_t, float* d_J, int64_t* d_segment_count,
+                                               int8_t* h_levels, void* stream);
 
 /* Validation: the Voigt function H(a_i, x_i) = Re w(x_i + i a_i) of PAPER.md:329 ("HUM1WEI24") exactly as the
  * Core-and-Voigt march evaluates it, for n (damping, frequency offset) pairs in device memory.  mode 0: as the

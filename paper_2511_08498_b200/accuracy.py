@@ -44,7 +44,7 @@ PAPER_CAPS = (6.0, 24.0, 96.0, 384.0)   # level <= 0, 1, 2, 3 below these distan
 
 
 def run(workload: str, n=None, n_dirs=None, n_probes=None, metric=None, thr=None, gate=None, max_level=None,
-        caps=None, device="cuda:0") -> dict:
+        caps=None, device="cuda:0", single_direction=False) -> dict:
     import torch
     from . import binding as B
     from . import pipeline
@@ -77,6 +77,23 @@ def run(workload: str, n=None, n_dirs=None, n_probes=None, metric=None, thr=None
         mips.destroy()
         return J.cpu().numpy().astype(np.float64), int(seg.item()), a.elapsed_time(b), lv
 
+    def solve_single_direction():
+        # PAPER.md:396 / DESIGN.md T11: per-direction Classic fields -> ISO VLM -> one-direction march, accumulated
+        seg = torch.zeros(1, dtype=torch.int64, device=device)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        pipeline.mean_intensity_single_direction(dw, grid, level_caps=caps)        # warm the pool
+        a.record(stream)
+        J, lvs = pipeline.mean_intensity_single_direction(dw, grid, level_caps=caps, segment_count=seg, want_levels=True)
+        b.record(stream)
+        torch.cuda.synchronize()
+        return J.cpu().numpy().astype(np.float64), int(seg.item()), a.elapsed_time(b), lvs
+
+    sd = None
+    if single_direction:
+        if wl.variant == B.DEX_ISO:
+            raise SystemExit("--single-direction needs an anisotropic workload (C3, C4, C5)")
+        J_sd, seg_sd, ms_sd, lv_sd = solve_single_direction()
+        sd = (J_sd, seg_sd, ms_sd, lv_sd)
     J_vlm, seg_vlm, ms_vlm, lv = solve(use_caps=True)
     if wl.variant == B.DEX_ISO:
         J_ex, seg_ex, ms_ex, _ = solve(max_level=0)
@@ -89,7 +106,18 @@ def run(workload: str, n=None, n_dirs=None, n_probes=None, metric=None, thr=None
     rel = np.abs(J_vlm[lit] - J_ex[lit]) / J_ex[lit]
     assert (J_vlm[~lit] == 0.0).all()
     hist = np.asarray(level_histogram(lv, wl.max_level))
+    extra = {}
+    if sd is not None:
+        J_sd, seg_sd, ms_sd, lv_sd = sd
+        h_sd = np.asarray(level_histogram(lv_sd.reshape(-1, lv_sd.shape[-1]), wl.max_level))
+        extra["single_direction"] = {
+            "what": "dex_mean_intensity_single_direction: per direction Classic fields -> ISO VLM -> march (PAPER.md:396); "
+                    "ms covers fields + mips builds + marches of all directions",
+            "rel_err_J": percentiles(np.abs(J_sd[lit] - J_ex[lit]) / J_ex[lit]), "segments": seg_sd, "ms_total": ms_sd,
+            "level_histogram_mean_fraction": (h_sd.mean(axis=0) / h_sd[0].sum()).round(4).tolist(),
+        }
     return {
+        **extra,
         "report": "vlm_accuracy_J", "workload": wl.name, "dims": list(wl.dims[:wl.ndim]), "variant": int(wl.variant),
         "metric": "relvar" if wl.metric == 1 else "iod_log", "thr": float(wl.thr_eta), "tau_gate": float(wl.tau_gate),
         "max_level": int(wl.max_level), "level_cap_t": list(caps) if caps else [], "n_probes": int(wl.probe_pos.shape[0]), "n_dirs": int(wl.dirs.shape[0]),
@@ -114,11 +142,14 @@ def main():
     ap.add_argument("--max-level", type=int, default=None)
     ap.add_argument("--caps", default=None,
                     help="near-field MIP cap thresholds: 'paper' (6,24,96,384 voxels) or a comma separated list")
+    ap.add_argument("--single-direction", action="store_true",
+                    help="also solve with per-direction VLM (dex_mean_intensity_single_direction) and report it")
     a = ap.parse_args()
     caps = None
     if a.caps:
         caps = PAPER_CAPS if a.caps == "paper" else tuple(float(v) for v in a.caps.split(","))
-    print(json.dumps(run(a.workload, a.n, a.n_dirs, a.n_probes, a.metric, a.thr, a.gate, a.max_level, caps)))
+    print(json.dumps(run(a.workload, a.n, a.n_dirs, a.n_probes, a.metric, a.thr, a.gate, a.max_level, caps,
+                         single_direction=a.single_direction)))
 
 
 if __name__ == "__main__":

@@ -28,7 +28,8 @@ EXPORTS = (
     "dex_last_error", "dex_version", "dex_build_sparse_grid", "dex_grid_info", "dex_grid_get_slots",
     "dex_destroy_grid", "dex_build_vlm_mips", "dex_mips_get_levels", "dex_mips_set_levels", "dex_mips_set_level_caps", "dex_mips_velocity_bin_report",
     "dex_mips_get_packed_levels", "dex_mips_get_level_data", "dex_destroy_mips", "dex_formal_solution",
-    "dex_mean_intensity", "dex_mean_intensity_host", "dex_mean_intensity_pipelined", "dex_pool_high_water", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read", "dex_march_work_read",
+    "dex_mean_intensity", "dex_mean_intensity_host", "dex_mean_intensity_pipelined", "dex_pool_high_water", "dex_direction_fields",
+    "dex_mean_intensity_single_direction", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read", "dex_march_work_read",
     "dex_set_lanes_per_ray", "dex_set_tuning",
 )
 
@@ -58,7 +59,7 @@ class _MipsDesc(C.Structure):
 class _Rays(C.Structure):
     _fields_ = [("n_probes", C.c_int64), ("d_probe_pos", C.c_void_p), ("n_dirs", C.c_int), ("d_dirs", C.c_void_p),
                 ("d_weights", C.c_void_p), ("d_i0", C.c_void_p), ("d_sin_incl", C.c_void_p),
-                ("t_begin", C.c_float), ("t_end", C.c_float)]
+                ("t_begin", C.c_float), ("t_end", C.c_float), ("accumulate", C.c_int)]
 
 
 class _Capture(C.Structure):
@@ -97,6 +98,10 @@ def _load():
                                           C.c_void_p]
     L.dex_mean_intensity_pipelined.argtypes = [C.c_void_p, C.POINTER(_MipsDesc), C.POINTER(_Rays), C.c_int, C.c_int,
                                                C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.dex_direction_fields.argtypes = [C.c_void_p, C.POINTER(_MipsDesc), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                       C.c_void_p]
+    L.dex_mean_intensity_single_direction.argtypes = [C.c_void_p, C.POINTER(_MipsDesc), C.POINTER(_Rays), C.c_int,
+                                                      C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     L.dex_pool_high_water.argtypes = [C.POINTER(C.c_int64), C.c_int]
     L.dex_voigt_profile.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_int, C.c_void_p]
     L.dex_march_timing_enable.argtypes = [C.c_int]
@@ -414,6 +419,43 @@ def dex_mean_intensity_pipelined(grid: Grid, mips_args: dict, rays: Rays, J: tor
                                            t.ctypes.data if t.size else None, _ptr(J, torch.float32),
                                            _ptr(segment_count, torch.int64), lv.ctypes.data if lv is not None else None,
                                            _stream(stream)))
+    del keep
+    return lv
+
+
+_MIPS_DEFAULTS = dict(eta=None, chi=None, lam=None, eta_bg=None, chi_bg=None, vel=None, lambda0=None, eta_star0=None,
+                      chi_star0=None, a0=None, inv_dlamD=None, active_lines=None, n_vbins=0, c_light=299792.458)
+
+
+def dex_direction_fields(grid: Grid, mips_args: dict, omega: torch.Tensor, eta: torch.Tensor, chi: torch.Tensor,
+                         sin_incl: Optional[torch.Tensor] = None, stream=None):
+    """include/dex.h dex_direction_fields: Classic eta, chi along the direction `omega` (device fp32 [ndim]) into the
+    dense device tensors eta, chi [nvox][n_lambda]."""
+    a = dict(_MIPS_DEFAULTS)
+    a.update(mips_args)
+    d, _, keep = _mips_desc(**a)
+    _check(_L.dex_direction_fields(grid.handle, C.byref(d), _ptr(omega, torch.float32), _ptr(sin_incl, torch.float32),
+                                   _ptr(eta, torch.float32), _ptr(chi, torch.float32), _stream(stream)))
+    del keep
+
+
+def dex_mean_intensity_single_direction(grid: Grid, mips_args: dict, rays: Rays, J: torch.Tensor, level_caps=None,
+                                        segment_count: Optional[torch.Tensor] = None, want_levels=False, stream=None):
+    """include/dex.h dex_mean_intensity_single_direction.  Returns the level tables [n_dirs][n_batch][n_bricks] when
+    `want_levels`, else None."""
+    a = dict(_MIPS_DEFAULTS)
+    a.update(mips_args)
+    d, _, keep = _mips_desc(**a)
+    r = rays.struct()
+    t = np.ascontiguousarray([] if level_caps is None else level_caps, dtype=np.float32)
+    lv = None
+    if want_levels:
+        nb, _ = grid.info()
+        lv = np.empty((rays.n_dirs, int(a["n_lambda"]) // int(a["lambda_batch"]), nb), dtype=np.int8)
+    _check(_L.dex_mean_intensity_single_direction(grid.handle, C.byref(d), C.byref(r), int(t.size),
+                                                  t.ctypes.data if t.size else None, _ptr(J, torch.float32),
+                                                  _ptr(segment_count, torch.int64),
+                                                  lv.ctypes.data if lv is not None else None, _stream(stream)))
     del keep
     return lv
 

@@ -72,6 +72,7 @@ dex_status check_rays(const dex_grid* grid, const dex_mips* mips, const dex_rays
   out->sin_incl = rays->d_sin_incl;
   out->t_begin = rays->t_begin;
   out->t_end = rays->t_end;
+  out->accumulate = rays->accumulate;
   if (rays->t_end > 0.0f && !(rays->t_begin >= 0.0f && rays->t_begin < rays->t_end)) {
     dex_set_error("radiance interval needs 0 <= t_begin < t_end");
     return DEX_ERR_INVALID_ARG;
@@ -775,6 +776,132 @@ dex_status dex_mean_intensity_pipelined(const dex_grid* grid, const dex_mips_des
   if (s != DEX_OK) return s;
   DEX_CUDA_CHECK(e);
   DEX_CUDA_CHECK(cudaGetLastError());
+  return DEX_OK;
+}
+
+// ------------------------------------------------------------------------------------------- single-direction VLM
+namespace {
+dex_status check_aniso_desc(const dex_mips_desc* desc) {
+  if (desc->variant == DEX_ISO) { dex_set_error("a static (DEX_ISO) medium has no direction dependence"); return DEX_ERR_INVALID_ARG; }
+  if (desc->lambda_batch != DEX_W) { dex_set_error("lambda_batch must be 8 in this build"); return DEX_ERR_UNSUPPORTED; }
+  if (desc->n_lambda <= 0 || desc->n_lambda % DEX_W) { dex_set_error("n_lambda must be a positive multiple of lambda_batch"); return DEX_ERR_SHAPE; }
+  if (desc->lambda_stride != 0 && desc->lambda_stride < desc->n_lambda) { dex_set_error("lambda_stride must be 0 (dense) or >= n_lambda"); return DEX_ERR_SHAPE; }
+  if (!desc->d_eta_bg || !desc->d_chi_bg || !desc->d_vel || !desc->d_lambda || !desc->h_active_lines) {
+    dex_set_error("anisotropic media need d_eta_bg, d_chi_bg, d_vel, d_lambda, h_active_lines");
+    return DEX_ERR_INVALID_ARG;
+  }
+  if (desc->n_lines < 0 || desc->n_lines > DEX_MAX_LINES) { dex_set_error("n_lines must be 0..4"); return DEX_ERR_SHAPE; }
+  if (desc->n_lines > 0 && (!desc->h_lambda0 || !desc->d_eta_star0 || !desc->d_chi_star0 || !desc->d_a0 || !desc->d_inv_dlamD)) {
+    dex_set_error("line arrays are NULL");
+    return DEX_ERR_INVALID_ARG;
+  }
+  const int n_batch = desc->n_lambda / DEX_W;
+  for (int i = 0; i < n_batch * DEX_MAX_LINES; ++i) {
+    const int l = desc->h_active_lines[i];
+    if (l < -1 || l >= desc->n_lines) { dex_set_error("active line id out of range"); return DEX_ERR_SHAPE; }
+  }
+  if (!(desc->c_light > 0.0f)) { dex_set_error("c_light must be > 0"); return DEX_ERR_INVALID_ARG; }
+  return DEX_OK;
+}
+
+dex_status upload_active_lines(const dex_mips_desc* desc, signed char** d_al, cudaStream_t st) {
+  const size_t n = (size_t)(desc->n_lambda / DEX_W) * DEX_MAX_LINES;
+  dex_status s = dmalloc(d_al, n, st);
+  if (s != DEX_OK) return s;
+  cudaError_t e = cudaMemcpyAsync(*d_al, desc->h_active_lines, n, cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) { dex_free(*d_al, st); *d_al = nullptr; DEX_CUDA_CHECK(e); }
+  return DEX_OK;
+}
+}  // namespace
+
+dex_status dex_direction_fields(const dex_grid* grid, const dex_mips_desc* desc, const float* d_omega,
+                                const float* d_sin_incl, float* d_eta, float* d_chi, void* stream) {
+  if (!grid || !desc || !d_omega || !d_eta || !d_chi) { dex_set_error("NULL grid / desc / d_omega / d_eta / d_chi"); return DEX_ERR_INVALID_ARG; }
+  if (d_sin_incl && grid->dev.ndim != 2) { dex_set_error("d_sin_incl (2.5D rays) needs a 2D grid"); return DEX_ERR_INVALID_ARG; }
+  dex_status s = check_aniso_desc(desc);
+  if (s != DEX_OK) return s;
+  if (!have_device()) return DEX_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  signed char* d_al = nullptr;
+  s = upload_active_lines(desc, &d_al, st);
+  if (s != DEX_OK) return s;
+  s = dex_launch_direction_fields(grid, desc, d_al, d_omega, d_sin_incl, d_eta, d_chi, st);
+  dex_free(d_al, st);
+  return s;
+}
+
+dex_status dex_mean_intensity_single_direction(const dex_grid* grid, const dex_mips_desc* desc, const dex_rays* rays,
+                                               int n_caps, const float* h_cap_t, float* d_J, int64_t* d_segment_count,
+                                               int8_t* h_levels, void* stream) {
+  if (!grid || !desc || !rays) { dex_set_error("NULL grid / desc / rays"); return DEX_ERR_INVALID_ARG; }
+  dex_status s = check_aniso_desc(desc);
+  if (s != DEX_OK) return s;
+  if (rays->n_probes < 0 || rays->n_dirs < 0) { dex_set_error("negative n_probes / n_dirs"); return DEX_ERR_INVALID_ARG; }
+  if (rays->n_probes == 0) return DEX_OK;
+  if (!d_J) { dex_set_error("d_J is NULL"); return DEX_ERR_INVALID_ARG; }
+  if (rays->n_dirs > 0 && (!rays->d_weights || !rays->d_dirs || !rays->d_probe_pos)) {
+    dex_set_error("d_probe_pos / d_dirs / d_weights is NULL");
+    return DEX_ERR_INVALID_ARG;
+  }
+  if (rays->d_sin_incl && grid->dev.ndim != 2) { dex_set_error("d_sin_incl (2.5D rays) needs a 2D grid"); return DEX_ERR_INVALID_ARG; }
+  if (!have_device()) return DEX_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t nl = (size_t)desc->n_lambda, D = (size_t)grid->dev.ndim;
+  const size_t n_batch = nl / DEX_W;
+  DEX_CUDA_CHECK(cudaMemsetAsync(d_J, 0, sizeof(float) * (size_t)rays->n_probes * nl, st));   // n_dirs == 0: J = 0
+  if (rays->n_dirs == 0) return DEX_OK;
+  float *d_eta = nullptr, *d_chi = nullptr;
+  signed char* d_al = nullptr;
+  int* d_perm = nullptr;
+  s = dmalloc(&d_eta, (size_t)grid->nvox * nl, st);
+  if (s == DEX_OK) s = dmalloc(&d_chi, (size_t)grid->nvox * nl, st);
+  if (s == DEX_OK) s = upload_active_lines(desc, &d_al, st);
+  if (s == DEX_OK && g_tile_probes.load() != 0) {     // one probe tiling serves every direction
+    DexRaysDev R;
+    R.n_probes = rays->n_probes;
+    R.probe_pos = rays->d_probe_pos;
+    s = dex_make_probe_tiling(grid, R, &d_perm, st);
+  }
+  dex_mips_desc iso = *desc;
+  iso.variant = DEX_ISO;
+  iso.d_eta = d_eta;
+  iso.d_chi = d_chi;
+  iso.lambda_stride = 0;
+  cudaError_t e = cudaSuccess;
+  for (int k = 0; k < rays->n_dirs && s == DEX_OK && e == cudaSuccess; ++k) {
+    s = dex_launch_direction_fields(grid, desc, d_al, rays->d_dirs + (size_t)k * D,
+                                    rays->d_sin_incl ? rays->d_sin_incl + k : nullptr, d_eta, d_chi, st);
+    if (s != DEX_OK) break;
+    dex_mips* m = nullptr;
+    s = dex_build_vlm_mips(grid, &iso, stream, &m);
+    if (s != DEX_OK) break;
+    s = dex_mips_set_level_caps(m, n_caps, h_cap_t);
+    if (s == DEX_OK && h_levels)
+      e = cudaMemcpyAsync(h_levels + (size_t)k * n_batch * grid->n_bricks, m->d_levels, n_batch * (size_t)grid->n_bricks,
+                          cudaMemcpyDeviceToHost, st);
+    dex_rays rk = *rays;
+    rk.n_dirs = 1;
+    rk.d_dirs = rays->d_dirs + (size_t)k * D;
+    rk.d_weights = rays->d_weights + k;
+    rk.d_i0 = rays->d_i0 ? rays->d_i0 + (size_t)k * nl : nullptr;
+    rk.d_sin_incl = rays->d_sin_incl ? rays->d_sin_incl + k : nullptr;
+    rk.accumulate = 1;
+    DexRaysDev R;
+    if (s == DEX_OK) s = check_rays(grid, m, &rk, &R);
+    if (s == DEX_OK) {
+      MarchTimer tm(st);
+      s = dex_launch_march(grid, m, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), false, st,
+                           d_perm);
+    }
+    dex_destroy_mips(m);     // stream-ordered: released after the march above
+  }
+  if (d_perm) cudaFreeAsync(d_perm, st);
+  dex_free(d_al, st);
+  dex_free(d_eta, st);
+  dex_free(d_chi, st);
+  if (s == DEX_OK && e == cudaSuccess && h_levels) e = cudaStreamSynchronize(st);
+  if (s != DEX_OK) return s;
+  DEX_CUDA_CHECK(e);
   return DEX_OK;
 }
 

@@ -71,6 +71,7 @@ struct DexRaysDev {
   const float* i0;
   const float* sin_incl;   // [n_dirs] or NULL: 2.5D rays
   float t_begin, t_end;    // finite radiance interval (T10); t_end <= 0: to the boundary
+  int accumulate;          // fused J: d_J += sum_k w_k I_k instead of = (single-direction VLM sums its per-direction solves)
 };
 
 // ---- exact (uncontracted) fp32 helpers -------------------------------------------------

@@ -55,6 +55,10 @@ dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStrea
 dex_status dex_launch_mips_build(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st);
 dex_status dex_launch_pack_levels(dex_mips* m, cudaStream_t st);
 dex_status dex_launch_vbin_report(const dex_mips* m, float factor, unsigned* d_max, unsigned long long* d_cnt, cudaStream_t st);
+// single-direction VLM input: Classic fields along the direction d_omega[D] (device), dense [nvox][n_lambda]
+dex_status dex_launch_direction_fields(const dex_grid* g, const dex_mips_desc* desc, const signed char* d_active_lines,
+                                       const float* d_omega, const float* d_sin_incl, float* d_eta, float* d_chi,
+                                       cudaStream_t st);
 dex_status dex_launch_level_data(const dex_mips* m, int chain, int level, float* d_dense, cudaStream_t st);
 // march.cu
 dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,

@@ -531,7 +531,10 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   if (FUSE_J && valid) {
     float* dst = out + (size_t)gid * M.io_stride + M.io_base + lam_off;
 #pragma unroll
-    for (int i = 0; i < LPT; ++i) dst[i] = Jsm[i * DEX_MARCH_THREADS + threadIdx.x];
+    for (int i = 0; i < LPT; ++i) {
+      const float j = Jsm[i * DEX_MARCH_THREADS + threadIdx.x];
+      dst[i] = R.accumulate ? __fadd_rn(dst[i], j) : j;
+    }
   }
   if (seg_count != nullptr) {
     unsigned v = (sub == 0) ? nseg : 0u;

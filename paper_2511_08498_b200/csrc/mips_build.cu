@@ -521,6 +521,105 @@ BuildCtx make_ctx(const dex_mips* m) {
   return X;
 }
 
+// ---- single-direction VLM input (T11) -------------------------------------------
+// eta, chi of an anisotropic medium seen along ONE direction, at full resolution, from the caller's dense arrays:
+// the Classic formula (eqs. 10-20) with v_proj = v . omega (times sin_incl for a 2.5D ray), fp64, rounded once.
+// One thread per (voxel, wavelength); voxels of empty bricks are written as 0.
+struct DirFieldArgs {
+  DexGridDev G;
+  int n_lambda, in_stride, n_lines;
+  const float* lam;                  // [n_lambda]
+  const float* eta_bg;               // [nvox][in_stride]
+  const float* chi_bg;
+  const float* vel;                  // [nvox][D]
+  const float* eta_star0;            // [n_lines][nvox]
+  const float* chi_star0;
+  const float* a0;
+  const float* inv_dlamD;
+  const signed char* active_lines;   // [n_batch][DEX_NLINES] device
+  float lambda0[DEX_NLINES];
+  const float* om;                   // [D] device: the direction
+  const float* sin_incl;             // device scalar or NULL (2.5D ray)
+  double c_light;
+  double wei_c[24];
+  double wei_L;
+};
+
+template <int D>
+__global__ void direction_fields_kernel(const DirFieldArgs A, long long nvox, float* __restrict__ eta,
+                                        float* __restrict__ chi) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nvox * A.n_lambda) return;
+  const int j = (int)(i % A.n_lambda);
+  const long long v = i / A.n_lambda;
+  const int x = (int)(v % A.G.dims[0]);
+  const int y = (int)((v / A.G.dims[0]) % A.G.dims[1]);
+  const int z = (D == 3) ? (int)(v / ((long long)A.G.dims[0] * A.G.dims[1])) : 0;
+  const int brick = ((z >> A.G.logB) * A.G.nb[1] + (y >> A.G.logB)) * A.G.nb[0] + (x >> A.G.logB);
+  if (A.G.slot[brick] < 0) {
+    eta[i] = 0.0f;
+    chi[i] = 0.0f;
+    return;
+  }
+  double vproj = 0.0;
+#pragma unroll
+  for (int a = 0; a < D; ++a) vproj = vproj + (double)A.vel[v * D + a] * (double)__ldg(A.om + a);
+  if (A.sin_incl != nullptr) vproj = vproj * (double)__ldg(A.sin_incl);
+  const int b = j / DEX_W;
+  const double lam = (double)A.lam[j];
+  double e = (double)A.eta_bg[v * A.in_stride + j];
+  double c = (double)A.chi_bg[v * A.in_stride + j];
+  for (int q = 0; q < DEX_NLINES; ++q) {
+    const int l = A.active_lines[b * DEX_NLINES + q];
+    if (l < 0) continue;
+    const size_t k = (size_t)l * nvox + v;
+    double el, cl;
+    dex_line_terms(A.wei_c, A.wei_L, lam, (double)A.lambda0[l], (double)A.eta_star0[k], (double)A.chi_star0[k],
+                   (double)A.a0[k], (double)A.inv_dlamD[k], vproj, A.c_light, el, cl);
+    e = e + el;
+    c = c + cl;
+  }
+  eta[i] = (float)e;
+  chi[i] = (float)c;
+}
+
+}  // namespace
+
+dex_status dex_launch_direction_fields(const dex_grid* g, const dex_mips_desc* desc, const signed char* d_active_lines,
+                                       const float* d_omega, const float* d_sin_incl, float* d_eta, float* d_chi,
+                                       cudaStream_t st) {
+  DirFieldArgs A;
+  A.G = g->dev;
+  A.n_lambda = desc->n_lambda;
+  A.in_stride = desc->lambda_stride ? desc->lambda_stride : desc->n_lambda;
+  A.n_lines = desc->n_lines;
+  A.lam = desc->d_lambda;
+  A.eta_bg = desc->d_eta_bg;
+  A.chi_bg = desc->d_chi_bg;
+  A.vel = desc->d_vel;
+  A.eta_star0 = desc->d_eta_star0;
+  A.chi_star0 = desc->d_chi_star0;
+  A.a0 = desc->d_a0;
+  A.inv_dlamD = desc->d_inv_dlamD;
+  A.active_lines = d_active_lines;
+  for (int l = 0; l < DEX_NLINES; ++l) A.lambda0[l] = (l < desc->n_lines) ? desc->h_lambda0[l] : 0.0f;
+  A.om = d_omega;
+  A.sin_incl = d_sin_incl;
+  A.c_light = (double)desc->c_light;
+  dex_weideman_coefficients(A.wei_c, &A.wei_L);
+  const long long total = g->nvox * desc->n_lambda;
+  if (total <= 0) return DEX_OK;
+  if (g->desc.ndim == 2)
+    direction_fields_kernel<2><<<blocks_for(total, 256), 256, 0, st>>>(A, g->nvox, d_eta, d_chi);
+  else
+    direction_fields_kernel<3><<<blocks_for(total, 256), 256, 0, st>>>(A, g->nvox, d_eta, d_chi);
+  dex_count_launch();
+  DEX_CUDA_CHECK(cudaGetLastError());
+  return DEX_OK;
+}
+
+namespace {
+
 template <int D>
 dex_status build_t(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st) {
   const BuildCtx X = make_ctx(m);

@@ -100,6 +100,29 @@ def mean_intensity_pipelined(dw: DeviceWorkload, grid: B.Grid, batches_per_stage
     return J, lv
 
 
+def direction_fields(dw: DeviceWorkload, grid: B.Grid, k: int, stream=None):
+    """Classic eta, chi of the workload's anisotropic medium along quadrature direction k (dense device tensors)."""
+    wl, t = dw.wl, dw.t
+    dev = t["probe_pos"].device
+    eta = torch.empty((wl.nvox, wl.n_lambda), dtype=torch.float32, device=dev)
+    chi = torch.empty_like(eta)
+    si = t.get("sin_incl")
+    B.dex_direction_fields(grid, _mips_args(wl, t), t["dirs"][k], eta, chi, None if si is None else si[k:k + 1], stream)
+    return eta, chi
+
+
+def mean_intensity_single_direction(dw: DeviceWorkload, grid: B.Grid, J: Optional[torch.Tensor] = None, level_caps=None,
+                                    segment_count: Optional[torch.Tensor] = None, want_levels=False, stream=None,
+                                    **override):
+    """Single-direction VLM (include/dex.h dex_mean_intensity_single_direction); returns (J, level tables or None)."""
+    r = rays(dw)
+    if J is None:
+        J = torch.empty((r.n_probes, dw.wl.n_lambda), dtype=torch.float32, device=r.probe_pos.device)
+    lv = B.dex_mean_intensity_single_direction(grid, _mips_args(dw.wl, dw.t, **override), r, J, level_caps,
+                                               segment_count, want_levels, stream)
+    return J, lv
+
+
 def formal_solution(dw: DeviceWorkload, grid: B.Grid, mips: B.Mips, capture_batch: Optional[int] = None,
                     segment_count: Optional[torch.Tensor] = None, want_I=True, room: Optional[int] = None, stream=None):
     r = rays(dw)
