@@ -377,7 +377,7 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": config_dict(wl, args, {"lanes_per_ray": args.lanes or 1,
+            "config": config_dict(wl, args, {"lanes_per_ray": args.lanes or ("auto: 8" if wl.probe_pos.shape[0] < 148 * 128 else "auto: 1"),
                                              "segments_per_step": segs_total // max(1, args.steps),
                                              "path": (f"rebuild pipeline, {args.pipeline} batch(es) per stage"
                                                       if args.pipeline > 0 else "whole-spectrum build + march"),

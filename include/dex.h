@@ -286,9 +286,10 @@ dex_status dex_march_timing_read(double* ms_total, int64_t* n_launches, int rese
  * number of active lines of the segment's batch, i.e. line-profile evaluations / W (bench.py's ALU roofline leg
  * multiplies by W and by the flops per evaluation stated in DESIGN.md).  Synchronises. */
 dex_status dex_march_work_read(int64_t* line_segments, int reset);
-/* Kernel configuration knob (performance experiments): lanes that share one ray, 1/2/4/8. */
+/* Kernel configuration knob: lanes that share one ray, 1/2/4/8, or 0 (default) = automatic: one thread per ray unless
+ * there are fewer probes than one wave of blocks (148 SMs x 128 threads), where 8 lanes per ray fill the machine better. */
 dex_status dex_set_lanes_per_ray(int lanes);
-/* Kernel-structure knobs for performance experiments (results do not change): "lanes_per_ray" 1/2/4/8;
+/* Kernel-structure knobs for performance experiments (results do not change): "lanes_per_ray" 0/1/2/4/8;
  * "tile_probes" 0/1 (1, default: probes are handed to warps in compact spatial tiles by an internal counting
  * sort instead of in the caller's order); "voigt_fp32" 0/1 (1, default: the Core-and-Voigt march evaluates H(a, x) in
  * its fp32 table form inside the damping window of csrc/dex_voigt.cuh; 0: the fp64 form everywhere -- results agree

@@ -14,7 +14,7 @@
 namespace {
 thread_local std::string g_last_error;
 std::atomic<long long> g_launches{0};
-std::atomic<int> g_lanes_per_ray{1};  // measured fastest on B200 (profiles/)
+std::atomic<int> g_lanes_per_ray{0};  // 0 = automatic, see lanes_for()
 std::atomic<int> g_timing{0};
 std::atomic<int> g_tile_probes{1};
 std::atomic<int> g_voigt_fp32{1};
@@ -22,6 +22,17 @@ std::mutex g_timing_mu;
 struct EvPair { cudaEvent_t a, b; };
 std::vector<EvPair> g_events;
 unsigned long long* g_d_line_segs = nullptr;   // device counter of (segment, active line) pairs, timing mode only
+
+// Lanes that share one ray.  One thread per ray (all W wavelengths in registers) is the fastest mapping whenever the
+// probes fill the machine (profiles/r01_march_ncu_full.md: 1.6-2.2x over 8 lanes on C2).  A small problem -- fewer
+// probes than one wave of 128-thread blocks on 148 SMs, e.g. C1's 4096 -- leaves most SMs idle with that mapping;
+// 8 lanes per ray give it 8x the threads (C1 march 0.403 -> 0.267 ms).  Depends on n_probes only, so every wavelength
+// stage of a pipelined solve takes the same mapping as the whole-spectrum call.
+int lanes_for(long long n_probes) {
+  const int set = g_lanes_per_ray.load();
+  if (set != 0) return set;
+  return (n_probes < 148LL * 128) ? 8 : 1;
+}
 
 int ilog2_exact(int v) {
   if (v <= 0 || (v & (v - 1))) return -1;
@@ -208,8 +219,8 @@ dex_status dex_pool_high_water(int64_t* bytes_in_use_high, int reset) {
 }
 
 dex_status dex_set_lanes_per_ray(int lanes) {
-  if (lanes != 1 && lanes != 2 && lanes != 4 && lanes != 8) {
-    dex_set_error("lanes per ray must be 1, 2, 4 or 8");
+  if (lanes != 0 && lanes != 1 && lanes != 2 && lanes != 4 && lanes != 8) {
+    dex_set_error("lanes per ray must be 0 (automatic), 1, 2, 4 or 8");
     return DEX_ERR_INVALID_ARG;
   }
   g_lanes_per_ray.store(lanes);
@@ -614,7 +625,7 @@ dex_status dex_formal_solution(const dex_grid* grid, const dex_mips* mips, const
   cudaStream_t st = (cudaStream_t)stream;
   if (d_I) {
     MarchTimer tm(st);
-    s = dex_launch_march(grid, mips, R, d_I, false, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), g_tile_probes.load() != 0, st);
+    s = dex_launch_march(grid, mips, R, d_I, false, (unsigned long long*)d_segment_count, lanes_for(R.n_probes), g_tile_probes.load() != 0, st);
     if (s != DEX_OK) return s;
   }
   if (capture) {
@@ -648,7 +659,7 @@ dex_status dex_mean_intensity(const dex_grid* grid, const dex_mips* mips, const 
   cudaStream_t st = (cudaStream_t)stream;
   if (d_I) return dex_launch_reduce_j(R, mips->n_lambda, d_I, d_J, st);
   MarchTimer tm(st);
-  return dex_launch_march(grid, mips, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), g_tile_probes.load() != 0, st);
+  return dex_launch_march(grid, mips, R, d_J, true, (unsigned long long*)d_segment_count, lanes_for(R.n_probes), g_tile_probes.load() != 0, st);
 }
 
 // ------------------------------------------------------------------------------------------- rebuild pipeline
@@ -746,7 +757,7 @@ dex_status dex_mean_intensity_pipelined(const dex_grid* grid, const dex_mips_des
       if (s == DEX_OK) {
         cudaStreamWaitEvent(ms, ev_built[sg & 1], 0);
         MarchTimer tm(ms);
-        s = dex_launch_march(grid, cur, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(),
+        s = dex_launch_march(grid, cur, R, d_J, true, (unsigned long long*)d_segment_count, lanes_for(R.n_probes),
                              false, ms, d_perm);
       }
     }
@@ -890,7 +901,7 @@ dex_status dex_mean_intensity_single_direction(const dex_grid* grid, const dex_m
     if (s == DEX_OK) s = check_rays(grid, m, &rk, &R);
     if (s == DEX_OK) {
       MarchTimer tm(st);
-      s = dex_launch_march(grid, m, R, d_J, true, (unsigned long long*)d_segment_count, g_lanes_per_ray.load(), false, st,
+      s = dex_launch_march(grid, m, R, d_J, true, (unsigned long long*)d_segment_count, lanes_for(R.n_probes), false, st,
                            d_perm);
     }
     dex_destroy_mips(m);     // stream-ordered: released after the march above

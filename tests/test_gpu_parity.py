@@ -26,6 +26,9 @@ def P():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     import paper_2511_08498_b200 as pkg
+    # the tests run the production mapping (one thread per ray) unless they say otherwise; the library's default is
+    # automatic (8 lanes per ray for problems smaller than one wave of blocks), exercised by test_c1_full
+    pkg.dex_set_lanes_per_ray(1)
     return pkg
 
 
@@ -106,7 +109,13 @@ def test_c1_full(P):
     M = orc.build_mips(wl)
     dw, grid, mips = _build(P, wl)
     _check_build(P, wl, M, grid, mips)
-    _solve_and_compare(P, wl, M, dw, grid, mips)
+    ref = _solve_and_compare(P, wl, M, dw, grid, mips)
+    P.dex_set_lanes_per_ray(0)             # automatic: 4096 probes < one wave of blocks -> 8 lanes per ray
+    try:
+        J = P.pipeline.mean_intensity(dw, grid, mips)
+        assert max_rel(J.cpu().numpy(), orc.mean_intensity(ref.I, wl.weights)) <= TOL
+    finally:
+        P.dex_set_lanes_per_ray(1)
 
 
 @pytest.mark.parametrize("metric,thr,gate", [(1, 1e-2, -1.0), (0, 1.0, 0.25), (1, 0.0, -1.0)])
