@@ -626,3 +626,49 @@ def test_single_direction_vlm_parity(P, name, kw, thr, tilt):
     assert max_rel(J2.cpu().numpy(), J.cpu().numpy()) <= 2e-6
     with pytest.raises(P.DexError):       # a static medium has no direction dependence
         P.pipeline.mean_intensity_single_direction(dw, grid, variant=P.DEX_ISO)
+
+
+def test_edge_cases_pipelined_and_single_direction(P):
+    """Degenerate inputs of the two composite entries: no probes, one batch (a single stage), all bricks empty, no
+    directions; argument errors."""
+    # no probes: nothing to write, the level table is still built and returned
+    wl = make("C2", n=64, n_dirs=4, n_probes=20)
+    full = wl.probe_pos
+    wl.probe_pos = full[:0]
+    M = orc.build_mips(wl)
+    dw = P.pipeline.upload(wl, "cuda:0")
+    grid = P.pipeline.build_grid(dw)
+    J, lv = P.pipeline.mean_intensity_pipelined(dw, grid, 1, want_levels=True)
+    assert J.shape == (0, wl.n_lambda) and np.array_equal(lv, M.levels)
+    # all bricks empty, boundary intensity only: J = sum_k w_k i0[k] exactly as the whole-spectrum path gives it
+    wl2 = make("C2", n=64, n_dirs=4, n_probes=33)
+    wl2.active[:] = 0
+    wl2.eta[:] = 0
+    wl2.chi[:] = 0
+    wl2.i0 = np.random.default_rng(3).uniform(0, 1, size=(4, wl2.n_lambda)).astype(np.float32)
+    dw2, g2, m2 = _build(P, wl2)
+    J0 = P.pipeline.mean_intensity(dw2, g2, m2)
+    seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+    J1, lv1 = P.pipeline.mean_intensity_pipelined(dw2, g2, 3, segment_count=seg, want_levels=True)
+    assert torch.equal(J0, J1) and (lv1 == -1).all() and int(seg.item()) == 0
+    assert max_rel(J1.cpu().numpy(), orc.mean_intensity(np.broadcast_to(wl2.i0, (33,) + wl2.i0.shape), wl2.weights)) <= 1e-6
+    # single direction: no directions -> J = 0 (and overwritten, not added to); no probes -> no-op
+    wl3 = make("C4", n=64, n_dirs=4, n_probes=25)
+    dw3 = P.pipeline.upload(wl3, "cuda:0")
+    g3 = P.pipeline.build_grid(dw3)
+    J3 = torch.full((25, wl3.n_lambda), 7.0, dtype=torch.float32, device="cuda:0")
+    r0 = P.Rays(dw3.t["probe_pos"], dw3.t["dirs"][:0], dw3.t["weights"][:0])
+    P.dex_mean_intensity_single_direction(g3, P.pipeline._mips_args(wl3, dw3.t), r0, J3)
+    assert (J3 == 0).all()
+    # ... and a second call overwrites the first (J is not accumulated across calls)
+    Ja, _ = P.pipeline.mean_intensity_single_direction(dw3, g3)
+    Jb, _ = P.pipeline.mean_intensity_single_direction(dw3, g3, J=Ja.clone())
+    assert torch.equal(Ja, Jb)
+    rn = P.Rays(dw3.t["probe_pos"][:0], dw3.t["dirs"], dw3.t["weights"])
+    P.dex_mean_intensity_single_direction(g3, P.pipeline._mips_args(wl3, dw3.t), rn,
+                                          torch.empty((0, wl3.n_lambda), dtype=torch.float32, device="cuda:0"))
+    # argument errors: max_level beyond log2(brick) is refused by both
+    with pytest.raises(P.DexError):
+        P.pipeline.mean_intensity_pipelined(dw, grid, 1, max_level=5)
+    with pytest.raises(P.DexError):
+        P.pipeline.mean_intensity_single_direction(dw3, g3, max_level=5)
