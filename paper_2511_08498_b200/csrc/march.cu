@@ -379,6 +379,14 @@ constexpr int dex_march_minb(int var) {
 #define DEX_CROSS_QUORUM 8
 #endif
 
+
+#ifdef DEX_MARCH_STATS
+// diagnostic build only (-DDEX_MARCH_STATS): lane-iteration census of the warp-synchronous loop
+// [0] warp iterations x 32, [1] lanes alive, [2] lanes blocked at a brick face, [3] lanes that emitted,
+// [4] iterations in which the general crossing ran, [5] lanes that took it
+__device__ unsigned long long g_dex_stats[8];
+#endif
+
 template <int D, int VAR, int LPR, bool FUSE_J, bool CLIP>
 __global__ void __launch_bounds__(DEX_MARCH_THREADS, dex_march_minb(VAR))
 dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ perm,
@@ -395,6 +403,9 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   const int sub = threadIdx.x % LPR;
   const int lam_off = batch * DEX_W + sub * LPT;
   unsigned nseg = 0;
+#ifdef DEX_MARCH_STATS
+  unsigned long long st_it = 0, st_alive = 0, st_blocked = 0, st_xit = 0, st_xl = 0;
+#endif
   const int* binfo = M.binfo + (size_t)batch * G.n_bricks;
   asm volatile("" : "+l"(binfo));   // opaque for the same reason as iso0 / iso1 below
   const size_t batch_base = ((size_t)batch * G.n_active) * M.cps;
@@ -483,6 +494,10 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
         for (int i = 0; i < LPT; ++i) { DEX_IH(i) += I[i]; I[i] = 0.0f; }
       }
       const unsigned bm = __ballot_sync(FULL, blocked);
+#ifdef DEX_MARCH_STATS
+      st_it += 32; st_alive += __popc(am); st_blocked += __popc(bm);
+      if (bm == am || __popc(bm) >= DEX_CROSS_QUORUM) { st_xit += 1; st_xl += __popc(bm); }
+#endif
       if (bm == am || __popc(bm) >= DEX_CROSS_QUORUM) {
         if (blocked) {
           alive = dex_ray_cross<D>(ray, G, M, binfo, probe, om);
@@ -536,6 +551,13 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
       dst[i] = R.accumulate ? __fadd_rn(dst[i], j) : j;
     }
   }
+#ifdef DEX_MARCH_STATS
+  if ((threadIdx.x & 31) == 0) {
+    atomicAdd(&g_dex_stats[0], st_it); atomicAdd(&g_dex_stats[1], st_alive); atomicAdd(&g_dex_stats[2], st_blocked);
+    atomicAdd(&g_dex_stats[4], st_xit); atomicAdd(&g_dex_stats[5], st_xl);
+  }
+  atomicAdd(&g_dex_stats[3], (unsigned long long)nseg);
+#endif
   if (seg_count != nullptr) {
     unsigned v = (sub == 0) ? nseg : 0u;
     v = __reduce_add_sync(FULL, v);
@@ -868,3 +890,12 @@ dex_status dex_launch_reduce_j(const DexRaysDev& rays, int n_lambda, const float
   DEX_CUDA_CHECK(cudaGetLastError());
   return DEX_OK;
 }
+
+#ifdef DEX_MARCH_STATS
+extern "C" int dex_debug_read_stats(unsigned long long* out8, int reset) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out8, g_dex_stats, sizeof(unsigned long long) * 8);
+  if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(g_dex_stats, z, sizeof(z)); }
+  return 0;
+}
+#endif
