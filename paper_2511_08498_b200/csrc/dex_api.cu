@@ -61,7 +61,7 @@ dex_status dmalloc(T** p, size_t count, cudaStream_t st) {
 }
 
 void free_mips_memory(dex_mips* m) {
-  void* ptrs[] = {m->d_store, m->d_mrec, m->d_line, m->d_vel, m->d_vtab, m->d_lam, m->d_active_lines, m->d_levels,
+  void* ptrs[] = {m->d_store, m->d_mrec, m->d_aux, m->d_vtab, m->d_lam, m->d_active_lines, m->d_levels,
                   m->d_packed, m->d_fail, m->d_binfo, m->d_vftab};
   for (void* q : ptrs) dex_free(q, m->stream);
 }
@@ -444,8 +444,7 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
   if (s == DEX_OK) s = dmalloc(&m->d_binfo, (size_t)n_batch * grid->n_bricks, st);
   if (s == DEX_OK) s = dmalloc(&m->d_fail, (size_t)n_batch * A * (max_level + 1), st);
   if (s == DEX_OK && v != DEX_ISO) {
-    s = dmalloc(&m->d_vel, A * cps, st);
-    if (s == DEX_OK) s = dmalloc(&m->d_line, A * cps * (size_t)(d.n_lines > 0 ? d.n_lines : 1), st);
+    s = dmalloc(&m->d_aux, A * cps * (size_t)(d.n_lines + 1), st);
     if (s == DEX_OK) s = dmalloc(&m->d_lam, (size_t)desc->n_lambda, st);
     if (s == DEX_OK) s = dmalloc(&m->d_active_lines, (size_t)n_batch * DEX_MAX_LINES, st);
     if (s == DEX_OK) s = dmalloc(&m->d_vftab, (size_t)DEX_VF_NODES * 5, st);
@@ -473,8 +472,9 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
     d.store = m->d_store;
     d.mrec = m->d_mrec;
     d.mplane = m->store_floats / 2;
-    d.line = m->d_line;
-    d.vel = m->d_vel;
+    d.aux = m->d_aux;
+    if (v == DEX_VELINTERP) { d.aux_vs = 1; d.aux_lo = A * cps; d.aux_ls = d.n_lines; }      // dense velocities, lines behind
+    else { d.aux_vs = d.n_lines + 1; d.aux_lo = 1; d.aux_ls = d.n_lines + 1; }             // one record per cell
     d.vtab = m->d_vtab;
     d.lam = m->d_lam;
     d.active_lines = m->d_active_lines;

@@ -42,8 +42,10 @@ struct DexMipsDev {
   const float* mrec;                 // ISO march records (make_march_records_kernel), what the ISO march reads: two planes
   size_t mplane;                     // [2][n_batch][n_active][cps][DEX_W], plane 0 chi log2(e), plane 1 S = eta/chi;
                                      // mplane = floats per plane
-  const float4* line;                // [n_active][cps][n_lines]  (eta*, chi*, a0, 1/dlamD)
-  const float4* vel;                 // [n_active][cps]           (vx, vy, vz, max|v|)
+  const float4* aux;                 // [n_active][cps][1 + n_lines]: (vx, vy, vz, max|v|) then per line (eta*, chi*, a0,
+                                     // 1/dlamD), see dex_aux_vel / dex_aux_line
+  int aux_vs, aux_ls;                // float4 strides of the velocity and of a cell's line records
+  size_t aux_lo;                     // float4 index of the first line record
   const float* vtab;                 // [n_batch][n_active][cps][n_vbins][DEX_REC]
   const float* lam;                  // [n_lambda] device
   const signed char* active_lines;   // [n_batch][DEX_NLINES] device
@@ -61,6 +63,17 @@ struct DexMipsDev {
   int io_stride, io_base;            // row length and first column of this handle's wavelengths in I / J / i0: n_lambda and
                                      // 0 unless the handle is one stage of dex_mean_intensity_pipelined
 };
+
+// Auxiliary chains of the anisotropic variants in one array `aux` of float4: velocity (vx, vy, vz, max|v|) and per line
+// (eta*, chi*, a0, 1/dlamD).  Core-and-Voigt / Classic marches read both at every segment, so there a cell's record is
+// contiguous, [velocity, line_0 .. line_{n-1}]: ONE 32-byte sector for one line (two for three lines) instead of a
+// sector each from two arrays (C5 is bound by DRAM sectors: 184.7 -> 171.8 ms, profiles/r01k).  The velocity-
+// interpolation march reads the velocity only, so there the velocities stay dense (16 B per cell) and the line records,
+// which only the build uses, follow them.  vel(cell) = aux[cell * aux_vs], line(cell, l) = aux[aux_lo + cell * aux_ls + l].
+__device__ __forceinline__ size_t dex_aux_vel(const DexMipsDev& M, size_t cell) { return cell * (size_t)M.aux_vs; }
+__device__ __forceinline__ size_t dex_aux_line(const DexMipsDev& M, size_t cell, int l) {
+  return M.aux_lo + cell * (size_t)M.aux_ls + (size_t)l;
+}
 
 struct DexRaysDev {
   long long n_probes;

@@ -26,8 +26,7 @@ struct dex_mips {
   // owned device memory
   float* d_store = nullptr;
   float* d_mrec = nullptr;
-  float4* d_line = nullptr;
-  float4* d_vel = nullptr;
+  float4* d_aux = nullptr;                   // [n_active][cps][1 + n_lines] velocity + line records (dex_aux_vel / dex_aux_line)
   float* d_vtab = nullptr;
   float* d_lam = nullptr;
   signed char* d_active_lines = nullptr;

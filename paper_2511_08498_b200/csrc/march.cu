@@ -232,7 +232,10 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
     return;
   }
   // projected velocity of the cell's box-filtered bulk velocity, fp64 (DESIGN.md R-vel)
-  const float4 v4 = __ldg(M.vel + cell);
+  // velocity-interpolation marches keep the velocities dense (stride 1, compile time); Core-and-Voigt / Classic read
+  // the cell's contiguous [velocity, lines] record (dex_device.cuh)
+  const float4* __restrict__ arec = M.aux + ((VAR == DEX_VELINTERP) ? (size_t)cell : dex_aux_vel(M, (size_t)cell));
+  const float4 v4 = __ldg(arec);
   double vproj = __dmul_rn((double)v4.x, (double)__ldg(om));
   vproj = __dadd_rn(vproj, __dmul_rn((double)v4.y, (double)__ldg(om + 1)));
   if (D == 3) vproj = __dadd_rn(vproj, __dmul_rn((double)v4.z, (double)__ldg(om + D - 1)));
@@ -268,7 +271,7 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
   for (int q = 0; q < DEX_NLINES; ++q) {   // not unrolled: the body is ~500 instructions and would be copied 4 times
     const int l = CT.line[q];
     if (l < 0) continue;               // block-uniform
-    const float4 ln = __ldg(M.line + (size_t)cell * M.n_lines + l);
+    const float4 ln = __ldg(arec + 1 + l);
     const double shift = vproj * CT.lam0_over_c[q];
     const float sh_h = (float)shift, sh_l = (float)(shift - (double)sh_h);
     const float es = ln.x * ln.w, cs = ln.y * ln.w;

@@ -22,8 +22,7 @@ struct BuildCtx {
   double thr_eta, thr_chi, tau_gate, h;
   int* fail;                  // [n_batch][n_active][max_level+1]
   float* store;
-  float4* line;
-  float4* vel;
+  float4* aux;                // [n_active][cps][1 + n_lines], dex_aux_vel / dex_aux_line
   float* vtab;
 };
 
@@ -204,14 +203,14 @@ __global__ void gather_aux_kernel(const BuildCtx X, const float* __restrict__ ve
   if (D == 3) s2 = s2 + (double)o.z * (double)o.z;
   o.w = (float)sqrt(s2);
   const size_t dst = (size_t)slot * X.M.cps + cell;
-  X.vel[dst] = o;
+  X.aux[dex_aux_vel(X.M, dst)] = o;
   for (int l = 0; l < X.M.n_lines; ++l) {
     float4 q;
     q.x = es[(size_t)l * nvox + v];
     q.y = cs[(size_t)l * nvox + v];
     q.z = a0[(size_t)l * nvox + v];
     q.w = inv[(size_t)l * nvox + v];
-    X.line[dst * X.M.n_lines + l] = q;
+    X.aux[dex_aux_line(X.M, dst, l)] = q;
   }
 }
 
@@ -232,7 +231,7 @@ __global__ void reduce_aux_kernel(const BuildCtx X, int m) {
   float vm = 0.0f;
 #pragma unroll
   for (int ch = 0; ch < NC; ++ch) {
-    const float4 v = X.vel[base + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc)];
+    const float4 v = X.aux[dex_aux_vel(X.M, base + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc))];
     if (ch == 0) { sx = (double)v.x; sy = (double)v.y; sz = (double)v.z; vm = v.w; }
     else { sx = sx + (double)v.x; sy = sy + (double)v.y; sz = sz + (double)v.z; vm = fmaxf(vm, v.w); }
   }
@@ -241,12 +240,12 @@ __global__ void reduce_aux_kernel(const BuildCtx X, int m) {
   o.y = (float)(sy * (1.0 / NC));
   o.z = (float)(sz * (1.0 / NC));
   o.w = vm;
-  X.vel[base + X.M.lvloff[m] + cell] = o;
+  X.aux[dex_aux_vel(X.M, base + X.M.lvloff[m] + cell)] = o;
   for (int l = 0; l < X.M.n_lines; ++l) {
     double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
 #pragma unroll
     for (int ch = 0; ch < NC; ++ch) {
-      const float4 q = X.line[(base + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc)) * X.M.n_lines + l];
+      const float4 q = X.aux[dex_aux_line(X.M, base + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc), l)];
       if (ch == 0) { s0 = (double)q.x; s1 = (double)q.y; s2 = (double)q.z; s3 = (double)q.w; }
       else { s0 = s0 + (double)q.x; s1 = s1 + (double)q.y; s2 = s2 + (double)q.z; s3 = s3 + (double)q.w; }
     }
@@ -255,7 +254,7 @@ __global__ void reduce_aux_kernel(const BuildCtx X, int m) {
     q.y = (float)(s1 * (1.0 / NC));
     q.z = (float)(s2 * (1.0 / NC));
     q.w = (float)(s3 * (1.0 / NC));
-    X.line[(base + X.M.lvloff[m] + cell) * X.M.n_lines + l] = q;
+    X.aux[dex_aux_line(X.M, base + X.M.lvloff[m] + cell, l)] = q;
   }
 }
 
@@ -267,7 +266,7 @@ __device__ __forceinline__ void line_sum(const BuildCtx& X, size_t cell, int b, 
   for (int q = 0; q < DEX_NLINES; ++q) {
     const int l = X.M.active_lines[b * DEX_NLINES + q];
     if (l < 0) continue;
-    const float4 ln = X.line[cell * X.M.n_lines + l];
+    const float4 ln = X.aux[dex_aux_line(X.M, cell, l)];
     double el, cl;
     dex_line_terms(X.M.wei_c, X.M.wei_L, lam, (double)X.M.lambda0[l], (double)ln.x, (double)ln.y, (double)ln.z,
                    (double)ln.w, vp_per_line ? vp[q] : vp[0], X.M.c_light, el, cl);
@@ -300,7 +299,7 @@ __global__ void cav_test_kernel(const BuildCtx X, int m) {
     const size_t cc = (size_t)slot * X.M.cps + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc);
     const size_t rb = ((size_t)b * X.G.n_active) * X.M.cps + cc;
     const float2 bg = make_float2(X.store[dex_rec_eta(rb, j)], X.store[dex_rec_chi(rb, j)]);
-    const double Vc = (double)X.vel[cc].w;
+    const double Vc = (double)X.aux[dex_aux_vel(X.M, cc)].w;
     double vd[DEX_NLINES];
     for (int q = 0; q < DEX_NLINES; ++q) {
       const int l = X.M.active_lines[b * DEX_NLINES + q];
@@ -332,7 +331,7 @@ __global__ void vtab_level0_kernel(const BuildCtx X) {
   const int slot = (int)(r % X.G.n_active);
   const int b = (int)(r / X.G.n_active);
   const size_t cc = (size_t)slot * X.M.cps + cell;
-  const double V = (double)X.vel[cc].w;
+  const double V = (double)X.aux[dex_aux_vel(X.M, cc)].w;
   const double vk = -V + (2.0 * V) * ((double)k / (double)(n - 1));
   const size_t rb = ((size_t)b * X.G.n_active) * X.M.cps + cc;
   double e, c;
@@ -379,14 +378,14 @@ __global__ void vtab_reduce_kernel(const BuildCtx X, int m) {
   cell_coords<D>(cell, nbm, pc);
   const size_t sbase = (size_t)slot * X.M.cps;
   const size_t bbase = ((size_t)b * X.G.n_active) * X.M.cps;
-  const double Vp = (double)X.vel[sbase + X.M.lvloff[m] + cell].w;
+  const double Vp = (double)X.aux[dex_aux_vel(X.M, sbase + X.M.lvloff[m] + cell)].w;
   const double vk = -Vp + (2.0 * Vp) * ((double)k / (double)(n - 1));
   double se = 0, sc = 0;
 #pragma unroll
   for (int ch = 0; ch < NC; ++ch) {
     const size_t cc = sbase + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc);
     double e, c;
-    vtab_interp(X.vtab + (bbase + cc) * n * DEX_REC, n, j, (double)X.vel[cc].w, vk, e, c);
+    vtab_interp(X.vtab + (bbase + cc) * n * DEX_REC, n, j, (double)X.aux[dex_aux_vel(X.M, cc)].w, vk, e, c);
     if (ch == 0) { se = e; sc = c; } else { se = se + e; sc = sc + c; }
   }
   const size_t ro = (bbase + sbase + X.M.lvloff[m] + cell) * n + k;
@@ -418,7 +417,7 @@ __global__ void vtab_test_kernel(const BuildCtx X, int m) {
 #pragma unroll
   for (int ch = 0; ch < NC; ++ch) {
     const size_t cc = sbase + X.M.lvloff[m - 1] + child_index<D>(pc, ch, nbc);
-    vtab_interp(X.vtab + (bbase + cc) * n * DEX_REC, n, j, (double)X.vel[cc].w, 0.0, e[ch], c[ch]);
+    vtab_interp(X.vtab + (bbase + cc) * n * DEX_REC, n, j, (double)X.aux[dex_aux_vel(X.M, cc)].w, 0.0, e[ch], c[ch]);
   }
   if (!cell_passes<NC>(e, c, X)) X.fail[((size_t)b * X.G.n_active + slot) * (X.M.max_level + 1) + m] = 1;
 }
@@ -487,9 +486,9 @@ __global__ void level_data_kernel(const BuildCtx X, int chain, int m, int width 
     const size_t rec = ((size_t)b * X.G.n_active) * X.M.cps + cc;
     v = X.store[(chain == DEX_CHAIN_CHI) ? dex_rec_chi(rec, j) : dex_rec_eta(rec, j)];
   } else if (chain == DEX_CHAIN_VEL) {                               // width = 4
-    v = reinterpret_cast<const float*>(X.vel)[cc * 4 + q];
+    v = reinterpret_cast<const float*>(X.aux)[dex_aux_vel(X.M, cc) * 4 + q];
   } else if (chain == DEX_CHAIN_LINE) {                              // width = n_lines * 4
-    v = reinterpret_cast<const float*>(X.line)[cc * X.M.n_lines * 4 + q];
+    v = reinterpret_cast<const float*>(X.aux)[dex_aux_line(X.M, cc, 0) * 4 + q];
   } else {                                                           // VTAB: width = n_vbins * n_lambda * 2
     const int f = q & 1;
     const int lam = (q >> 1) % X.M.n_lambda;
@@ -515,8 +514,7 @@ BuildCtx make_ctx(const dex_mips* m) {
   X.h = (double)m->grid->desc.voxel_size;
   X.fail = m->d_fail;
   X.store = m->d_store;
-  X.line = m->d_line;
-  X.vel = m->d_vel;
+  X.aux = m->d_aux;
   X.vtab = m->d_vtab;
   return X;
 }
@@ -708,10 +706,10 @@ __global__ void vbin_report_kernel(const BuildCtx X, int cells0, float factor, u
   const long long slot = i / cells0;
   const int c = (int)(i - slot * cells0);
   const size_t cell = (size_t)slot * X.M.cps + c;        // level 0 starts at lvloff[0] = 0
-  const double V = (double)X.M.vel[cell].w;
+  const double V = (double)X.M.aux[dex_aux_vel(X.M, cell)].w;
   const double spacing = 2.0 * V / (double)(X.M.n_vbins - 1);
   for (int l = 0; l < X.M.n_lines; ++l) {
-    const double invD = (double)X.M.line[cell * X.M.n_lines + l].w;
+    const double invD = (double)X.M.aux[dex_aux_line(X.M, cell, l)].w;
     const double ratio = spacing * invD * (double)X.M.lambda0[l] / X.M.c_light;
     const float rf = (float)ratio;
     atomicMax(out + l, __float_as_uint(rf));
