@@ -367,7 +367,7 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
 // resident blocks per SM asked of the compiler per variant: the ISO march fits 64 registers; the velocity tables
 // want two records in flight, and Core-and-Voigt runs 8 independent fp64 Goertzel chains per line
 #ifndef DEX_MINB_VEL
-#define DEX_MINB_VEL 5
+#define DEX_MINB_VEL 7   // swept 4..8 on C3: 774 / 675 / 665 / 631 / 678 ms (profiles/r01k)
 #endif
 #ifndef DEX_MINB_CAV
 #define DEX_MINB_CAV 4
