@@ -289,6 +289,66 @@ def _line_sum(wl, lam_idx, lines, es, cs, a0, inv, vproj_per_line, bg_eta, bg_ch
     return e, c
 
 
+def velinterp_parent_table(child_tabs, child_V, Vp, n_vbins):
+    """DESIGN.md reading R-vel (the construction of the higher levels is not stated): the parent's
+    velocity grid is uniform on [-Vp, Vp], Vp = max over its children; its bin value is the mean, over the 2^D
+    children in child order, of the CHILD's table linearly interpolated on the CHILD's own grid [-V_child, V_child]
+    at the parent's bin velocity (clamped to the child's range).  child_tabs: 2^D arrays [cells..., n_vbins,
+    n_lambda, 2] fp32; child_V: 2^D arrays [cells...]; Vp: [cells...].  Returns fp32 [cells..., n_vbins, n_lambda, 2]."""
+    n = n_vbins
+    Vp = Vp.astype(np.float64)
+    tab = np.zeros(Vp.shape + (n,) + child_tabs[0].shape[-2:], dtype=np.float32)
+    for k in range(n):
+        vk = -Vp + 2.0 * Vp * (float(k) / float(n - 1))
+        acc = None
+        for cti, cV in zip(child_tabs, child_V):
+            val = _velinterp_at(cti, cV, vk, n)
+            acc = val if acc is None else acc + val
+        acc = acc * (1.0 / len(child_tabs))
+        tab[..., k, :, :] = acc.astype(np.float32)
+    return tab
+
+
+def velinterp_rest_frame(tab, V, n_vbins):
+    """the VLM test of the velocity-interpolation scheme sees "the values for the emissivity and opacity
+    in the rest frame of each voxel (i.e. the centre of the velocity grid, with a velocity of 0)": the cell's table
+    interpolated at v = 0.  Returns (eta, chi) fp64 [cells..., n_lambda]."""
+    z = np.zeros(V.shape, dtype=np.float64)
+    t = _velinterp_at(tab, V, z, n_vbins)
+    return t[..., 0], t[..., 1]
+
+
+def cav_worst_case_shift(lam, lam0, V, c_light):
+    """eq. 17: the Doppler shift v_D in [-V, V] that minimises |lam0 (1 - v/c) - lam|, i.e. that
+    brings the line core as close to wavelength lam as the cell's velocities allow: v_D = clamp(c (1 - lam/lam0), -V, V).
+    lam: [W] fp64, V: [cells...] fp64 (max |v| over the cell's voxels).  Returns [cells..., W] fp64."""
+    want = c_light * (1.0 - lam / float(lam0))
+    return np.clip(want, -V[..., None], V[..., None])
+
+
+def cav_test_fields(wl, M, m):
+    """V6: what the VLM test of the Core-and-Voigt scheme sees in the cells of level m: background
+    plus the sum over the batch's active lines of the line terms (eqs. 10-20) at each cell's worst-case Doppler shift
+    (eq. 17) -- "summing the emissivity and opacity from each line at a Doppler shift of v_D".  Returns (eta, chi) fp64
+    [cells_m..., n_lambda]."""
+    W, nl = wl.lambda_batch, wl.n_lambda
+    te = np.zeros(grid_shape(wl, m) + (nl,), dtype=np.float64)
+    tc = np.zeros_like(te)
+    Vc = M.vmax[m].astype(np.float64)
+    for b in range(wl.n_batch):
+        lines = [int(l) for l in wl.active_lines[b] if l >= 0]
+        idx = np.arange(b * W, (b + 1) * W)
+        lam = wl.lam[idx].astype(np.float64)
+        vd = {}
+        for l in lines:   # eq. 17: Doppler shift closest to the line core reachable in the cell
+            vd[l] = cav_worst_case_shift(lam, wl.lambda0[l], Vc, wl.c_light)     # [cells..., W]
+        ee, cc = _line_sum(wl, idx, lines, M.eta_star[m], M.chi_star[m], M.a0[m], M.inv_dlamD[m], vd,
+                           M.eta[m][..., idx], M.chi[m][..., idx])
+        te[..., idx] = ee
+        tc[..., idx] = cc
+    return te, tc
+
+
 def build_mips(wl, max_level=None, metric=None, thr_eta=None, thr_chi=None, tau_gate=None,
                variant=None) -> OracleMips:
     """Mip chains (V1), per-cell VLM test (V2-V4, V6) and per-brick level per batch (V5, V7).
@@ -358,19 +418,7 @@ def build_mips(wl, max_level=None, metric=None, thr_eta=None, thr_chi=None, tau_
         for m in range(1, max_level + 1):
             # DESIGN.md reading R-vel: parent bin = mean over children of the child's table interpolated
             # at the parent's bin velocity (clamped to the child's grid)
-            Vp = M.vmax[m].astype(np.float64)
-            prev = M.vtab[-1]
-            chs = children(prev, nd)
-            chV = children(M.vmax[m - 1], nd)
-            tab = np.zeros(grid_shape(wl, m) + (n, nl, 2), dtype=np.float32)
-            for k in range(n):
-                vk = -Vp + 2.0 * Vp * (float(k) / float(n - 1))
-                acc = None
-                for cti, cV in zip(chs, chV):
-                    val = _velinterp_at(cti, cV, vk, n)
-                    acc = val if acc is None else acc + val
-                acc = acc * (1.0 / len(chs))
-                tab[..., k, :, :] = acc.astype(np.float32)
+            tab = velinterp_parent_table(children(M.vtab[-1], nd), children(M.vmax[m - 1], nd), M.vmax[m], n)
             M.vtab.append(tab)
 
     # ---- per-cell test (V2-V6) and brick levels (V5) ----
@@ -382,25 +430,9 @@ def build_mips(wl, max_level=None, metric=None, thr_eta=None, thr_chi=None, tau_
         if variant == ISO:
             te, tc = M.eta[m - 1].astype(np.float64), M.chi[m - 1].astype(np.float64)
         elif variant == VELINTERP:
-            z = np.zeros(M.vmax[m - 1].shape, dtype=np.float64)
-            t = _velinterp_at(M.vtab[m - 1], M.vmax[m - 1], z, wl.n_vbins)   # rest frame
-            te, tc = t[..., 0], t[..., 1]
+            te, tc = velinterp_rest_frame(M.vtab[m - 1], M.vmax[m - 1], wl.n_vbins)
         else:
-            te = np.zeros(grid_shape(wl, m - 1) + (nl,), dtype=np.float64)
-            tc = np.zeros_like(te)
-            Vc = M.vmax[m - 1].astype(np.float64)
-            for b in range(nb):
-                lines = [int(l) for l in wl.active_lines[b] if l >= 0]
-                idx = np.arange(b * W, (b + 1) * W)
-                lam = wl.lam[idx].astype(np.float64)
-                vd = {}
-                for l in lines:   # eq. 17: Doppler shift closest to the line core reachable in the cell
-                    want = wl.c_light * (1.0 - lam / float(wl.lambda0[l]))
-                    vd[l] = np.clip(want, -Vc[..., None], Vc[..., None])     # [cells..., W]
-                ee, cc = _line_sum(wl, idx, lines, M.eta_star[m - 1], M.chi_star[m - 1], M.a0[m - 1],
-                                   M.inv_dlamD[m - 1], vd, M.eta[m - 1][..., idx], M.chi[m - 1][..., idx])
-                te[..., idx] = ee
-                tc[..., idx] = cc
+            te, tc = cav_test_fields(wl, M, m - 1)
         ch_e = children(te, nd)
         ch_c = children(tc, nd)
         me = cell_metric(ch_e, metric, h)

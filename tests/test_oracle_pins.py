@@ -826,3 +826,232 @@ def test_t11_direction_fields_and_single_direction_solve():
     s3 = orc.single_direction_workload(wv, 3)
     assert np.array_equal(orc.build_mips(s3, variant=orc.ISO).levels, lv1[3])
     assert np.percentile(np.abs(J1 - JA) / JA, 99) < 0.2
+
+
+# ------------------------------------------------------------------------------------------------
+# P14-P17: the anisotropic VLM tests and the velocity-table pyramid (V6, R-vel).  Every C3 / C4 / C5
+# level table -- hence every timed segment count -- hangs on these three readings.
+# ------------------------------------------------------------------------------------------------
+def _one_line_medium(n, u_kms, vth_kms, speeds_x, chi_star=None, n_vbins=9, max_level=1, thr=1e-2):
+    """Hand-controlled one-line moving medium on an n x n grid (brick 16, all active): uniform line parameters
+    (a = 0.01, thermal width vth_kms), wavelengths at Doppler offsets u_kms from the line centre, velocity (speeds_x, 0)
+    per voxel, no background.  Everything of C3's generated fields is overwritten."""
+    wl = make("C3", n=n, n_dirs=4, n_probes=4, n_lambda=len(u_kms), max_level=max_level, n_vbins=n_vbins)
+    nv = n * n
+    lam0 = 500.0
+    wl.active[:] = 1
+    wl.lam = (lam0 * (1.0 + np.asarray(u_kms, dtype=np.float64) / wl.c_light)).astype(np.float32)
+    wl.lambda0 = np.array([lam0], dtype=np.float32)
+    dlamD = lam0 * vth_kms / wl.c_light
+    cs = np.full(nv, 2.0) if chi_star is None else np.asarray(chi_star, dtype=np.float64).ravel()
+    wl.chi_star0 = (cs * math.sqrt(math.pi) * dlamD).astype(np.float32)[None, :]
+    wl.eta_star0 = (1.5 * wl.chi_star0).astype(np.float32)
+    wl.a0 = np.full((1, nv), 0.01, dtype=np.float32)
+    wl.inv_dlamD = np.full((1, nv), 1.0 / dlamD, dtype=np.float32)
+    wl.eta_bg = np.zeros((nv, len(u_kms)), dtype=np.float32)
+    wl.chi_bg = np.zeros((nv, len(u_kms)), dtype=np.float32)
+    wl.vel = np.zeros((nv, 2), dtype=np.float32)
+    wl.vel[:, 0] = np.asarray(speeds_x, dtype=np.float32).ravel()
+    wl.thr_eta = wl.thr_chi = thr
+    return wl
+
+
+def test_p14_cav_test_quantity_is_the_worst_case_shift_brute_force():
+    """eq. 17: the Core-and-Voigt VLM test sums, per line, the terms "Doppler shifted to the
+    wavelength closest to the line core possible in the current voxel".  Brute force, independent of the oracle's
+    clamp formula: (i) over 401 velocities in [-V, V], |lam0 (1 - v/c) - lam| is never smaller than at the oracle's
+    v_D; (ii) the test quantity of build_mips (cav_test_fields) equals background + sum over the active lines of the
+    MAXIMUM over those velocities of the textbook line term (scipy's Faddeeva function, not HUM1WEI24): the line
+    opacity falls monotonically away from the core, so the closest shift is the strongest one."""
+    from scipy.special import wofz
+    wl = make("C4", n=64, n_dirs=4, n_probes=4)
+    M = orc.build_mips(wl, max_level=2)
+    c = wl.c_light
+    rng = np.random.default_rng(17)
+    n_clamped = n_free = n_pos = n_neg = 0
+    for m in (0, 1, 2):
+        te, tc = orc.cav_test_fields(wl, M, m)
+        shape = orc.grid_shape(wl, m)
+        V = M.vmax[m].astype(np.float64)
+        cells = np.argwhere(M.chi_star[m][0] > 0)
+        pick = cells[rng.choice(len(cells), size=min(60, len(cells)), replace=False)]
+        for (cy, cx) in pick:
+            Vc = float(V[cy, cx])
+            vgrid = np.linspace(-Vc, Vc, 401)
+            for j in rng.choice(wl.n_lambda, size=24, replace=False):
+                b = j // wl.lambda_batch
+                lam = float(wl.lam[j])
+                e_max, c_max = float(M.eta[m][cy, cx, j]), float(M.chi[m][cy, cx, j])
+                lines = [int(q) for q in wl.active_lines[b] if q >= 0]
+                for l in lines:
+                    lam0 = float(wl.lambda0[l])
+                    vD = float(orc.cav_worst_case_shift(np.array([lam]), lam0, np.array([Vc]), c)[0, 0])
+                    assert -Vc <= vD <= Vc
+                    f = np.abs(lam0 * (1.0 - vgrid / c) - lam)
+                    assert abs(lam0 * (1.0 - vD / c) - lam) <= f.min() * (1 + 1e-12) + 1e-12
+                    n_clamped += abs(vD) == Vc
+                    n_free += abs(vD) < Vc
+                    n_pos += vD > 0
+                    n_neg += vD < 0
+                    inv = float(M.inv_dlamD[m][l][cy, cx])
+                    x = (lam - lam0 + vgrid / c * lam0) * inv
+                    a = (lam / lam0) ** 2 * float(M.a0[m][l][cy, cx])
+                    phi = wofz(x + 1j * a).real * inv / math.sqrt(math.pi)
+                    e_max += lam0 / lam * float(M.eta_star[m][l][cy, cx]) * phi.max()
+                    c_max += lam0 / lam * float(M.chi_star[m][l][cy, cx]) * phi.max()
+                # the grid maximum can only fall short of the true one by the grid spacing: (dx/2)^2 with dx the step
+                # in Doppler widths; HUM1WEI24 against wofz: 3e-6 in the far wings (P13)
+                dx = max([(2.0 * Vc / 400.0) / c * float(wl.lambda0[l]) * float(M.inv_dlamD[m][l][cy, cx]) for l in lines] + [0.0])
+                slack = 3e-6 + 0.3 * dx * dx
+                assert c_max * (1 - 3e-6) <= tc[cy, cx, j] <= c_max * (1 + slack), (m, cy, cx, j)
+                assert e_max * (1 - 3e-6) <= te[cy, cx, j] <= e_max * (1 + slack), (m, cy, cx, j)
+    assert min(n_clamped, n_free, n_pos, n_neg) > 50        # both regimes and both signs were exercised
+
+
+def test_p14_cav_level_decision_hand_example():
+    """eq. 17 on a hand example: one line, thermal width 10 km/s, eight wavelengths 0.25 .. 2 km/s redward of the
+    core; columns alternate |v| = 1 and 2 km/s, so every level-1 cell has children (1, 2, 1, 2) km/s.  Shifted TOWARDS
+    the core the reddest wavelength sits at x = (2 - 1)/10 = 0.1 in the slow children and at x = 0 in the fast ones:
+    H = e^-0.01 against 1, relative variance (0.005 / 0.995)^2 = 2.5e-5.  (Shifted AWAY from the core it would be
+    x = 0.3 against 0.4: 1.2e-3.)  So the brick coarsens at a threshold of 2e-4 and does not at 1e-5."""
+    n = 16
+    u = 0.25 * np.arange(1, 9)
+    speeds = np.where(np.arange(n)[None, :] % 2 == 0, 1.0, 2.0) * np.ones((n, 1))
+    wl = _one_line_medium(n, u, 10.0, speeds)
+    assert (orc.build_mips(wl, variant=orc.CAV, thr_eta=2e-4, thr_chi=2e-4).levels == 1).all()
+    assert (orc.build_mips(wl, variant=orc.CAV, thr_eta=1e-5, thr_chi=1e-5).levels == 0).all()
+    # the same blueward of the core (the other sign of v_D)
+    wl = _one_line_medium(n, -u, 10.0, speeds)
+    assert (orc.build_mips(wl, variant=orc.CAV, thr_eta=2e-4, thr_chi=2e-4).levels == 1).all()
+    assert (orc.build_mips(wl, variant=orc.CAV, thr_eta=1e-5, thr_chi=1e-5).levels == 0).all()
+    # every wavelength within reach of every child's velocity range: all children are tested AT the core, where a
+    # medium with uniform line parameters is uniform -- coarsens at any positive threshold
+    wl = _one_line_medium(n, u, 10.0, speeds * 3.0)
+    assert (orc.build_mips(wl, variant=orc.CAV, thr_eta=1e-9, thr_chi=1e-9).levels == 1).all()
+
+
+def test_p15_max_speed_chain_hand_example():
+    """PAPER.md:196 / :311: the velocity range of a MIP N voxel is taken "over the set of voxels MIP 0 contained
+    within" it: max |v| of the children, level by level.  4 x 4 typed-in speeds (3-4-5 triangles)."""
+    a = np.array([[1, 5, 2, 2], [3, 4, 2, 9], [7, 1, 1, 1], [0, 6, 1, 8]], dtype=np.float32)
+    assert np.array_equal(orc.mip_max(a, 2), np.array([[5, 9], [7, 8]], dtype=np.float32))
+    assert np.array_equal(orc.mip_max(orc.mip_max(a, 2), 2), np.array([[9]], dtype=np.float32))
+    a3 = np.zeros((2, 2, 2), dtype=np.float32)
+    a3[1, 0, 1] = 4.0
+    a3[0, 1, 0] = 2.5
+    assert np.array_equal(orc.mip_max(a3, 3), np.array([[[4.0]]], dtype=np.float32))
+    # through build_mips: speeds are the Euclidean norm of the velocity, (3, 4) -> 5
+    n = 16
+    wl = _one_line_medium(n, np.linspace(-20, 20, 8), 10.0, np.zeros((n, n)), max_level=2)
+    vx = np.zeros((n, n))
+    vy = np.zeros((n, n))
+    vx[5, 6], vy[5, 6] = 3.0, -4.0
+    vx[0, 0] = -2.0
+    wl.vel[:, 0], wl.vel[:, 1] = vx.ravel(), vy.ravel()
+    M = orc.build_mips(wl, variant=orc.CAV)
+    assert M.vmax[0][5, 6] == 5.0 and M.vmax[1][2, 3] == 5.0 and M.vmax[2][1, 1] == 5.0
+    assert M.vmax[1][0, 0] == 2.0 and M.vmax[2][0, 0] == 2.0
+    assert M.vmax[1].sum() == 7.0 and M.vmax[2].sum() == 7.0          # and nothing anywhere else
+    # the box-filtered velocity (what the ray projects) is the mean, not the max
+    assert M.vbar[1][2, 3, 0] == 0.75 and M.vbar[1][2, 3, 1] == -1.0 and M.vbar[2][1, 1, 0] == 0.1875
+
+
+def test_p16_velocity_table_pyramid():
+    """R-vel (the higher levels are not spelled out).  (i) Hand example: five bins, children
+    A (V = 10, nodes -10 -5 0 5 10) and B (V = 20, nodes -20 .. 20), twice each; the parent spans [-20, 20] and each
+    child is read ON ITS OWN grid, clamped: at v = -10 child A gives its first node, not its second.  (ii) Children
+    with equal V and equal tables reproduce themselves bit for bit.  (iii) On a generated atmosphere every parent
+    table equals the mean of numpy.interp over explicit child grids (a library routine, clamping at the ends).
+    (iv) A static medium (v = 0) with mips on: level tables and intensities of the velocity-interpolation build equal
+    those of the ISO build of the rest-frame fields."""
+    A = np.array([1.0, 2.0, 4.0, 8.0, 16.0], dtype=np.float32)
+    B = np.array([32.0, 64.0, 128.0, 256.0, 512.0], dtype=np.float32)
+
+    def tab(vals):                       # one cell, 5 bins, 1 wavelength, (eta, chi) = (vals, 3 vals)
+        return np.stack([vals, 3 * vals], axis=-1).reshape(1, 5, 1, 2).astype(np.float32)
+
+    V = lambda v: np.array([v], dtype=np.float32)
+    parent = orc.velinterp_parent_table([tab(A), tab(B), tab(A), tab(B)], [V(10), V(20), V(10), V(20)], V(20), 5)
+    # parent bins -20 -10 0 10 20: A -> 1 1 4 16 16 (clamped outside its +-10), B -> its own nodes
+    want = (np.array([1, 1, 4, 16, 16]) + np.array([32, 64, 128, 256, 512])) / 2.0
+    assert np.array_equal(parent[0, :, 0, 0], want.astype(np.float32))
+    assert np.array_equal(parent[0, :, 0, 1], (3 * want).astype(np.float32))
+    # between nodes: child A (V = 10) at parent bins of V = 16: -16 -8 0 8 16 -> 1, 1.4, 4, 12.8, 16
+    parent = orc.velinterp_parent_table([tab(A)] * 4, [V(10)] * 4, V(16), 5)
+    assert np.allclose(parent[0, :, 0, 0], [1.0, 1.4, 4.0, 12.8, 16.0], rtol=1e-7)
+    # (ii)
+    same = orc.velinterp_parent_table([tab(B)] * 4, [V(20)] * 4, V(20), 5)
+    assert np.array_equal(same, tab(B))
+    wl = make("C3", n=64, n_dirs=4, n_probes=30, max_level=3)
+    for name in ("eta_bg", "chi_bg", "vel"):
+        a = getattr(wl, name).reshape(64, 64, -1)
+        setattr(wl, name, np.ascontiguousarray(np.repeat(np.repeat(a[::2, ::2], 2, axis=0), 2, axis=1).reshape(64 * 64, -1)))
+    for name in ("eta_star0", "chi_star0", "a0", "inv_dlamD"):
+        a = getattr(wl, name).reshape(1, 64, 64)
+        setattr(wl, name, np.ascontiguousarray(np.repeat(np.repeat(a[:, ::2, ::2], 2, axis=1), 2, axis=2).reshape(1, -1)))
+    M2 = orc.build_mips(wl)
+    assert np.array_equal(M2.vtab[1], M2.vtab[0][::2, ::2]) and np.array_equal(M2.vmax[1], M2.vmax[0][::2, ::2])
+    # (iii)
+    wl = make("C3", n=64, n_dirs=4, n_probes=30, max_level=3)
+    M = orc.build_mips(wl)
+    nb = wl.n_vbins
+    rng = np.random.default_rng(23)
+    differs = 0
+    for m in (1, 2, 3):
+        ny, nx = orc.grid_shape(wl, m)
+        for _ in range(40):
+            cy, cx = int(rng.integers(ny)), int(rng.integers(nx))
+            Vp = float(M.vmax[m][cy, cx])
+            if Vp == 0.0:
+                continue
+            vk = np.linspace(-Vp, Vp, nb)
+            kids = [(2 * cy + dy, 2 * cx + dx) for dy in (0, 1) for dx in (0, 1)]
+            assert Vp == max(float(M.vmax[m - 1][k]) for k in kids)
+            for j in rng.choice(wl.n_lambda, size=5, replace=False):
+                for q in (0, 1):
+                    acc = np.zeros(nb)
+                    for k in kids:
+                        Vc = float(M.vmax[m - 1][k])
+                        vals = M.vtab[m - 1][k][:, j, q].astype(np.float64)
+                        acc += np.interp(vk, np.linspace(-Vc, Vc, nb), vals) if Vc > 0 else vals[0]
+                        differs += Vc < 0.9 * Vp
+                    assert np.allclose(M.vtab[m][cy, cx, :, j, q], acc / 4.0, rtol=3e-7, atol=0)
+    assert differs > 100                                      # children whose range is well inside the parent's
+    # (iv)
+    ws = make("C3", n=64, n_dirs=6, n_probes=40, max_level=3)
+    ws.vel[:] = 0.0
+    ws.thr_eta = ws.thr_chi = 0.2                               # a mix of levels 1 and 2 on this 64^2 atmosphere
+    Mv = orc.build_mips(ws)
+    assert Mv.levels.max() >= 2 and (Mv.levels == 1).any()
+    rest = Mv.vtab[0][:, :, 0]                                  # [ny][nx][lambda][2]: every bin holds the static value
+    assert all(np.array_equal(Mv.vtab[0][:, :, k], rest) for k in range(ws.n_vbins))
+    iso = iso_workload((64, 64), ws.brick, rest[..., 0], rest[..., 1], ws.probe_pos, ws.dirs, active=ws.active,
+                       max_level=3, thr=0.2)
+    Mi = orc.build_mips(iso)
+    assert np.array_equal(Mi.levels, Mv.levels)
+    a, b = orc.hdda_march(ws, Mv, capture_batch=0), orc.hdda_march(iso, Mi, capture_batch=0)
+    assert np.array_equal(a.records, b.records) and max_rel(a.I, b.I) < 1e-14
+
+
+def test_p17_velinterp_tests_the_rest_frame():
+    """the level test of the velocity-interpolation scheme is "computed ... using the values ... in the
+    rest frame of each voxel (i.e. the centre of the velocity grid, with a velocity of 0)".  A medium whose line
+    parameters are uniform but whose speeds differ from voxel to voxel is uniform at rest and varies in every shifted
+    bin: it must coarsen fully.  The converse -- uniform speeds, line strength varying 1 : 3 inside every level-1
+    cell -- must not coarsen.  (Nine bins: the centre node is v = 0 exactly.)"""
+    n = 16
+    u = np.linspace(-20.0, 20.0, 8)
+    rng = np.random.default_rng(4)
+    speeds = rng.uniform(2.0, 25.0, size=(n, n))
+    wl = _one_line_medium(n, u, 10.0, speeds, n_vbins=9, max_level=4)
+    M = orc.build_mips(wl, variant=orc.VELINTERP)
+    assert (M.levels == 4).all()
+    last = M.vtab[0][:, :, -1, :, 1]                           # the shifted bins do vary (by far more than 1e-2)
+    assert (last.std(axis=(0, 1)) / last.mean(axis=(0, 1))).max() > 0.1
+    e0, c0 = orc.velinterp_rest_frame(M.vtab[0], M.vmax[0], 9)
+    assert (c0 == c0[0, 0]).all() and (e0 == e0[0, 0]).all()
+    cs = np.where(np.arange(n)[:, None] % 2 == 0, 1.0, 3.0) * np.ones((1, n))
+    wl = _one_line_medium(n, u, 10.0, np.full((n, n), 7.0), chi_star=cs, n_vbins=9, max_level=4, thr=0.2)
+    assert (orc.build_mips(wl, variant=orc.VELINTERP).levels == 0).all()        # relvar of (1,1,3,3) is 0.25 > 0.2
+    wl.thr_eta = wl.thr_chi = 0.26
+    assert (orc.build_mips(wl, variant=orc.VELINTERP).levels >= 1).all()
