@@ -289,6 +289,14 @@ dex_status dex_march_work_read(int64_t* line_segments, int reset);
 /* Kernel configuration knob: lanes that share one ray, 1/2/4/8, or 0 (default) = automatic: one thread per ray unless
  * there are fewer probes than one wave of blocks (148 SMs x 128 threads), where 8 lanes per ray fill the machine better. */
 dex_status dex_set_lanes_per_ray(int lanes);
+/* The lanes-per-ray mapping a march over `n_probes` probes will take under the current setting (the automatic rule
+ * depends on the probe count only); bench.py reports it instead of restating the rule. */
+dex_status dex_get_lanes_per_ray(int64_t n_probes, int* lanes);
+/* MEASURED fp32 arithmetic peak of the current device in TFLOP/s (an FMA counts 2 flops): register-resident chains of
+ * scalar FFMA (*tflops_ffma) and of the packed two-wide FFMA2 the march's integrators use (*tflops_ffma2), ~15 ms in all,
+ * timed with CUDA events on `stream`.  The denominator of the "alu" roofline of the Core-and-Voigt / Classic march
+ * (SURVEY.md 8(d) caveat 2).  Either pointer may be NULL.  Synchronises. */
+dex_status dex_measure_fp32_peak(double* tflops_ffma, double* tflops_ffma2, void* stream);
 /* Kernel-structure knobs for performance experiments (results do not change): "lanes_per_ray" 0/1/2/4/8;
  * "tile_probes" 0/1 (1, default: probes are handed to warps in compact spatial tiles by an internal counting
  * sort instead of in the caller's order); "voigt_fp32" 0/1 (1, default: the Core-and-Voigt march evaluates H(a, x) in

@@ -15,6 +15,7 @@ SOURCES = {
     "grid_build.cu": [],
     "mips_build.cu": ["-fmad=false"],
     "march.cu": [],
+    "peaks.cu": [],
 }
 
 

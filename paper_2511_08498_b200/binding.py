@@ -30,7 +30,7 @@ EXPORTS = (
     "dex_mips_get_packed_levels", "dex_mips_get_level_data", "dex_destroy_mips", "dex_formal_solution",
     "dex_mean_intensity", "dex_mean_intensity_host", "dex_mean_intensity_pipelined", "dex_pool_high_water", "dex_direction_fields",
     "dex_mean_intensity_single_direction", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read", "dex_march_work_read",
-    "dex_set_lanes_per_ray", "dex_set_tuning",
+    "dex_set_lanes_per_ray", "dex_get_lanes_per_ray", "dex_measure_fp32_peak", "dex_set_tuning",
 )
 
 
@@ -110,6 +110,8 @@ def _load():
     L.dex_march_work_read.argtypes = [C.POINTER(C.c_int64), C.c_int]
     L.dex_set_lanes_per_ray.argtypes = [C.c_int]
     L.dex_set_tuning.argtypes = [C.c_char_p, C.c_int]
+    L.dex_get_lanes_per_ray.argtypes = [C.c_int64, C.POINTER(C.c_int)]
+    L.dex_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]
     return L
 
 
@@ -151,6 +153,19 @@ def dex_launch_count() -> int:
 
 def dex_set_lanes_per_ray(lanes: int):
     _check(_L.dex_set_lanes_per_ray(int(lanes)))
+
+
+def dex_get_lanes_per_ray(n_probes: int) -> int:
+    v = C.c_int(0)
+    _check(_L.dex_get_lanes_per_ray(int(n_probes), C.byref(v)))
+    return v.value
+
+
+def dex_measure_fp32_peak(stream=None):
+    """(TFLOP/s of scalar FFMA chains, TFLOP/s of packed FFMA2 chains), measured on the current device."""
+    a, b = C.c_double(0), C.c_double(0)
+    _check(_L.dex_measure_fp32_peak(C.byref(a), C.byref(b), _stream(stream)))
+    return a.value, b.value
 
 
 def dex_set_tuning(name: str, value: int):

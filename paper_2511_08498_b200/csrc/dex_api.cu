@@ -227,6 +227,12 @@ dex_status dex_set_lanes_per_ray(int lanes) {
   return DEX_OK;
 }
 
+dex_status dex_get_lanes_per_ray(int64_t n_probes, int* lanes) {
+  if (!lanes) { dex_set_error("NULL lanes"); return DEX_ERR_INVALID_ARG; }
+  *lanes = lanes_for((long long)n_probes);
+  return DEX_OK;
+}
+
 dex_status dex_set_tuning(const char* name, int value) {
   if (!name) { dex_set_error("NULL tuning name"); return DEX_ERR_INVALID_ARG; }
   if (!strcmp(name, "lanes_per_ray")) return dex_set_lanes_per_ray(value);

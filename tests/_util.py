@@ -3,7 +3,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from workloads.gen import Workload, VARIANT_ISO, METRIC_RELVAR
+from workloads.gen import Workload, VARIANT_ISO, METRIC_RELVAR, batch_workload  # noqa: F401
 
 
 def iso_workload(dims, brick, eta, chi, probes, dirs, active=None, weights=None, max_level=0,
@@ -139,3 +139,4 @@ def crop_brick_ids(wl, lo, size):
             for bx in range(lo[0] // b, (lo[0] + size[0]) // b):
                 ids.append((bz * bd[1] + by) * bd[0] + bx)
     return np.asarray(ids, dtype=np.int64)
+

@@ -15,7 +15,7 @@ torch = pytest.importorskip("torch")
 from oracle import oracle as orc           # noqa: E402
 from workloads import make                 # noqa: E402
 from workloads.gen import dirs_2d          # noqa: E402
-from _util import (crop_brick_ids, crop_workload, fig5_levels, iso_workload, max_rel, random_unit_dirs,   # noqa: E402
+from _util import (batch_workload, crop_brick_ids, crop_workload, fig5_levels, iso_workload, max_rel, random_unit_dirs,   # noqa: E402
                    unit_dirs_2d)
 
 TOL = 1e-5
@@ -398,36 +398,75 @@ def test_full_size_build_on_crops(P, name, side):
             vel = full[(P.DEX_CHAIN_VEL, m)][sl]
             assert np.array_equal(vel[mask][:, :nd].view(np.uint32), np.ascontiguousarray(Mc.vbar[m])[mask].view(np.uint32))
             assert np.array_equal(vel[mask][:, 3].view(np.uint32), np.ascontiguousarray(Mc.vmax[m])[mask].view(np.uint32))
+            # the four mip chains per line: bit-exact
+            if (P.DEX_CHAIN_LINE, m) not in full:
+                full[(P.DEX_CHAIN_LINE, m)] = mips.level_data(P.DEX_CHAIN_LINE, m)
+            line = full[(P.DEX_CHAIN_LINE, m)][sl]
+            for l in range(wl.n_lines):
+                for q, ref in enumerate((Mc.eta_star, Mc.chi_star, Mc.a0, Mc.inv_dlamD)):
+                    assert np.array_equal(line[mask][:, l, q].view(np.uint32),
+                                          np.ascontiguousarray(ref[m][l])[mask].view(np.uint32)), f"{name}: line chain {q}"
+            # the velocity tables the C3 march reads (4 GB at level 0), every batch, every level: 2e-6 (DESIGN tolerances)
+            if wl.variant == orc.VELINTERP:
+                tab = mips.level_data(P.DEX_CHAIN_VTAB, m)[sl]
+                assert max_rel(tab[mask], Mc.vtab[m][mask]) <= 2e-6, f"{name}: vtab level {m}"
+                del tab
     hist = [int((lv == m).sum()) for m in range(-1, wl.max_level + 1)]
     assert sum(hist) == lv.size          # Table-2 style histogram covers every (batch, brick)
 
 
+# wavelength batches whose oracle pyramid is built over the WHOLE grid (numpy, 3-26 s each): C3 far wing + line core;
+# C4 core of the blended pair (two active lines), core of the 600 nm line (one), continuum (none); C5 line core
+FULL_SIZE_BATCHES = {"C3": (0, 4), "C4": (3, 20, 25), "C5": (1,)}
+
+
 @pytest.mark.parametrize("name", ["C3", "C4", "C5"])
 def test_full_size_march_sampled(P, name):
-    """BASELINE-size grids (configs[2..4]): (i) Classic (level 0, per-voxel velocity) I and J of seeded probes
-    against the oracle's plain AW87 march over the dense arrays -- needs no oracle mip build; (ii) the fused VLM march
-    over ALL probes (the launch configuration bench.py times) against the materialised-I path on the sampled probes.
-    C4 (45 s for all probes x 128 directions x 208 wavelengths) runs (ii) on a seeded 1/16 of its probes and (i) on 6."""
+    """BASELINE-size grids (configs[2..4]), the workload's own VLM variant, the launch bench.py times (fused J over all
+    probes) against the ORACLE: for the batches of FULL_SIZE_BATCHES the oracle pyramid is built over the whole grid
+    (batches are independent, batch_workload) -- level table and packed words exact over the whole grid, every mip
+    chain of the batch bit-exact over the whole grid (velocity tables 2e-6), visit lists and path lengths bit-exact on
+    32 seeded probes x all directions, I of those rays and J of those probes (from the all-probe fused launch) within
+    1e-5.  Then (ii) the Classic (level 0, per-voxel velocity) march against the oracle's plain AW87 march."""
     wl = make(name)
-    if name == "C4":
-        keep = np.sort(np.random.default_rng(41).choice(wl.probe_pos.shape[0], size=65536, replace=False))
-        wl.probe_pos = np.ascontiguousarray(wl.probe_pos[keep])
     dw, grid, mips = _build(P, wl)
     all_probes = wl.probe_pos
     seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
     J_all = P.pipeline.mean_intensity(dw, grid, mips, segment_count=seg).cpu().numpy()
     assert int(seg.item()) > 0 and np.isfinite(J_all).all() and (J_all >= 0).all()
+    lv = mips.levels()
+    act = orc.brick_active(wl)
     rng = np.random.default_rng(31)
-    idx = np.sort(rng.choice(all_probes.shape[0], size=96, replace=False))
+    idx = np.sort(rng.choice(all_probes.shape[0], size=32, replace=False))
     wl.probe_pos = np.ascontiguousarray(all_probes[idx])
     dw.t["probe_pos"] = torch.from_numpy(wl.probe_pos).cuda()
-    P.dex_set_lanes_per_ray(8)
-    I, _ = P.pipeline.formal_solution(dw, grid, mips)
-    P.dex_set_lanes_per_ray(1)
-    J2 = torch.empty((idx.size, wl.n_lambda), dtype=torch.float32, device="cuda:0")
-    P.dex_mean_intensity(grid, mips, P.pipeline.rays(dw), J2, I)
-    assert max_rel(J_all[idx], J2.cpu().numpy().astype(np.float64)) <= 2e-6
-    # (i) exact side at full size against the oracle
+    I = P.pipeline.formal_solution(dw, grid, mips)[0].cpu().numpy()
+    chains = {}
+    for b in FULL_SIZE_BATCHES[name]:
+        sub, lam_idx = batch_workload(wl, [b])
+        Mb = orc.build_mips(sub)
+        assert np.array_equal(lv[b], Mb.levels[0]), f"{name} batch {b}: {(lv[b] != Mb.levels[0]).sum()} brick levels differ"
+        assert np.array_equal(mips.packed_levels(b), orc.pack_levels(Mb.levels[0], Mb.max_level))
+        for m in range(Mb.max_level + 1):
+            mask = _active_cell_mask(wl, act, m)
+            for chain, ref in ((P.DEX_CHAIN_ETA, Mb.eta[m]), (P.DEX_CHAIN_CHI, Mb.chi[m])):
+                if (chain, m) not in chains:
+                    chains[(chain, m)] = mips.level_data(chain, m)
+                got = np.ascontiguousarray(chains[(chain, m)][..., lam_idx])
+                assert np.array_equal(got[mask].view(np.uint32), np.ascontiguousarray(ref)[mask].view(np.uint32))
+            if wl.variant == orc.VELINTERP:
+                tab = mips.level_data(P.DEX_CHAIN_VTAB, m)[mask][:, :, lam_idx]
+                assert max_rel(tab, Mb.vtab[m][mask]) <= 2e-6, f"{name} batch {b}: vtab level {m}"
+                del tab
+        ref = orc.hdda_march(sub, Mb, capture_batch=0)
+        _, cap = P.pipeline.formal_solution(dw, grid, mips, capture_batch=b, want_I=False)
+        _check_lists(cap, ref, cap.room)
+        del cap
+        assert ref.segments > 0 and ref.counts.max() > 64        # long rays through several levels
+        assert max_rel(I[:, :, lam_idx], ref.I) <= TOL, f"{name} batch {b}: I"
+        assert max_rel(J_all[idx][:, lam_idx], orc.mean_intensity(ref.I, wl.weights)) <= TOL, f"{name} batch {b}: J"
+    chains.clear()
+    # (ii) exact side at full size against the oracle
     wl.probe_pos = np.ascontiguousarray(wl.probe_pos[:6 if name == "C4" else 24])
     dw.t["probe_pos"] = torch.from_numpy(wl.probe_pos).cuda()
     A = orc.plain_march(wl, variant=orc.CLASSIC)

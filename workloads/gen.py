@@ -500,3 +500,27 @@ def make(name: str, n: Optional[int] = None, n_dirs: Optional[int] = None,
     if n_probes is not None:
         wl.probe_pos = sample_probes(wl.probe_pos, int(n_probes), seed + 17)
     return wl
+
+
+def batch_workload(wl, batches):
+    """The same atmosphere and rays restricted to the wavelength batches `batches` (a list of batch indices): pure
+    column selection, returns (workload, wavelength indices).  Batches are independent (one level table per batch,
+    PAPER.md:351; pinned by test_batches_are_independent_in_the_oracle), so the oracle's pyramid, level table, lists, I
+    and J of the restricted workload are those columns / rows of the full one: this is how the BASELINE-size configs
+    are compared with (and bench.py's cpu_baseline is timed on) the oracle without a numpy build of every batch."""
+    import copy
+    W = wl.lambda_batch
+    idx = np.concatenate([np.arange(b * W, (b + 1) * W) for b in batches])
+    out = copy.copy(wl)
+    out.n_lambda = int(idx.size)
+    for name in ("eta", "chi", "eta_bg", "chi_bg"):
+        a = getattr(wl, name)
+        if a is not None:
+            setattr(out, name, np.ascontiguousarray(a[:, idx]))
+    if wl.lam is not None:
+        out.lam = np.ascontiguousarray(wl.lam[idx])
+    if wl.active_lines is not None:
+        out.active_lines = np.ascontiguousarray(wl.active_lines[list(batches)])
+    if wl.i0 is not None:
+        out.i0 = np.ascontiguousarray(wl.i0[:, idx])
+    return out, idx
