@@ -195,19 +195,19 @@ def cpu_baseline(wl, n_probes, target_s=10.0, one_thread_s=4.0):
     from workloads.gen import sample_probes
     sub, which = oracle_sample(wl)
     M = orc.build_mips(sub)
+    cores = orc.max_threads()     # asked for explicitly below: a one-thread march leaves OpenMP at one thread
     total = wl.probe_pos.shape[0]
     n_probes = min(n_probes, total)
     best, segs, pp = None, 0, None
     for attempt in range(3):      # a pilot sample sizes the timed one
         pp = sample_probes(wl.probe_pos, n_probes, 4242)
         t0 = time.perf_counter()
-        res = orc.hdda_march(sub, M, probe_pos=pp)
+        res = orc.hdda_march(sub, M, probe_pos=pp, n_threads=cores)
         best = time.perf_counter() - t0
         segs = res.segments
         if best >= 0.6 * target_s or n_probes >= total:
             break
         n_probes = min(total, max(n_probes + 1, int(n_probes * target_s / max(best, 1e-3))))
-    cores = orc.max_threads()
     out = {
         "value": segs * wl.lambda_batch / best, "unit": UNIT, "cores": cores, "kind": "oracle",
         "sample": f"{pp.shape[0]} seeded probes x {wl.dirs.shape[0]} directions x {which} of the same workload "
@@ -489,6 +489,40 @@ class Bench:
                              "out: H2D + grid build + mips build + fused march + D2H inside), max over ranks"}
             del pinned, J_host
 
+        # Core-and-Voigt in 2D (C4): the alternative the paper itself names for many rays per voxel and direction --
+        # single-direction VLM (dex_mean_intensity_single_direction): per direction the Classic fields over
+        # the grid, an ISO pyramid of their own, a one-direction ISO march.  Same rays, same J; timed beside the scheme
+        # the config prescribes.
+        alt = None
+        if wl.variant == 2 and wl.ndim == 2 and args.pipeline == 0 and not (args.shard == "probes" and self.world > 1):
+            J2 = torch.empty_like(J)
+            seg2 = torch.zeros(1, dtype=torch.int64, device=self.dev)
+            grid = P.pipeline.build_grid(dw)
+            if warmup > 1:
+                P.pipeline.mean_intensity_single_direction(dw, grid, J=J2)
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            n_alt = 1 if name in STEP_CAPS and name != args.workload else max(1, min(steps, 3))
+            a.record(stream)
+            for _ in range(n_alt):
+                P.pipeline.mean_intensity_single_direction(dw, grid, J=J2, segment_count=seg2)
+            b.record(stream)
+            torch.cuda.synchronize()
+            ms_alt = a.elapsed_time(b) / n_alt
+            d = ((J2 - J).abs() / J.abs().clamp_min(1e-30)).flatten()
+            k = max(1, int(round(0.999 * d.numel())))
+            p999 = float(torch.kthvalue(d[: 1 << 26] if d.numel() > (1 << 26) else d, min(k, 1 << 26) if d.numel() > (1 << 26)
+                                        else k).values.item()) if d.numel() else 0.0
+            alt = {"path": "single-direction VLM (PAPER.md:396): dex_mean_intensity_single_direction, everything inside "
+                           "(per-direction Classic fields, ISO mips, one-direction ISO march, J accumulated)",
+                   "ms_per_step": ms_alt, "steps": n_alt, "segments_per_step": int(seg2.item()) // n_alt,
+                   "value": int(seg2.item()) / n_alt * W / (ms_alt * 1e-3), "unit": UNIT,
+                   "p999_rel_diff_of_J_vs_core_and_voigt": p999,
+                   "note": "both are approximations of the Classic (level-0, per-voxel velocity) solve; their p99.9 errors "
+                           "against it are in profiles/ (accuracy report)"}
+            grid.destroy()
+            del J2, d
+
         out = None
         if self.rank == 0:
             march_avg_ms = march_ms / max(1, march_n)
@@ -506,6 +540,8 @@ class Bench:
             }
             if shard_check:
                 out["shard_check"] = shard_check
+            if alt:
+                out["alt_single_direction"] = alt
             if want_cpu and self.world == 1:
                 ncpu = args.cpu_probes or CPU_PROBES[wl.name]
                 out["cpu_baseline"] = cpu_baseline(wl, ncpu, cpu_target_s, one_thread_s)

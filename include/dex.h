@@ -156,6 +156,9 @@ typedef enum {
 } dex_chain;
 /* Canonical dense level-m array of a chain (cells of empty bricks are 0). */
 dex_status dex_mips_get_level_data(const dex_mips* mips, int chain, int level, float* h_dense);
+/* Releases the handle's device memory with a stream-ordered free on the stream the handle was BUILT on.  Work that
+ * uses the handle on another stream must be ordered before the destroy by the caller (event / synchronise): the pool
+ * may hand the memory to the next allocation on the build stream at once.  The same holds for dex_destroy_grid. */
 void dex_destroy_mips(dex_mips* mips);
 
 /* ------------------------------------------------------------------------------------------
@@ -275,9 +278,13 @@ dex_status dex_mean_intensity_host(const dex_grid_desc* desc, const uint8_t* h_a
 /* Number of kernel launches this library has enqueued since load (bench.py's gpu_launches). */
 int64_t dex_launch_count(void);
 /* High-water mark (bytes) of the device memory this library's handles and temporaries have held at once since the last
- * reset (all of it comes from the device's default stream-ordered pool; a caller that uses that pool too is counted
- * with it).  Synchronises.  bench.py reports it to show what the rebuild pipeline keeps resident. */
+ * reset.  All of it comes from a stream-ordered pool of the library's own (one per device, created at first use), which
+ * keeps freed memory for the next build instead of returning it to the driver; the device's default pool and other
+ * allocators are not touched.  Synchronises.  bench.py reports it to show what the rebuild pipeline keeps resident. */
 dex_status dex_pool_high_water(int64_t* bytes_in_use_high, int reset);
+/* Return the pool's unused memory to the driver (e.g. before another allocator in the process needs the GBs that C3's
+ * velocity tables held); *bytes_reserved_after (may be NULL) = what the pool still holds for live handles.  Synchronises. */
+dex_status dex_trim(int64_t* bytes_reserved_after);
 /* Device time (ms) and launch count of the march kernels since the last reset, measured with CUDA
  * events on the launching stream when timing is enabled (bench.py roofline leg).  Synchronises. */
 void dex_march_timing_enable(int on);
@@ -301,7 +308,9 @@ dex_status dex_measure_fp32_peak(double* tflops_ffma, double* tflops_ffma2, void
  * "tile_probes" 0/1 (1, default: probes are handed to warps in compact spatial tiles by an internal counting
  * sort instead of in the caller's order); "voigt_fp32" 0/1 (1, default: the Core-and-Voigt march evaluates H(a, x) in
  * its fp32 table form inside the damping window of csrc/dex_voigt.cuh; 0: the fp64 form everywhere -- results agree
- * to ~1e-6). */
+ * to ~1e-6); "dir_split" -1 (default: automatic), 0, n: a fused-J march over fewer probes than one wave of blocks is
+ * launched as one block per (probe tile, batch, n directions) into a temporary I and summed by the reduction kernel in
+ * the fused kernel's order (bit-identical J); 0 never, n > 0 always. */
 dex_status dex_set_tuning(const char* name, int value);
 
 #ifdef __cplusplus

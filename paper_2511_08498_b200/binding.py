@@ -28,7 +28,7 @@ EXPORTS = (
     "dex_last_error", "dex_version", "dex_build_sparse_grid", "dex_grid_info", "dex_grid_get_slots",
     "dex_destroy_grid", "dex_build_vlm_mips", "dex_mips_get_levels", "dex_mips_set_levels", "dex_mips_set_level_caps", "dex_mips_velocity_bin_report",
     "dex_mips_get_packed_levels", "dex_mips_get_level_data", "dex_destroy_mips", "dex_formal_solution",
-    "dex_mean_intensity", "dex_mean_intensity_host", "dex_mean_intensity_pipelined", "dex_pool_high_water", "dex_direction_fields",
+    "dex_mean_intensity", "dex_mean_intensity_host", "dex_mean_intensity_pipelined", "dex_pool_high_water", "dex_trim", "dex_direction_fields",
     "dex_mean_intensity_single_direction", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read", "dex_march_work_read",
     "dex_set_lanes_per_ray", "dex_get_lanes_per_ray", "dex_measure_fp32_peak", "dex_set_tuning",
 )
@@ -110,6 +110,7 @@ def _load():
     L.dex_march_work_read.argtypes = [C.POINTER(C.c_int64), C.c_int]
     L.dex_set_lanes_per_ray.argtypes = [C.c_int]
     L.dex_set_tuning.argtypes = [C.c_char_p, C.c_int]
+    L.dex_trim.argtypes = [C.POINTER(C.c_int64)]
     L.dex_get_lanes_per_ray.argtypes = [C.c_int64, C.POINTER(C.c_int)]
     L.dex_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]
     return L
@@ -153,6 +154,13 @@ def dex_launch_count() -> int:
 
 def dex_set_lanes_per_ray(lanes: int):
     _check(_L.dex_set_lanes_per_ray(int(lanes)))
+
+
+def dex_trim() -> int:
+    """Return the library pool's unused device memory to the driver; returns the bytes it still holds."""
+    v = C.c_int64(0)
+    _check(_L.dex_trim(C.byref(v)))
+    return v.value
 
 
 def dex_get_lanes_per_ray(n_probes: int) -> int:

@@ -18,13 +18,14 @@ std::atomic<int> g_lanes_per_ray{0};  // 0 = automatic, see lanes_for()
 std::atomic<int> g_timing{0};
 std::atomic<int> g_tile_probes{1};
 std::atomic<int> g_voigt_fp32{1};
+std::atomic<int> g_dir_split{-1};
 std::mutex g_timing_mu;
 struct EvPair { cudaEvent_t a, b; };
 std::vector<EvPair> g_events;
 unsigned long long* g_d_line_segs = nullptr;   // device counter of (segment, active line) pairs, timing mode only
 
 // Lanes that share one ray.  One thread per ray (all W wavelengths in registers) is the fastest mapping whenever the
-// probes fill the machine (profiles/r01_march_ncu_full.md: 1.6-2.2x over 8 lanes on C2).  A small problem -- fewer
+// probes fill the machine (profiles/r01_history.md: 1.6-2.2x over 8 lanes on C2).  A small problem -- fewer
 // probes than one wave of 128-thread blocks on 148 SMs, e.g. C1's 4096 -- leaves most SMs idle with that mapping;
 // 8 lanes per ray give it 8x the threads (C1 march 0.403 -> 0.267 ms).  Depends on n_probes only, so every wavelength
 // stage of a pipelined solve takes the same mapping as the whole-spectrum call.
@@ -84,6 +85,7 @@ dex_status check_rays(const dex_grid* grid, const dex_mips* mips, const dex_rays
   out->t_begin = rays->t_begin;
   out->t_end = rays->t_end;
   out->accumulate = rays->accumulate;
+  out->k_per_block = 0;
   if (rays->t_end > 0.0f && !(rays->t_begin >= 0.0f && rays->t_begin < rays->t_end)) {
     dex_set_error("radiance interval needs 0 <= t_begin < t_end");
     return DEX_ERR_INVALID_ARG;
@@ -168,23 +170,40 @@ const float* dex_voigt_fast_table_host() {
   return tab.data();
 }
 
-cudaError_t dex_alloc(void** p, size_t bytes, cudaStream_t st) {
-  static std::mutex mu;
-  static bool warm[64] = {false};
+// The library's own stream-ordered pool, one per device, created at first use: nothing is returned to the driver
+// until dex_trim(), so a rebuild per iteration pays no cudaMalloc / cudaFree.  A PRIVATE pool: the device's default
+// pool (and with it every other cudaMallocAsync user of the process) keeps its own release threshold and statistics.
+namespace {
+std::mutex g_pool_mu;
+cudaMemPool_t g_pool[64] = {nullptr};
+cudaMemPool_t pool_of_current_device() {
   int dev = 0;
-  if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64) {
-    std::lock_guard<std::mutex> lk(mu);
-    if (!warm[dev]) {
-      cudaMemPool_t pool;
-      if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-        unsigned long long keep = ~0ULL;
-        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-      }
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return nullptr; }
+  std::lock_guard<std::mutex> lk(g_pool_mu);
+  if (!g_pool[dev]) {
+    cudaMemPoolProps props;
+    memset(&props, 0, sizeof(props));
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t pool = nullptr;
+    if (cudaMemPoolCreate(&pool, &props) == cudaSuccess) {
+      unsigned long long keep = ~0ULL;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+      g_pool[dev] = pool;
+    } else {
       cudaGetLastError();
-      warm[dev] = true;
     }
   }
-  return cudaMallocAsync(p, bytes, st);
+  return g_pool[dev];
+}
+}  // namespace
+
+cudaError_t dex_alloc(void** p, size_t bytes, cudaStream_t st) {
+  cudaMemPool_t pool = pool_of_current_device();
+  if (!pool) return cudaMallocAsync(p, bytes, st);     // pool creation failed: the default pool, untouched
+  return cudaMallocFromPoolAsync(p, bytes, pool, st);
 }
 void dex_free(void* p, cudaStream_t st) {
   if (p) cudaFreeAsync(p, st);
@@ -193,6 +212,7 @@ void dex_free(void* p, cudaStream_t st) {
 void dex_set_error(const std::string& msg) { g_last_error = msg; }
 void dex_count_launch(int n) { g_launches.fetch_add(n); }
 int dex_tuning_voigt_fp32() { return g_voigt_fp32.load(); }
+int dex_tuning_dir_split() { return g_dir_split.load(); }
 unsigned long long* dex_line_segment_counter() { return g_timing.load() ? g_d_line_segs : nullptr; }
 
 extern "C" {
@@ -203,10 +223,8 @@ int64_t dex_launch_count(void) { return (int64_t)g_launches.load(); }
 
 dex_status dex_pool_high_water(int64_t* bytes_in_use_high, int reset) {
   if (!have_device()) return DEX_ERR_CUDA;
-  int dev = 0;
-  DEX_CUDA_CHECK(cudaGetDevice(&dev));
-  cudaMemPool_t pool;
-  DEX_CUDA_CHECK(cudaDeviceGetDefaultMemPool(&pool, dev));
+  cudaMemPool_t pool = pool_of_current_device();
+  if (!pool) { dex_set_error("the library's memory pool could not be created"); return DEX_ERR_CUDA; }
   DEX_CUDA_CHECK(cudaDeviceSynchronize());
   unsigned long long v = 0;
   DEX_CUDA_CHECK(cudaMemPoolGetAttribute(pool, cudaMemPoolAttrUsedMemHigh, &v));
@@ -215,6 +233,18 @@ dex_status dex_pool_high_water(int64_t* bytes_in_use_high, int reset) {
     v = 0;
     DEX_CUDA_CHECK(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrUsedMemHigh, &v));
   }
+  return DEX_OK;
+}
+
+dex_status dex_trim(int64_t* bytes_reserved_after) {
+  if (!have_device()) return DEX_ERR_CUDA;
+  cudaMemPool_t pool = pool_of_current_device();
+  if (!pool) { dex_set_error("the library's memory pool could not be created"); return DEX_ERR_CUDA; }
+  DEX_CUDA_CHECK(cudaDeviceSynchronize());
+  DEX_CUDA_CHECK(cudaMemPoolTrimTo(pool, 0));
+  unsigned long long v = 0;
+  DEX_CUDA_CHECK(cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReservedMemCurrent, &v));
+  if (bytes_reserved_after) *bytes_reserved_after = (int64_t)v;
   return DEX_OK;
 }
 
@@ -238,6 +268,7 @@ dex_status dex_set_tuning(const char* name, int value) {
   if (!strcmp(name, "lanes_per_ray")) return dex_set_lanes_per_ray(value);
   if (!strcmp(name, "tile_probes")) { g_tile_probes.store(value ? 1 : 0); return DEX_OK; }
   if (!strcmp(name, "voigt_fp32")) { g_voigt_fp32.store(value ? 1 : 0); return DEX_OK; }
+  if (!strcmp(name, "dir_split")) { g_dir_split.store(value < 0 ? -1 : value); return DEX_OK; }
   dex_set_error("unknown tuning knob");
   return DEX_ERR_INVALID_ARG;
 }
@@ -937,6 +968,10 @@ dex_status dex_mean_intensity_host(const dex_grid_desc* desc, const uint8_t* h_a
   if (desc->ndim != 2 && desc->ndim != 3) { dex_set_error("ndim must be 2 or 3"); return DEX_ERR_INVALID_ARG; }
   if (hm->n_lambda <= 0 || hr->n_probes < 0 || hr->n_dirs < 0 || hm->n_lines < 0 || hm->n_lines > DEX_MAX_LINES) {
     dex_set_error("bad n_lambda / n_probes / n_dirs / n_lines");
+    return DEX_ERR_SHAPE;
+  }
+  if (hm->lambda_stride != 0 && hm->lambda_stride != hm->n_lambda) {
+    dex_set_error("the host entry uploads dense [nvox][n_lambda] spectra: lambda_stride must be 0 (or n_lambda)");
     return DEX_ERR_SHAPE;
   }
   if (!have_device()) return DEX_ERR_CUDA;

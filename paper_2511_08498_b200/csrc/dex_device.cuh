@@ -85,6 +85,8 @@ struct DexRaysDev {
   const float* sin_incl;   // [n_dirs] or NULL: 2.5D rays
   float t_begin, t_end;    // finite radiance interval (T10); t_end <= 0: to the boundary
   int accumulate;          // fused J: d_J += sum_k w_k I_k instead of = (single-direction VLM sums its per-direction solves)
+  int k_per_block;         // > 0: blockIdx.z selects a run of this many directions (materialised I only: small problems
+                           // are spread over the machine direction by direction, dex_launch_march); 0: all directions
 };
 
 // ---- exact (uncontracted) fp32 helpers -------------------------------------------------

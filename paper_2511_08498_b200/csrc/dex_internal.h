@@ -46,6 +46,7 @@ cudaError_t dex_alloc(void** p, size_t bytes, cudaStream_t st);
 void dex_free(void* p, cudaStream_t st);
 void dex_count_launch(int n = 1);
 int dex_tuning_voigt_fp32();
+int dex_tuning_dir_split();   // -1 automatic, 0 never, n > 0: n directions per block whenever J is fused
 unsigned long long* dex_line_segment_counter();   // device counter, NULL unless march timing is enabled
 
 // grid_build.cu

@@ -137,6 +137,32 @@ __device__ __forceinline__ void dex_accumulate_all_S(const float (&S)[LPT], cons
   }
 }
 
+// Providers that deliver (eta, chi) instead of march records (velocity interpolation, Core-and-Voigt, Classic): the
+// record form is made on the fly, chi' = max(chi, 2^-60), S = eta rcp(chi'), and the S integrator above does the rest
+// -- one MUFU.RCP per wavelength buys ~10 fewer issue slots per wavelength pair than the E(tau) form below (the kernel
+// is issue-bound, profiles/).  chi < 2^-60 (a pure emitter) gives S (1 - e^-tau) = eta h ds to 1e-18 h ds.
+#define DEX_CHI_TINY 8.673617379884035e-19f      // 2^-60
+template <int LPT>
+__device__ __forceinline__ void dex_accumulate_all_EC(const float (&eta)[LPT], const float (&chi)[LPT], float hds,
+                                                      float (&I)[LPT], float (&T)[LPT]) {
+  const float nhl = hds * -1.4426950408889634f;      // y = chi' (-h ds log2 e)
+  if (LPT == 1) {
+    const float c = fmaxf(chi[0], DEX_CHI_TINY);
+    dex_accumulate_S1(eta[0] * dex_rcp(c), c, nhl, I[0], T[0]);
+  } else {
+    const float2 nhl2 = make_float2(nhl, nhl);
+#pragma unroll
+    for (int i = 0; i < LPT / 2; ++i) {
+      const float2 c = make_float2(fmaxf(chi[2 * i], DEX_CHI_TINY), fmaxf(chi[2 * i + 1], DEX_CHI_TINY));
+      const float2 S = __fmul2_rn(make_float2(eta[2 * i], eta[2 * i + 1]), make_float2(dex_rcp(c.x), dex_rcp(c.y)));
+      float2 Ii = make_float2(I[2 * i], I[2 * i + 1]), Ti = make_float2(T[2 * i], T[2 * i + 1]);
+      dex_accumulate_S2(S, c, nhl2, Ii, Ti);
+      I[2 * i] = Ii.x; I[2 * i + 1] = Ii.y;
+      T[2 * i] = Ti.x; T[2 * i + 1] = Ti.y;
+    }
+  }
+}
+
 template <int LPT>
 __device__ __forceinline__ void dex_accumulate_all(const float (&eta)[LPT], const float (&chi)[LPT], float hds,
                                                    float (&I)[LPT], float (&T)[LPT]) {
@@ -178,7 +204,10 @@ template <int LPT>
 __device__ __forceinline__ void dex_load_rec(const float* __restrict__ rec, int sub, float (&eta)[LPT], float (&chi)[LPT]) {
   const float* pc = rec + sub * LPT;
   const float* pe = rec + DEX_W + sub * LPT;
-  if (LPT == 1) {
+  if (LPT == 8) {          // one thread per ray: each 32-byte plane of the 64-byte record is one LDG.E.256
+    dex_load_plane<LPT>(pc, chi);
+    dex_load_plane<LPT>(pe, eta);
+  } else if (LPT == 1) {
     chi[0] = __ldg(pc);
     eta[0] = __ldg(pe);
   } else if (LPT == 2) {
@@ -222,7 +251,7 @@ __device__ __noinline__ float dex_voigt_H_outside_window(const double* __restric
 // eta, chi of one cell for this lane's wavelengths, seen along propagation direction om (a7)
 template <int D, int VAR, int LPT>
 __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_base, int cell, int sub,
-                                             const float* __restrict__ om, float sin_incl, const DexCavTab& CT,
+                                             const float (&om)[D], float sin_incl, const DexCavTab& CT,
                                              const float4* __restrict__ vfw, const float* __restrict__ vfc,
                                              const float* __restrict__ iso0, const float* __restrict__ iso1,
                                              float (&eta)[LPT], float (&chi)[LPT]) {
@@ -234,39 +263,58 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
   // projected velocity of the cell's box-filtered bulk velocity, fp64 (DESIGN.md R-vel)
   // velocity-interpolation marches keep the velocities dense (stride 1, compile time); Core-and-Voigt / Classic read
   // the cell's contiguous [velocity, lines] record (dex_device.cuh)
-  const float4* __restrict__ arec = M.aux + ((VAR == DEX_VELINTERP) ? (size_t)cell : dex_aux_vel(M, (size_t)cell));
+  const float4* __restrict__ arec = M.aux + ((VAR == DEX_VELINTERP) ? (size_t)(unsigned)cell : dex_aux_vel(M, (size_t)(unsigned)cell));
   const float4 v4 = __ldg(arec);
-  double vproj = __dmul_rn((double)v4.x, (double)__ldg(om));
-  vproj = __dadd_rn(vproj, __dmul_rn((double)v4.y, (double)__ldg(om + 1)));
-  if (D == 3) vproj = __dadd_rn(vproj, __dmul_rn((double)v4.z, (double)__ldg(om + D - 1)));
+  double vproj = __dmul_rn((double)v4.x, (double)om[0]);
+  vproj = __dadd_rn(vproj, __dmul_rn((double)v4.y, (double)om[1]));
+  if (D == 3) vproj = __dadd_rn(vproj, __dmul_rn((double)v4.z, (double)om[D - 1]));
   if (D == 2) vproj = __dmul_rn(vproj, (double)sin_incl);   // 2.5D: in-plane part of the 3D direction (1 for in-plane rays)
   if (VAR == DEX_VELINTERP) {
-    // linear interpolation on the cell's uniform velocity grid [-V, V]
+    // linear interpolation on the cell's uniform velocity grid [-V, V]:
+    // f = (vproj + V) / (2V) (n - 1) clamped to [0, n-1], i0 = min(floor f, n-2), w = f - i0.  f needs fp64 (adjacent
+    // bins of a Gaussian core differ by factors of 1e2, so an fp32 f would cost 1e-4 in eta), the division does not:
+    // 1/(2V) is the fp32 MUFU.RCP refined by one fp64 Newton step (2^-44).  The bin is taken from f rounded to fp32;
+    // where that rounding crosses an integer the pair (i0, w) describes the same point of the same piecewise-linear
+    // function from the neighbouring interval (w within 3e-7 of 0 or 1), so only the two ends need the clamp.
     const int nvb = M.n_vbins;
-    const double V = (double)v4.w;
     int i0 = 0;
     float w = 0.0f;
-    if (V > 0.0) {
-      double f = __dmul_rn(__ddiv_rn(__dadd_rn(vproj, V), __dmul_rn(2.0, V)), (double)(nvb - 1));
-      f = fmin(fmax(f, 0.0), (double)(nvb - 1));
-      i0 = min((int)floor(f), nvb - 2);
-      w = (float)(f - (double)i0);
+    if (v4.w > 0.0f) {
+      const double V = (double)v4.w, d2 = V + V;
+      double r = (double)dex_rcp(v4.w + v4.w);
+      r = fma(r, fma(-d2, r, 1.0), r);
+      const double f = (vproj + V) * (r * (double)(nvb - 1));
+      const float top = (float)(nvb - 2);
+      const float fi = fminf(fmaxf(floorf((float)f), 0.0f), top);
+      i0 = (int)fi;
+      w = (float)(f - (double)fi);
+      w = fminf(fmaxf(w, (fi <= 0.0f) ? 0.0f : -1.0f), (fi >= top) ? 1.0f : 2.0f);
     }
-    const float* r0 = M.vtab + ((batch_base + (size_t)cell) * nvb + i0) * DEX_REC;
+    // this batch's tables start at vt0 (kept in a register pair by the caller through iso0); 32-bit record index
+    const float* r0 = iso0 + (size_t)((unsigned)cell * (unsigned)nvb + (unsigned)i0) * DEX_REC;
     float e1[LPT], c1[LPT];
     dex_load_rec<LPT>(r0, sub, eta, chi);
     dex_load_rec<LPT>(r0 + DEX_REC, sub, e1, c1);
+    const float omw = 1.0f - w;
+    if (LPT == 1) {
+      eta[0] = fmaf(w, e1[0], omw * eta[0]);
+      chi[0] = fmaf(w, c1[0], omw * chi[0]);
+    } else {
+      const float2 w2 = dex_f2(w), omw2 = dex_f2(omw);
 #pragma unroll
-    for (int i = 0; i < LPT; ++i) {
-      eta[i] = fmaf(w, e1[i], (1.0f - w) * eta[i]);
-      chi[i] = fmaf(w, c1[i], (1.0f - w) * chi[i]);
+      for (int i = 0; i < LPT / 2; ++i) {
+        const float2 e = __ffma2_rn(w2, make_float2(e1[2 * i], e1[2 * i + 1]), __fmul2_rn(omw2, make_float2(eta[2 * i], eta[2 * i + 1])));
+        const float2 c = __ffma2_rn(w2, make_float2(c1[2 * i], c1[2 * i + 1]), __fmul2_rn(omw2, make_float2(chi[2 * i], chi[2 * i + 1])));
+        eta[2 * i] = e.x; eta[2 * i + 1] = e.y;
+        chi[2 * i] = c.x; chi[2 * i + 1] = c.y;
+      }
     }
     return;
   }
   // Core-and-Voigt / Classic: background + sum over the active lines (eqs. 10-11).  Only H(a, x) needs fp64 (the
   // Weideman form cancels in the wings); the line sum itself is fp32.  Everything that depends
   // on (wavelength, line) alone comes from the block's shared table CT (one batch per block).
-  dex_load_rec<LPT>(M.store + (batch_base + (size_t)cell) * DEX_REC, sub, eta, chi);
+  dex_load_rec<LPT>(iso0 + (size_t)(unsigned)cell * DEX_REC, sub, eta, chi);   // iso0 = this batch's background records
 #pragma unroll 1
   for (int q = 0; q < DEX_NLINES; ++q) {   // not unrolled: the body is ~500 instructions and would be copied 4 times
     const int l = CT.line[q];
@@ -383,12 +431,6 @@ constexpr int dex_march_minb(int var) {
 #endif
 
 
-#ifdef DEX_MARCH_STATS
-// diagnostic build only (-DDEX_MARCH_STATS): lane-iteration census of the warp-synchronous loop
-// [0] warp iterations x 32, [1] lanes alive, [2] lanes blocked at a brick face, [3] lanes that emitted,
-// [4] iterations in which the general crossing ran, [5] lanes that took it
-__device__ unsigned long long g_dex_stats[8];
-#endif
 
 template <int D, int VAR, int LPR, bool FUSE_J, bool CLIP>
 __global__ void __launch_bounds__(DEX_MARCH_THREADS, dex_march_minb(VAR))
@@ -406,17 +448,17 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   const int sub = threadIdx.x % LPR;
   const int lam_off = batch * DEX_W + sub * LPT;
   unsigned nseg = 0;
-#ifdef DEX_MARCH_STATS
-  unsigned long long st_it = 0, st_alive = 0, st_blocked = 0, st_xit = 0, st_xl = 0;
-#endif
   const int* binfo = M.binfo + (size_t)batch * G.n_bricks;
   asm volatile("" : "+l"(binfo));   // opaque for the same reason as iso0 / iso1 below
   const size_t batch_base = ((size_t)batch * G.n_active) * M.cps;
   // this lane's rows of the two ISO record planes (cell 0 of the batch); kept opaque so that the pointers stay in
   // registers instead of being rebuilt from the kernel parameters at every segment
-  const float* iso0 = M.mrec + batch_base * DEX_W + sub * LPT;
+  // (velocity interpolation: iso0 = this batch's velocity tables; Core-and-Voigt / Classic: its background records)
+  const float* iso0 = (VAR == DEX_ISO) ? M.mrec + batch_base * DEX_W + sub * LPT
+                      : (VAR == DEX_VELINTERP) ? M.vtab + batch_base * (size_t)M.n_vbins * DEX_REC
+                                               : M.store + batch_base * DEX_REC;
   const float* iso1 = iso0 + M.mplane;
-  if (VAR == DEX_ISO) asm volatile("" : "+l"(iso0), "+l"(iso1));
+  asm volatile("" : "+l"(iso0), "+l"(iso1));
   const float* __restrict__ probe = R.probe_pos + gid * D;
   __shared__ DexCavTab CT;
   __shared__ float4 vfw[VAR == DEX_CAV ? DEX_VF_NODES : 1];
@@ -480,8 +522,13 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   }
   DexRay3<D> ray;
   // one direction at a time: the lanes of a warp trace the same direction together (coherent fetches)
-  for (int k = 0; k < R.n_dirs; ++k) {
+  const int k_begin = (!FUSE_J && R.k_per_block > 0) ? (int)blockIdx.z * R.k_per_block : 0;
+  const int k_end = (!FUSE_J && R.k_per_block > 0) ? min(R.n_dirs, k_begin + R.k_per_block) : R.n_dirs;
+  for (int k = k_begin; k < k_end; ++k) {
     const float* __restrict__ om = R.dirs + k * D;
+    float omf[D];
+#pragma unroll
+    for (int a = 0; a < D; ++a) omf[a] = __ldg(om + a);
     // 2.5D rays: path lengths are divided by the sine of the inclination to the homogeneous axis (dex.h d_sin_incl)
     const float sin_incl = (D == 2 && R.sin_incl != nullptr) ? __ldg(R.sin_incl + k) : 1.0f;
     const float hk = (D == 2 && R.sin_incl != nullptr) ? __fdiv_rn(G.h, sin_incl) : G.h;
@@ -497,10 +544,6 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
         for (int i = 0; i < LPT; ++i) { DEX_IH(i) += I[i]; I[i] = 0.0f; }
       }
       const unsigned bm = __ballot_sync(FULL, blocked);
-#ifdef DEX_MARCH_STATS
-      st_it += 32; st_alive += __popc(am); st_blocked += __popc(bm);
-      if (bm == am || __popc(bm) >= DEX_CROSS_QUORUM) { st_xit += 1; st_xl += __popc(bm); }
-#endif
       if (bm == am || __popc(bm) >= DEX_CROSS_QUORUM) {
         if (blocked) {
           alive = dex_ray_cross<D>(ray, G, M, binfo, probe, om);
@@ -522,9 +565,12 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
           ++nseg;
           const float hds = hk * ds;
           float eta[LPT], chi[LPT];
-          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, om, sin_incl, CT, vfw, vfc, iso0, iso1, eta, chi);
+          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, omf, sin_incl, CT, vfw, vfc, iso0, iso1, eta, chi);
           if (VAR == DEX_ISO) dex_accumulate_all_S<LPT>(eta, chi, hds, I, T);
-          else dex_accumulate_all<LPT>(eta, chi, hds, I, T);
+          // velocity interpolation keeps the E(tau) integrator: the record form costs it registers it does not have at
+          // 7 blocks per SM (measured on C3: 583 ms against 616; Core-and-Voigt gains 3 % from the record form)
+          else if (VAR == DEX_VELINTERP) dex_accumulate_all<LPT>(eta, chi, hds, I, T);
+          else dex_accumulate_all_EC<LPT>(eta, chi, hds, I, T);
         }
       }
     }
@@ -554,13 +600,6 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
       dst[i] = R.accumulate ? __fadd_rn(dst[i], j) : j;
     }
   }
-#ifdef DEX_MARCH_STATS
-  if ((threadIdx.x & 31) == 0) {
-    atomicAdd(&g_dex_stats[0], st_it); atomicAdd(&g_dex_stats[1], st_alive); atomicAdd(&g_dex_stats[2], st_blocked);
-    atomicAdd(&g_dex_stats[4], st_xit); atomicAdd(&g_dex_stats[5], st_xl);
-  }
-  atomicAdd(&g_dex_stats[3], (unsigned long long)nseg);
-#endif
   if (seg_count != nullptr) {
     unsigned v = (sub == 0) ? nseg : 0u;
     v = __reduce_add_sync(FULL, v);
@@ -696,15 +735,16 @@ __global__ void dex_tile_rank_kernel(const DexTiling TL, long long n, const floa
 
 // J(p, lambda) = sum_k w_k I(p, k, lambda) from a materialised I: one thread per (probe, lambda);
 // consecutive threads read consecutive lambda (coalesced).
+// The sum runs in direction order with one fma per term, exactly as the fused march accumulates it: both give the same bits.
 __global__ void dex_reduce_j_kernel(long long n_probes, int n_dirs, int n_lambda, const float* __restrict__ w,
-                                    const float* __restrict__ I, float* __restrict__ J) {
+                                    const float* __restrict__ I, float* __restrict__ J, int accumulate) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_probes * n_lambda) return;
   const long long p = i / n_lambda;
   const int j = (int)(i - p * n_lambda);
   float acc = 0.0f;
   for (int k = 0; k < n_dirs; ++k) acc = fmaf(__ldg(w + k), __ldg(I + (p * n_dirs + k) * n_lambda + j), acc);
-  J[i] = acc;
+  J[i] = accumulate ? __fadd_rn(J[i], acc) : acc;
 }
 
 // validation (dex_voigt_profile): the march's own Voigt routines on caller-supplied (a, x)
@@ -735,7 +775,10 @@ dex_status launch_march_t(const dex_grid* g, const dex_mips* m, const DexRaysDev
     dex_set_error("march: problem too large for one launch");
     return DEX_ERR_UNSUPPORTED;
   }
-  dim3 grid((unsigned)gx, (unsigned)m->n_batch, 1);
+  unsigned gz = 1;
+  if (!fuse_j && rays.k_per_block > 0) gz = (unsigned)((rays.n_dirs + rays.k_per_block - 1) / rays.k_per_block);
+  if (gz > 65535u) { dex_set_error("march: too many direction groups for one launch"); return DEX_ERR_UNSUPPORTED; }
+  dim3 grid((unsigned)gx, (unsigned)m->n_batch, gz);
   DexMipsDev md = m->dev;
   md.voigt_fp32 = dex_tuning_voigt_fp32();
   unsigned long long* d_work = dex_line_segment_counter();   // NULL unless march timing is enabled
@@ -801,15 +844,15 @@ static dex_status tile_probes_t(const dex_grid* g, const DexRaysDev& rays, int**
   if (nt_total > (1LL << 28)) return DEX_OK;
   TL.n_tiles = (int)nt_total;
   int* d_count = nullptr;
-  DEX_CUDA_CHECK(cudaMallocAsync((void**)&d_count, sizeof(int) * (size_t)(TL.n_tiles + 1), st));
-  cudaError_t e = cudaMallocAsync((void**)d_perm, sizeof(int) * (size_t)n, st);
+  DEX_CUDA_CHECK(dex_alloc((void**)&d_count, sizeof(int) * (size_t)(TL.n_tiles + 1), st));
+  cudaError_t e = dex_alloc((void**)d_perm, sizeof(int) * (size_t)n, st);
   if (e != cudaSuccess) { cudaFreeAsync(d_count, st); *d_perm = nullptr; DEX_CUDA_CHECK(e); }
   cudaMemsetAsync(d_count, 0, sizeof(int) * (size_t)(TL.n_tiles + 1), st);
   const unsigned blocks = (unsigned)((n + 255) / 256);
   dex_tile_count_kernel<D><<<blocks, 256, 0, st>>>(TL, n, rays.probe_pos, d_count);
   dex_tile_scan_kernel<<<1, 1024, 0, st>>>(d_count, TL.n_tiles);
   int* d_arrival = nullptr;
-  e = cudaMallocAsync((void**)&d_arrival, sizeof(int) * (size_t)n, st);
+  e = dex_alloc((void**)&d_arrival, sizeof(int) * (size_t)n, st);
   if (e != cudaSuccess) { cudaFreeAsync(d_count, st); cudaFreeAsync(*d_perm, st); *d_perm = nullptr; DEX_CUDA_CHECK(e); }
   dex_tile_scatter_kernel<D><<<blocks, 256, 0, st>>>(TL, n, rays.probe_pos, d_count, d_arrival);
   dex_tile_rank_kernel<D><<<blocks, 256, 0, st>>>(TL, n, rays.probe_pos, d_count, d_arrival, *d_perm);
@@ -831,10 +874,30 @@ dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysD
   dex_status s = DEX_OK;
   if (tile && !perm_in) s = dex_make_probe_tiling(g, rays, &d_perm, st);
   const int* perm = perm_in ? perm_in : d_perm;
-  if (s == DEX_OK) {
-    if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, perm, st);
-    else s = launch_march_d<3>(g, m, rays, d_out, fuse_j, d_seg, lanes_per_ray, perm, st);
+  // Small problems (fewer probes than one wave of blocks) leave most SMs idle while every thread walks its directions
+  // one after the other (C1: 4096 probes x 16 directions).  There the fused J is taken apart: one block per (probe tile,
+  // batch, direction) writes I (a few MB), and dex_reduce_j_kernel sums it in the fused kernel's own order, so J is
+  // bit-identical to the fused path.  Whole-spectrum handles only (a pipeline stage writes a window of J's columns).
+  DexRaysDev r = rays;
+  r.k_per_block = 0;
+  float* d_I = nullptr;
+  const size_t i_floats = (size_t)rays.n_probes * (size_t)rays.n_dirs * (size_t)m->n_lambda;
+  const int split = dex_tuning_dir_split();
+  const bool small = rays.n_probes < 148LL * 128 && rays.n_dirs > 1 && i_floats <= (64u << 20);
+  if (s == DEX_OK && fuse_j && (split > 0 || (split < 0 && small)) && m->dev.io_base == 0 && m->dev.io_stride == m->n_lambda &&
+      rays.t_end <= 0.0f) {
+    cudaError_t e = dex_alloc((void**)&d_I, sizeof(float) * i_floats, st);
+    if (e != cudaSuccess) { cudaGetLastError(); d_I = nullptr; }     // no room: the fused path needs none
+    else r.k_per_block = (split > 0) ? split : 1;
   }
+  if (s == DEX_OK) {
+    float* out = d_I ? d_I : d_out;
+    const bool fj = d_I ? false : fuse_j;
+    if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st);
+    else s = launch_march_d<3>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st);
+    if (s == DEX_OK && d_I) s = dex_launch_reduce_j(r, m->n_lambda, d_I, d_out, st);
+  }
+  if (d_I) dex_free(d_I, st);
   if (d_perm) cudaFreeAsync(d_perm, st);
   return s;
 }
@@ -869,7 +932,7 @@ dex_status dex_launch_voigt_profile(const float* d_a, const double* d_x, long lo
   DexWeideman Wc;
   dex_weideman_coefficients(Wc.c, &Wc.L);
   float* d_tab = nullptr;
-  DEX_CUDA_CHECK(cudaMallocAsync((void**)&d_tab, sizeof(float) * DEX_VF_NODES * 5, st));
+  DEX_CUDA_CHECK(dex_alloc((void**)&d_tab, sizeof(float) * DEX_VF_NODES * 5, st));
   cudaError_t e = cudaMemcpyAsync(d_tab, dex_voigt_fast_table_host(), sizeof(float) * DEX_VF_NODES * 5, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) {
     const long long gx = (n + 255) / 256;
@@ -888,17 +951,10 @@ dex_status dex_launch_reduce_j(const DexRaysDev& rays, int n_lambda, const float
   if (n <= 0) return DEX_OK;
   const int threads = 256;
   const long long gx = (n + threads - 1) / threads;
-  dex_reduce_j_kernel<<<(unsigned)gx, threads, 0, st>>>(rays.n_probes, rays.n_dirs, n_lambda, rays.weights, d_I, d_J);
+  dex_reduce_j_kernel<<<(unsigned)gx, threads, 0, st>>>(rays.n_probes, rays.n_dirs, n_lambda, rays.weights, d_I, d_J,
+                                                        rays.accumulate);
   dex_count_launch();
   DEX_CUDA_CHECK(cudaGetLastError());
   return DEX_OK;
 }
 
-#ifdef DEX_MARCH_STATS
-extern "C" int dex_debug_read_stats(unsigned long long* out8, int reset) {
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(out8, g_dex_stats, sizeof(unsigned long long) * 8);
-  if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(g_dex_stats, z, sizeof(z)); }
-  return 0;
-}
-#endif

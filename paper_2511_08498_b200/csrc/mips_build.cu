@@ -166,18 +166,19 @@ __global__ void reduce_spec_kernel(const BuildCtx X, int m) {
 // wavelength), and with chi2 = chi log2(e) the exponent is a single product, e^{-tau} = 2^(-chi2 h ds).
 // Records hold (chi2, S) for every level of the pyramid in two planes of 32-byte rows (one LDG.E.256 each; four
 // cells per 128-byte line, so the neighbouring rays of a warp share L1 lines); the pyramid itself keeps (eta, chi)
-// exactly (it is what the VLM test and the validation accessors see).  chi < 2^-100 (including chi = 0, a pure
-// emitter: I_out = I_in + eta h ds) is represented by chi = 2^-100, S = eta 2^100: then tau is ~1e-30 h ds,
-// e^{-tau} = 1 and S (1 - e^{-tau}) = eta h ds to 1e-7, so the E(0) = 1 limit of DESIGN.md is kept.
+// exactly (it is what the VLM test and the validation accessors see).  chi < 2^-60 (including chi = 0, a pure
+// emitter: I_out = I_in + eta h ds) is represented by chi = 2^-60, S = eta 2^60: then tau is ~1e-18 h ds,
+// e^{-tau} = 1 and S (1 - e^{-tau}) = eta h ds to 1e-7, so the E(0) = 1 limit of DESIGN.md is kept.  (2^-100 / 2^100
+// in round 1: S overflowed to inf for eta above 2.7e8.)
 __global__ void make_march_records_kernel(const float* __restrict__ store, float* __restrict__ mrec, long long n_rec) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_rec * DEX_W) return;
   const int j = (int)(i % DEX_W);
   const size_t r = (size_t)(i / DEX_W);
   const float eta = store[dex_rec_eta(r, j)], chi = store[dex_rec_chi(r, j)];
-  const float tiny = 7.888609052210118e-31f;   // 2^-100
+  const float tiny = 8.673617379884035e-19f;   // 2^-60
   float c = chi, S;
-  if (chi < tiny) { c = tiny; S = eta * 1.2676506002282294e30f; }   // 2^100, exact scaling
+  if (chi < tiny) { c = tiny; S = eta * 1.152921504606846976e18f; }   // 2^60, exact scaling (finite for eta < 2.9e20)
   else S = eta / chi;
   mrec[i] = c * 1.4426950408889634f;
   mrec[(size_t)n_rec * DEX_W + i] = S;

@@ -201,7 +201,7 @@ def test_edge_cases(P):
     eta = rng.uniform(0.0, 1.0, size=(64, 64, 8))
     chi[:, 20:40] = 0.0
     eta[30:50, 30:60] = 0.0
-    chi[5:9, 5:9] = 1e-36           # far below 2^-100: treated as chi = 0 by the march records
+    chi[5:9, 5:9] = 1e-36           # far below 2^-60: treated as chi = 0 by the march records
     wl4 = iso_workload((64, 64), 16, eta, chi, rng.uniform(0, 64, size=(200, 2)), dirs_2d(12)[0], h=1.7)
     M4 = orc.build_mips(wl4)
     dw, grid, mips = _build(P, wl4)
@@ -305,6 +305,36 @@ def test_c2_full_size_sampled(P):
     assert np.isfinite(J).all() and (J >= 0).all()
 
 
+def test_direction_split_bit_identical(P):
+    """Small problems (fewer probes than one wave of blocks) are launched one block per (probe tile, batch, direction)
+    into a temporary I and summed by the reduction kernel in the fused kernel's order: J and the segment count are bit
+    for bit those of the fused launch, for every lanes-per-ray mapping, with boundary intensity; pool memory is returned
+    by dex_trim."""
+    wl = make("C2", n=128, n_dirs=12, n_probes=700)
+    wl.i0 = np.random.default_rng(5).uniform(0, 1, size=(12, wl.n_lambda)).astype(np.float32)
+    M = orc.build_mips(wl)
+    ref = orc.hdda_march(wl, M)
+    dw, grid, mips = _build(P, wl)
+    try:
+        for lpr in (1, 8):
+            P.dex_set_lanes_per_ray(lpr)
+            out = {}
+            for split in (0, -1, 1, 5):
+                P.dex_set_tuning("dir_split", split)
+                seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+                out[split] = P.pipeline.mean_intensity(dw, grid, mips, segment_count=seg)
+                assert int(seg.item()) == ref.segments
+            assert max_rel(out[0].cpu().numpy(), orc.mean_intensity(ref.I, wl.weights)) <= TOL
+            for split in (-1, 1, 5):
+                assert torch.equal(out[0], out[split]), f"lanes={lpr} dir_split={split}"
+    finally:
+        P.dex_set_tuning("dir_split", -1)
+        P.dex_set_lanes_per_ray(1)
+    mips.destroy(); grid.destroy()
+    torch.cuda.synchronize()
+    assert P.dex_trim() >= 0
+
+
 # ------------------------------------------------------------------------------------------ host entry
 @pytest.mark.parametrize("name,kw", [("C2", dict(n=128, n_dirs=8, n_probes=333)), ("C5", dict(n=32, n_dirs=6, n_probes=200)),
                                      ("C3", dict(n=128, n_dirs=6, n_probes=150))])
@@ -321,6 +351,20 @@ def test_host_entry_matches_device_path(P, name, kw):
         assert nseg == int(seg.item()) and nseg > 0
         assert np.array_equal(Jh.view(np.uint32), J.view(np.uint32))
         assert d2h == J.size * 4 + 8 and 0 < h2d <= dw.h2d_bytes
+    # the host entry uploads dense spectra: a wavelength stride is refused (it would read past the uploads)
+    import paper_2511_08498_b200.binding as Bm
+    orig = Bm._mips_desc
+
+    def strided(*a, **k):
+        d, n, keep = orig(*a, **k)
+        d.lambda_stride = 2 * wl.n_lambda
+        return d, n, keep
+    Bm._mips_desc = strided
+    try:
+        with pytest.raises(P.DexError):
+            P.pipeline.solve_J_from_host(wl, "cuda:0")
+    finally:
+        Bm._mips_desc = orig
     # argument errors surface as a status, not a crash
     with pytest.raises(P.DexError):
         P.dex_mean_intensity_host(2, (64, 60), 16, 1.0, None, dict(variant=0, n_lambda=8, lambda_batch=8, max_level=0,

@@ -416,7 +416,18 @@ def _c4(n, n_dirs, rng, n_line_lambda=64, n_cont=16, max_level=4):
     )
 
 
-def _c5(n, n_dirs, rng, n_lambda=32, max_level=2, probe_stride=4):
+# C5 brick classes (smooth / mild / structured / rough): small-scale amplitudes (A of G_4, F of white noise) in ln chi and
+# the small-scale share of the velocity field.  Round 2 retune (SURVEY.md 8(d) allows it, "stating so"): with the round-1
+# recipe (ln chi on 24 voxels, velocities on 16, scale height 12) the eq. 17 Core-and-Voigt test left 99.4 % of the
+# populated bricks at level 0, so the config timed brick skipping only; a 20 km/s field must vary on >~ 100 voxels for
+# 2^3 / 4^3 cells to pass at relative variance 1e-2 (the Gaussian core turns dv into d ln(phi) = 2 x dv / v_th).
+_C5_CLASS_AF = np.array([[0.0, 0.0], [0.1, 0.0], [0.4, 0.0], [0.0, 0.5]])
+_C5_CLASS_VEL = (0.0, 0.005, 0.05, 0.2)
+_C5_CLASS_P = (0.5, 0.3, 0.1, 0.1)
+
+
+def _c5(n, n_dirs, rng, n_lambda=32, max_level=2, probe_stride=4, lnf_len=128.0, vel_len=128.0, hs0=48.0, s_len=96.0,
+        vel_small=_C5_CLASS_VEL, cls_af=_C5_CLASS_AF, cls_p=_C5_CLASS_P):
     b = 8
     nb = n // b
     sc = n / 256.0
@@ -425,20 +436,23 @@ def _c5(n, n_dirs, rng, n_lambda=32, max_level=2, probe_stride=4):
     zb = np.arange(nb, dtype=np.float64)[:, None, None]
     dist = np.abs(zb - nb / 2.0 + (nb / 8.0) * g4[None, :, :])
     occ_b = _occupancy_top(-dist, int(round(0.3 * nb ** 3)))
-    cls = _brick_classes(rng, occ_b)
-    A = _brick_expand(_CLASS_AF[cls, 0], b)
-    F = _brick_expand(_CLASS_AF[cls, 1], b)
+    cls = _brick_classes(rng, occ_b, cls_p)
+    caf = np.asarray(cls_af, dtype=np.float64)
+    A = _brick_expand(caf[cls, 0], b)
+    F = _brick_expand(caf[cls, 1], b)
     occ = _brick_expand(occ_b, b)
     zs = n / 2.0 + (n / 8.0) * grf((n, n), 32.0 * sc, rng)          # z_s(x, y)
     z = np.arange(n, dtype=np.float64)[:, None, None]
     dz = np.abs(z - zs[None, :, :])
     sh = (n, n, n)
-    lnf = 1.5 * grf(sh, 24.0 * sc, rng) + A * grf(sh, 4.0 * sc, rng) + F * rng.standard_normal(sh)
-    hs = 12.0 * sc
+    lnf = 1.5 * grf(sh, lnf_len * sc, rng) + A * grf(sh, 4.0 * sc, rng) + F * rng.standard_normal(sh)
+    hs = hs0 * sc
     chi_lc = 0.3 * np.exp(-dz / hs) * np.exp(lnf)
     del lnf
-    S = (1.0 + 2.0 * np.exp(-dz / hs)) * np.exp(0.3 * grf(sh, 32.0 * sc, rng))
-    vel = np.stack([20.0 * grf(sh, 16.0 * sc, rng) for _ in range(3)], axis=-1)
+    S = (1.0 + 2.0 * np.exp(-dz / hs)) * np.exp(0.3 * grf(sh, s_len * sc, rng))
+    Av = _brick_expand(np.asarray(vel_small, dtype=np.float64)[cls], b)
+    vel = np.stack([20.0 * (np.sqrt(1.0 - Av * Av) * grf(sh, vel_len * sc, rng) + Av * grf(sh, 4.0 * sc, rng))
+                    for _ in range(3)], axis=-1)
     T = 6000.0 + 2000.0 * np.exp(-dz / hs)
     vth = 12.85 * np.sqrt(T / 1.0e4)
     lam0 = 500.0
@@ -469,7 +483,7 @@ def _c5(n, n_dirs, rng, n_lambda=32, max_level=2, probe_stride=4):
         n_lines=1, lambda0=np.array([lam0], dtype=np.float32),
         eta_star0=f32(es.reshape(1, nv)), chi_star0=f32(cs.reshape(1, nv)),
         a0=f32(a0.reshape(1, nv)), inv_dlamD=f32(inv.reshape(1, nv)),
-        active_lines=al, n_vbins=0,
+        active_lines=al, n_vbins=0, notes={"brick_class": cls},
     )
 
 
