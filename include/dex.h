@@ -294,11 +294,12 @@ dex_status dex_march_timing_read(double* ms_total, int64_t* n_launches, int rese
  * multiplies by W and by the flops per evaluation stated in DESIGN.md).  Synchronises. */
 dex_status dex_march_work_read(int64_t* line_segments, int reset);
 /* Kernel configuration knob: lanes that share one ray, 1/2/4/8, or 0 (default) = automatic: one thread per ray unless
- * there are fewer probes than one wave of blocks (148 SMs x 128 threads), where 8 lanes per ray fill the machine better. */
+ * there are fewer probes than one wave of blocks (148 SMs x 128 threads), where 8 lanes per ray fill the machine better
+ * (2 when the march is also spread over the machine direction by direction, see "dir_split"). */
 dex_status dex_set_lanes_per_ray(int lanes);
-/* The lanes-per-ray mapping a march over `n_probes` probes will take under the current setting (the automatic rule
- * depends on the probe count only); bench.py reports it instead of restating the rule. */
-dex_status dex_get_lanes_per_ray(int64_t n_probes, int* lanes);
+/* The lanes-per-ray mapping a whole-spectrum fused-J march over `n_probes` probes x `n_dirs` directions will take under
+ * the current settings; bench.py reports it instead of restating the rule. */
+dex_status dex_get_lanes_per_ray(int64_t n_probes, int n_dirs, int* lanes);
 /* MEASURED fp32 arithmetic peak of the current device in TFLOP/s (an FMA counts 2 flops): register-resident chains of
  * scalar FFMA (*tflops_ffma) and of the packed two-wide FFMA2 the march's integrators use (*tflops_ffma2), ~15 ms in all,
  * timed with CUDA events on `stream`.  The denominator of the "alu" roofline of the Core-and-Voigt / Classic march

@@ -111,7 +111,7 @@ def _load():
     L.dex_set_lanes_per_ray.argtypes = [C.c_int]
     L.dex_set_tuning.argtypes = [C.c_char_p, C.c_int]
     L.dex_trim.argtypes = [C.POINTER(C.c_int64)]
-    L.dex_get_lanes_per_ray.argtypes = [C.c_int64, C.POINTER(C.c_int)]
+    L.dex_get_lanes_per_ray.argtypes = [C.c_int64, C.c_int, C.POINTER(C.c_int)]
     L.dex_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]
     return L
 
@@ -163,9 +163,9 @@ def dex_trim() -> int:
     return v.value
 
 
-def dex_get_lanes_per_ray(n_probes: int) -> int:
+def dex_get_lanes_per_ray(n_probes: int, n_dirs: int) -> int:
     v = C.c_int(0)
-    _check(_L.dex_get_lanes_per_ray(int(n_probes), C.byref(v)))
+    _check(_L.dex_get_lanes_per_ray(int(n_probes), int(n_dirs), C.byref(v)))
     return v.value
 
 

@@ -25,15 +25,10 @@ std::vector<EvPair> g_events;
 unsigned long long* g_d_line_segs = nullptr;   // device counter of (segment, active line) pairs, timing mode only
 
 // Lanes that share one ray.  One thread per ray (all W wavelengths in registers) is the fastest mapping whenever the
-// probes fill the machine (profiles/r01_history.md: 1.6-2.2x over 8 lanes on C2).  A small problem -- fewer
-// probes than one wave of 128-thread blocks on 148 SMs, e.g. C1's 4096 -- leaves most SMs idle with that mapping;
-// 8 lanes per ray give it 8x the threads (C1 march 0.403 -> 0.267 ms).  Depends on n_probes only, so every wavelength
-// stage of a pipelined solve takes the same mapping as the whole-spectrum call.
-int lanes_for(long long n_probes) {
-  const int set = g_lanes_per_ray.load();
-  if (set != 0) return set;
-  return (n_probes < 148LL * 128) ? 8 : 1;
-}
+// probes fill the machine (profiles/r01_history.md: 1.6-2.2x over 8 lanes on C2).  0 = automatic: dex_launch_march
+// (march.cu) decides from the probe count -- small problems take 8 lanes per ray, or 2 when they are also spread over
+// the machine direction by direction (C1: 0.415 -> 0.236 ms per step).
+int lanes_for(long long) { return g_lanes_per_ray.load(); }
 
 int ilog2_exact(int v) {
   if (v <= 0 || (v & (v - 1))) return -1;
@@ -257,9 +252,9 @@ dex_status dex_set_lanes_per_ray(int lanes) {
   return DEX_OK;
 }
 
-dex_status dex_get_lanes_per_ray(int64_t n_probes, int* lanes) {
+dex_status dex_get_lanes_per_ray(int64_t n_probes, int n_dirs, int* lanes) {
   if (!lanes) { dex_set_error("NULL lanes"); return DEX_ERR_INVALID_ARG; }
-  *lanes = lanes_for((long long)n_probes);
+  *lanes = dex_auto_lanes(lanes_for((long long)n_probes), (long long)n_probes, dex_auto_dir_split((long long)n_probes, n_dirs, 1));
   return DEX_OK;
 }
 

@@ -101,20 +101,27 @@ __device__ __forceinline__ bool dex_crossed(int k, float inv, float off, float t
 }
 
 // level-0 coordinate on axis a (inside the cell [lo, lo+size)) that the plain DDA would hold when
-// the ray crosses the exit plane of axis s at time th.  Guess from the position, then correct with
-// the monotone `crossed` predicate -- the result is the unique one defined by T5.
+// the ray crosses the exit plane of axis s at time th: the unique G in [lo, hi] with every plane up to G
+// crossed and none beyond (T5; `crossed` is monotone along the ray).  The position o + th d locates it to
+// within one voxel (plane times and position are fp32 evaluations of the same line, ~1e-4 voxel apart at
+// coordinates below 2^18), so the guess is corrected by one step from two evaluations of the predicate --
+// straight-line code (the correction loops this replaces were 11 % of the instructions of C2's march).
 __device__ __forceinline__ int dex_fine_coord(float o, float d, float inv, float off, int lo, int size,
                                               float th, bool lower_axis) {
   if (d == 0.0f) return (int)floorf(o);
   const int hi = lo + size - 1;
   int g = (int)floorf(__fmaf_rn(th, d, o));
   g = max(lo, min(hi, g));
+  const bool c0 = dex_crossed(g, inv, off, th, lower_axis);        // plane g
+  const bool c1 = dex_crossed(g + 1, inv, off, th, lower_axis);    // plane g + 1
   if (d > 0.0f) {
-    while (g < hi && dex_crossed(g + 1, inv, off, th, lower_axis)) ++g;
-    while (g > lo && !dex_crossed(g, inv, off, th, lower_axis)) --g;
+    // cell g holds the ray iff plane g is crossed (or g == lo) and plane g + 1 is not (or g == hi)
+    if (c1 && g < hi) return g + 1;
+    if (!c0 && g > lo) return g - 1;
   } else {
-    while (g > lo && dex_crossed(g, inv, off, th, lower_axis)) --g;
-    while (g < hi && !dex_crossed(g + 1, inv, off, th, lower_axis)) ++g;
+    // moving down: cell g holds the ray iff plane g + 1 is crossed (or g == hi) and plane g is not (or g == lo)
+    if (c0 && g > lo) return g - 1;
+    if (!c1 && g < hi) return g + 1;
   }
   return g;
 }
@@ -308,4 +315,73 @@ __device__ __forceinline__ bool dex_ray_cross(DexRay3<D>& r, const DexGridDev& G
     dex_set_cell<D>(r, G, M, info, x);
   }
   return alive;
+}
+
+// ---- the same two routines without the near-field cap (M.n_caps == 0, the default): the march kernel picks the pair
+// once per block.  The cap's threshold loops sit in the middle of the general routines; without them a crossing is
+// straight-line code apart from the rare re-entry into a finer brick (profiles/r02: the crossing was 25 % of the
+// instructions of C3's march).
+template <int D>
+__device__ __forceinline__ void dex_set_cell_nocap(DexRay3<D>& r, const DexGridDev& G, int info, const int* x) {
+  const int m = (info & 15) - 1;
+  const int sh = (m < 0) ? G.logB : m;
+  const int size = 1 << sh, lsh = G.logB - sh, bmask = G.B - 1;
+  const float fsize = (float)size;
+  r.info = info;
+  r.sh = sh;
+  int idx = 0;
+  float tb = __int_as_float(0x7f800000);
+#pragma unroll
+  for (int a = 0; a < D; ++a) {
+    const bool pos = r.dk[a] > 0.0f;
+    const int c = x[a] & -size;
+    r.kf[a] = (float)(pos ? c + size : c);
+    r.tn[a] = __fmaf_rn(r.kf[a], r.inv[a], r.off[a]);
+    r.dk[a] = pos ? fsize : -fsize;
+    const int bexit = pos ? (x[a] | bmask) + 1 : (x[a] & ~bmask);
+    tb = fminf(tb, __fmaf_rn((float)bexit, r.inv[a], r.off[a]));
+    idx += ((c & bmask) >> sh) << (a * lsh);
+    const int st = 1 << (a * lsh);
+    r.cstep[a] = pos ? st : -st;
+  }
+  r.tb = tb;
+  r.cell = (m < 0) ? -1 : (info >> 4) + idx;
+}
+
+template <int D>
+__device__ __forceinline__ bool dex_ray_cross_nocap(DexRay3<D>& r, const DexGridDev& G, const int* __restrict__ binfo,
+                                                    const float* __restrict__ probe, const float* __restrict__ omega) {
+  int s;
+  float th;
+  dex_ray_next_plane<D>(r, s, th);
+  const int size = 1 << r.sh;
+  int x[D], c[D];
+  bool alive = true, newbrick = false;
+#pragma unroll
+  for (int a = 0; a < D; ++a) {
+    const bool pos = r.dk[a] > 0.0f;
+    const int kp = (int)r.kf[a];                 // exit plane of the current cell (T3)
+    c[a] = pos ? kp - size : kp;                 // its low corner
+    const int xe = pos ? kp : kp - 1;            // level-0 coordinate just beyond the exit plane (T5)
+    const bool mv = (a == s);
+    x[a] = mv ? xe : c[a];
+    if (mv) {                                    // only the crossed axis can leave the grid or its brick
+      alive = (unsigned)xe < (unsigned)G.dims[a];
+      newbrick = ((xe ^ c[a]) >> G.logB) != 0;
+    }
+  }
+  if (!alive) return false;
+  int info = r.info;
+  if (newbrick) {
+    info = __ldg(binfo + dex_brick_of<D>(G, x));
+    const int m2 = (info & 15) - 1;
+    const int sh2 = (m2 < 0) ? G.logB : m2;
+    if (sh2 < r.sh) {
+#pragma unroll
+      for (int a = 0; a < D; ++a)
+        if (a != s) x[a] = dex_fine_coord(__ldg(probe + a), -__ldg(omega + a), r.inv[a], r.off[a], c[a], size, th, a < s);
+    }
+  }
+  dex_set_cell_nocap<D>(r, G, info, x);
+  return true;
 }

@@ -46,7 +46,11 @@ cudaError_t dex_alloc(void** p, size_t bytes, cudaStream_t st);
 void dex_free(void* p, cudaStream_t st);
 void dex_count_launch(int n = 1);
 int dex_tuning_voigt_fp32();
-int dex_tuning_dir_split();   // -1 automatic, 0 never, n > 0: n directions per block whenever J is fused
+int dex_tuning_dir_split();
+// automatic mapping of small problems (march.cu): does a fused-J march over n_probes x n_dirs spread its directions over
+// blocks (n_lambda only bounds the temporary I), and how many lanes share a ray (`set` = the caller's knob, 0 = automatic)
+bool dex_auto_dir_split(long long n_probes, int n_dirs, int n_lambda);
+int dex_auto_lanes(int set, long long n_probes, bool dir_split);   // -1 automatic, 0 never, n > 0: n directions per block whenever J is fused
 unsigned long long* dex_line_segment_counter();   // device counter, NULL unless march timing is enabled
 
 // grid_build.cu

@@ -239,7 +239,8 @@ struct DexCavTab {
   float r2lo[DEX_NLINES], r2hi[DEX_NLINES];   // min / max of r2f over the batch (slightly widened): damping window test
   float scale[DEX_NLINES][DEX_W];    // (lambda0 / lambda) / sqrt(pi): eta*(lambda) phi = eta*0 invD scale H (eqs. 18-19)
   double lam0_over_c[DEX_NLINES];    // Doppler shift of the line centre per unit projected velocity     (eq. 14)
-  int line[DEX_NLINES];              // active line of slot q or -1
+  int line[DEX_NLINES];              // the batch's active lines, compacted: slots 0 .. nq-1
+  int nq;                            // number of active lines of the batch
 };
 
 // the literal fp64 formula for damping outside the fp32 window: rare, so kept out of line (it would otherwise be
@@ -315,10 +316,10 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
   // Weideman form cancels in the wings); the line sum itself is fp32.  Everything that depends
   // on (wavelength, line) alone comes from the block's shared table CT (one batch per block).
   dex_load_rec<LPT>(iso0 + (size_t)(unsigned)cell * DEX_REC, sub, eta, chi);   // iso0 = this batch's background records
+  const int nq = CT.nq;                    // block-uniform
 #pragma unroll 1
-  for (int q = 0; q < DEX_NLINES; ++q) {   // not unrolled: the body is ~500 instructions and would be copied 4 times
+  for (int q = 0; q < nq; ++q) {           // not unrolled: the body is ~350 instructions and would be copied 4 times
     const int l = CT.line[q];
-    if (l < 0) continue;               // block-uniform
     const float4 ln = __ldg(arec + 1 + l);
     const double shift = vproj * CT.lam0_over_c[q];
     const float sh_h = (float)shift, sh_l = (float)(shift - (double)sh_h);
@@ -429,6 +430,9 @@ constexpr int dex_march_minb(int var) {
 #ifndef DEX_CROSS_QUORUM
 #define DEX_CROSS_QUORUM 8
 #endif
+#ifndef DEX_PREFETCH
+#define DEX_PREFETCH 0   // 0 none, 1 prefetch.global.L1, 2 prefetch.global.L2 of the next cell's records (Core-and-Voigt)
+#endif
 
 
 
@@ -469,9 +473,17 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
       vfc[i] = __ldg(M.vf_core + i);
     }
     if (threadIdx.x < DEX_NLINES * DEX_W) {
-      const int q = threadIdx.x / DEX_W, j = threadIdx.x % DEX_W;
-      const int l = M.active_lines[batch * DEX_NLINES + q];
-      if (j == 0) CT.line[q] = l;
+      // the caller's active set may have gaps (-1 anywhere): slot q of the table = the q-th ACTIVE line
+      const int q0 = threadIdx.x / DEX_W, j = threadIdx.x % DEX_W;
+      const int l = M.active_lines[batch * DEX_NLINES + q0];
+      int q = 0, total = 0;
+      for (int qq = 0; qq < DEX_NLINES; ++qq) {
+        const int on = (M.active_lines[batch * DEX_NLINES + qq] >= 0) ? 1 : 0;
+        q += (qq < q0) ? on : 0;
+        total += on;
+      }
+      if (threadIdx.x == 0) CT.nq = total;
+      if (j == 0 && l >= 0) CT.line[q] = l;
       if (l >= 0) {
         const double lm = (double)__ldg(M.lam + batch * DEX_W + j), l0 = (double)M.lambda0[l];
         const double r = lm / l0;
@@ -521,6 +533,7 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
     for (int i = 0; i < LPT; ++i) Jsm[i * DEX_MARCH_THREADS + threadIdx.x] = 0.0f;
   }
   DexRay3<D> ray;
+  const bool caps = M.n_caps > 0;     // block-uniform: which of the two crossing routines (dex_device.cuh) this launch runs
   // one direction at a time: the lanes of a warp trace the same direction together (coherent fetches)
   const int k_begin = (!FUSE_J && R.k_per_block > 0) ? (int)blockIdx.z * R.k_per_block : 0;
   const int k_end = (!FUSE_J && R.k_per_block > 0) ? min(R.n_dirs, k_begin + R.k_per_block) : R.n_dirs;
@@ -546,7 +559,7 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
       const unsigned bm = __ballot_sync(FULL, blocked);
       if (bm == am || __popc(bm) >= DEX_CROSS_QUORUM) {
         if (blocked) {
-          alive = dex_ray_cross<D>(ray, G, M, binfo, probe, om);
+          alive = caps ? dex_ray_cross<D>(ray, G, M, binfo, probe, om) : dex_ray_cross_nocap<D>(ray, G, binfo, probe, om);
           blocked = false;
         }
       }
@@ -561,11 +574,31 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
           emit = emit && ds > 0.0f;
           if (ray.t >= R.t_end) { alive = false; blocked = false; }
         }
+#if DEX_PREFETCH
+        // Core-and-Voigt in 3D waits on the latency of its per-cell records (profiles/r02: long_scoreboard 2.2 of 3.6
+        // warps per scheduler, DRAM at 27 %): after the in-brick step the NEXT cell is known one whole profile evaluation
+        // (~700 instructions) before its records are needed, so they are requested now
+        if ((VAR == DEX_CAV) && !blocked && ray.cell >= 0) {
+          const float* pb = iso0 + (size_t)(unsigned)ray.cell * DEX_REC;
+          const float4* pa = M.aux + dex_aux_vel(M, (size_t)(unsigned)ray.cell);
+#if DEX_PREFETCH == 1
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(pb));
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(pa));
+#else
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(pb));
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(pa));
+#endif
+        }
+#endif
         if (emit) {
           ++nseg;
           const float hds = hk * ds;
           float eta[LPT], chi[LPT];
+#ifdef DEX_FAKE_CELL   // experiment: every fetch from a tiny, cache-resident window of cells (results are wrong)
+          dex_provider<D, VAR, LPT>(M, batch_base, cell & 1023, sub, omf, sin_incl, CT, vfw, vfc, iso0, iso1, eta, chi);
+#else
           dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, omf, sin_incl, CT, vfw, vfc, iso0, iso1, eta, chi);
+#endif
           if (VAR == DEX_ISO) dex_accumulate_all_S<LPT>(eta, chi, hds, I, T);
           // velocity interpolation keeps the E(tau) integrator: the record form costs it registers it does not have at
           // 7 blocks per SM (measured on C3: 583 ms against 616; Core-and-Voigt gains 3 % from the record form)
@@ -606,9 +639,7 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
     if ((threadIdx.x & 31) == 0 && v) atomicAdd(seg_count, (unsigned long long)v);
   }
   if (VAR == DEX_CAV && line_seg_count != nullptr) {   // bench.py's ALU roofline: segments x active lines of the batch
-    int nact = 0;
-#pragma unroll
-    for (int q = 0; q < DEX_NLINES; ++q) nact += (CT.line[q] >= 0) ? 1 : 0;
+    const int nact = CT.nq;
     unsigned v = (sub == 0) ? nseg : 0u;
     v = __reduce_add_sync(FULL, v);
     if ((threadIdx.x & 31) == 0 && v && nact) atomicAdd(line_seg_count, (unsigned long long)v * (unsigned long long)nact);
@@ -867,6 +898,19 @@ dex_status dex_make_probe_tiling(const dex_grid* g, const DexRaysDev& rays, int*
   return (g->desc.ndim == 2) ? tile_probes_t<2>(g, rays, d_perm, st) : tile_probes_t<3>(g, rays, d_perm, st);
 }
 
+bool dex_auto_dir_split(long long n_probes, int n_dirs, int n_lambda) {
+  const int split = dex_tuning_dir_split();
+  const size_t i_floats = (size_t)n_probes * (size_t)n_dirs * (size_t)n_lambda;
+  const bool small = n_probes < 148LL * 128 && n_dirs > 1 && i_floats <= (64u << 20);
+  return split > 0 || (split < 0 && small);
+}
+
+int dex_auto_lanes(int set, long long n_probes, bool dir_split) {
+  if (set != 0) return set;
+  if (n_probes >= 148LL * 128) return 1;
+  return dir_split ? 2 : 8;      // swept on C1 with the split: 1 / 2 / 4 / 8 lanes give 0.254 / 0.236 / 0.251 / 0.265 ms per step
+}
+
 dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out, bool fuse_j,
                             unsigned long long* d_seg, int lanes_per_ray, bool tile, cudaStream_t st,
                             const int* perm_in) {
@@ -883,13 +927,13 @@ dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysD
   float* d_I = nullptr;
   const size_t i_floats = (size_t)rays.n_probes * (size_t)rays.n_dirs * (size_t)m->n_lambda;
   const int split = dex_tuning_dir_split();
-  const bool small = rays.n_probes < 148LL * 128 && rays.n_dirs > 1 && i_floats <= (64u << 20);
-  if (s == DEX_OK && fuse_j && (split > 0 || (split < 0 && small)) && m->dev.io_base == 0 && m->dev.io_stride == m->n_lambda &&
-      rays.t_end <= 0.0f) {
+  if (s == DEX_OK && fuse_j && dex_auto_dir_split(rays.n_probes, rays.n_dirs, m->n_lambda) && m->dev.io_base == 0 &&
+      m->dev.io_stride == m->n_lambda && rays.t_end <= 0.0f) {
     cudaError_t e = dex_alloc((void**)&d_I, sizeof(float) * i_floats, st);
     if (e != cudaSuccess) { cudaGetLastError(); d_I = nullptr; }     // no room: the fused path needs none
     else r.k_per_block = (split > 0) ? split : 1;
   }
+  lanes_per_ray = dex_auto_lanes(lanes_per_ray, rays.n_probes, d_I != nullptr);
   if (s == DEX_OK) {
     float* out = d_I ? d_I : d_out;
     const bool fj = d_I ? false : fuse_j;
