@@ -341,16 +341,23 @@ class Bench:
         eff_gbs = ALGO_BYTES[wl.variant] * sl / t / 1e9 if t > 0 else 0.0
         pk = self.measure_fp32_peak()
         fp32_peak = max(pk["ffma_tflops"], pk["ffma2_tflops"])
+        # the library counts provider evaluations (dex_march_work_read): one per emitted segment when eta, chi are evaluated
+        # inside the march, one per (cell, direction, batch) when they are memoised per direction
+        evals = line_segs_per_launch * W                          # per wavelength (x active lines for Core-and-Voigt)
+        memoised = wl.variant != 0 and line_segs_per_launch < 0.5 * segs_per_launch
+        integral = FLOPS_INTEGRAL * sl + FLOPS_HDDA_PER_SEGMENT * segs_per_launch
         if wl.variant in (2, 3):
-            flops = CAV_FLOPS_PER_LINE_EVAL * line_segs_per_launch * W + CAV_FLOPS_PER_SEG_LAMBDA * sl
-            what = (f"{CAV_FLOPS_PER_LINE_EVAL:g} per (segment, lambda, active line) for the fp32 profile + line sum, "
-                    f"{CAV_FLOPS_PER_SEG_LAMBDA:g} per seg*lambda for the integral; the library counts segments x active lines")
-            binds = "fp32 arithmetic (one Voigt profile per segment, wavelength and active line)"
+            flops = CAV_FLOPS_PER_LINE_EVAL * evals + integral
+            what = (f"{CAV_FLOPS_PER_LINE_EVAL:g} per fp32 Voigt profile evaluation + line sum (the library counts them: "
+                    f"{evals:.3g} per launch, {'memoised per (cell, direction)' if memoised else 'one per segment, wavelength and active line'}), "
+                    f"{FLOPS_INTEGRAL:g} per seg*lambda for the segment integral, {FLOPS_HDDA_PER_SEGMENT:g} per segment of HDDA stepping")
+            binds = ("instruction issue of the ISO march over per-direction records (the Voigt profiles are evaluated once per cell "
+                     "and direction)" if memoised else "fp32 arithmetic (one Voigt profile per segment, wavelength and active line)")
         else:
-            per = FLOPS_INTEGRAL + (FLOPS_VEL_LERP if wl.variant == 1 else 0.0)
-            flops = per * sl + FLOPS_HDDA_PER_SEGMENT * segs_per_launch
-            what = (f"{per:g} per seg*lambda (segment integral{' + two velocity-bin lerps' if wl.variant == 1 else ''}) + "
-                    f"{FLOPS_HDDA_PER_SEGMENT:g} per segment of HDDA stepping")
+            flops = integral + FLOPS_VEL_LERP * evals
+            what = (f"{FLOPS_INTEGRAL:g} per seg*lambda (segment integral) + {FLOPS_HDDA_PER_SEGMENT:g} per segment of HDDA stepping"
+                    + (f" + {FLOPS_VEL_LERP:g} per velocity-bin interpolation ({evals:.3g} per launch, "
+                       f"{'memoised per (cell, direction)' if memoised else 'one per seg*lambda'})" if wl.variant == 1 else ""))
             binds = ("instruction issue (fp32 / integer pipes + one MUFU ex2 per seg*lambda); the batch's records are "
                      "L1/L2-resident because every cell is revisited by 1e2-1e3 rays, so DRAM is idle by construction")
         ach = flops / t / 1e12 if t > 0 else 0.0

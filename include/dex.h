@@ -289,9 +289,10 @@ dex_status dex_trim(int64_t* bytes_reserved_after);
  * events on the launching stream when timing is enabled (bench.py roofline leg).  Synchronises. */
 void dex_march_timing_enable(int on);
 dex_status dex_march_timing_read(double* ms_total, int64_t* n_launches, int reset);
-/* Work counter of the Core-and-Voigt / Classic march while timing is enabled: sum over emitted segments of the
- * number of active lines of the segment's batch, i.e. line-profile evaluations / W (bench.py's ALU roofline leg
- * multiplies by W and by the flops per evaluation stated in DESIGN.md).  Synchronises. */
+/* Work counter of the anisotropic marches while timing is enabled: provider evaluations / W -- one per emitted segment
+ * when eta, chi are evaluated inside the march, one per (cell, direction, batch) record when they are memoised per
+ * direction ("memo" below) -- times the number of active lines of the batch for Core-and-Voigt / Classic (bench.py's
+ * roofline leg multiplies by W and by the flops per evaluation stated in DESIGN.md).  Synchronises. */
 dex_status dex_march_work_read(int64_t* line_segments, int reset);
 /* Kernel configuration knob: lanes that share one ray, 1/2/4/8, or 0 (default) = automatic: one thread per ray unless
  * there are fewer probes than one wave of blocks (148 SMs x 128 threads), where 8 lanes per ray fill the machine better
@@ -311,7 +312,10 @@ dex_status dex_measure_fp32_peak(double* tflops_ffma, double* tflops_ffma2, void
  * its fp32 table form inside the damping window of csrc/dex_voigt.cuh; 0: the fp64 form everywhere -- results agree
  * to ~1e-6); "dir_split" -1 (default: automatic), 0, n: a fused-J march over fewer probes than one wave of blocks is
  * launched as one block per (probe tile, batch, n directions) into a temporary I and summed by the reduction kernel in
- * the fused kernel's order (bit-identical J); 0 never, n > 0 always. */
+ * the fused kernel's order (bit-identical J); 0 never, n > 0 always; "memo" -1 (default: automatic), 0, 1: the
+ * anisotropic marches (velocity interpolation, Core-and-Voigt, Classic) evaluate eta, chi once per (cell, direction,
+ * batch) into per-direction march records and march those with the ISO kernel, instead of once per ray segment, when a
+ * cell is crossed by many rays per direction (a probe in every voxel: hundreds); same routine, same numbers up to the last bits of the record rounding. */
 dex_status dex_set_tuning(const char* name, int value);
 
 #ifdef __cplusplus

@@ -19,6 +19,7 @@ std::atomic<int> g_timing{0};
 std::atomic<int> g_tile_probes{1};
 std::atomic<int> g_voigt_fp32{1};
 std::atomic<int> g_dir_split{-1};
+std::atomic<int> g_memo{-1};
 std::mutex g_timing_mu;
 struct EvPair { cudaEvent_t a, b; };
 std::vector<EvPair> g_events;
@@ -208,6 +209,7 @@ void dex_set_error(const std::string& msg) { g_last_error = msg; }
 void dex_count_launch(int n) { g_launches.fetch_add(n); }
 int dex_tuning_voigt_fp32() { return g_voigt_fp32.load(); }
 int dex_tuning_dir_split() { return g_dir_split.load(); }
+int dex_tuning_memo() { return g_memo.load(); }
 unsigned long long* dex_line_segment_counter() { return g_timing.load() ? g_d_line_segs : nullptr; }
 
 extern "C" {
@@ -264,6 +266,7 @@ dex_status dex_set_tuning(const char* name, int value) {
   if (!strcmp(name, "tile_probes")) { g_tile_probes.store(value ? 1 : 0); return DEX_OK; }
   if (!strcmp(name, "voigt_fp32")) { g_voigt_fp32.store(value ? 1 : 0); return DEX_OK; }
   if (!strcmp(name, "dir_split")) { g_dir_split.store(value < 0 ? -1 : value); return DEX_OK; }
+  if (!strcmp(name, "memo")) { g_memo.store(value < 0 ? -1 : (value ? 1 : 0)); return DEX_OK; }
   dex_set_error("unknown tuning knob");
   return DEX_ERR_INVALID_ARG;
 }

@@ -42,6 +42,8 @@ struct DexMipsDev {
   const float* mrec;                 // ISO march records (make_march_records_kernel), what the ISO march reads: two planes
   size_t mplane;                     // [2][n_batch][n_active][cps][DEX_W], plane 0 chi log2(e), plane 1 S = eta/chi;
                                      // mplane = floats per plane
+  size_t mdir;                       // 0, or floats between the records of consecutive DIRECTIONS (Core-and-Voigt memoised
+                                     // per direction, march.cu: mrec then holds [n_dirs][2][n_batch][n_active][cps][DEX_W])
   const float4* aux;                 // [n_active][cps][1 + n_lines]: (vx, vy, vz, max|v|) then per line (eta*, chi*, a0,
                                      // 1/dlamD), see dex_aux_vel / dex_aux_line
   int aux_vs, aux_ls;                // float4 strides of the velocity and of a cell's line records
@@ -356,20 +358,28 @@ __device__ __forceinline__ bool dex_ray_cross_nocap(DexRay3<D>& r, const DexGrid
   dex_ray_next_plane<D>(r, s, th);
   const int size = 1 << r.sh;
   int x[D], c[D];
-  bool alive = true, newbrick = false;
-#pragma unroll
-  for (int a = 0; a < D; ++a) {
-    const bool pos = r.dk[a] > 0.0f;
-    const int kp = (int)r.kf[a];                 // exit plane of the current cell (T3)
-    c[a] = pos ? kp - size : kp;                 // its low corner
-    const int xe = pos ? kp : kp - 1;            // level-0 coordinate just beyond the exit plane (T5)
-    const bool mv = (a == s);
-    x[a] = mv ? xe : c[a];
-    if (mv) {                                    // only the crossed axis can leave the grid or its brick
-      alive = (unsigned)xe < (unsigned)G.dims[a];
-      newbrick = ((xe ^ c[a]) >> G.logB) != 0;
-    }
+  // exit plane kp, low corner c of the current cell per axis (T3); scalars of the crossed axis by select, not by index
+  int kps = (int)r.kf[0], dims_s = G.dims[0];
+  bool poss = r.dk[0] > 0.0f;
+  c[0] = poss ? kps - size : kps;
+  if (D >= 2) {
+    const int kp1 = (int)r.kf[1];
+    const bool pos1 = r.dk[1] > 0.0f;
+    c[1] = pos1 ? kp1 - size : kp1;
+    if (s == 1) { kps = kp1; poss = pos1; dims_s = G.dims[1]; }
   }
+  if (D == 3) {
+    const int kp2 = (int)r.kf[D - 1];
+    const bool pos2 = r.dk[D - 1] > 0.0f;
+    c[D - 1] = pos2 ? kp2 - size : kp2;
+    if (s == D - 1) { kps = kp2; poss = pos2; dims_s = G.dims[D - 1]; }
+  }
+  const int xe = poss ? kps : kps - 1;           // level-0 coordinate just beyond the exit plane (T5)
+  const int cs = poss ? kps - size : kps;
+  const bool alive = (unsigned)xe < (unsigned)dims_s;
+  const bool newbrick = ((xe ^ cs) >> G.logB) != 0;
+#pragma unroll
+  for (int a = 0; a < D; ++a) x[a] = (a == s) ? xe : c[a];
   if (!alive) return false;
   int info = r.info;
   if (newbrick) {

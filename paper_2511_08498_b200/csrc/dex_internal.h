@@ -46,6 +46,7 @@ cudaError_t dex_alloc(void** p, size_t bytes, cudaStream_t st);
 void dex_free(void* p, cudaStream_t st);
 void dex_count_launch(int n = 1);
 int dex_tuning_voigt_fp32();
+int dex_tuning_memo();    // -1 automatic, 0 never, 1 always: anisotropic provider memoised per direction (march.cu)
 int dex_tuning_dir_split();
 // automatic mapping of small problems (march.cu): does a fused-J march over n_probes x n_dirs spread its directions over
 // blocks (n_lambda only bounds the temporary I), and how many lanes share a ray (`set` = the caller's knob, 0 = automatic)

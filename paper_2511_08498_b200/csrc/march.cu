@@ -399,76 +399,11 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
   }
 }
 
-// Each lane group owns one probe and loops over the quadrature directions.
-//
-// Control structure (profiles/r01c-r01e): the loop over HDDA events is warp-synchronous.  Every iteration each live
-// lane leaves one cell (dex_ray_advance: segment, in-brick move) and the emitting lanes integrate together.  A lane
-// whose ray reaches a brick face does NOT take the general crossing at once: it waits (`blocked`) until a quorum of
-// the warp's lanes wait too, or nobody else can move, and then they cross together.  With 29 rays per warp each
-// meeting a face every ~17 steps, crossing at once would run the ~100-instruction general path on 4 lanes in 82 % of
-// the iterations (measured); batched, it runs on >= DEX_CROSS_QUORUM lanes a quarter as often.
-#ifndef DEX_MARCH_THREADS
-#define DEX_MARCH_THREADS 128
-#endif
-#ifndef DEX_MARCH_MINB
-#define DEX_MARCH_MINB 8
-#endif
-// resident blocks per SM asked of the compiler per variant: the ISO march fits 64 registers; the velocity tables
-// want two records in flight, and Core-and-Voigt runs 8 independent fp64 Goertzel chains per line
-#ifndef DEX_MINB_VEL
-#define DEX_MINB_VEL 7   // swept 4..8 on C3: 774 / 675 / 665 / 631 / 678 ms (profiles/r01k)
-#endif
-#ifndef DEX_MINB_CAV
-#define DEX_MINB_CAV 4
-#endif
-constexpr int dex_march_minb(int var) {
-  return var == DEX_ISO ? DEX_MARCH_MINB : (var == DEX_VELINTERP ? DEX_MINB_VEL : DEX_MINB_CAV);
-}
-#ifndef DEX_FOLD_EVERY
-#define DEX_FOLD_EVERY 32   // power of two
-#endif
-#ifndef DEX_CROSS_QUORUM
-#define DEX_CROSS_QUORUM 8
-#endif
-#ifndef DEX_PREFETCH
-#define DEX_PREFETCH 0   // 0 none, 1 prefetch.global.L1, 2 prefetch.global.L2 of the next cell's records (Core-and-Voigt)
-#endif
-
-
-
-template <int D, int VAR, int LPR, bool FUSE_J, bool CLIP>
-__global__ void __launch_bounds__(DEX_MARCH_THREADS, dex_march_minb(VAR))
-dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ perm,
-                 float* __restrict__ out, unsigned long long* __restrict__ seg_count,
-                 unsigned long long* __restrict__ line_seg_count) {
-  constexpr int LPT = DEX_W / LPR;
-  constexpr unsigned FULL = 0xffffffffu;
-  __shared__ float Jsm[FUSE_J ? LPT * DEX_MARCH_THREADS : 1];
-  const int batch = blockIdx.y;
-  const long long slot_id = ((long long)blockIdx.x * blockDim.x + threadIdx.x) / LPR;
-  const bool valid = slot_id < R.n_probes;          // lanes past the end stay in the warp-synchronous loops, idle
-  // probes are handed to lanes in tile order (dex_tile_probes): a warp's probes are spatial neighbours
-  const long long gid = !valid ? 0 : (perm != nullptr ? (long long)perm[slot_id] : slot_id);
-  const int sub = threadIdx.x % LPR;
-  const int lam_off = batch * DEX_W + sub * LPT;
-  unsigned nseg = 0;
-  const int* binfo = M.binfo + (size_t)batch * G.n_bricks;
-  asm volatile("" : "+l"(binfo));   // opaque for the same reason as iso0 / iso1 below
-  const size_t batch_base = ((size_t)batch * G.n_active) * M.cps;
-  // this lane's rows of the two ISO record planes (cell 0 of the batch); kept opaque so that the pointers stay in
-  // registers instead of being rebuilt from the kernel parameters at every segment
-  // (velocity interpolation: iso0 = this batch's velocity tables; Core-and-Voigt / Classic: its background records)
-  const float* iso0 = (VAR == DEX_ISO) ? M.mrec + batch_base * DEX_W + sub * LPT
-                      : (VAR == DEX_VELINTERP) ? M.vtab + batch_base * (size_t)M.n_vbins * DEX_REC
-                                               : M.store + batch_base * DEX_REC;
-  const float* iso1 = iso0 + M.mplane;
-  asm volatile("" : "+l"(iso0), "+l"(iso1));
-  const float* __restrict__ probe = R.probe_pos + gid * D;
-  __shared__ DexCavTab CT;
-  __shared__ float4 vfw[VAR == DEX_CAV ? DEX_VF_NODES : 1];
-  __shared__ float vfc[VAR == DEX_CAV ? DEX_VF_NODES : 1];
-  if (VAR == DEX_CAV) {
-    for (int i = threadIdx.x; i < DEX_VF_NODES; i += DEX_MARCH_THREADS) {
+// Block prologue of the Core-and-Voigt evaluation: the fp32 Voigt tables and everything that depends on (wavelength of
+// the batch, active line) only go to shared memory (eqs. 14, 18-20).  Ends with a barrier.
+__device__ __forceinline__ void dex_cav_block_setup(const DexMipsDev& M, int batch, DexCavTab& CT, float4* vfw, float* vfc) {
+  {
+    for (int i = threadIdx.x; i < DEX_VF_NODES; i += blockDim.x) {
       vfw[i] = __ldg(M.vf_wing + i);
       vfc[i] = __ldg(M.vf_core + i);
     }
@@ -513,6 +448,81 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
     }
     __syncthreads();
   }
+}
+
+// Each lane group owns one probe and loops over the quadrature directions.
+//
+// Control structure (profiles/r01c-r01e): the loop over HDDA events is warp-synchronous.  Every iteration each live
+// lane leaves one cell (dex_ray_advance: segment, in-brick move) and the emitting lanes integrate together.  A lane
+// whose ray reaches a brick face does NOT take the general crossing at once: it waits (`blocked`) until a quorum of
+// the warp's lanes wait too, or nobody else can move, and then they cross together.  With 29 rays per warp each
+// meeting a face every ~17 steps, crossing at once would run the ~100-instruction general path on 4 lanes in 82 % of
+// the iterations (measured); batched, it runs on >= DEX_CROSS_QUORUM lanes a quarter as often.
+#ifndef DEX_MARCH_THREADS
+#define DEX_MARCH_THREADS 128
+#endif
+#ifndef DEX_MARCH_MINB
+#define DEX_MARCH_MINB 8
+#endif
+// resident blocks per SM asked of the compiler per variant: the ISO march fits 64 registers; the velocity tables
+// want two records in flight, and Core-and-Voigt runs 8 independent fp64 Goertzel chains per line
+#ifndef DEX_MINB_VEL
+#define DEX_MINB_VEL 7   // swept 4..8 on C3: 774 / 675 / 665 / 631 / 678 ms (profiles/r01k)
+#endif
+#ifndef DEX_MINB_CAV
+#define DEX_MINB_CAV 4
+#endif
+constexpr int dex_march_minb(int var) {
+  return var == DEX_ISO ? DEX_MARCH_MINB : (var == DEX_VELINTERP ? DEX_MINB_VEL : DEX_MINB_CAV);
+}
+#ifndef DEX_FOLD_EVERY
+#define DEX_FOLD_EVERY 32   // power of two
+#endif
+#ifndef DEX_CROSS_QUORUM
+#define DEX_CROSS_QUORUM 8
+#endif
+#ifndef DEX_MEMO_MIN_REUSE
+#define DEX_MEMO_MIN_REUSE 12.0   // rays per (cell, direction) from which the memoised march is taken:
+                                      // C5 (5 rays per cell and direction) is 1.26x slower memoised, a 1/32 probe band of C4 (18) 2.5x faster
+#endif
+#ifndef DEX_PREFETCH
+#define DEX_PREFETCH 0   // 0 none, 1 prefetch.global.L1, 2 prefetch.global.L2 of the next cell's records (Core-and-Voigt)
+#endif
+
+
+
+template <int D, int VAR, int LPR, bool FUSE_J, bool CLIP>
+__global__ void __launch_bounds__(DEX_MARCH_THREADS, dex_march_minb(VAR))
+dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ perm,
+                 float* __restrict__ out, unsigned long long* __restrict__ seg_count,
+                 unsigned long long* __restrict__ line_seg_count) {
+  constexpr int LPT = DEX_W / LPR;
+  constexpr unsigned FULL = 0xffffffffu;
+  __shared__ float Jsm[FUSE_J ? LPT * DEX_MARCH_THREADS : 1];
+  const int batch = blockIdx.y;
+  const long long slot_id = ((long long)blockIdx.x * blockDim.x + threadIdx.x) / LPR;
+  const bool valid = slot_id < R.n_probes;          // lanes past the end stay in the warp-synchronous loops, idle
+  // probes are handed to lanes in tile order (dex_tile_probes): a warp's probes are spatial neighbours
+  const long long gid = !valid ? 0 : (perm != nullptr ? (long long)perm[slot_id] : slot_id);
+  const int sub = threadIdx.x % LPR;
+  const int lam_off = batch * DEX_W + sub * LPT;
+  unsigned nseg = 0;
+  const int* binfo = M.binfo + (size_t)batch * G.n_bricks;
+  asm volatile("" : "+l"(binfo));   // opaque for the same reason as iso0 / iso1 below
+  const size_t batch_base = ((size_t)batch * G.n_active) * M.cps;
+  // this lane's rows of the two ISO record planes (cell 0 of the batch); kept opaque so that the pointers stay in
+  // registers instead of being rebuilt from the kernel parameters at every segment
+  // (velocity interpolation: iso0 = this batch's velocity tables; Core-and-Voigt / Classic: its background records)
+  const float* iso0 = (VAR == DEX_ISO) ? M.mrec + batch_base * DEX_W + sub * LPT
+                      : (VAR == DEX_VELINTERP) ? M.vtab + batch_base * (size_t)M.n_vbins * DEX_REC
+                                               : M.store + batch_base * DEX_REC;
+  const float* iso1 = iso0 + M.mplane;
+  asm volatile("" : "+l"(iso0), "+l"(iso1));
+  const float* __restrict__ probe = R.probe_pos + gid * D;
+  __shared__ DexCavTab CT;
+  __shared__ float4 vfw[VAR == DEX_CAV ? DEX_VF_NODES : 1];
+  __shared__ float vfc[VAR == DEX_CAV ? DEX_VF_NODES : 1];
+  if (VAR == DEX_CAV) dex_cav_block_setup(M, batch, CT, vfw, vfc);
   // J is touched once per direction, I and T once per segment: J lives in shared memory ([i][thread], conflict-free)
   // I is accumulated on two levels: I[] (registers) holds the sum over the last <= DEX_FOLD_EVERY iterations of the
   // warp's loop, Ih[] (shared memory, [i][thread], conflict free) everything before.  With one level, a ray of ~1000
@@ -536,6 +546,10 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   const bool caps = M.n_caps > 0;     // block-uniform: which of the two crossing routines (dex_device.cuh) this launch runs
   // one direction at a time: the lanes of a warp trace the same direction together (coherent fetches)
   const int k_begin = (!FUSE_J && R.k_per_block > 0) ? (int)blockIdx.z * R.k_per_block : 0;
+  if (VAR == DEX_ISO && M.mdir != 0) {   // per-direction records (memoised Core-and-Voigt, below): direction k's start at k mdir
+    iso0 += (size_t)k_begin * M.mdir;
+    iso1 += (size_t)k_begin * M.mdir;
+  }
   const int k_end = (!FUSE_J && R.k_per_block > 0) ? min(R.n_dirs, k_begin + R.k_per_block) : R.n_dirs;
   for (int k = k_begin; k < k_end; ++k) {
     const float* __restrict__ om = R.dirs + k * D;
@@ -607,6 +621,7 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
         }
       }
     }
+    if (VAR == DEX_ISO && M.mdir != 0) { iso0 += M.mdir; iso1 += M.mdir; }
     if (valid) {
 #pragma unroll
       for (int i = 0; i < LPT; ++i) I[i] += DEX_IH(i);
@@ -638,11 +653,69 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
     v = __reduce_add_sync(FULL, v);
     if ((threadIdx.x & 31) == 0 && v) atomicAdd(seg_count, (unsigned long long)v);
   }
-  if (VAR == DEX_CAV && line_seg_count != nullptr) {   // bench.py's ALU roofline: segments x active lines of the batch
-    const int nact = CT.nq;
+  if (VAR != DEX_ISO && line_seg_count != nullptr) {   // bench.py's roofline: provider evaluations (x active lines of the batch)
+    const int nact = (VAR == DEX_CAV) ? CT.nq : 1;
     unsigned v = (sub == 0) ? nseg : 0u;
     v = __reduce_add_sync(FULL, v);
     if ((threadIdx.x & 31) == 0 && v && nact) atomicAdd(line_seg_count, (unsigned long long)v * (unsigned long long)nact);
+  }
+}
+
+// ---- anisotropic providers, memoised per direction ----------------------------------------------------------------
+// eta, chi of a cell along direction k (eqs. 10-20; the velocity-bin interpolation of PAPER.md:196-198) depend on
+// (cell, k, wavelength) only, and with a probe in every voxel each (cell, direction) is crossed by hundreds of rays
+// (C3, C4: ~600), every one of which would evaluate the same Voigt profiles / interpolate the same two bins.
+// This kernel evaluates the provider ONCE per (cell of the brick's selected level, direction, batch)
+// -- the very routine the march calls, so the numbers are the march's own -- and stores them as march records
+// (chi' log2 e | S, the ISO layout); the rays are then marched by the ISO kernel with M.mdir stepping the record
+// pointers from direction to direction.
+template <int D, int VAR>
+__global__ void __launch_bounds__(DEX_MARCH_THREADS)
+dex_dir_records_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ active_bricks,
+                       int b0, float* __restrict__ rec, size_t plane, unsigned long long* __restrict__ line_eval_count) {
+  __shared__ DexCavTab CT;
+  __shared__ float4 vfw[VAR == DEX_CAV ? DEX_VF_NODES : 1];
+  __shared__ float vfc[VAR == DEX_CAV ? DEX_VF_NODES : 1];
+  const int bl = blockIdx.y, batch = b0 + bl, k = blockIdx.z;
+  if (VAR == DEX_CAV) dex_cav_block_setup(M, batch, CT, vfw, vfc);
+  // one thread per pyramid cell of an active brick: the brick's selected level for this batch is the one the rays visit;
+  // under a near-field cap (T8) they also visit the finer levels of the same brick
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  bool work = t < (long long)G.n_active * M.cps;
+  const int cell = (int)t;                         // record index: slot * cps + position in the slot's pyramid
+  if (work) {
+    const int slot = (int)(t / M.cps), c = (int)(t - (long long)slot * M.cps);
+    const int info = __ldg(M.binfo + (size_t)batch * G.n_bricks + active_bricks[slot]);
+    const int m = (info & 15) - 1;
+    int l = 0;
+    for (int i = 1; i <= M.max_level; ++i) l += (c >= M.lvloff[i]) ? 1 : 0;
+    work = m >= 0 && (l == m || (M.n_caps > 0 && l < m));
+  }
+  unsigned done = 0;
+  if (work) {
+    float omf[D];
+#pragma unroll
+    for (int a = 0; a < D; ++a) omf[a] = __ldg(R.dirs + (size_t)k * D + a);
+    const float sin_incl = (D == 2 && R.sin_incl != nullptr) ? __ldg(R.sin_incl + k) : 1.0f;
+    const size_t batch_base = ((size_t)batch * G.n_active) * M.cps;
+    // what the march keeps in iso0: this batch's background records (Core-and-Voigt) / velocity tables
+    const float* bg = (VAR == DEX_VELINTERP) ? M.vtab + batch_base * (size_t)M.n_vbins * DEX_REC : M.store + batch_base * DEX_REC;
+    float eta[DEX_W], chi[DEX_W];
+    dex_provider<D, VAR, DEX_W>(M, batch_base, cell, 0, omf, sin_incl, CT, vfw, vfc, bg, bg, eta, chi);
+    float* o0 = rec + (size_t)k * M.mdir + (((size_t)bl * G.n_active) * M.cps + (size_t)(unsigned)cell) * DEX_W;
+    float* o1 = o0 + plane;
+#pragma unroll
+    for (int j = 0; j < DEX_W; ++j) {
+      const float cj = fmaxf(chi[j], DEX_CHI_TINY);
+      o0[j] = cj * 1.4426950408889634f;
+      o1[j] = eta[j] * dex_rcp(cj);
+    }
+    done = 1;
+  }
+  if (line_eval_count != nullptr) {    // bench.py's roofline counts provider evaluations: records (x active lines) here
+    const unsigned v = __reduce_add_sync(0xffffffffu, done);
+    const int nact = (VAR == DEX_CAV) ? CT.nq : 1;
+    if ((threadIdx.x & 31) == 0 && v && nact) atomicAdd(line_eval_count, (unsigned long long)v * (unsigned long long)nact);
   }
 }
 
@@ -898,6 +971,77 @@ dex_status dex_make_probe_tiling(const dex_grid* g, const DexRaysDev& rays, int*
   return (g->desc.ndim == 2) ? tile_probes_t<2>(g, rays, d_perm, st) : tile_probes_t<3>(g, rays, d_perm, st);
 }
 
+// Anisotropic marches with many rays per (cell, direction): evaluate the provider once per (cell, direction, batch) into
+// per-direction march records (dex_dir_records_kernel) and march them with the ISO kernel, a group of
+// wavelength batches at a time so that the records fit the memory set aside for them.  J columns of different batches
+// are disjoint, so the groups need no accumulation.
+template <int D>
+static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out,
+                                        bool fuse_j, unsigned long long* d_seg, int lpr, const int* perm, cudaStream_t st,
+                                        int batches_per_group) {
+  const size_t A = (size_t)g->n_active, cps = (size_t)m->dev.cps;
+  for (int b0 = 0; b0 < m->n_batch; b0 += batches_per_group) {
+    const int nb = (b0 + batches_per_group <= m->n_batch) ? batches_per_group : m->n_batch - b0;
+    const size_t plane = (size_t)nb * A * cps * DEX_W;
+    float* d_rec = nullptr;
+    DEX_CUDA_CHECK(dex_alloc((void**)&d_rec, sizeof(float) * 2 * plane * (size_t)rays.n_dirs, st));
+    dex_mips mm = *m;                       // a view of the group's batches as an ISO handle over the records
+    mm.variant = DEX_ISO;
+    mm.n_batch = nb;
+    DexMipsDev& d = mm.dev;
+    d.variant = DEX_ISO;
+    d.n_batch = nb;
+    d.mdir = 2 * plane;
+    const long long tasks = (long long)A * (long long)cps;
+    dim3 grid((unsigned)((tasks + DEX_MARCH_THREADS - 1) / DEX_MARCH_THREADS), (unsigned)nb, (unsigned)rays.n_dirs);
+    DexMipsDev full = m->dev;
+    full.mdir = 2 * plane;
+    full.voigt_fp32 = dex_tuning_voigt_fp32();
+    dex_status s = DEX_OK;
+    if (rays.n_dirs > 65535) { dex_set_error("march: too many directions for the per-direction record launch"); s = DEX_ERR_UNSUPPORTED; }
+    if (s == DEX_OK && tasks > 0) {
+      if (m->variant == DEX_VELINTERP)
+        dex_dir_records_kernel<D, DEX_VELINTERP><<<grid, DEX_MARCH_THREADS, 0, st>>>(g->dev, full, rays, g->d_active_bricks, b0,
+                                                                                    d_rec, plane, dex_line_segment_counter());
+      else
+        dex_dir_records_kernel<D, DEX_CAV><<<grid, DEX_MARCH_THREADS, 0, st>>>(g->dev, full, rays, g->d_active_bricks, b0, d_rec,
+                                                                              plane, dex_line_segment_counter());
+      dex_count_launch();
+      if (cudaGetLastError() != cudaSuccess) { dex_set_error("record kernel launch failed"); s = DEX_ERR_CUDA; }
+    }
+    if (s == DEX_OK) {
+      d.mrec = d_rec;
+      d.mplane = plane;
+      d.binfo = m->dev.binfo + (size_t)b0 * g->n_bricks;
+      d.io_base = m->dev.io_base + b0 * DEX_W;
+      s = launch_march_v<D, DEX_ISO>(g, &mm, rays, d_out, fuse_j, d_seg, lpr, perm, st);
+    }
+    dex_free(d_rec, st);
+    if (s != DEX_OK) return s;
+  }
+  return DEX_OK;
+}
+
+// How many wavelength batches' per-direction records the memoised march may hold at once; 0 = do not memoise (a static
+// medium, too few rays per cell and direction for the evaluation to be shared, or no room for one batch).
+static int memo_group(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays) {
+  if (m->variant == DEX_ISO) return 0;
+  const int knob = dex_tuning_memo();
+  if (knob == 0 || rays.n_dirs <= 0 || g->n_active <= 0) return 0;
+  const int D = g->desc.ndim;
+  double cells0 = 1.0, mean_dim = 0.0;
+  for (int a = 0; a < D; ++a) { cells0 *= (double)g->dev.B; mean_dim += (double)g->dev.dims[a] / D; }
+  // rays through a level-0 cell per direction: probes x a typical path length (0.4 of the box) / active cells
+  const double reuse = (double)rays.n_probes * 0.4 * mean_dim / ((double)g->n_active * cells0);
+  if (knob < 0 && reuse < DEX_MEMO_MIN_REUSE) return 0;
+  const double per_batch = (double)rays.n_dirs * 2.0 * (double)g->n_active * (double)m->dev.cps * DEX_W * sizeof(float);
+  size_t free_b = 0, total_b = 0;
+  if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); return 0; }
+  const double budget = fmin(0.5 * (double)free_b, 64.0e9);
+  const int nb = (int)fmin((double)m->n_batch, floor(budget / per_batch));
+  return nb < 1 ? 0 : nb;
+}
+
 bool dex_auto_dir_split(long long n_probes, int n_dirs, int n_lambda) {
   const int split = dex_tuning_dir_split();
   const size_t i_floats = (size_t)n_probes * (size_t)n_dirs * (size_t)n_lambda;
@@ -937,7 +1081,10 @@ dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysD
   if (s == DEX_OK) {
     float* out = d_I ? d_I : d_out;
     const bool fj = d_I ? false : fuse_j;
-    if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st);
+    const int memo = memo_group(g, m, r);
+    if (memo > 0 && g->desc.ndim == 2) s = launch_march_memo<2>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st, memo);
+    else if (memo > 0) s = launch_march_memo<3>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st, memo);
+    else if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st);
     else s = launch_march_d<3>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st);
     if (s == DEX_OK && d_I) s = dex_launch_reduce_j(r, m->n_lambda, d_I, d_out, st);
   }

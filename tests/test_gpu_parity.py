@@ -261,6 +261,69 @@ def test_cav_small(P, name, n, metric, thr, gate):
     _solve_and_compare(P, wl, M, dw, grid, mips, lanes=(8, 2))
 
 
+@pytest.mark.parametrize("name,kw,thr,extra", [("C4", dict(n=128, n_dirs=8, n_probes=300), 0.3, "plain"),
+                                                ("C4", dict(n=128, n_dirs=6, n_probes=200), 0.3, "caps+interval"),
+                                                ("C4", dict(n=64, n_dirs=4, n_probes=150), 0.3, "25d"),
+                                                ("C5", dict(n=64, n_dirs=8, n_probes=300), 5.0, "plain"),
+                                                ("C4", dict(n=64, n_dirs=6, n_probes=100), 0.3, "classic"),
+                                                ("C3", dict(n=128, n_dirs=8, n_probes=300), None, "plain")])
+def test_memo_parity(P, name, kw, thr, extra):
+    """Core-and-Voigt memoised per direction (tuning knob "memo": eta, chi evaluated once per (cell, direction,
+    batch) into march records, then the ISO march) against the oracle and against the in-march evaluation: segment
+    counts exact, I and J within 1e-5 of the oracle in both modes (and of each other); with the
+    near-field cap + a radiance interval, 2.5D rays, the Classic variant, 8 lanes per ray, the direction split and the
+    rebuild pipeline's wavelength windows."""
+    from workloads.gen import dirs_25d
+    wl = make(name, **kw)
+    if thr is not None:
+        wl.thr_eta = wl.thr_chi = thr
+    nd = wl.dirs.shape[0]
+    caps = None
+    if extra == "25d":
+        wl.dirs, wl.weights, wl.sin_incl = dirs_25d(3, 4)
+        nd = wl.dirs.shape[0]
+    wl.i0 = np.random.default_rng(21).uniform(0, 1, size=(nd, wl.n_lambda)).astype(np.float32)
+    if extra == "caps+interval":
+        caps = [6.0, 24.0]
+        wl.interval = (2.0, 70.0)
+    variant = orc.CLASSIC if extra == "classic" else None
+    if variant is None:
+        M = orc.build_mips(wl)
+        ref = orc.hdda_march(wl, M, level_cap_t=caps)
+        dw, grid, mips = _build(P, wl)
+    else:
+        ref = orc.plain_march(wl, variant=orc.CLASSIC)
+        dw, grid, mips = _build(P, wl, variant=P.DEX_CLASSIC)
+    mips.set_level_caps(caps)
+    Jref = orc.mean_intensity(ref.I, wl.weights)
+    out = {}
+    try:
+        for memo in (0, 1):
+            P.dex_set_tuning("memo", memo)
+            for lpr, split in ((1, 0), (8, 0), (1, 1)):
+                P.dex_set_lanes_per_ray(lpr)
+                P.dex_set_tuning("dir_split", split)
+                seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+                I, _ = P.pipeline.formal_solution(dw, grid, mips, segment_count=seg)
+                if variant is None:
+                    assert int(seg.item()) == ref.segments
+                assert max_rel(I.cpu().numpy(), ref.I) <= TOL, f"memo={memo} lanes={lpr}"
+                J = P.pipeline.mean_intensity(dw, grid, mips)
+                assert max_rel(J.cpu().numpy(), Jref) <= TOL, f"memo={memo} lanes={lpr} split={split}"
+                out[(memo, lpr, split)] = J
+            if variant is None and extra == "plain":      # wavelength windows of the rebuild pipeline (io_base != 0)
+                P.dex_set_lanes_per_ray(1)
+                P.dex_set_tuning("dir_split", 0)
+                Jp, _ = P.pipeline.mean_intensity_pipelined(dw, grid, 2)
+                assert torch.equal(Jp, out[(memo, 1, 0)])
+        assert max_rel(out[(1, 1, 0)].cpu().numpy(), out[(0, 1, 0)].cpu().numpy()) <= TOL
+        assert torch.equal(out[(1, 1, 0)], out[(1, 1, 1)])       # the direction split sums in the fused order
+    finally:
+        P.dex_set_tuning("memo", -1)
+        P.dex_set_tuning("dir_split", -1)
+        P.dex_set_lanes_per_ray(1)
+
+
 def test_classic_equals_plain_march(P):
     wl = make("C4", n=64, n_dirs=6, n_probes=100)
     A = orc.plain_march(wl, variant=orc.CLASSIC)
