@@ -158,3 +158,40 @@ def test_crop_workload_is_brick_local():
         for m in range(M.max_level + 1):
             sl = tuple(slice(lo[a] >> m, (lo[a] + size[a]) >> m) for a in reversed(range(wl.ndim)))
             assert np.array_equal(M.eta[m][sl], Mc.eta[m]) and np.array_equal(M.vmax[m][sl], Mc.vmax[m])
+
+
+def test_batch_workload_is_a_column_selection():
+    """workloads.gen.batch_workload (full-size GPU comparisons, bench.py's cpu_baseline): the oracle's level table and I
+    of a workload restricted to some wavelength batches are the rows / columns of the full workload's, bit for bit."""
+    from oracle import oracle as orc
+    from workloads import make
+    from workloads.gen import batch_workload
+    for name, kw, batches in (("C2", dict(n=64, n_dirs=4, n_probes=40), [1, 3]), ("C4", dict(n=64, n_dirs=4, n_probes=30), [3, 20, 25]),
+                              ("C3", dict(n=64, n_dirs=4, n_probes=30), [0, 4])):
+        wl = make(name, **kw)
+        wl.i0 = np.random.default_rng(2).uniform(0, 1, size=(4, wl.n_lambda)).astype(np.float32)
+        M = orc.build_mips(wl)
+        full = orc.hdda_march(wl, M)
+        sub, idx = batch_workload(wl, batches)
+        assert sub.n_lambda == 8 * len(batches) and sub.n_batch == len(batches)
+        Ms = orc.build_mips(sub)
+        assert np.array_equal(Ms.levels, M.levels[batches])
+        part = orc.hdda_march(sub, Ms)
+        assert np.array_equal(part.I, full.I[:, :, idx])
+
+
+def test_bench_reference_arm_line():
+    """bench.py --impl reference (the oracle on the host cores): one JSON line with the contract's keys."""
+    import json
+    import subprocess
+    import sys
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "C1", "--steps", "1",
+                          "--warmup", "0", "--cpu-probes", "64"], capture_output=True, text=True, timeout=600, check=True).stdout
+    line = [ln for ln in out.splitlines() if ln.startswith("{")]
+    assert len(line) == 1
+    d = json.loads(line[0])
+    for key in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e", "gpu_launches"):
+        assert key in d, key
+    assert d["impl"] == "reference" and d["value"] > 0 and d["gpu_launches"] == 0
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["cpu_baseline"]["kind"] == "oracle" and "workload" in d["config"]
