@@ -352,6 +352,7 @@ dex_status dex_build_sparse_grid(const dex_grid_desc* desc, const uint8_t* d_act
   g->stream = (cudaStream_t)stream;
   dex_status s = dmalloc(&g->d_slot, (size_t)nbr, g->stream);
   if (s == DEX_OK) s = dmalloc(&g->d_active_bricks, (size_t)nbr, g->stream);
+  if (s == DEX_OK) s = dmalloc(&g->d_edist, (size_t)nbr, g->stream);
   if (s == DEX_OK) { d.slot = g->d_slot; s = dex_launch_grid_build(g, d_active, (cudaStream_t)stream); }
   if (s != DEX_OK) { dex_destroy_grid(g); return s; }
   *out = g;
@@ -376,6 +377,7 @@ void dex_destroy_grid(dex_grid* grid) {
   if (!grid) return;
   dex_free(grid->d_slot, grid->stream);
   dex_free(grid->d_active_bricks, grid->stream);
+  dex_free(grid->d_edist, grid->stream);
   delete grid;
 }
 

@@ -12,6 +12,7 @@ struct dex_grid {
   DexGridDev dev;          // device view (pointers into memory owned by this handle)
   int* d_slot = nullptr;   // [n_bricks]
   int* d_active_bricks = nullptr;  // [n_active] slot -> brick
+  int* d_edist = nullptr;          // [n_bricks] 0 populated, else Chebyshev distance in bricks to the nearest populated brick
   int64_t n_bricks = 0, n_active = 0;
   int64_t nvox = 0;
   cudaStream_t stream = nullptr;   // the stream the handle was built on; its memory is released on it

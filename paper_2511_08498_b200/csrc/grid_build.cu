@@ -59,6 +59,36 @@ dex_scan_slots_kernel(const int* __restrict__ flag, int n, int* __restrict__ slo
   if (t == 1023) *n_active = part[1023];
 }
 
+// Empty-space distance: for an empty brick, the Chebyshev distance (in bricks, capped at DEX_EDIST_MAX) to the nearest
+// populated brick; 0 for a populated one.  The (2d-1)^D box of bricks centred on an empty brick at distance d holds no
+// populated brick, so a ray inside it can be taken to the box's face in ONE HDDA step (dex_set_cell_nocap): empty visits
+// are never emitted, and the face a ray leaves through is the face of the brick it enters, so emitted lists are unchanged.
+#define DEX_EDIST_MAX 8
+template <int D>
+__global__ void dex_empty_distance_kernel(const DexGridDev G, const int* __restrict__ flag, int* __restrict__ edist) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= G.n_bricks) return;
+  if (flag[b] != 0) { edist[b] = 0; return; }
+  const int bx = b % G.nb[0], by = (b / G.nb[0]) % G.nb[1], bz = (D == 3) ? b / (G.nb[0] * G.nb[1]) : 0;
+  int d = DEX_EDIST_MAX;
+  for (int r = 1; r < DEX_EDIST_MAX && d == DEX_EDIST_MAX; ++r) {       // shells of growing radius, stop at the first hit
+    const int z0 = (D == 3) ? max(0, bz - r) : 0, z1 = (D == 3) ? min(G.nb[2] - 1, bz + r) : 0;
+    for (int z = z0; z <= z1 && d == DEX_EDIST_MAX; ++z)
+      for (int y = max(0, by - r); y <= min(G.nb[1] - 1, by + r) && d == DEX_EDIST_MAX; ++y) {
+        const bool edge_zy = (D == 3 && (z == bz - r || z == bz + r)) || y == by - r || y == by + r;
+        const int x0 = max(0, bx - r), x1 = min(G.nb[0] - 1, bx + r);
+        if (edge_zy) {
+          for (int x = x0; x <= x1; ++x)
+            if (flag[(z * G.nb[1] + y) * G.nb[0] + x] != 0) { d = r; break; }
+        } else {      // interior row of the shell: only its two end points belong to it
+          if (bx - r >= 0 && flag[(z * G.nb[1] + y) * G.nb[0] + bx - r] != 0) d = r;
+          if (bx + r < G.nb[0] && flag[(z * G.nb[1] + y) * G.nb[0] + bx + r] != 0) d = r;
+        }
+      }
+  }
+  edist[b] = d;
+}
+
 }  // namespace
 
 dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStream_t st) {
@@ -77,7 +107,9 @@ dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStrea
   }
   dex_count_launch();
   dex_scan_slots_kernel<<<1, 1024, 0, st>>>(d_flag, nb, g->d_slot, g->d_active_bricks, d_count);
-  dex_count_launch();
+  if (g->desc.ndim == 2) dex_empty_distance_kernel<2><<<(nb + 127) / 128, 128, 0, st>>>(g->dev, d_flag, g->d_edist);
+  else dex_empty_distance_kernel<3><<<(nb + 127) / 128, 128, 0, st>>>(g->dev, d_flag, g->d_edist);
+  dex_count_launch(2);
   int h_count = 0;
   cudaError_t e = cudaMemcpyAsync(&h_count, d_count, sizeof(int), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);

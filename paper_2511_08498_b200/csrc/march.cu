@@ -1001,8 +1001,7 @@ static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const 
     full.mdir = 2 * plane;
     full.voigt_fp32 = dex_tuning_voigt_fp32();
     dex_status s = DEX_OK;
-    if (rays.n_dirs > 65535) { dex_set_error("march: too many directions for the per-direction record launch"); s = DEX_ERR_UNSUPPORTED; }
-    if (s == DEX_OK && tasks > 0) {
+    if (tasks > 0) {
       if (m->variant == DEX_VELINTERP)
         dex_dir_records_kernel<D, DEX_VELINTERP><<<grid, DEX_MARCH_THREADS, 0, st>>>(g->dev, full, rays, g->d_active_bricks, b0,
                                                                                     d_rec, plane, dex_line_segment_counter());
@@ -1030,7 +1029,7 @@ static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const 
 static int memo_group(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays) {
   if (m->variant == DEX_ISO) return 0;
   const int knob = dex_tuning_memo();
-  if (knob == 0 || rays.n_dirs <= 0 || g->n_active <= 0) return 0;
+  if (knob == 0 || rays.n_dirs <= 0 || rays.n_dirs > 65535 || g->n_active <= 0) return 0;   // directions are the records kernel's grid.z
   const int D = g->desc.ndim;
   double cells0 = 1.0, mean_dim = 0.0;
   for (int a = 0; a < D; ++a) { cells0 *= (double)g->dev.B; mean_dim += (double)g->dev.dims[a] / D; }

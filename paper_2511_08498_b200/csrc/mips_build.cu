@@ -444,7 +444,9 @@ __global__ void select_levels_kernel(const BuildCtx X, signed char* __restrict__
 
 // state = level + 1 in `bits` bits, floor(64/bits) bricks per 64-bit word.  The same pass
 // writes the march's own table: one 4-byte word (first record of the brick's level << 4) | state per (batch, brick).
-__global__ void pack_levels_kernel(const signed char* __restrict__ levels, const int* __restrict__ slot, int n_batch,
+// For an empty brick the word is (empty-space distance << 4) | 0 (grid_build.cu): the traversal skips the whole empty box.
+__global__ void pack_levels_kernel(const signed char* __restrict__ levels, const int* __restrict__ slot,
+                                   const int* __restrict__ edist, int n_batch,
                                    int n_bricks, int bits, int per_word, int words, const DexMipsDev M,
                                    unsigned long long* __restrict__ packed, int* __restrict__ binfo) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -457,7 +459,7 @@ __global__ void pack_levels_kernel(const signed char* __restrict__ levels, const
     if (bi >= n_bricks) break;
     const int state = levels[(size_t)b * n_bricks + bi] + 1;
     word |= (unsigned long long)state << (q * bits);
-    binfo[(size_t)b * n_bricks + bi] = (state > 0) ? (((slot[bi] * M.cps + M.lvloff[state - 1]) << 4) | state) : 0;
+    binfo[(size_t)b * n_bricks + bi] = (state > 0) ? (((slot[bi] * M.cps + M.lvloff[state - 1]) << 4) | state) : (edist[bi] << 4);
   }
   packed[i] = word;
 }
@@ -687,7 +689,7 @@ dex_status dex_launch_mips_build(dex_mips* m, const dex_mips_desc* desc, cudaStr
 
 dex_status dex_launch_pack_levels(dex_mips* m, cudaStream_t st) {
   const long long total = (long long)m->n_batch * m->dev.words_per_batch;
-  pack_levels_kernel<<<blocks_for(total, 256), 256, 0, st>>>(m->d_levels, m->grid->d_slot, m->n_batch,
+  pack_levels_kernel<<<blocks_for(total, 256), 256, 0, st>>>(m->d_levels, m->grid->d_slot, m->grid->d_edist, m->n_batch,
                                                              (int)m->grid->n_bricks, m->dev.bits, m->dev.per_word,
                                                              m->dev.words_per_batch, m->dev, m->d_packed, m->d_binfo);
   dex_count_launch();
