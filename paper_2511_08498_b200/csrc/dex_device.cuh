@@ -401,7 +401,7 @@ __device__ __forceinline__ bool dex_ray_cross_nocap(DexRay3<D>& r, const DexGrid
   const int xe = poss ? kps : kps - 1;           // level-0 coordinate just beyond the exit plane (T5)
   const int cs = poss ? kps - size : kps;
   const bool alive = (unsigned)xe < (unsigned)dims_s;
-  const bool box = r.sh > G.logB;               // leaving a multi-brick box of empty space
+  const bool box = (D == 2) && r.sh > G.logB;   // leaving a multi-brick box of empty space (2D only, dex_set_cell_nocap)
   const bool newbrick = box || ((xe ^ cs) >> G.logB) != 0;
 #pragma unroll
   for (int a = 0; a < D; ++a) x[a] = (a == s) ? xe : c[a];
