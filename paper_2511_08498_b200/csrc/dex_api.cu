@@ -58,8 +58,8 @@ dex_status dmalloc(T** p, size_t count, cudaStream_t st) {
 }
 
 void free_mips_memory(dex_mips* m) {
-  void* ptrs[] = {m->d_store, m->d_mrec, m->d_aux, m->d_vtab, m->d_lam, m->d_active_lines, m->d_levels,
-                  m->d_packed, m->d_fail, m->d_binfo, m->d_vftab};
+  void* ptrs[] = {m->d_store, m->d_mrec, m->aux_borrowed ? nullptr : (void*)m->d_aux, m->d_vtab, m->d_lam, m->d_active_lines,
+                  m->d_levels, m->d_packed, m->d_fail, m->d_binfo, m->aux_borrowed ? nullptr : (void*)m->d_vftab};
   for (void* q : ptrs) dex_free(q, m->stream);
 }
 
@@ -382,7 +382,13 @@ void dex_destroy_grid(dex_grid* grid) {
 }
 
 // ------------------------------------------------------------------------------------------- mips
-dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, void* stream, dex_mips** out) {
+}  // extern "C"
+
+// dex_build_vlm_mips with the wavelength-independent chains (velocity, line parameters: "shared by all
+// batches") and the fp32 Voigt tables optionally BORROWED from an earlier build of the same atmosphere: the rebuild
+// pipeline builds them with its first stage only.
+static dex_status build_vlm_mips_impl(const dex_grid* grid, const dex_mips_desc* desc, void* stream, float4* donor_aux,
+                                      float* donor_vftab, dex_mips** out) {
   if (!grid || !desc || !out) { dex_set_error("NULL grid / desc / out"); return DEX_ERR_INVALID_ARG; }
   *out = nullptr;
   const int v = (int)desc->variant;
@@ -481,10 +487,12 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
   if (s == DEX_OK) s = dmalloc(&m->d_binfo, (size_t)n_batch * grid->n_bricks, st);
   if (s == DEX_OK) s = dmalloc(&m->d_fail, (size_t)n_batch * A * (max_level + 1), st);
   if (s == DEX_OK && v != DEX_ISO) {
-    s = dmalloc(&m->d_aux, A * cps * (size_t)(d.n_lines + 1), st);
+    m->aux_borrowed = donor_aux != nullptr && donor_vftab != nullptr;
+    if (m->aux_borrowed) { m->d_aux = donor_aux; m->d_vftab = donor_vftab; }
+    else s = dmalloc(&m->d_aux, A * cps * (size_t)(d.n_lines + 1), st);
     if (s == DEX_OK) s = dmalloc(&m->d_lam, (size_t)desc->n_lambda, st);
     if (s == DEX_OK) s = dmalloc(&m->d_active_lines, (size_t)n_batch * DEX_MAX_LINES, st);
-    if (s == DEX_OK) s = dmalloc(&m->d_vftab, (size_t)DEX_VF_NODES * 5, st);
+    if (s == DEX_OK && !m->aux_borrowed) s = dmalloc(&m->d_vftab, (size_t)DEX_VF_NODES * 5, st);
     if (s == DEX_OK && v == DEX_VELINTERP) {
       m->vtab_floats = m->store_floats * (size_t)d.n_vbins;
       s = dmalloc(&m->d_vtab, m->vtab_floats, st);
@@ -495,7 +503,7 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
       if (e == cudaSuccess)
         e = cudaMemcpyAsync(m->d_active_lines, desc->h_active_lines, (size_t)n_batch * DEX_MAX_LINES,
                             cudaMemcpyHostToDevice, st);
-      if (e == cudaSuccess)
+      if (e == cudaSuccess && !m->aux_borrowed)
         e = cudaMemcpyAsync(m->d_vftab, dex_voigt_fast_table_host(), sizeof(float) * DEX_VF_NODES * 5,
                             cudaMemcpyHostToDevice, st);
       if (e != cudaSuccess) { dex_set_error(cudaGetErrorString(e)); s = DEX_ERR_CUDA; }
@@ -520,6 +528,12 @@ dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, v
   if (s != DEX_OK) { free_mips_memory(m); delete m; return s; }
   *out = m;
   return DEX_OK;
+}
+
+extern "C" {
+
+dex_status dex_build_vlm_mips(const dex_grid* grid, const dex_mips_desc* desc, void* stream, dex_mips** out) {
+  return build_vlm_mips_impl(grid, desc, stream, nullptr, nullptr, out);
 }
 
 dex_status dex_mips_get_levels(const dex_mips* mips, int8_t* h_level) {
@@ -756,6 +770,8 @@ dex_status dex_mean_intensity_pipelined(const dex_grid* grid, const dex_mips_des
   cudaStreamWaitEvent(sm[0], ev_in, 0);
   cudaStreamWaitEvent(sm[1], ev_in, 0);
 
+  float4* keep_aux = nullptr;            // built by the first stage on `sb`, read by every stage, freed after the join
+  float* keep_vftab = nullptr;
   dex_mips* prev = nullptr;              // stage s-1, released on the build stream once its march has finished
   int prev_ev = 0;
   for (int sg = 0; sg < n_stage && s == DEX_OK && e == cudaSuccess; ++sg) {
@@ -772,8 +788,14 @@ dex_status dex_mean_intensity_pipelined(const dex_grid* grid, const dex_mips_des
     if (desc->d_chi_bg) sub.d_chi_bg = desc->d_chi_bg + off;
     if (aniso && desc->h_active_lines) sub.h_active_lines = desc->h_active_lines + (size_t)b0 * DEX_MAX_LINES;
     dex_mips* cur = nullptr;
-    s = dex_build_vlm_mips(grid, &sub, (void*)sb, &cur);
+    s = build_vlm_mips_impl(grid, &sub, (void*)sb, keep_aux, keep_vftab, &cur);
     if (s != DEX_OK) break;
+    if (aniso && !keep_aux && cur->d_aux && cur->d_vftab) {
+      // the first stage's wavelength-independent chains and Voigt tables serve every later stage: this call keeps them
+      keep_aux = cur->d_aux;
+      keep_vftab = cur->d_vftab;
+      cur->aux_borrowed = true;
+    }
     cur->dev.io_stride = desc->n_lambda;
     cur->dev.io_base = (int)off;
     s = dex_mips_set_level_caps(cur, n_caps, h_cap_t);
@@ -815,6 +837,8 @@ dex_status dex_mean_intensity_pipelined(const dex_grid* grid, const dex_mips_des
   cudaEventRecord(ev_in, sb);
   cudaStreamWaitEvent(st, ev_in, 0);
   if (d_perm) cudaFreeAsync(d_perm, st);
+  dex_free(keep_aux, st);                // `st` has just been made to wait for every march and for the build stream
+  dex_free(keep_vftab, st);
   if (h_levels && e == cudaSuccess) e = cudaStreamSynchronize(sb);
   cudaEventDestroy(ev_in);
   for (int i = 0; i < 2; ++i) { cudaEventDestroy(ev_built[i]); cudaEventDestroy(ev_marched[i]); }

@@ -37,6 +37,8 @@ struct dex_mips {
   float* d_vftab = nullptr;                  // fp32 Voigt tables: [NODES][4] wing then [NODES] core (anisotropic variants)
   int* d_fail = nullptr;                     // [n_batch][n_active][max_level+1]
   size_t store_floats = 0, vtab_floats = 0;
+  bool aux_borrowed = false;       // d_aux / d_vftab belong to the caller (the rebuild pipeline shares the wavelength-
+                                   // independent chains between its stages): not built, not freed by this handle
   cudaStream_t stream = nullptr;   // the stream the handle was built on; its memory is released on it
 };
 

@@ -641,7 +641,8 @@ dex_status build_t(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st) {
   const float* chi = iso ? desc->d_chi : desc->d_chi_bg;
   gather_spec_kernel<D><<<blocks_for((long long)m->n_batch * A * cells_at(0) * DEX_W, T), T, 0, st>>>(X, eta, chi);
   dex_count_launch();
-  if (!iso) {
+  const bool own_aux = !iso && !m->aux_borrowed;      // a pipeline stage after the first borrows the finished chains
+  if (own_aux) {
     gather_aux_kernel<D><<<blocks_for(A * cells_at(0), T), T, 0, st>>>(X, desc->d_vel, desc->d_eta_star0, desc->d_chi_star0,
                                                                   desc->d_a0, desc->d_inv_dlamD, m->grid->nvox);
     dex_count_launch();
@@ -655,7 +656,7 @@ dex_status build_t(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st) {
     if (iso) reduce_spec_kernel<D, true><<<blocks_for(nspec, T), T, 0, st>>>(X, lv);
     else reduce_spec_kernel<D, false><<<blocks_for(nspec, T), T, 0, st>>>(X, lv);
     dex_count_launch();
-    if (!iso) {
+    if (own_aux) {
       reduce_aux_kernel<D><<<blocks_for(A * cells_at(lv), T), T, 0, st>>>(X, lv);
       dex_count_launch();
     }
