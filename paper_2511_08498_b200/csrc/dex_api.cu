@@ -201,6 +201,17 @@ cudaError_t dex_alloc(void** p, size_t bytes, cudaStream_t st) {
   if (!pool) return cudaMallocAsync(p, bytes, st);     // pool creation failed: the default pool, untouched
   return cudaMallocFromPoolAsync(p, bytes, pool, st);
 }
+size_t dex_pool_idle_bytes() {
+  cudaMemPool_t pool = pool_of_current_device();
+  if (!pool) return 0;
+  unsigned long long reserved = 0, used = 0;
+  if (cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReservedMemCurrent, &reserved) != cudaSuccess ||
+      cudaMemPoolGetAttribute(pool, cudaMemPoolAttrUsedMemCurrent, &used) != cudaSuccess) {
+    cudaGetLastError();
+    return 0;
+  }
+  return reserved > used ? (size_t)(reserved - used) : 0;
+}
 void dex_free(void* p, cudaStream_t st) {
   if (p) cudaFreeAsync(p, st);
 }

@@ -47,6 +47,7 @@ void dex_set_error(const std::string& msg);
 // rebuild per iteration does not pay cudaMalloc / cudaFree (page mapping, device-wide synchronisation) every time.
 cudaError_t dex_alloc(void** p, size_t bytes, cudaStream_t st);
 void dex_free(void* p, cudaStream_t st);
+size_t dex_pool_idle_bytes();      // memory the library's pool holds but no live allocation uses (reusable at once)
 void dex_count_launch(int n = 1);
 int dex_tuning_voigt_fp32();
 int dex_tuning_memo();    // -1 automatic, 0 never, 1 always: anisotropic provider memoised per direction (march.cu)

@@ -485,6 +485,9 @@ constexpr int dex_march_minb(int var) {
 #define DEX_MEMO_MIN_REUSE 12.0   // rays per (cell, direction) from which the memoised march is taken:
                                       // C5 (5 rays per cell and direction) is 1.26x slower memoised, a 1/32 probe band of C4 (18) 2.5x faster
 #endif
+#ifndef DEX_ROTATE
+#define DEX_ROTATE 0     // 1: ISO iterations run step -> request records -> batched crossing -> integrate (experiment)
+#endif
 #ifndef DEX_PREFETCH
 #define DEX_PREFETCH 0   // 0 none, 1 prefetch.global.L1, 2 prefetch.global.L2 of the next cell's records (Core-and-Voigt)
 #endif
@@ -570,6 +573,39 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
 #pragma unroll
         for (int i = 0; i < LPT; ++i) { DEX_IH(i) += I[i]; I[i] = 0.0f; }
       }
+#if DEX_ROTATE
+      if (VAR == DEX_ISO) {
+        // rotated iteration (ISO): step, REQUEST the records, run the batched crossing of the lanes waiting at brick
+        // faces, then integrate -- the crossing's ~110 instructions sit between the two LDG.E.256 and their first use
+        bool emit = false;
+        int cell = 0;
+        float ds = 0.0f;
+        if (alive && !blocked) {
+          const float t0 = ray.t;
+          blocked = !dex_ray_advance<D>(ray, emit, cell, ds);
+          if (CLIP) {
+            ds = __fsub_rn(fminf(ray.t, R.t_end), fmaxf(t0, R.t_begin));
+            emit = emit && ds > 0.0f;
+            if (ray.t >= R.t_end) { alive = false; blocked = false; }
+          }
+        }
+        float eta[LPT], chi[LPT];
+        if (emit) {
+          ++nseg;
+          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, omf, sin_incl, CT, vfw, vfc, iso0, iso1, eta, chi);
+        }
+        const unsigned bm = __ballot_sync(FULL, blocked);
+        const unsigned am2 = __ballot_sync(FULL, alive);
+        if (bm != 0u && (bm == am2 || __popc(bm) >= DEX_CROSS_QUORUM)) {
+          if (blocked) {
+            alive = caps ? dex_ray_cross<D>(ray, G, M, binfo, probe, om) : dex_ray_cross_nocap<D>(ray, G, binfo, probe, om);
+            blocked = false;
+          }
+        }
+        if (emit) dex_accumulate_all_S<LPT>(eta, chi, hk * ds, I, T);
+        continue;
+      }
+#endif
       const unsigned bm = __ballot_sync(FULL, blocked);
       if (bm == am || __popc(bm) >= DEX_CROSS_QUORUM) {
         if (blocked) {
@@ -1039,7 +1075,8 @@ static int memo_group(const dex_grid* g, const dex_mips* m, const DexRaysDev& ra
   const double per_batch = (double)rays.n_dirs * 2.0 * (double)g->n_active * (double)m->dev.cps * DEX_W * sizeof(float);
   size_t free_b = 0, total_b = 0;
   if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); return 0; }
-  const double budget = fmin(0.5 * (double)free_b, 64.0e9);
+  // half of what is available: the driver's free memory plus what the library's own pool holds idle from earlier calls
+  const double budget = fmin(0.5 * ((double)free_b + (double)dex_pool_idle_bytes()), 64.0e9);
   const int nb = (int)fmin((double)m->n_batch, floor(budget / per_batch));
   return nb < 1 ? 0 : nb;
 }
