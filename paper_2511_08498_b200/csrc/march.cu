@@ -485,12 +485,6 @@ constexpr int dex_march_minb(int var) {
 #define DEX_MEMO_MIN_REUSE 12.0   // rays per (cell, direction) from which the memoised march is taken:
                                       // C5 (5 rays per cell and direction) is 1.26x slower memoised, a 1/32 probe band of C4 (18) 2.5x faster
 #endif
-#ifndef DEX_ROTATE
-#define DEX_ROTATE 0     // 1: ISO iterations run step -> request records -> batched crossing -> integrate (experiment)
-#endif
-#ifndef DEX_PREFETCH
-#define DEX_PREFETCH 0   // 0 none, 1 prefetch.global.L1, 2 prefetch.global.L2 of the next cell's records (Core-and-Voigt)
-#endif
 
 
 
@@ -573,39 +567,6 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
 #pragma unroll
         for (int i = 0; i < LPT; ++i) { DEX_IH(i) += I[i]; I[i] = 0.0f; }
       }
-#if DEX_ROTATE
-      if (VAR == DEX_ISO) {
-        // rotated iteration (ISO): step, REQUEST the records, run the batched crossing of the lanes waiting at brick
-        // faces, then integrate -- the crossing's ~110 instructions sit between the two LDG.E.256 and their first use
-        bool emit = false;
-        int cell = 0;
-        float ds = 0.0f;
-        if (alive && !blocked) {
-          const float t0 = ray.t;
-          blocked = !dex_ray_advance<D>(ray, emit, cell, ds);
-          if (CLIP) {
-            ds = __fsub_rn(fminf(ray.t, R.t_end), fmaxf(t0, R.t_begin));
-            emit = emit && ds > 0.0f;
-            if (ray.t >= R.t_end) { alive = false; blocked = false; }
-          }
-        }
-        float eta[LPT], chi[LPT];
-        if (emit) {
-          ++nseg;
-          dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, omf, sin_incl, CT, vfw, vfc, iso0, iso1, eta, chi);
-        }
-        const unsigned bm = __ballot_sync(FULL, blocked);
-        const unsigned am2 = __ballot_sync(FULL, alive);
-        if (bm != 0u && (bm == am2 || __popc(bm) >= DEX_CROSS_QUORUM)) {
-          if (blocked) {
-            alive = caps ? dex_ray_cross<D>(ray, G, M, binfo, probe, om) : dex_ray_cross_nocap<D>(ray, G, binfo, probe, om);
-            blocked = false;
-          }
-        }
-        if (emit) dex_accumulate_all_S<LPT>(eta, chi, hk * ds, I, T);
-        continue;
-      }
-#endif
       const unsigned bm = __ballot_sync(FULL, blocked);
       if (bm == am || __popc(bm) >= DEX_CROSS_QUORUM) {
         if (blocked) {
@@ -624,31 +585,11 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
           emit = emit && ds > 0.0f;
           if (ray.t >= R.t_end) { alive = false; blocked = false; }
         }
-#if DEX_PREFETCH
-        // Core-and-Voigt in 3D waits on the latency of its per-cell records (profiles/r02: long_scoreboard 2.2 of 3.6
-        // warps per scheduler, DRAM at 27 %): after the in-brick step the NEXT cell is known one whole profile evaluation
-        // (~700 instructions) before its records are needed, so they are requested now
-        if ((VAR == DEX_CAV) && !blocked && ray.cell >= 0) {
-          const float* pb = iso0 + (size_t)(unsigned)ray.cell * DEX_REC;
-          const float4* pa = M.aux + dex_aux_vel(M, (size_t)(unsigned)ray.cell);
-#if DEX_PREFETCH == 1
-          asm volatile("prefetch.global.L1 [%0];" ::"l"(pb));
-          asm volatile("prefetch.global.L1 [%0];" ::"l"(pa));
-#else
-          asm volatile("prefetch.global.L2 [%0];" ::"l"(pb));
-          asm volatile("prefetch.global.L2 [%0];" ::"l"(pa));
-#endif
-        }
-#endif
         if (emit) {
           ++nseg;
           const float hds = hk * ds;
           float eta[LPT], chi[LPT];
-#ifdef DEX_FAKE_CELL   // experiment: every fetch from a tiny, cache-resident window of cells (results are wrong)
-          dex_provider<D, VAR, LPT>(M, batch_base, cell & 1023, sub, omf, sin_incl, CT, vfw, vfc, iso0, iso1, eta, chi);
-#else
           dex_provider<D, VAR, LPT>(M, batch_base, cell, sub, omf, sin_incl, CT, vfw, vfc, iso0, iso1, eta, chi);
-#endif
           if (VAR == DEX_ISO) dex_accumulate_all_S<LPT>(eta, chi, hds, I, T);
           // velocity interpolation keeps the E(tau) integrator: the record form costs it registers it does not have at
           // 7 blocks per SM (measured on C3: 583 ms against 616; Core-and-Voigt gains 3 % from the record form)
