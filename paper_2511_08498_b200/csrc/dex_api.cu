@@ -527,7 +527,7 @@ static dex_status build_vlm_mips_impl(const dex_grid* grid, const dex_mips_desc*
     d.binfo = m->d_binfo;
     d.store = m->d_store;
     d.mrec = m->d_mrec;
-    d.mplane = m->store_floats / 2;
+    d.mplane = (grid->dev.ndim == 3) ? (size_t)DEX_W : m->store_floats / 2;   // 3D: interleaved records (dex_device.cuh)
     d.aux = m->d_aux;
     if (v == DEX_VELINTERP) { d.aux_vs = 1; d.aux_lo = A * cps; d.aux_ls = d.n_lines; }      // dense velocities, lines behind
     else { d.aux_vs = d.n_lines + 1; d.aux_lo = 1; d.aux_ls = d.n_lines + 1; }             // one record per cell

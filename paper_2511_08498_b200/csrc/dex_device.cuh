@@ -11,6 +11,8 @@
 #define DEX_W 8            // wavelengths per batch
 #define DEX_REC (2 * DEX_W) // floats per cell record: chi[0..W-1] then eta[0..W-1] (pairs of wavelengths feed FFMA2)
 #define DEX_MAXLEV 6
+// floats between the march records of consecutive cells: 8 in 2D (two planes), 16 in 3D (interleaved), see DexMipsDev::mrec
+template <int D> struct DexRecStride { static constexpr int value = (D == 3) ? 2 * DEX_W : DEX_W; };
 #define DEX_NLINES 4
 
 // cell record accessors: record r (in units of DEX_REC floats) of a store, wavelength j of the batch
@@ -39,9 +41,11 @@ struct DexMipsDev {
   int cps;                           // cells per slot (all levels)
   int lvloff[DEX_MAXLEV];            // first cell of level m inside a slot
   const float* store;                // [n_batch][n_active][cps][DEX_REC]  chi|eta (ISO) or background
-  const float* mrec;                 // ISO march records (make_march_records_kernel), what the ISO march reads: two planes
-  size_t mplane;                     // [2][n_batch][n_active][cps][DEX_W], plane 0 chi log2(e), plane 1 S = eta/chi;
-                                     // mplane = floats per plane
+  const float* mrec;                 // ISO march records (make_march_records_kernel), what the ISO march reads.  2D: two planes
+  size_t mplane;                     // [2][n_batch][n_active][cps][DEX_W], plane 0 chi log2(e), plane 1 S = eta/chi, mplane =
+                                     // floats per plane (lanes in x-adjacent cells share L1 lines).  3D: one 64-byte record per
+                                     // cell, [n_batch][n_active][cps][chi log2(e) x 8 | S x 8], mplane = DEX_W: rays are sparse
+                                     // there, and a record that misses the L2 costs one 64-byte DRAM burst instead of two
   size_t mdir;                       // 0, or floats between the records of consecutive DIRECTIONS (Core-and-Voigt memoised
                                      // per direction, march.cu: mrec then holds [n_dirs][2][n_batch][n_active][cps][DEX_W])
   const float4* aux;                 // [n_active][cps][1 + n_lines]: (vx, vy, vz, max|v|) then per line (eta*, chi*, a0,

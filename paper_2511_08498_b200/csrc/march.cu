@@ -7,6 +7,8 @@
 // direction at the same time, so brick / level lookups and cell fetches of a warp hit the same lines.
 // Each lane group loops over all quadrature directions and accumulates J in registers: the angular
 // reduction needs no atomics and is deterministic.
+#include <mutex>
+
 #include "dex_internal.h"
 #include "dex_voigt.cuh"
 
@@ -245,8 +247,14 @@ struct DexCavTab {
 
 // the literal fp64 formula for damping outside the fp32 window: rare, so kept out of line (it would otherwise be
 // inlined 8 x DEX_NLINES times and set the register count of the whole kernel)
-__device__ __noinline__ float dex_voigt_H_outside_window(const double* __restrict__ wc, double L, double a, double x) {
-  return (float)dex_voigt_H_march(wc, L, a, x);
+// The Weideman coefficients come from __constant__ memory, not from the kernel's DexMipsDev parameter: passing
+// &M.wei_c[0] to an out-of-line function needs a generic address, for which the compiler copied the whole 464-byte
+// parameter struct to local memory at the start of EVERY thread (58 STL.64: invisible in the march, whose threads live
+// for millions of segments, but 3x the DRAM writes of the records themselves in dex_dir_records_kernel).
+__constant__ double dex_c_wei[DEX_WEI_N];
+__constant__ double dex_c_wei_L;
+__device__ __noinline__ float dex_voigt_H_outside_window(double a, double x) {
+  return (float)dex_voigt_H_march(dex_c_wei, dex_c_wei_L, a, x);
 }
 
 // eta, chi of one cell for this lane's wavelengths, seen along propagation direction om (a7)
@@ -257,8 +265,8 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
                                              const float* __restrict__ iso0, const float* __restrict__ iso1,
                                              float (&eta)[LPT], float (&chi)[LPT]) {
   if (VAR == DEX_ISO) {   // march records, two planes of 32-byte rows: chi[] receives chi log2(e), eta[] S = eta/chi
-    dex_load_plane<LPT>(iso0 + (unsigned)cell * DEX_W, chi);
-    dex_load_plane<LPT>(iso1 + (unsigned)cell * DEX_W, eta);
+    dex_load_plane<LPT>(iso0 + (unsigned)cell * DexRecStride<D>::value, chi);
+    dex_load_plane<LPT>(iso1 + (unsigned)cell * DexRecStride<D>::value, eta);
     return;
   }
   // projected velocity of the cell's box-filtered bulk velocity, fp64 (DESIGN.md R-vel)
@@ -373,11 +381,14 @@ __device__ __forceinline__ void dex_provider(const DexMipsDev& M, size_t batch_b
           if (fabsf(xh[i]) + af[i] >= 15.0f) H[i] = dex_voigt_H_region1(af[i], xh[i]);
       }
     } else {
-#pragma unroll 1
+      // unrolled on purpose: a run-time index into H[] would put H -- and with it the fast path's results -- into local
+      // memory (two STL.128 per segment in the march; in the records kernel, whose threads each own fresh local lines,
+      // 5x the DRAM writes of the records themselves).  The callee is out of line, so this is 8 call sites, not 8 bodies.
+#pragma unroll
       for (int i = 0; i < LPT; ++i) {
         const int j = sub * LPT + i;
         const double x = (CT.dlam[q][j] + shift) * (double)ln.w;
-        H[i] = dex_voigt_H_outside_window(M.wei_c, M.wei_L, CT.r2[q][j] * (double)ln.z, x);
+        H[i] = dex_voigt_H_outside_window(CT.r2[q][j] * (double)ln.z, x);
       }
     }
     if (LPT == 1) {
@@ -482,8 +493,8 @@ constexpr int dex_march_minb(int var) {
 #define DEX_CROSS_QUORUM 8
 #endif
 #ifndef DEX_MEMO_MIN_REUSE
-#define DEX_MEMO_MIN_REUSE 12.0   // rays per (cell, direction) from which the memoised march is taken:
-                                      // C5 (5 rays per cell and direction) is 1.26x slower memoised, a 1/32 probe band of C4 (18) 2.5x faster
+#define DEX_MEMO_MIN_REUSE 3.0   // estimated rays per (cell, direction) from which the memoised march is taken: C5 (estimate
+                                 // 5.3; 3.4 segments per evaluated record) is 1.35x faster memoised, C3 / C4 (590) 1.8x / 5.9x
 #endif
 
 
@@ -510,7 +521,7 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
   // this lane's rows of the two ISO record planes (cell 0 of the batch); kept opaque so that the pointers stay in
   // registers instead of being rebuilt from the kernel parameters at every segment
   // (velocity interpolation: iso0 = this batch's velocity tables; Core-and-Voigt / Classic: its background records)
-  const float* iso0 = (VAR == DEX_ISO) ? M.mrec + batch_base * DEX_W + sub * LPT
+  const float* iso0 = (VAR == DEX_ISO) ? M.mrec + batch_base * DexRecStride<D>::value + sub * LPT
                       : (VAR == DEX_VELINTERP) ? M.vtab + batch_base * (size_t)M.n_vbins * DEX_REC
                                                : M.store + batch_base * DEX_REC;
   const float* iso1 = iso0 + M.mplane;
@@ -653,11 +664,15 @@ dex_dir_records_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev 
   __shared__ DexCavTab CT;
   __shared__ float4 vfw[VAR == DEX_CAV ? DEX_VF_NODES : 1];
   __shared__ float vfc[VAR == DEX_CAV ? DEX_VF_NODES : 1];
-  const int bl = blockIdx.y, batch = b0 + bl, k = blockIdx.z;
+  // blockIdx.x = cell block * n_dirs + direction: the blocks that evaluate the same cells for different directions are
+  // neighbours in launch order and share the cells' background / line / velocity records in the L2 (direction-major
+  // order re-read them from DRAM for every direction: 63 GB per C5 step)
+  const int bl = blockIdx.y, batch = b0 + bl, k = (int)(blockIdx.x % (unsigned)R.n_dirs);
+  const unsigned cell_block = blockIdx.x / (unsigned)R.n_dirs;
   if (VAR == DEX_CAV) dex_cav_block_setup(M, batch, CT, vfw, vfc);
   // one thread per pyramid cell of an active brick: the brick's selected level for this batch is the one the rays visit;
   // under a near-field cap (T8) they also visit the finer levels of the same brick
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long t = (long long)cell_block * blockDim.x + threadIdx.x;
   bool work = t < (long long)G.n_active * M.cps;
   const int cell = (int)t;                         // record index: slot * cps + position in the slot's pyramid
   if (work) {
@@ -679,23 +694,31 @@ dex_dir_records_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev 
     const float* bg = (VAR == DEX_VELINTERP) ? M.vtab + batch_base * (size_t)M.n_vbins * DEX_REC : M.store + batch_base * DEX_REC;
     float eta[DEX_W], chi[DEX_W];
     dex_provider<D, VAR, DEX_W>(M, batch_base, cell, 0, omf, sin_incl, CT, vfw, vfc, bg, bg, eta, chi);
-    float* o0 = rec + (size_t)k * M.mdir + (((size_t)bl * G.n_active) * M.cps + (size_t)(unsigned)cell) * DEX_W;
-    float* o1 = o0 + plane;
+    float* o0 = rec + (size_t)k * M.mdir + (((size_t)bl * G.n_active) * M.cps + (size_t)(unsigned)cell) * DexRecStride<D>::value;
+    float* o1 = o0 + ((D == 3) ? (size_t)DEX_W : plane);
+    float c2[DEX_W], S[DEX_W];
 #pragma unroll
     for (int j = 0; j < DEX_W; ++j) {
       const float cj = fmaxf(chi[j], DEX_CHI_TINY);
-      o0[j] = cj * 1.4426950408889634f;
-      o1[j] = eta[j] * dex_rcp(cj);
+      c2[j] = cj * 1.4426950408889634f;
+      S[j] = eta[j] * dex_rcp(cj);
+    }
+    // whole 32-byte rows: scalar stores left every sector half written, and the L2 read each one back from DRAM to merge
+    // (C5: 103 GB written + 46 GB read for 53 GB of records)
+#pragma unroll
+    for (int j = 0; j < DEX_W; j += 4) {
+      *reinterpret_cast<float4*>(o0 + j) = make_float4(c2[j], c2[j + 1], c2[j + 2], c2[j + 3]);
+      *reinterpret_cast<float4*>(o1 + j) = make_float4(S[j], S[j + 1], S[j + 2], S[j + 3]);
     }
     done = 1;
   }
-  if (line_eval_count != nullptr && blockIdx.z == 0) {
+  if (line_eval_count != nullptr && k == 0) {
     // bench.py's roofline counts provider evaluations: records (x active lines) here.  Every direction evaluates the same
     // cells, so direction 0 counts for all of them: one atomic per block instead of 1e8 on one address (C4)
     const int n = __syncthreads_count(done != 0u);
     const int nact = (VAR == DEX_CAV) ? CT.nq : 1;
     if (threadIdx.x == 0 && n && nact)
-      atomicAdd(line_eval_count, (unsigned long long)n * (unsigned long long)nact * (unsigned long long)gridDim.z);
+      atomicAdd(line_eval_count, (unsigned long long)n * (unsigned long long)nact * (unsigned long long)R.n_dirs);
   }
 }
 
@@ -973,7 +996,9 @@ static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const 
     d.n_batch = nb;
     d.mdir = 2 * plane;
     const long long tasks = (long long)A * (long long)cps;
-    dim3 grid((unsigned)((tasks + DEX_MARCH_THREADS - 1) / DEX_MARCH_THREADS), (unsigned)nb, (unsigned)rays.n_dirs);
+    const long long gx = ((tasks + DEX_MARCH_THREADS - 1) / DEX_MARCH_THREADS) * (long long)rays.n_dirs;
+    if (gx > 2147483647LL) { dex_free(d_rec, st); dex_set_error("march: too many (cell, direction) blocks for one records launch"); return DEX_ERR_UNSUPPORTED; }
+    dim3 grid((unsigned)gx, (unsigned)nb, 1);
     DexMipsDev full = m->dev;
     full.mdir = 2 * plane;
     full.voigt_fp32 = dex_tuning_voigt_fp32();
@@ -990,7 +1015,7 @@ static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const 
     }
     if (s == DEX_OK) {
       d.mrec = d_rec;
-      d.mplane = plane;
+      d.mplane = (D == 3) ? (size_t)DEX_W : plane;
       d.binfo = m->dev.binfo + (size_t)b0 * g->n_bricks;
       d.io_base = m->dev.io_base + b0 * DEX_W;
       s = launch_march_v<D, DEX_ISO>(g, &mm, rays, d_out, fuse_j, d_seg, lpr, perm, st);
@@ -1006,7 +1031,7 @@ static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const 
 static int memo_group(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays) {
   if (m->variant == DEX_ISO) return 0;
   const int knob = dex_tuning_memo();
-  if (knob == 0 || rays.n_dirs <= 0 || rays.n_dirs > 65535 || g->n_active <= 0) return 0;   // directions are the records kernel's grid.z
+  if (knob == 0 || rays.n_dirs <= 0 || g->n_active <= 0) return 0;
   const int D = g->desc.ndim;
   double cells0 = 1.0, mean_dim = 0.0;
   for (int a = 0; a < D; ++a) { cells0 *= (double)g->dev.B; mean_dim += (double)g->dev.dims[a] / D; }
@@ -1017,9 +1042,27 @@ static int memo_group(const dex_grid* g, const dex_mips* m, const DexRaysDev& ra
   size_t free_b = 0, total_b = 0;
   if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); return 0; }
   // half of what is available: the driver's free memory plus what the library's own pool holds idle from earlier calls
-  const double budget = fmin(0.5 * ((double)free_b + (double)dex_pool_idle_bytes()), 64.0e9);
+  const double budget = fmin(0.5 * ((double)free_b + (double)dex_pool_idle_bytes()), 96.0e9);
   const int nb = (int)fmin((double)m->n_batch, floor(budget / per_batch));
   return nb < 1 ? 0 : nb;
+}
+
+// one upload of the Weideman coefficients per device (they are constants of the method)
+static dex_status ensure_march_constants() {
+  static std::mutex mu;
+  static bool done[64] = {false};
+  int dev = 0;
+  DEX_CUDA_CHECK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return DEX_OK;
+  std::lock_guard<std::mutex> lk(mu);
+  if (!done[dev]) {
+    double c[DEX_WEI_N], L = 0.0;
+    dex_weideman_coefficients(c, &L);
+    DEX_CUDA_CHECK(cudaMemcpyToSymbol(dex_c_wei, c, sizeof(c)));
+    DEX_CUDA_CHECK(cudaMemcpyToSymbol(dex_c_wei_L, &L, sizeof(L)));
+    done[dev] = true;
+  }
+  return DEX_OK;
 }
 
 bool dex_auto_dir_split(long long n_probes, int n_dirs, int n_lambda) {
@@ -1039,7 +1082,8 @@ dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysD
                             unsigned long long* d_seg, int lanes_per_ray, bool tile, cudaStream_t st,
                             const int* perm_in) {
   int* d_perm = nullptr;
-  dex_status s = DEX_OK;
+  dex_status s = (m->variant == DEX_ISO) ? DEX_OK : ensure_march_constants();
+  if (s != DEX_OK) return s;
   if (tile && !perm_in) s = dex_make_probe_tiling(g, rays, &d_perm, st);
   const int* perm = perm_in ? perm_in : d_perm;
   // Small problems (fewer probes than one wave of blocks) leave most SMs idle while every thread walks its directions

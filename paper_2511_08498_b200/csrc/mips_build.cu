@@ -170,7 +170,8 @@ __global__ void reduce_spec_kernel(const BuildCtx X, int m) {
 // emitter: I_out = I_in + eta h ds) is represented by chi = 2^-60, S = eta 2^60: then tau is ~1e-18 h ds,
 // e^{-tau} = 1 and S (1 - e^{-tau}) = eta h ds to 1e-7, so the E(0) = 1 limit of DESIGN.md is kept.  (2^-100 / 2^100
 // in round 1: S overflowed to inf for eta above 2.7e8.)
-__global__ void make_march_records_kernel(const float* __restrict__ store, float* __restrict__ mrec, long long n_rec) {
+__global__ void make_march_records_kernel(const float* __restrict__ store, float* __restrict__ mrec, long long n_rec,
+                                          int interleaved /* 3D: one [chi' | S] record per cell, DexMipsDev::mrec */) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_rec * DEX_W) return;
   const int j = (int)(i % DEX_W);
@@ -180,8 +181,13 @@ __global__ void make_march_records_kernel(const float* __restrict__ store, float
   float c = chi, S;
   if (chi < tiny) { c = tiny; S = eta * 1.152921504606846976e18f; }   // 2^60, exact scaling (finite for eta < 2.9e20)
   else S = eta / chi;
-  mrec[i] = c * 1.4426950408889634f;
-  mrec[(size_t)n_rec * DEX_W + i] = S;
+  if (interleaved) {
+    mrec[r * DEX_REC + j] = c * 1.4426950408889634f;
+    mrec[r * DEX_REC + DEX_W + j] = S;
+  } else {
+    mrec[i] = c * 1.4426950408889634f;
+    mrec[(size_t)n_rec * DEX_W + i] = S;
+  }
 }
 
 // ---- line parameters and velocity: level 0 gather and box filter ------------------------------------
@@ -671,7 +677,7 @@ dex_status build_t(dex_mips* m, const dex_mips_desc* desc, cudaStream_t st) {
   }
   if (iso) {
     const long long n_rec = (long long)m->n_batch * A * X.M.cps;
-    make_march_records_kernel<<<blocks_for(n_rec * DEX_W, T), T, 0, st>>>(m->d_store, m->d_mrec, n_rec);
+    make_march_records_kernel<<<blocks_for(n_rec * DEX_W, T), T, 0, st>>>(m->d_store, m->d_mrec, n_rec, D == 3 ? 1 : 0);
     dex_count_launch();
   }
   select_levels_kernel<<<blocks_for((long long)m->n_batch * X.G.n_bricks, T), T, 0, st>>>(X, m->d_levels);
