@@ -388,8 +388,23 @@ class Bench:
             tr_launch = tr * (segs_per_launch / cap_segs)
             roof.update({"traffic": int(tr_launch), "dram_gbs": tr_launch / t / 1e9, "dram_frac": tr_launch / t / 1e9 / self.hbm_peak,
                          "l2_hit_pct": float(row["l2_hit_pct"]) if row.get("l2_hit_pct") else None,
-                         "traffic_source": f"profiles/traffic.csv (ncu --set full, builder-run: {row.get('source', '')}); "
+                         "traffic_source": f"profiles/traffic.csv (ncu, builder-run: {row.get('source', '')}); "
                                            "dram_gbs = that traffic / this run's kernel time"})
+            if roof["dram_frac"] >= 0.25:
+                # the launch moves a quarter of the HBM peak or more (C5: per-direction records read once per segment with
+                # little reuse): the binding roofline is HBM.  Algorithmic bytes: the 8 B record per seg*lambda the march reads,
+                # plus the 8 B per memoised record*lambda the records kernel writes
+                # (evals counts (record, wavelength) pairs, times the active lines of the batch for Core-and-Voigt: one for C5)
+                algo = ALGO_BYTES[wl.variant] * sl + (8.0 * evals if memoised else 0.0)
+                gbs = algo / t / 1e9
+                roof.update({"alu_achieved_tflops": roof["achieved"], "alu_frac": roof["frac"], "alu_peak_tflops": roof["peak"],
+                             "bound": "hbm", "achieved": gbs, "peak": self.hbm_peak, "unit": "GB/s", "frac": gbs / self.hbm_peak,
+                             "binds": "HBM: the ISO march reads one 64-byte per-direction record per segment with an L2 hit rate "
+                                      "below 40 % (the records of all directions of a batch are 17.6 GB)",
+                             "peak_source": self.hbm_src,
+                             "note": f"achieved = ALGORITHMIC bytes ({ALGO_BYTES[wl.variant]:g} B per seg*lambda read by the march"
+                                     + (" + 8 B per memoised record*lambda written by the records kernel" if memoised else "")
+                                     + ") / time of the library's march region (records kernel + march) from CUDA events"})
         return roof
 
     def measure(self, name, steps, warmup, e2e_steps, want_cpu, cpu_target_s, one_thread_s):

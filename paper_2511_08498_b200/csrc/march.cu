@@ -483,8 +483,11 @@ __device__ __forceinline__ void dex_cav_block_setup(const DexMipsDev& M, int bat
 #ifndef DEX_MINB_CAV
 #define DEX_MINB_CAV 4
 #endif
-constexpr int dex_march_minb(int var) {
-  return var == DEX_ISO ? DEX_MARCH_MINB : (var == DEX_VELINTERP ? DEX_MINB_VEL : DEX_MINB_CAV);
+#ifndef DEX_MINB_ISO3D
+#define DEX_MINB_ISO3D 7   // swept on C5 memoised: 6 / 7 / 8 / 10 blocks per SM give 97.2 / 94.0 / 99.2 / 126.8 ms (8 spills 40 B at 64 registers)
+#endif
+constexpr int dex_march_minb(int var, int ndim) {
+  return var == DEX_ISO ? (ndim == 3 ? DEX_MINB_ISO3D : DEX_MARCH_MINB) : (var == DEX_VELINTERP ? DEX_MINB_VEL : DEX_MINB_CAV);
 }
 #ifndef DEX_FOLD_EVERY
 #define DEX_FOLD_EVERY 32   // power of two
@@ -500,7 +503,7 @@ constexpr int dex_march_minb(int var) {
 
 
 template <int D, int VAR, int LPR, bool FUSE_J, bool CLIP>
-__global__ void __launch_bounds__(DEX_MARCH_THREADS, dex_march_minb(VAR))
+__global__ void __launch_bounds__(DEX_MARCH_THREADS, dex_march_minb(VAR, D))
 dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ perm,
                  float* __restrict__ out, unsigned long long* __restrict__ seg_count,
                  unsigned long long* __restrict__ line_seg_count) {
@@ -595,6 +598,13 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
           ds = __fsub_rn(fminf(ray.t, R.t_end), fmaxf(t0, R.t_begin));
           emit = emit && ds > 0.0f;
           if (ray.t >= R.t_end) { alive = false; blocked = false; }
+        }
+        // 3D ISO march over records that miss the L2 (C5 memoised: long_scoreboard 9 warps per issue, DRAM at 45 %): after an
+        // in-brick step the next cell's 64-byte record is known one iteration early and is requested into the L2 now
+        // (C5 102.5 -> 99.2 ms; into the L1, or one request per 32-byte half, is slower: profiles/r02_experiments.md)
+        if (D == 3 && VAR == DEX_ISO && !blocked && ray.cell >= 0) {
+          const float* pn = iso0 + (size_t)(unsigned)ray.cell * DexRecStride<D>::value;
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(pn));
         }
         if (emit) {
           ++nseg;
@@ -1042,7 +1052,8 @@ static int memo_group(const dex_grid* g, const dex_mips* m, const DexRaysDev& ra
   size_t free_b = 0, total_b = 0;
   if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); return 0; }
   // half of what is available: the driver's free memory plus what the library's own pool holds idle from earlier calls
-  const double budget = fmin(0.5 * ((double)free_b + (double)dex_pool_idle_bytes()), 96.0e9);
+  // at most 64 GB in 2D (C4: 7 batches per group 7.44 s, 11 per group 7.60 s), 96 GB in 3D (C5's four batches in one launch)
+  const double budget = fmin(0.5 * ((double)free_b + (double)dex_pool_idle_bytes()), D == 3 ? 96.0e9 : 64.0e9);
   const int nb = (int)fmin((double)m->n_batch, floor(budget / per_batch));
   return nb < 1 ? 0 : nb;
 }
