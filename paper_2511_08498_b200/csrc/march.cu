@@ -483,6 +483,9 @@ __device__ __forceinline__ void dex_cav_block_setup(const DexMipsDev& M, int bat
 #ifndef DEX_MINB_CAV
 #define DEX_MINB_CAV 4
 #endif
+#ifndef DEX_REC_THREADS
+#define DEX_REC_THREADS 128   // block of dex_dir_records_kernel
+#endif
 #ifndef DEX_MINB_ISO3D
 #define DEX_MINB_ISO3D 7   // swept on C5 memoised: 6 / 7 / 8 / 10 blocks per SM give 97.2 / 94.0 / 99.2 / 126.8 ms (8 spills 40 B at 64 registers)
 #endif
@@ -668,7 +671,7 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
 // (chi' log2 e | S, the ISO layout); the rays are then marched by the ISO kernel with M.mdir stepping the record
 // pointers from direction to direction.
 template <int D, int VAR>
-__global__ void __launch_bounds__(DEX_MARCH_THREADS)
+__global__ void __launch_bounds__(DEX_REC_THREADS)
 dex_dir_records_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, const int* __restrict__ active_bricks,
                        int b0, float* __restrict__ rec, size_t plane, unsigned long long* __restrict__ line_eval_count) {
   __shared__ DexCavTab CT;
@@ -1006,7 +1009,7 @@ static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const 
     d.n_batch = nb;
     d.mdir = 2 * plane;
     const long long tasks = (long long)A * (long long)cps;
-    const long long gx = ((tasks + DEX_MARCH_THREADS - 1) / DEX_MARCH_THREADS) * (long long)rays.n_dirs;
+    const long long gx = ((tasks + DEX_REC_THREADS - 1) / DEX_REC_THREADS) * (long long)rays.n_dirs;
     if (gx > 2147483647LL) { dex_free(d_rec, st); dex_set_error("march: too many (cell, direction) blocks for one records launch"); return DEX_ERR_UNSUPPORTED; }
     dim3 grid((unsigned)gx, (unsigned)nb, 1);
     DexMipsDev full = m->dev;
@@ -1015,10 +1018,10 @@ static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const 
     dex_status s = DEX_OK;
     if (tasks > 0) {
       if (m->variant == DEX_VELINTERP)
-        dex_dir_records_kernel<D, DEX_VELINTERP><<<grid, DEX_MARCH_THREADS, 0, st>>>(g->dev, full, rays, g->d_active_bricks, b0,
+        dex_dir_records_kernel<D, DEX_VELINTERP><<<grid, DEX_REC_THREADS, 0, st>>>(g->dev, full, rays, g->d_active_bricks, b0,
                                                                                     d_rec, plane, dex_line_segment_counter());
       else
-        dex_dir_records_kernel<D, DEX_CAV><<<grid, DEX_MARCH_THREADS, 0, st>>>(g->dev, full, rays, g->d_active_bricks, b0, d_rec,
+        dex_dir_records_kernel<D, DEX_CAV><<<grid, DEX_REC_THREADS, 0, st>>>(g->dev, full, rays, g->d_active_bricks, b0, d_rec,
                                                                               plane, dex_line_segment_counter());
       dex_count_launch();
       if (cudaGetLastError() != cudaSuccess) { dex_set_error("record kernel launch failed"); s = DEX_ERR_CUDA; }
