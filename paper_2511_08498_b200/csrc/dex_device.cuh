@@ -327,7 +327,7 @@ __device__ __forceinline__ bool dex_ray_cross(DexRay3<D>& r, const DexGridDev& G
 // once per block.  The cap's threshold loops sit in the middle of the general routines; without them a crossing is
 // straight-line code apart from the rare re-entry into a finer brick (profiles/r02: the crossing was 25 % of the
 // instructions of C3's march).
-template <int D>
+template <int D, bool BOX>
 __device__ __forceinline__ void dex_set_cell_nocap(DexRay3<D>& r, const DexGridDev& G, int info, const int* x) {
   const int m = (info & 15) - 1;
   r.info = info;
@@ -337,7 +337,7 @@ __device__ __forceinline__ void dex_set_cell_nocap(DexRay3<D>& r, const DexGridD
     // leaves it through the face of the brick it enters next, so the times of the emitted visits are unchanged.
     // (2D only: in 3D the two extra coordinate searches per box exit and their registers cost the Core-and-Voigt march
     //  more than the skipped bricks save -- C5 139.7 -> 142.0 ms with boxes, C2 45.7 -> 44.4, C3 317.0 -> 311.5)
-    const int d = (D == 2) ? max(1, info >> 4) : 1;
+    const int d = BOX ? max(1, info >> 4) : 1;
     r.sh = (d > 1) ? G.logB + 1 : G.logB;        // sh > logB marks a multi-brick box (dex_ray_cross_nocap)
     const float fB = (float)G.B;
     float tb = __int_as_float(0x7f800000);
@@ -378,7 +378,7 @@ __device__ __forceinline__ void dex_set_cell_nocap(DexRay3<D>& r, const DexGridD
   r.cell = (info >> 4) + idx;
 }
 
-template <int D>
+template <int D, bool BOX>
 __device__ __forceinline__ bool dex_ray_cross_nocap(DexRay3<D>& r, const DexGridDev& G, const int* __restrict__ binfo,
                                                     const float* __restrict__ probe, const float* __restrict__ omega) {
   int s;
@@ -405,7 +405,7 @@ __device__ __forceinline__ bool dex_ray_cross_nocap(DexRay3<D>& r, const DexGrid
   const int xe = poss ? kps : kps - 1;           // level-0 coordinate just beyond the exit plane (T5)
   const int cs = poss ? kps - size : kps;
   const bool alive = (unsigned)xe < (unsigned)dims_s;
-  const bool box = (D == 2) && r.sh > G.logB;   // leaving a multi-brick box of empty space (2D only, dex_set_cell_nocap)
+  const bool box = BOX && r.sh > G.logB;        // leaving a multi-brick box of empty space (dex_set_cell_nocap)
   const bool newbrick = box || ((xe ^ cs) >> G.logB) != 0;
 #pragma unroll
   for (int a = 0; a < D; ++a) x[a] = (a == s) ? xe : c[a];
@@ -428,6 +428,6 @@ __device__ __forceinline__ bool dex_ray_cross_nocap(DexRay3<D>& r, const DexGrid
         if (a != s) x[a] = dex_fine_coord(__ldg(probe + a), -__ldg(omega + a), r.inv[a], r.off[a], c[a], size, th, a < s);
     }
   }
-  dex_set_cell_nocap<D>(r, G, info, x);
+  dex_set_cell_nocap<D, BOX>(r, G, info, x);
   return true;
 }

@@ -108,7 +108,7 @@ dex_status dex_launch_grid_build(dex_grid* g, const uint8_t* d_active, cudaStrea
   dex_count_launch();
   dex_scan_slots_kernel<<<1, 1024, 0, st>>>(d_flag, nb, g->d_slot, g->d_active_bricks, d_count);
   if (g->desc.ndim == 2) dex_empty_distance_kernel<2><<<(nb + 127) / 128, 128, 0, st>>>(g->dev, d_flag, g->d_edist);
-  else dex_fill_int_kernel<<<(nb + 255) / 256, 256, 0, st>>>(g->d_edist, nb, 1);   // 3D rays take empty bricks one at a time (dex_device.cuh)
+  else dex_fill_int_kernel<<<(nb + 255) / 256, 256, 0, st>>>(g->d_edist, nb, 1);   // 3D rays take empty bricks one at a time (march.cu DEX_BOX)
   dex_count_launch(2);
   int h_count = 0;
   cudaError_t e = cudaMemcpyAsync(&h_count, d_count, sizeof(int), cudaMemcpyDeviceToHost, st);

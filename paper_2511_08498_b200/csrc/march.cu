@@ -483,6 +483,10 @@ __device__ __forceinline__ void dex_cav_block_setup(const DexMipsDev& M, int bat
 #ifndef DEX_MINB_CAV
 #define DEX_MINB_CAV 4
 #endif
+// which marches cross a whole box of empty bricks in one step (dex_device.cuh): the 2D ones.  In 3D the two extra
+// coordinate searches per box exit cost what the skipped bricks save (C5 in the ray loop 139.7 -> 142.0 ms, C5 memoised
+// with the 3D ISO march 94.2 -> 95.1 ms), so 3D rays take empty bricks one at a time
+#define DEX_BOX(D, VAR) ((D) == 2)
 #ifndef DEX_REC_THREADS
 #define DEX_REC_THREADS 128   // block of dex_dir_records_kernel
 #endif
@@ -587,7 +591,7 @@ dex_march_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, con
       const unsigned bm = __ballot_sync(FULL, blocked);
       if (bm == am || __popc(bm) >= DEX_CROSS_QUORUM) {
         if (blocked) {
-          alive = caps ? dex_ray_cross<D>(ray, G, M, binfo, probe, om) : dex_ray_cross_nocap<D>(ray, G, binfo, probe, om);
+          alive = caps ? dex_ray_cross<D>(ray, G, M, binfo, probe, om) : dex_ray_cross_nocap<D, DEX_BOX(D, VAR)>(ray, G, binfo, probe, om);
           blocked = false;
         }
       }
