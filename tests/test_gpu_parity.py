@@ -265,6 +265,7 @@ def test_cav_small(P, name, n, metric, thr, gate):
                                                 ("C4", dict(n=128, n_dirs=6, n_probes=200), 0.3, "caps+interval"),
                                                 ("C4", dict(n=64, n_dirs=4, n_probes=150), 0.3, "25d"),
                                                 ("C5", dict(n=64, n_dirs=8, n_probes=300), 5.0, "plain"),
+                                                ("C5", dict(n=64, n_dirs=6, n_probes=200), 5.0, "caps+interval"),
                                                 ("C4", dict(n=64, n_dirs=6, n_probes=100), 0.3, "classic"),
                                                 ("C3", dict(n=128, n_dirs=8, n_probes=300), None, "plain")])
 def test_memo_parity(P, name, kw, thr, extra):
