@@ -490,6 +490,9 @@ __device__ __forceinline__ void dex_cav_block_setup(const DexMipsDev& M, int bat
 #ifndef DEX_REC_THREADS
 #define DEX_REC_THREADS 128   // block of dex_dir_records_kernel
 #endif
+#ifndef DEX_REC_GROUP
+#define DEX_REC_GROUP 8       // runs of DEX_REC_THREADS cells per block of dex_dir_records_kernel
+#endif
 #ifndef DEX_MINB_ISO3D
 #define DEX_MINB_ISO3D 7   // swept on C5 memoised: 6 / 7 / 8 / 10 blocks per SM give 97.2 / 94.0 / 99.2 / 126.8 ms (8 spills 40 B at 64 registers)
 #endif
@@ -685,11 +688,16 @@ dex_dir_records_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev 
   // neighbours in launch order and share the cells' background / line / velocity records in the L2 (direction-major
   // order re-read them from DRAM for every direction: 63 GB per C5 step)
   const int bl = blockIdx.y, batch = b0 + bl, k = (int)(blockIdx.x % (unsigned)R.n_dirs);
-  const unsigned cell_block = blockIdx.x / (unsigned)R.n_dirs;
+  const unsigned cell_group = blockIdx.x / (unsigned)R.n_dirs;
   if (VAR == DEX_CAV) dex_cav_block_setup(M, batch, CT, vfw, vfc);
+  unsigned done = 0;
+  // a block evaluates DEX_REC_GROUP consecutive runs of blockDim.x cells, so that the table set-up above (9.6 KB of Voigt
+  // tables into shared memory, the per-line constants in fp64, a barrier) is paid once per ~1000 evaluations
+#pragma unroll 1
+  for (int run = 0; run < DEX_REC_GROUP; ++run) {
   // one thread per pyramid cell of an active brick: the brick's selected level for this batch is the one the rays visit;
   // under a near-field cap (T8) they also visit the finer levels of the same brick
-  const long long t = (long long)cell_block * blockDim.x + threadIdx.x;
+  const long long t = ((long long)cell_group * DEX_REC_GROUP + run) * blockDim.x + threadIdx.x;
   bool work = t < (long long)G.n_active * M.cps;
   const int cell = (int)t;                         // record index: slot * cps + position in the slot's pyramid
   if (work) {
@@ -700,7 +708,6 @@ dex_dir_records_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev 
     for (int i = 1; i <= M.max_level; ++i) l += (c >= M.lvloff[i]) ? 1 : 0;
     work = m >= 0 && (l == m || (M.n_caps > 0 && l < m));
   }
-  unsigned done = 0;
   if (work) {
     float omf[D];
 #pragma unroll
@@ -727,15 +734,21 @@ dex_dir_records_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev 
       *reinterpret_cast<float4*>(o0 + j) = make_float4(c2[j], c2[j + 1], c2[j + 2], c2[j + 3]);
       *reinterpret_cast<float4*>(o1 + j) = make_float4(S[j], S[j + 1], S[j + 2], S[j + 3]);
     }
-    done = 1;
+    done += 1;
+  }
   }
   if (line_eval_count != nullptr && k == 0) {
     // bench.py's roofline counts provider evaluations: records (x active lines) here.  Every direction evaluates the same
     // cells, so direction 0 counts for all of them: one atomic per block instead of 1e8 on one address (C4)
-    const int n = __syncthreads_count(done != 0u);
+    __shared__ unsigned n_done;
+    if (threadIdx.x == 0) n_done = 0;
+    __syncthreads();
+    const unsigned w = __reduce_add_sync(0xffffffffu, done);
+    if ((threadIdx.x & 31) == 0 && w) atomicAdd(&n_done, w);
+    __syncthreads();
     const int nact = (VAR == DEX_CAV) ? CT.nq : 1;
-    if (threadIdx.x == 0 && n && nact)
-      atomicAdd(line_eval_count, (unsigned long long)n * (unsigned long long)nact * (unsigned long long)R.n_dirs);
+    if (threadIdx.x == 0 && n_done && nact)
+      atomicAdd(line_eval_count, (unsigned long long)n_done * (unsigned long long)nact * (unsigned long long)R.n_dirs);
   }
 }
 
@@ -1013,7 +1026,8 @@ static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const 
     d.n_batch = nb;
     d.mdir = 2 * plane;
     const long long tasks = (long long)A * (long long)cps;
-    const long long gx = ((tasks + DEX_REC_THREADS - 1) / DEX_REC_THREADS) * (long long)rays.n_dirs;
+    const long long per_block = (long long)DEX_REC_THREADS * DEX_REC_GROUP;
+    const long long gx = ((tasks + per_block - 1) / per_block) * (long long)rays.n_dirs;
     if (gx > 2147483647LL) { dex_free(d_rec, st); dex_set_error("march: too many (cell, direction) blocks for one records launch"); return DEX_ERR_UNSUPPORTED; }
     dim3 grid((unsigned)gx, (unsigned)nb, 1);
     DexMipsDev full = m->dev;
