@@ -9,10 +9,10 @@ dex_build_sparse_grid + dex_build_vlm_mips + dex_mean_intensity (fused HDDA marc
 
 BASELINE.json's `metric` names no config, so the headline (`value`, `ms_per_step`, `roofline`, `e2e`,
 `cpu_baseline` at the top level of the JSON line) is quoted on the largest single-GPU configuration that
-fits K = 20 timed steps in a minute: C3 (configs[2], 1024x1024, velocity interpolation, 0.6 s per step).
+fits K = 20 timed steps in a minute: C3 (configs[2], 1024x1024, velocity interpolation, 0.3 s per step).
 The same process then measures every other BASELINE config into `per_config` (own step counts, own clock
-sample, own roofline / e2e / cpu_baseline); C4 (configs[3], tens of seconds per step) takes 1 warm-up + 1
-timed step there, stated in its entry.
+sample, own roofline / e2e / cpu_baseline); C4 (configs[3], 7 s per step) takes 1 timed + 1 end-to-end
+step there, stated in its entry.  The whole default run takes two minutes.
 
 N > 1 (torchrun): `--shard replicas` (default): every rank solves its own seeded atmosphere of the same
 size (weak scaling, no data-path collective -- rays are independent); NCCL is used only for
