@@ -74,6 +74,30 @@ dex_status dex_grid_info(const dex_grid* grid, int64_t* n_bricks, int64_t* n_act
 dex_status dex_grid_get_slots(const dex_grid* grid, int32_t* h_slot /*[n_bricks]*/);
 void dex_destroy_grid(dex_grid* grid);
 
+/* a1 for callers that must not allocate device memory (same numbering as
+ * dex_build_sparse_grid: active bricks get slots 0..A-1 in brick-index order).
+ * Meant for code that runs where an allocation is not an option: a solver confined to a memory budget fixed at
+ * start-up, a plug-in inside a host application that owns the device allocator, a latency-bound loop that cannot
+ * wait on the driver's allocation lock.  dex_build_sparse_grid takes its flag array, its counter and the handle's
+ * tables from the library's pool; this entry calls no cudaMalloc / cudaFree / pool routine and never synchronises:
+ *   outputs   d_slot [n_bricks] (slot, -1 = empty brick), d_active_bricks [n_bricks] (entry s = brick of slot s for
+ *             s < A; entries from A on are left as they were), d_n_active [1] (A) -- CALLER-OWNED DEVICE memory,
+ *             written asynchronously on `stream`; no handle is created (the other calls of this header do not take
+ *             these tables -- this entry serves callers that run the brick bookkeeping themselves);
+ *   scratch   the per-brick occupancy flags sit in a fixed array inside the library image: DEX_STATIC_MAX_BRICKS
+ *             ints (4 MiB), held by every GPU that loads libdex.so until the process exits.  More bricks than that
+ *             -> DEX_ERR_SHAPE with a message naming the limit, nothing launched.
+ * The first call on each device looks up the array's device address (cudaGetSymbolAddress, with the caller's
+ * current device) and keeps it; make that first call outside any stream capture.  All calls on a device share the
+ * array and it keeps the last call's contents; each call rewrites the part it reads, so nothing needs clearing, but
+ * two calls that can overlap on the GPU (two streams with no ordering between them) race on it -- order them.
+ * d_active: [nvox] device bytes or NULL (all active).
+ * Errors: DEX_ERR_INVALID_ARG (NULL desc / outputs, ndim), DEX_ERR_SHAPE (brick, dims, too many bricks),
+ * DEX_ERR_UNSUPPORTED (device ordinal >= 64), DEX_ERR_CUDA. */
+#define DEX_STATIC_MAX_BRICKS (1 << 20)
+dex_status dex_brick_slots_static(const dex_grid_desc* desc, const uint8_t* d_active /*[nvox] or NULL*/,
+                                  int32_t* d_slot, int32_t* d_active_bricks, int32_t* d_n_active, void* stream);
+
 /* ------------------------------------------------------------------------------------------
  * MIP pyramid + variance-limited mipmapping
  * ---------------------------------------------------------------------------------------- */

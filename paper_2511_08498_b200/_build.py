@@ -13,6 +13,7 @@ COMMON = ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-Xcompiler",
 SOURCES = {
     "dex_api.cu": [],
     "grid_build.cu": [],
+    "grid_static.cu": [],
     "mips_build.cu": ["-fmad=false"],
     "march.cu": [],
     "peaks.cu": [],

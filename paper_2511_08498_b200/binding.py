@@ -31,7 +31,9 @@ EXPORTS = (
     "dex_mean_intensity", "dex_mean_intensity_host", "dex_mean_intensity_pipelined", "dex_pool_high_water", "dex_trim", "dex_direction_fields",
     "dex_mean_intensity_single_direction", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read", "dex_march_work_read",
     "dex_set_lanes_per_ray", "dex_get_lanes_per_ray", "dex_measure_fp32_peak", "dex_set_tuning",
+    "dex_brick_slots_static",
 )
+DEX_STATIC_MAX_BRICKS = 1 << 20
 
 
 class DexError(RuntimeError):
@@ -76,6 +78,7 @@ def _load():
     L.dex_version.restype = C.c_char_p
     L.dex_launch_count.restype = C.c_int64
     L.dex_build_sparse_grid.argtypes = [C.POINTER(_GridDesc), C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p)]
+    L.dex_brick_slots_static.argtypes = [C.POINTER(_GridDesc), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     L.dex_grid_info.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.dex_grid_get_slots.argtypes = [C.c_void_p, C.c_void_p]
     L.dex_destroy_grid.argtypes = [C.c_void_p]
@@ -234,6 +237,24 @@ def dex_build_sparse_grid(ndim, dims, brick, voxel_size, active: Optional[torch.
     h = C.c_void_p()
     _check(_L.dex_build_sparse_grid(C.byref(d), _ptr(active, torch.uint8), _stream(stream), C.byref(h)))
     return Grid(h, ndim, dd, brick, voxel_size)
+
+
+def dex_brick_slots_static(ndim, dims, brick, voxel_size, active: Optional[torch.Tensor], slot: torch.Tensor,
+                           active_bricks: torch.Tensor, n_active: torch.Tensor, stream=None):
+    """Step a1 for callers that cannot allocate on the device (a fixed memory budget, a host application that owns the
+    allocator, a loop that cannot wait on the driver): brick slots, slot -> brick list and active count written into
+    the caller's int32 CUDA tensors `slot` [n_bricks], `active_bricks` [n_bricks], `n_active` [1].  Nothing is
+    allocated, nothing synchronises; the flag scratch is a 4 MiB array inside libdex.so, so at most
+    DEX_STATIC_MAX_BRICKS bricks (DexError otherwise) and no two overlapping calls on one GPU.  See include/dex.h."""
+    d = _GridDesc()
+    d.ndim = ndim
+    dd = list(dims) + [1] * (3 - len(dims))
+    for a in range(3):
+        d.dims[a] = int(dd[a])
+    d.brick = int(brick)
+    d.voxel_size = float(voxel_size)
+    _check(_L.dex_brick_slots_static(C.byref(d), _ptr(active, torch.uint8), _ptr(slot, torch.int32),
+                                     _ptr(active_bricks, torch.int32), _ptr(n_active, torch.int32), _stream(stream)))
 
 
 class Mips:
