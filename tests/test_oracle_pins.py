@@ -1055,3 +1055,211 @@ def test_p17_velinterp_tests_the_rest_frame():
     assert (orc.build_mips(wl, variant=orc.VELINTERP).levels == 0).all()        # relvar of (1,1,3,3) is 0.25 > 0.2
     wl.thr_eta = wl.thr_chi = 0.26
     assert (orc.build_mips(wl, variant=orc.VELINTERP).levels >= 1).all()
+
+
+# ------------------------------------------------------------------------------------------------
+# The 3D half of the level selection (SURVEY.md 8(c) V1, V2, V5, P7, P10; PAPER.md:127-130 eq. 8, :142, :148).
+# Mutants these pins exist for: sample instead of population variance over the 8 children,
+# and a brick aggregation with two brick axes exchanged.
+# ------------------------------------------------------------------------------------------------
+def _iso_3d_from_c5(n=32, n_dirs=6, n_probes=40, seed=5):
+    """C5's occupancy, probes and directions around a static (ISO) 3D medium: a smooth stratification times log-normal
+    small-scale noise whose amplitude is drawn per brick (0 / 1 % / 5 % / 30 %) and grows with wavelength, so that
+    bricks and wavelength batches land on different levels.  Input recipe only: no method arithmetic."""
+    wl = make("C5", n=n, n_dirs=n_dirs, n_probes=n_probes)
+    rng = np.random.default_rng(seed)
+    b = wl.brick
+    nb = n // b
+    z = np.arange(n, dtype=np.float64)[:, None, None, None]
+    base = np.exp(-np.abs(z - n / 2.0) / (2.0 * n)) * np.ones((n, n, n, 1))
+    amp_b = rng.choice([0.0, 0.01, 0.05, 0.3], size=(nb, nb, nb))
+    amp = np.repeat(np.repeat(np.repeat(amp_b, b, 0), b, 1), b, 2)[..., None] * np.linspace(0.25, 1.0, wl.n_lambda)
+    occ = wl.active.reshape(n, n, n, 1).astype(bool)
+    eta = base * np.exp(amp * rng.standard_normal((n, n, n, wl.n_lambda))) * occ
+    chi = 0.3 * base * np.exp(amp * rng.standard_normal((n, n, n, wl.n_lambda))) * occ
+    return iso_workload((n, n, n), b, eta, chi, wl.probe_pos, wl.dirs, active=wl.active, weights=wl.weights,
+                        max_level=3, h=wl.voxel_size)
+
+
+def _levels_by_loops_3d(wl, max_level, metric, thr, tau_gate):
+    """Second implementation of V1-V5 for a 3D ISO medium, structured brick by brick: each populated brick builds its
+    own little pyramid in python floats and stops at the first level where one of its cells fails.  The statistic is
+    typed out for 8 children with the population variance (divide by 8, eq. 8 / V2), the mean as the V1 child-order sum
+    times 1/8 rounded once to fp32."""
+    nx, ny, nz = wl.dims
+    B, W, h = wl.brick, wl.lambda_batch, float(wl.voxel_size)
+    thr, tau_gate = float(np.float32(thr)), float(np.float32(tau_gate))
+    eta = wl.eta.reshape(nz, ny, nx, wl.n_lambda)
+    chi = wl.chi.reshape(nz, ny, nx, wl.n_lambda)
+    act = wl.active.reshape(nz, ny, nx)
+    nbx, nby, nbz = nx // B, ny // B, nz // B
+    out = np.zeros((wl.n_batch, nbx * nby * nbz), dtype=np.int8)
+
+    def kids(p, k, j, i, l):      # child order: x fastest, then y, then z (V1)
+        return [float(p[2 * k + dz, 2 * j + dy, 2 * i + dx, l]) for dz in (0, 1) for dy in (0, 1) for dx in (0, 1)]
+
+    def total(v):
+        return ((((((v[0] + v[1]) + v[2]) + v[3]) + v[4]) + v[5]) + v[6]) + v[7]
+
+    def stat(vals):
+        if all(v == vals[0] for v in vals):
+            return 0.0
+        if metric == orc.IOD_LOG:
+            if any(v <= 0 for v in vals):
+                return math.inf
+            X = [math.log(v * h) for v in vals]
+        else:
+            X = list(vals)
+        mean = total(X) / 8
+        var = total([(x - mean) ** 2 for x in X]) / 8            # population variance of the 8 children
+        if mean == 0:
+            return math.inf
+        return abs(var / mean) if metric == orc.IOD_LOG else var / (mean * mean)
+
+    for bz in range(nbz):
+        for by in range(nby):
+            for bx in range(nbx):
+                bi = (bz * nby + by) * nbx + bx
+                box = (slice(bz * B, (bz + 1) * B), slice(by * B, (by + 1) * B), slice(bx * B, (bx + 1) * B))
+                if not act[box].any():
+                    out[:, bi] = -1
+                    continue
+                for bt in range(wl.n_batch):
+                    pe = eta[box][..., bt * W:(bt + 1) * W].astype(np.float64)
+                    pc = chi[box][..., bt * W:(bt + 1) * W].astype(np.float64)
+                    level = 0
+                    for m in range(1, max_level + 1):
+                        s = pe.shape[0] // 2
+                        ne, nc = np.zeros((s, s, s, W)), np.zeros((s, s, s, W))
+                        ok = True
+                        for k in range(s):
+                            for j in range(s):
+                                for i in range(s):
+                                    for l in range(W):
+                                        ve, vc = kids(pe, k, j, i, l), kids(pc, k, j, i, l)
+                                        ne[k, j, i, l] = np.float32(total(ve) * 0.125)
+                                        nc[k, j, i, l] = np.float32(total(vc) * 0.125)
+                                        passed = stat(ve) < thr and stat(vc) < thr
+                                        if tau_gate >= 0 and (total(vc) / 8) * h <= tau_gate:
+                                            passed = True
+                                        ok = ok and passed
+                        if not ok:
+                            break
+                        level, pe, pc = m, ne, nc
+                    out[bt, bi] = level
+    return out
+
+
+@pytest.mark.parametrize("metric,thr,gate", [(orc.RELVAR, 1e-3, -1.0), (orc.RELVAR, 1e-4, -1.0),
+                                             (orc.IOD_LOG, 0.02, 0.2), (orc.IOD_LOG, 0.004, -1.0)])
+def test_p10_3d_level_selection_second_implementation(metric, thr, gate):
+    wl = _iso_3d_from_c5()
+    M = orc.build_mips(wl, max_level=3, metric=metric, thr_eta=thr, thr_chi=thr, tau_gate=gate)
+    ref = _levels_by_loops_3d(wl, 3, metric, thr, gate)
+    assert (ref == -1).any() and len(np.unique(ref[ref >= 0])) >= 2      # the case separates levels
+    assert np.array_equal(M.levels, ref)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_p10_3d_hand_example_population_variance(axis):
+    """2x2x2 children (1,1,1,1,3,3,3,3), the 3s on the upper half along `axis` (numpy order z, y, x): mean 2, population
+    variance 1 -> relvar 1/4 (the sample variance 8/7 would give 2/7 = 0.2857); X = ln x = (0 x4, ln3 x4): mean ln3/2,
+    variance (ln3/2)^2 -> IoD = ln3/2 = 0.5493 (sample variance: 0.6278)."""
+    dims = (8, 8, 8)
+    x = np.ones(dims)
+    sl = [slice(None)] * 3
+    sl[axis] = slice(1, None, 2)
+    x[tuple(sl)] = 3.0
+    wl = iso_workload(dims, 8, x, x, [[1.5, 1.5, 1.5]], [[1.0, 0.0, 0.0]], max_level=3)
+    assert (orc.build_mips(wl, metric=orc.RELVAR, thr_eta=0.2501, thr_chi=0.2501).levels >= 1).all()
+    assert (orc.build_mips(wl, metric=orc.RELVAR, thr_eta=0.2499, thr_chi=0.2499).levels == 0).all()
+    assert (orc.build_mips(wl, metric=orc.IOD_LOG, thr_eta=0.5494, thr_chi=0.5494).levels >= 1).all()
+    assert (orc.build_mips(wl, metric=orc.IOD_LOG, thr_eta=0.5492, thr_chi=0.5492).levels == 0).all()
+    # level-1 cells are all 2 -> once level 1 passes every higher level does (IoD = 0 < thr)
+    assert (orc.build_mips(wl, metric=orc.RELVAR, thr_eta=0.2501, thr_chi=0.2501).levels == 3).all()
+    # the statistic itself, on one cell: children in V1 order
+    ch = [np.array([v], dtype=np.float64) for v in (1, 1, 1, 1, 3, 3, 3, 3)]
+    assert orc.cell_metric(ch, orc.RELVAR, 1.0)[0] == 0.25
+    assert abs(orc.cell_metric(ch, orc.IOD_LOG, 1.0)[0] - math.log(3.0) / 2) < 1e-15
+    # gate (PAPER.md:144): mean chi h = 2
+    assert (orc.build_mips(wl, metric=orc.RELVAR, thr_eta=0.0, thr_chi=0.0, tau_gate=2.0).levels == 3).all()
+    assert (orc.build_mips(wl, metric=orc.RELVAR, thr_eta=0.0, thr_chi=0.0, tau_gate=1.99).levels == 0).all()
+
+
+def test_p10_3d_brick_aggregation_typed_in_levels():
+    """A 4 x 3 x 2 brick lattice (x, y, z) whose bricks are told apart by position: brick b = (bz*3 + by)*4 + bx (V5,
+    PAPER.md:148, :170).  Smooth everywhere (level 3) except four marked bricks; exchanging any two brick axes in the
+    aggregation moves the marks (or cannot even be reshaped)."""
+    nx, ny, nz, B = 32, 24, 16, 8
+    x = np.full((nz, ny, nx), 0.5)
+    act = np.ones((nz, ny, nx), dtype=np.uint8)
+
+    def box(bx, by, bz):
+        return (slice(bz * B, (bz + 1) * B), slice(by * B, (by + 1) * B), slice(bx * B, (bx + 1) * B))
+
+    # (3, 1, 0): one odd voxel -> its level-1 cell fails -> level 0
+    v = x[box(3, 1, 0)]; v[5, 2, 7] = 5.0
+    # (0, 2, 1): constant 2^3 blocks, one block different -> level 1 passes, its level-2 cell fails -> level 1
+    v = x[box(0, 2, 1)]; v[2:4, 6:8, 0:2] = 5.0
+    # (2, 0, 1): constant 4^3 blocks, one different -> levels 1, 2 pass, level 3 fails -> level 2
+    v = x[box(2, 0, 1)]; v[4:8, 0:4, 4:8] = 5.0
+    # (1, 2, 0): no active voxel -> empty
+    act[box(1, 2, 0)] = 0
+    want = np.full(4 * 3 * 2, 3, dtype=np.int8)
+    want[(0 * 3 + 1) * 4 + 3] = 0      # brick 7
+    want[(1 * 3 + 2) * 4 + 0] = 1      # brick 20
+    want[(1 * 3 + 0) * 4 + 2] = 2      # brick 14
+    want[(0 * 3 + 2) * 4 + 1] = -1     # brick 9
+    wl = iso_workload((nx, ny, nz), B, x, x, [[1.5, 1.5, 1.5]], [[1.0, 0.0, 0.0]], active=act.ravel(), max_level=3)
+    for metric in (orc.RELVAR, orc.IOD_LOG):
+        M = orc.build_mips(wl, max_level=3, metric=metric, thr_eta=1e-3, thr_chi=1e-3)
+        assert M.levels.shape == (1, 24)
+        assert np.array_equal(M.levels[0], want)
+    # occupancy in the same numbering
+    assert np.array_equal(orc.brick_active(wl), want >= 0)
+
+
+def test_v1_3d_mip_values_are_correctly_rounded_means():
+    rng = np.random.default_rng(4)
+    a = np.exp(rng.standard_normal((4, 6, 8, 2)) * 4).astype(np.float32)       # (z, y, x, channel), all sides differ
+    m = orc.mip_mean(a, 3)
+    assert m.shape == (2, 3, 4, 2)
+    from fractions import Fraction
+    for k in range(2):
+        for j in range(3):
+            for i in range(4):
+                for c in range(2):
+                    ex = sum(Fraction(float(a[2 * k + dz, 2 * j + dy, 2 * i + dx, c]))
+                             for dz in (0, 1) for dy in (0, 1) for dx in (0, 1)) / 8
+                    assert float(m[k, j, i, c]) == float(np.float32(float(ex)))
+
+
+def test_p7_3d_hdda_equals_plain_march_over_upsampled_field():
+    """P7 in 3D: segments of equal eta, chi compose exactly, so the VLM + HDDA solve equals the plain level-0 march
+    through the field in which every voxel carries the mip value of the cell its brick's level puts it in."""
+    wl = _iso_3d_from_c5(n=32, n_dirs=8, n_probes=60)
+    M = orc.build_mips(wl, max_level=3, metric=orc.RELVAR, thr_eta=1e-3, thr_chi=1e-3)
+    assert len(np.unique(M.levels[M.levels >= 0])) >= 3
+    Bm = orc.hdda_march(wl, M)
+    n, b, W = 32, wl.brick, wl.lambda_batch
+    eta_up = np.zeros((n, n, n, wl.n_lambda), dtype=np.float32)
+    chi_up = np.zeros_like(eta_up)
+    nbk = n // b
+    for bt in range(wl.n_batch):
+        sl = slice(bt * W, (bt + 1) * W)
+        for bi in range(wl.n_bricks):
+            m = int(M.levels[bt, bi])
+            if m < 0:
+                continue
+            bz, r = divmod(bi, nbk * nbk)
+            by, bx = divmod(r, nbk)
+            cb = b >> m
+            for name, up in (("eta", eta_up), ("chi", chi_up)):
+                src = getattr(M, name)[m][bz * cb:(bz + 1) * cb, by * cb:(by + 1) * cb, bx * cb:(bx + 1) * cb, sl]
+                for ax in range(3):
+                    src = np.repeat(src, 1 << m, axis=ax)
+                up[bz * b:(bz + 1) * b, by * b:(by + 1) * b, bx * b:(bx + 1) * b, sl] = src
+    wl_up = iso_workload((n, n, n), b, eta_up, chi_up, wl.probe_pos, wl.dirs, active=wl.active, weights=wl.weights)
+    A = orc.plain_march(wl_up)
+    assert Bm.segments < A.segments
+    assert max_rel(Bm.I, A.I) < 2e-6
