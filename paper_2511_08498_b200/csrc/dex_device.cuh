@@ -349,6 +349,7 @@ __device__ __forceinline__ void dex_set_cell_nocap(DexRay3<D>& r, const DexGridD
       r.kf[a] = (float)(face << G.logB);
       r.tn[a] = __fmaf_rn(r.kf[a], r.inv[a], r.off[a]);
       r.dk[a] = pos ? fB : -fB;                    // only the sign is read while the cell is empty
+      if (BOX) r.cstep[a] = x[a] & ~(G.B - 1);     // low corner of the brick the box is entered in (dex_ray_cross_nocap)
       tb = fminf(tb, r.tn[a]);
     }
     r.tb = tb;
@@ -411,11 +412,22 @@ __device__ __forceinline__ bool dex_ray_cross_nocap(DexRay3<D>& r, const DexGrid
   for (int a = 0; a < D; ++a) x[a] = (a == s) ? xe : c[a];
   if (!alive) return false;
   if (box) {
-    // the box spans several bricks on the other axes: the brick being entered is the one holding the plain DDA's
-    // coordinates at this event (T5), searched over the whole axis (the position locates them to within one voxel)
+    // the box spans several bricks on the other axes: the brick being entered is the one holding the HDDA's
+    // coordinates at this event (T5), searched over the whole axis (the position locates them to within one voxel).
+    // Taking the empty bricks one at a time clamps the T5 coordinate to the current brick at every step; over the
+    // box that composes to a clamp against the brick the box was entered in, on the side the ray comes from (the
+    // T5 coordinate is monotone along the ray).  It only acts when a probe sits exactly on a cell plane and the
+    // direction component is so small (|d| ~ 1e-16, a cos(pi/2) that is not quite 0) that the fp32 plane time of that
+    // very plane is rounding noise: the plane then does not count as crossed although the ray started beyond it.
 #pragma unroll
     for (int a = 0; a < D; ++a)
-      if (a != s) x[a] = dex_fine_coord(__ldg(probe + a), -__ldg(omega + a), r.inv[a], r.off[a], 0, G.dims[a], th, a < s);
+      if (a != s) {
+        const float da = -__ldg(omega + a);
+        int xa = dex_fine_coord(__ldg(probe + a), da, r.inv[a], r.off[a], 0, G.dims[a], th, a < s);
+        if (da > 0.0f) xa = max(xa, r.cstep[a]);
+        else if (da < 0.0f) xa = min(xa, r.cstep[a] + G.B - 1);
+        x[a] = xa;
+      }
   }
   int info = r.info;
   if (newbrick) {

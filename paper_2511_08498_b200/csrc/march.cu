@@ -753,7 +753,9 @@ dex_dir_records_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev 
 }
 
 // a10: traversal only, one thread per ray, for one batch's level table -- the same stepping code as
-// the march kernel, so the recorded list is the one the production path integrates over.
+// the march kernel, crossing routine included (the capped dex_ray_cross under a near-field cap, else the cap-free
+// dex_ray_cross_nocap with the march's empty-space boxes), so the recorded list is the one the production path
+// integrates over.
 template <int D>
 __global__ void __launch_bounds__(128)
 dex_capture_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, long long* __restrict__ counts,
@@ -771,6 +773,7 @@ dex_capture_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, l
   const long long room = ((ray_id + 1 < n_rays) ? offsets[ray_id + 1] : capacity) - begin;
   long long n = 0;
   DexRay3<D> ray;
+  const bool caps = M.n_caps > 0;     // as in dex_march_kernel
   bool alive = dex_ray_init3<D>(ray, G, M, binfo, probe, om);
   while (alive) {
     int c[D];
@@ -786,7 +789,9 @@ dex_capture_kernel(const DexGridDev G, const DexMipsDev M, const DexRaysDev R, l
       emit = emit && ds > 0.0f;
     }
     if (R.t_end > 0.0f && ray.t >= R.t_end) alive = false;
-    else if (!inside) alive = dex_ray_cross<D>(ray, G, M, binfo, probe, om);
+    else if (!inside)
+      alive = caps ? dex_ray_cross<D>(ray, G, M, binfo, probe, om)
+                   : dex_ray_cross_nocap<D, DEX_BOX(D, DEX_ISO)>(ray, G, binfo, probe, om);
     if (emit) {
       if (n < room) {
         unsigned long long rec = ((unsigned long long)(unsigned)m << 56) | (unsigned long long)(unsigned)(c[0] >> m);
@@ -1008,16 +1013,35 @@ dex_status dex_make_probe_tiling(const dex_grid* g, const DexRaysDev& rays, int*
 // per-direction march records (dex_dir_records_kernel) and march them with the ISO kernel, a group of
 // wavelength batches at a time so that the records fit the memory set aside for them.  J columns of different batches
 // are disjoint, so the groups need no accumulation.
+// Returns through *fell_back = true (and DEX_OK, nothing marched) when not even one batch's records could be allocated
+// before the first group: the caller then evaluates eta, chi in the ray loop instead (launch_march_d).
 template <int D>
 static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const DexRaysDev& rays, float* d_out,
                                         bool fuse_j, unsigned long long* d_seg, int lpr, const int* perm, cudaStream_t st,
-                                        int batches_per_group) {
+                                        int& batches_per_group, bool* fell_back) {
   const size_t A = (size_t)g->n_active, cps = (size_t)m->dev.cps;
-  for (int b0 = 0; b0 < m->n_batch; b0 += batches_per_group) {
-    const int nb = (b0 + batches_per_group <= m->n_batch) ? batches_per_group : m->n_batch - b0;
-    const size_t plane = (size_t)nb * A * cps * DEX_W;
+  *fell_back = false;
+  for (int b0 = 0; b0 < m->n_batch;) {
+    // The budget of memo_group is an estimate: the pool's idle bytes may be fragmented or still owned by another stream,
+    // and the rebuild pipeline's build stream allocates at the same time.  A failed allocation is retried with half
+    // the batches; if one batch does not fit, the first group falls back, a later one reports the failure (the
+    // batches already marched have been added to J and to the segment counter: they cannot be redone).
+    int nb = (b0 + batches_per_group <= m->n_batch) ? batches_per_group : m->n_batch - b0;
     float* d_rec = nullptr;
-    DEX_CUDA_CHECK(dex_alloc((void**)&d_rec, sizeof(float) * 2 * plane * (size_t)rays.n_dirs, st));
+    size_t plane = 0;
+    for (;;) {
+      plane = (size_t)nb * A * cps * DEX_W;
+      cudaError_t e = dex_tuning_memo_fail_alloc() ? cudaErrorMemoryAllocation
+                                                   : dex_alloc((void**)&d_rec, sizeof(float) * 2 * plane * (size_t)rays.n_dirs, st);
+      if (e == cudaSuccess) break;
+      cudaGetLastError();
+      d_rec = nullptr;
+      if (e != cudaErrorMemoryAllocation) { dex_set_error(std::string("march records: ") + cudaGetErrorString(e)); return DEX_ERR_CUDA; }
+      if (nb > 1) { nb = (nb + 1) / 2; batches_per_group = nb; continue; }
+      if (b0 == 0) { *fell_back = true; return DEX_OK; }
+      dex_set_error("march records: out of device memory for one wavelength batch of per-direction records");
+      return DEX_ERR_OOM;
+    }
     dex_mips mm = *m;                       // a view of the group's batches as an ISO handle over the records
     mm.variant = DEX_ISO;
     mm.n_batch = nb;
@@ -1053,6 +1077,7 @@ static dex_status launch_march_memo(const dex_grid* g, const dex_mips* m, const 
     }
     dex_free(d_rec, st);
     if (s != DEX_OK) return s;
+    b0 += nb;
   }
   return DEX_OK;
 }
@@ -1072,9 +1097,15 @@ static int memo_group(const dex_grid* g, const dex_mips* m, const DexRaysDev& ra
   const double per_batch = (double)rays.n_dirs * 2.0 * (double)g->n_active * (double)m->dev.cps * DEX_W * sizeof(float);
   size_t free_b = 0, total_b = 0;
   if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); return 0; }
-  // half of what is available: the driver's free memory plus what the library's own pool holds idle from earlier calls
-  // at most 64 GB in 2D (C4: 7 batches per group 7.44 s, 11 per group 7.60 s), 96 GB in 3D (C5's four batches in one launch)
-  const double budget = fmin(0.5 * ((double)free_b + (double)dex_pool_idle_bytes()), D == 3 ? 96.0e9 : 64.0e9);
+  // half of what is available (the driver's free memory plus what the library's own pool holds idle from earlier calls),
+  // at most 32 GB in 2D and 40 GB in 3D.  Measured in round 3 (profiles/r03_memo_budget.md): C3 36 -> 16 GB of records
+  // costs 0.8 % of a step, C4 65 -> 34 GB 1.6 %, C5 72 -> 37 GB 2.2 % (19 GB: 8.4 %); the round-2 caps (64 / 96 GB) left
+  // a second tenant of the GPU nothing.  "memo_budget_mb" moves the cap either way.
+  double budget = fmin(0.5 * ((double)free_b + (double)dex_pool_idle_bytes()), D == 3 ? 40.0e9 : 32.0e9);
+  const int cap_mb = dex_tuning_memo_budget_mb();       // "memo_budget_mb": the caller's own bound on these temporaries;
+  if (cap_mb > 0) {                                      // one batch is the smallest group, so it is taken even above the bound
+    budget = fmin(budget, fmax((double)cap_mb * 1.0e6, fmin(per_batch, budget)));
+  }
   const int nb = (int)fmin((double)m->n_batch, floor(budget / per_batch));
   return nb < 1 ? 0 : nb;
 }
@@ -1095,6 +1126,14 @@ static dex_status ensure_march_constants() {
     done[dev] = true;
   }
   return DEX_OK;
+}
+
+// what the last dex_launch_march of this thread actually ran with (dex_last_march_mapping)
+static thread_local int t_map_lanes = 0, t_map_dirs_per_block = 0, t_map_memo_group = 0;
+void dex_last_mapping(int* lanes_per_ray, int* dirs_per_block, int* memo_batches_per_group) {
+  if (lanes_per_ray) *lanes_per_ray = t_map_lanes;
+  if (dirs_per_block) *dirs_per_block = t_map_dirs_per_block;
+  if (memo_batches_per_group) *memo_batches_per_group = t_map_memo_group;
 }
 
 bool dex_auto_dir_split(long long n_probes, int n_dirs, int n_lambda) {
@@ -1137,11 +1176,20 @@ dex_status dex_launch_march(const dex_grid* g, const dex_mips* m, const DexRaysD
   if (s == DEX_OK) {
     float* out = d_I ? d_I : d_out;
     const bool fj = d_I ? false : fuse_j;
-    const int memo = memo_group(g, m, r);
-    if (memo > 0 && g->desc.ndim == 2) s = launch_march_memo<2>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st, memo);
-    else if (memo > 0) s = launch_march_memo<3>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st, memo);
-    else if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st);
-    else s = launch_march_d<3>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st);
+    int memo = memo_group(g, m, r);
+    if (memo > 0) {
+      bool fell_back = false;
+      if (g->desc.ndim == 2) s = launch_march_memo<2>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st, memo, &fell_back);
+      else s = launch_march_memo<3>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st, memo, &fell_back);
+      if (fell_back) memo = 0;         // no room for one batch of records: evaluate in the ray loop
+    }
+    t_map_lanes = lanes_per_ray;
+    t_map_dirs_per_block = r.k_per_block;
+    t_map_memo_group = memo;
+    if (memo == 0) {
+      if (g->desc.ndim == 2) s = launch_march_d<2>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st);
+      else s = launch_march_d<3>(g, m, r, out, fj, d_seg, lanes_per_ray, perm, st);
+    }
     if (s == DEX_OK && d_I) s = dex_launch_reduce_j(r, m->n_lambda, d_I, d_out, st);
   }
   if (d_I) dex_free(d_I, st);

@@ -325,6 +325,52 @@ def test_memo_parity(P, name, kw, thr, extra):
         P.dex_set_lanes_per_ray(1)
 
 
+
+def test_memo_budget_and_allocation_failure(P):
+    """The memoised march's temporaries under pressure: a caller-set bound ("memo_budget_mb") far below the whole spectrum's
+    records still takes the memoised path, in more groups of wavelength batches, with bit-identical J (batches are
+    independent columns); a records allocation that fails is retried with half the batches; when not even one batch
+    fits before anything was marched, the solve falls back to evaluating eta, chi in the ray loop -- the "memo" = 0
+    path bit for bit -- instead of failing.  Which path ran is read off the library's launch counter."""
+    wl = make("C4", n=128, n_dirs=6, n_probes=300)
+    wl.thr_eta = wl.thr_chi = 0.3
+    assert wl.n_batch >= 4
+    dw, grid, mips = _build(P, wl)
+
+    def run():
+        c0 = P.dex_launch_count()
+        seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+        J = P.pipeline.mean_intensity(dw, grid, mips, segment_count=seg)
+        torch.cuda.synchronize()
+        return J, int(seg.item()), P.dex_launch_count() - c0
+
+    try:
+        P.dex_set_tuning("memo", 0)
+        J0, s0, n0 = run()
+        P.dex_set_tuning("memo", 1)
+        assert P.dex_last_march_mapping()["memo_batches_per_group"] == 0
+        J1, s1, n1 = run()
+        assert P.dex_last_march_mapping()["memo_batches_per_group"] == wl.n_batch
+        assert s1 == s0 and n1 > n0                       # the records kernel is an extra launch
+        assert max_rel(J1.cpu().numpy(), J0.cpu().numpy()) <= TOL
+        P.dex_set_tuning("memo_budget_mb", 1)             # below one batch's records: one batch per group
+        Jb, sb, nb = run()
+        assert torch.equal(Jb, J1) and sb == s1 and nb >= n1 + wl.n_batch - 1
+        assert P.dex_last_march_mapping()["memo_batches_per_group"] == 1
+        P.dex_set_tuning("memo_budget_mb", 0)
+        P.dex_set_tuning("memo_fail_allocs", 1)           # the whole-spectrum allocation fails once: two groups
+        Jf, sf, nf = run()
+        assert torch.equal(Jf, J1) and sf == s1 and n1 < nf < nb
+        assert P.dex_last_march_mapping()["memo_batches_per_group"] == (wl.n_batch + 1) // 2
+        P.dex_set_tuning("memo_fail_allocs", 1000)        # nothing can be allocated: in-march evaluation
+        Jx, sx, nx = run()
+        assert torch.equal(Jx, J0) and sx == s0 and nx == n0
+        assert P.dex_last_march_mapping()["memo_batches_per_group"] == 0
+    finally:
+        P.dex_set_tuning("memo_fail_allocs", 0)
+        P.dex_set_tuning("memo_budget_mb", 0)
+        P.dex_set_tuning("memo", -1)
+
 def test_classic_equals_plain_march(P):
     wl = make("C4", n=64, n_dirs=6, n_probes=100)
     A = orc.plain_march(wl, variant=orc.CLASSIC)
@@ -367,6 +413,15 @@ def test_c2_full_size_sampled(P):
     assert max_rel(J[idx], Jref) <= TOL
     assert int(seg.item()) > 0
     assert np.isfinite(J).all() and (J >= 0).all()
+    # visit lists and path lengths of the timed launch's traversal at 512^2: 32 seeded probes x all 64 directions, every
+    # wavelength batch (each has its own level table), bit-exact against the oracle
+    sel = np.sort(rng.choice(wl.probe_pos.shape[0], size=32, replace=False))
+    wl.probe_pos = np.ascontiguousarray(wl.probe_pos[sel])
+    dw.t["probe_pos"] = torch.from_numpy(wl.probe_pos).cuda()
+    for b in range(wl.n_batch):
+        ref = orc.hdda_march(wl, M, capture_batch=b)
+        _, cap = P.pipeline.formal_solution(dw, grid, mips, capture_batch=b, want_I=False)
+        _check_lists(cap, ref, cap.room)
 
 
 def test_direction_split_bit_identical(P):
@@ -614,6 +669,71 @@ def test_level_cap_parity(P, name, kw, thr):
             assert ref.segments == base.segments
     with pytest.raises(P.DexError):
         mips.set_level_caps([5.0, 2.0])
+
+
+# ------------------------------------------------------------------------------------------ large coordinates
+def _large_void_workload(n=4096, brick=16, seed=31):
+    """A large, mostly empty 2D ISO medium: populated bricks in a few blobs and isolated single bricks, wide voids in
+    between (empty-space distance up to the cap of 8 bricks), brick-constant eta, chi so that any level table is a
+    valid one.  Probes anywhere (in voids, on voxel and brick planes); random, axis-parallel, diagonal and grazing
+    directions.  Input recipe only."""
+    rng = np.random.default_rng(seed)
+    nb = n // brick
+    yy, xx = np.mgrid[0:nb, 0:nb]
+    occ = np.zeros((nb, nb), dtype=bool)
+    for _ in range(14):
+        cx, cy, r = rng.uniform(0, nb), rng.uniform(0, nb), rng.uniform(3, 22)
+        occ |= (xx - cx) ** 2 + (yy - cy) ** 2 < r * r
+    occ |= rng.random((nb, nb)) < 0.004                      # isolated bricks inside the voids
+    occ[0, :] |= rng.random(nb) < 0.3                        # and some on the grid's edges and corners
+    occ[:, -1] |= rng.random(nb) < 0.3
+    occ[0, 0] = occ[-1, -1] = True
+    val = rng.uniform(0.002, 0.02, size=(nb, nb)).astype(np.float32) * occ
+    field = np.repeat(np.repeat(val, brick, axis=0), brick, axis=1)                    # [n][n] fp32
+    spec = np.ascontiguousarray(np.repeat(field.reshape(-1, 1), 8, axis=1))            # [nvox][8]
+    act = np.repeat(np.repeat(occ, brick, axis=0), brick, axis=1).astype(np.uint8).ravel()
+    probes = np.concatenate([
+        rng.uniform(0, n, size=(150, 2)),
+        rng.integers(0, n, size=(20, 2)).astype(np.float64),                 # on voxel corners
+        rng.integers(0, nb, size=(20, 2)).astype(np.float64) * brick,        # on brick corners
+        rng.integers(0, n, size=(20, 2)) + 0.5,                              # voxel centres
+        [[0.0, 0.0], [n - 0.001, n - 0.001], [n - 0.5, 0.5], [0.25, n - 0.25]]]).astype(np.float32)
+    ang = np.array([0.0, math.pi / 2, math.pi, 1.5 * math.pi, math.pi / 4, 0.75 * math.pi, 1.25 * math.pi, 1.75 * math.pi,
+                    1e-6, math.pi / 2 + 1e-5, math.pi - 3e-7, 1.5 * math.pi + 2e-4, math.atan2(1, 2), math.atan2(-3, 1)])
+    dirs = np.concatenate([unit_dirs_2d(ang), random_unit_dirs(10, 2, rng)]).astype(np.float32)
+    from workloads.gen import METRIC_RELVAR, VARIANT_ISO, Workload
+    wl = Workload(name="large-void", ndim=2, dims=(n, n, 1), brick=brick, voxel_size=1.0, active=act, variant=VARIANT_ISO,
+                  n_lambda=8, lambda_batch=8, max_level=4, metric=METRIC_RELVAR, thr_eta=1e-3, thr_chi=1e-3, tau_gate=-1.0,
+                  probe_pos=np.ascontiguousarray(probes), dirs=np.ascontiguousarray(dirs),
+                  weights=np.full(dirs.shape[0], 1.0 / dirs.shape[0], dtype=np.float32), eta=spec * np.float32(1.5), chi=spec)
+    levels = np.where(occ.ravel(), rng.integers(0, 5, size=nb * nb), -1).astype(np.int8)[None, :]
+    return wl, levels
+
+
+def test_large_grid_void_boxes_list_parity(P):
+    """Visit lists of the PRODUCTION traversal (cap-free crossing, whole boxes of empty bricks in one step, single-step
+    fine-coordinate correction) against the oracle's HDDA on a 4096^2 grid that is ~80 % empty: bit-exact records and
+    path lengths for 214 probes x 24 directions.  This is what holds dex_fine_coord to its claim that the fp32 position
+    locates the T5 cell to within one voxel at large coordinates and over a whole-axis search: a guess two voxels off
+    would enter a wrong cell or brick and change the list.  Repeated under a near-field cap (the other crossing routine)."""
+    wl, levels = _large_void_workload()
+    act_b = orc.brick_active(wl)
+    assert 0.1 < act_b.mean() < 0.35
+    M = orc.build_mips(wl, max_level=4)
+    M.levels = np.ascontiguousarray(levels)
+    dw, grid, mips = _build(P, wl, max_level=4)
+    assert np.array_equal(grid.slots() >= 0, act_b)
+    mips.set_levels(M.levels)
+    for caps in ([], [6.0, 24.0, 96.0, 384.0]):
+        mips.set_level_caps(caps)
+        ref = orc.hdda_march(wl, M, capture_batch=0, level_cap_t=caps if caps else None)
+        assert ref.segments > 100000
+        _, cap = P.pipeline.formal_solution(dw, grid, mips, capture_batch=0, want_I=False)
+        _check_lists(cap, ref, cap.room)
+        seg = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+        J = P.pipeline.mean_intensity(dw, grid, mips, segment_count=seg)
+        assert int(seg.item()) == ref.segments
+        assert max_rel(J.cpu().numpy(), orc.mean_intensity(ref.I, wl.weights)) <= TOL
 
 
 def test_velocity_bin_report(P):
