@@ -8,11 +8,13 @@ dex_build_sparse_grid + dex_build_vlm_mips + dex_mean_intensity (fused HDDA marc
                   [--configs C1,C2,...|none] [--shard replicas|probes]
 
 BASELINE.json's `metric` names no config, so the headline (`value`, `ms_per_step`, `roofline`, `e2e`,
-`cpu_baseline` at the top level of the JSON line) is quoted on the largest single-GPU configuration that
-fits K = 20 timed steps in a minute: C3 (configs[2], 1024x1024, velocity interpolation, 0.3 s per step).
-The same process then measures every other BASELINE config into `per_config` (own step counts, own clock
-sample, own roofline / e2e / cpu_baseline); C4 (configs[3], 7 s per step) takes 1 timed + 1 end-to-end
-step there, stated in its entry.  The whole default run takes two minutes.
+`cpu_baseline` at the top level of the JSON line) is quoted on the largest single-GPU configuration: C4
+(configs[3], 1024x1024, Core-and-Voigt, 208 wavelengths x 128 directions, 8.7e11 segments and ~7 s per
+step), timed for EXACTLY --steps steps after --warmup warm-up steps (20 + 5 take three minutes).  The same
+process then measures every other BASELINE config (own clock sample, own roofline / e2e / cpu_baseline)
+and prints each as its own JSON line {"per_config": "C1", ...} BEFORE the final headline line; the
+headline line's `config.all_configs` repeats every config's step time, value, e2e and roofline fraction in
+a few numbers, so that one line alone carries C1-C5.  The default run (5 + 3 steps) takes three minutes.
 
 N > 1 (torchrun): `--shard replicas` (default): every rank solves its own seeded atmosphere of the same
 size (weak scaling, no data-path collective -- rays are independent); NCCL is used only for
@@ -39,7 +41,7 @@ import numpy as np  # noqa: E402
 METRIC = "formal_solution_ray_voxel_segments_lambda_per_sec"
 UNIT = "seg*lambda/s"
 CONFIGS = ("C1", "C2", "C3", "C4", "C5")
-HEADLINE = "C3"
+HEADLINE = "C4"
 BASELINE_CONFIG = {"C1": "configs[0]", "C2": "configs[1]", "C3": "configs[2]", "C4": "configs[3]", "C5": "configs[4]"}
 VARIANT_NAME = {0: "iso", 1: "velinterp", 2: "cav", 3: "classic"}
 # ALGORITHMIC work per unit (restated in DESIGN.md section 6)
@@ -54,8 +56,11 @@ CAV_FLOPS_PER_LINE_EVAL = 75.0
 CAV_FLOPS_PER_SEG_LAMBDA = 25.0
 MUFU_PER_SM_PER_CLK = 16.0      # ex2 results per SM per clock (4 SMSPs x 4 lanes; Blackwell guide)
 N_SM = 148
-# per-config caps on (warm-up, timed, e2e) steps when the config is NOT the headline: C4 is tens of seconds per step
+# per-config caps on (warm-up, timed, e2e) steps when the config is NOT the headline: C4 is seconds per step
 STEP_CAPS = {"C4": (0, 1, 1)}
+# end-to-end steps and steps of the single-direction alternative per config (default: min(steps, 3)); C4: 7 s each
+E2E_STEPS = {"C4": 2}
+ALT_STEPS = {"C4": 1}
 CPU_PROBES = {"C1": 4096, "C2": 2048, "C3": 128, "C4": 24, "C5": 256}
 _HOST_THREADS = None
 
@@ -84,6 +89,8 @@ def parse():
     ap.add_argument("--pipeline", type=int, default=0,
                     help="time the per-iteration rebuild pipeline (dex_mean_intensity_pipelined) with this many "
                          "wavelength batches per stage instead of the whole-spectrum build + march")
+    ap.add_argument("--memo-budget-mb", type=int, default=None,
+                    help='"memo_budget_mb" tuning knob: cap on the memoised march\'s per-direction records (MB)')
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -178,15 +185,27 @@ class ClockSampler:
 
 
 def oracle_sample(wl):
-    """The workload restricted to its middle wavelength batch (pure column selection, workloads.gen.batch_workload):
-    the oracle's numpy mip build over every batch of a BASELINE-size grid takes minutes, its throughput in
-    seg*lambda/s does not depend on how many batches are marched."""
+    """The workload restricted to ONE wavelength batch (pure column selection, workloads.gen.batch_workload): the
+    oracle's numpy mip build over every batch of a BASELINE-size grid takes minutes.  The oracle evaluates the line
+    profiles per segment, so its seg*lambda/s falls with the number of active lines of the batch (the GPU's memoised
+    march does not); the batch taken is the one nearest the middle of the spectrum among those with the MEDIAN number
+    of active lines, and the sample string says how the batches are distributed."""
     from workloads.gen import batch_workload
     if wl.n_batch <= 1:
         return wl, "all wavelengths"
-    b = wl.n_batch // 2
+    mid = wl.n_batch // 2
+    if wl.active_lines is None:
+        b, lines = mid, ""
+    else:
+        n_act = (np.asarray(wl.active_lines) >= 0).sum(axis=1)
+        med = int(np.sort(n_act)[len(n_act) // 2])
+        cand = np.flatnonzero(n_act == med)
+        b = int(cand[np.argmin(np.abs(cand - mid))])
+        hist = np.bincount(n_act)
+        lines = (f", {med} active line(s) -- the median; batches with 0/1/2/.. active lines: "
+                 f"{'/'.join(str(int(v)) for v in hist)}; the oracle's rate falls with the line count")
     sub, _ = batch_workload(wl, [b])
-    return sub, f"wavelength batch {b} of {wl.n_batch} ({wl.lambda_batch} wavelengths)"
+    return sub, f"wavelength batch {b} of {wl.n_batch} ({wl.lambda_batch} wavelengths{lines})"
 
 
 def cpu_baseline(wl, n_probes, target_s=10.0, one_thread_s=4.0):
@@ -287,6 +306,8 @@ class Bench:
             P.dex_set_lanes_per_ray(args.lanes)
         if args.tile is not None:
             P.dex_set_tuning("tile_probes", args.tile)
+        if args.memo_budget_mb is not None:
+            P.dex_set_tuning("memo_budget_mb", args.memo_budget_mb)
         self.flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=self.dev)
         self.hbm_peak, self.hbm_src = peaks()
         self.fp32_peak = None
@@ -338,13 +359,24 @@ class Bench:
         W = wl.lambda_batch
         sl = segs_per_launch * W                                  # seg*lambda per launch
         t = march_avg_ms * 1e-3
-        eff_gbs = ALGO_BYTES[wl.variant] * sl / t / 1e9 if t > 0 else 0.0
         pk = self.measure_fp32_peak()
         fp32_peak = max(pk["ffma_tflops"], pk["ffma2_tflops"])
         # the library counts provider evaluations (dex_march_work_read): one per emitted segment when eta, chi are evaluated
         # inside the march, one per (cell, direction, batch) when they are memoised per direction
         evals = line_segs_per_launch * W                          # per wavelength (x active lines for Core-and-Voigt)
         memoised = wl.variant != 0 and line_segs_per_launch < 0.5 * segs_per_launch
+        # bytes the launched kernels REQUEST per march region: in the ray loop the variant's nominal bytes per seg*lambda;
+        # memoised: the ISO march reads an 8-byte (chi, S) record per seg*lambda, the records kernel writes 8 B per
+        # record*lambda and, for velocity interpolation, reads the two 8-byte velocity bins it interpolates between
+        # (evals counts record*lambda, times the batch's active lines for Core-and-Voigt: an upper bound there)
+        if memoised:
+            req_bytes = 8.0 * sl + 8.0 * evals + (16.0 * evals if wl.variant == 1 else 0.0)
+            req_what = ("8 B per seg*lambda read by the ISO march + 8 B per memoised record*lambda written"
+                        + (" + 16 B of velocity bins read per record*lambda" if wl.variant == 1 else "") + " by the records kernel")
+        else:
+            req_bytes = ALGO_BYTES[wl.variant] * sl
+            req_what = f"{ALGO_BYTES[wl.variant]:g} B per seg*lambda"
+        eff_gbs = req_bytes / t / 1e9 if t > 0 else 0.0
         integral = FLOPS_INTEGRAL * sl + FLOPS_HDDA_PER_SEGMENT * segs_per_launch
         if wl.variant in (2, 3):
             flops = CAV_FLOPS_PER_LINE_EVAL * evals + integral
@@ -375,7 +407,7 @@ class Bench:
             "segments_per_launch": segs_per_launch,
             # the HBM view BASELINE.json's metric asks for: effective (algorithmic bytes / time; exceeds 1 when the reuse
             # is served by L1/L2) and measured DRAM traffic (ncu, builder-run capture named in traffic_source)
-            "effective_gbs": eff_gbs, "effective_frac": eff_gbs / self.hbm_peak,
+            "effective_gbs": eff_gbs, "effective_frac": eff_gbs / self.hbm_peak, "effective_bytes": req_what,
             "hbm_peak_gbs": self.hbm_peak, "hbm_peak_source": self.hbm_src,
             "mufu_floor_ms": mufu_floor_ms, "mufu_floor_frac": mufu_floor_ms / march_avg_ms if march_avg_ms > 0 else None,
             "traffic": None, "dram_gbs": None, "dram_frac": None,
@@ -395,16 +427,18 @@ class Bench:
                 # little reuse): the binding roofline is HBM.  Algorithmic bytes: the 8 B record per seg*lambda the march reads,
                 # plus the 8 B per memoised record*lambda the records kernel writes
                 # (evals counts (record, wavelength) pairs, times the active lines of the batch for Core-and-Voigt: one for C5)
-                algo = ALGO_BYTES[wl.variant] * sl + (8.0 * evals if memoised else 0.0)
-                gbs = algo / t / 1e9
+                gbs = req_bytes / t / 1e9
+                hit = roof.get("l2_hit_pct")
                 roof.update({"alu_achieved_tflops": roof["achieved"], "alu_frac": roof["frac"], "alu_peak_tflops": roof["peak"],
                              "bound": "hbm", "achieved": gbs, "peak": self.hbm_peak, "unit": "GB/s", "frac": gbs / self.hbm_peak,
-                             "binds": "HBM: the ISO march reads one 64-byte per-direction record per segment with an L2 hit rate "
-                                      "below 40 % (the records of all directions of a batch are 17.6 GB)",
+                             "bound_source": "chosen from the builder-run ncu capture in profiles/traffic.csv (DRAM bytes per launch "
+                                             "at >= 0.25 of the HBM peak over this run's kernel time), not from a counter read in this run",
+                             "binds": "HBM: the ISO march reads one per-direction record per segment with little reuse"
+                                      + (f" (L2 hit rate {hit:.1f} % in the capture)" if hit is not None else "")
+                                      + (f"; the records of one launch are {8.0 * evals / 1e9:.1f} GB" if memoised else ""),
                              "peak_source": self.hbm_src,
-                             "note": f"achieved = ALGORITHMIC bytes ({ALGO_BYTES[wl.variant]:g} B per seg*lambda read by the march"
-                                     + (" + 8 B per memoised record*lambda written by the records kernel" if memoised else "")
-                                     + ") / time of the library's march region (records kernel + march) from CUDA events"})
+                             "note": f"achieved = ALGORITHMIC bytes ({req_what}) / time of the library's march region "
+                                     "(records kernel + march) from CUDA events"})
         return roof
 
     def measure(self, name, steps, warmup, e2e_steps, want_cpu, cpu_target_s, one_thread_s):
@@ -467,6 +501,7 @@ class Bench:
         t_wall = time.perf_counter() - t_wall0
         clk = clocks.stop()
         launches = P.dex_launch_count() - launches0
+        mapping = P.dex_last_march_mapping()     # what the timed marches ran with (same thread)
         pool_high = P.dex_pool_high_water()
         P.dex_march_timing_enable(False)
         march_ms, march_n = P.dex_march_timing_read(reset=True)
@@ -528,7 +563,7 @@ class Bench:
                 P.pipeline.mean_intensity_single_direction(dw, grid, J=J2)
             torch.cuda.synchronize()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            n_alt = 1 if name in STEP_CAPS and name != args.workload else max(1, min(steps, 3))
+            n_alt = ALT_STEPS.get(name, max(1, min(steps, 3)))
             a.record(stream)
             for _ in range(n_alt):
                 P.pipeline.mean_intensity_single_direction(dw, grid, J=J2, segment_count=seg2)
@@ -556,7 +591,8 @@ class Bench:
                                  march_ms / total_ms if total_ms else None, clk)
             out = {
                 "value": value, "unit": UNIT, "steps": steps, "warmup": warmup, "ms_per_step": max_ms / steps,
-                "config": config_dict(wl, args, {"lanes_per_ray": P.dex_get_lanes_per_ray(n_probes, wl.dirs.shape[0]),
+                "config": config_dict(wl, args, {"lanes_per_ray": mapping["lanes_per_ray"], "dirs_per_block": mapping["dirs_per_block"],
+                                                 "memo_batches_per_group": mapping["memo_batches_per_group"],
                                                  "segments_per_step": segs_total // max(1, steps),
                                                  "path": (f"rebuild pipeline, {args.pipeline} batch(es) per stage"
                                                           if args.pipeline > 0 else "whole-spectrum build + march"),
@@ -591,7 +627,8 @@ def main():
     else:
         extra = [c for c in args.configs.split(",") if c in CONFIGS and c != args.workload]
 
-    head = B.measure(args.workload, args.steps, args.warmup, max(1, min(args.steps, 3)), not args.no_cpu_baseline, 10.0, 4.0)
+    head = B.measure(args.workload, args.steps, args.warmup, E2E_STEPS.get(args.workload, max(1, min(args.steps, 3))),
+                     not args.no_cpu_baseline, 10.0, 4.0)
     per = {}
     for name in extra:
         cw, cs, ce = STEP_CAPS.get(name, (args.warmup, args.steps, max(1, min(args.steps, 3))))
@@ -612,16 +649,36 @@ def main():
             "wall_s_timed_region": head["wall_s_timed_region"],
         }
         out["config"]["headline"] = ("BASELINE.json's metric names no config; the headline is the largest single-GPU config "
-                                     "that fits 20 timed steps in a minute (C3); every config is in per_config")
+                                     f"({HEADLINE}) unless --workload says otherwise; every other config is printed as its own "
+                                     "{\"per_config\": ...} line before this one and summarised in all_configs")
         if "shard_check" in head:
             out["shard_check"] = head["shard_check"]
         if "cpu_baseline" in head:
             out["cpu_baseline"] = head["cpu_baseline"]
-        slim = dict(head)
-        per_all = {args.workload: slim}
+        per_all = {args.workload: head}
         per_all.update(per)
-        out["per_config"] = {k: {kk: vv for kk, vv in per_all[k].items() if kk != "wall_s_timed_region"}
-                             for k in sorted(per_all)}
+
+        def brief(r):
+            rf, e, c = r["roofline"], r.get("e2e") or {}, r.get("cpu_baseline") or {}
+            b = {"ms_per_step": round(r["ms_per_step"], 4), "steps": r["steps"], "warmup": r["warmup"], "value": float(f"{r['value']:.4g}"),
+                 "e2e_ms_per_step": round(e["ms_per_step"], 4) if e else None, "e2e_value": float(f"{e['value']:.4g}") if e else None,
+                 "segments_per_step": r["config"]["segments_per_step"], "gpu_launches": r["gpu_launches"],
+                 "bound": rf["bound"], "roofline_frac": round(rf["frac"], 4) if rf.get("frac") is not None else None,
+                 "march_ms_per_launch": round(rf["kernel_ms_per_launch"], 4), "march_share": round(rf["kernel_share_of_step"] or 0.0, 4),
+                 "dram_frac": round(rf["dram_frac"], 4) if rf.get("dram_frac") is not None else None,
+                 "sm_mhz": r["clocks"].get("sm_mhz"), "reasons": r["clocks"].get("reasons"),
+                 "device_bytes_high_water": r["config"]["library_device_bytes_high_water"]}
+            if c:
+                b["cpu_oracle_value"] = float(f"{c['value']:.4g}")
+            return b
+
+        out["config"]["all_configs"] = {k: brief(per_all[k]) for k in sorted(per_all)}
+        for k in sorted(per):          # the other configs in full, one line each, before the headline line
+            line = {"per_config": k}
+            line.update({kk: vv for kk, vv in per[k].items() if kk != "wall_s_timed_region"})
+            print(json.dumps(line))
+        if "alt_single_direction" in head:
+            out["alt_single_direction"] = head["alt_single_direction"]
         print(json.dumps(out))
     if B.world > 1:
         B.dist.barrier()

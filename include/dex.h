@@ -322,9 +322,17 @@ dex_status dex_march_work_read(int64_t* line_segments, int reset);
  * there are fewer probes than one wave of blocks (148 SMs x 128 threads), where 8 lanes per ray fill the machine better
  * (2 when the march is also spread over the machine direction by direction, see "dir_split"). */
 dex_status dex_set_lanes_per_ray(int lanes);
-/* The lanes-per-ray mapping a whole-spectrum fused-J march over `n_probes` probes x `n_dirs` directions will take under
- * the current settings; bench.py reports it instead of restating the rule. */
-dex_status dex_get_lanes_per_ray(int64_t n_probes, int n_dirs, int* lanes);
+/* PREDICTION of the lanes-per-ray mapping a whole-spectrum fused-J march over `n_probes` probes x `n_dirs` directions x
+ * `n_lambda` wavelengths takes under the current settings.  It cannot see what only the launch knows (a wavelength window
+ * of the rebuild pipeline, a finite radiance interval, a temporary I that fails to allocate -- each keeps the march
+ * unsplit); dex_last_march_mapping reports what a march actually ran with. */
+dex_status dex_get_lanes_per_ray(int64_t n_probes, int n_dirs, int n_lambda, int* lanes);
+/* The mapping the LAST dex_formal_solution / dex_mean_intensity* march launched from the calling thread ran with:
+ * lanes sharing a ray (1/2/4/8), directions per block of the direction-split launch (0 = not split: every thread walks
+ * all directions), wavelength batches per group of the memoised march (0 = eta, chi evaluated in the ray loop; smaller
+ * than the spectrum when the records budget or a failed allocation split it).  Any pointer may be NULL.  bench.py
+ * records these instead of restating the rules. */
+dex_status dex_last_march_mapping(int* lanes_per_ray, int* dirs_per_block, int* memo_batches_per_group);
 /* MEASURED fp32 arithmetic peak of the current device in TFLOP/s (an FMA counts 2 flops): register-resident chains of
  * scalar FFMA (*tflops_ffma) and of the packed two-wide FFMA2 the march's integrators use (*tflops_ffma2), ~15 ms in all,
  * timed with CUDA events on `stream`.  The denominator of the "alu" roofline of the Core-and-Voigt / Classic march
@@ -339,7 +347,13 @@ dex_status dex_measure_fp32_peak(double* tflops_ffma, double* tflops_ffma2, void
  * the fused kernel's order (bit-identical J); 0 never, n > 0 always; "memo" -1 (default: automatic), 0, 1: the
  * anisotropic marches (velocity interpolation, Core-and-Voigt, Classic) evaluate eta, chi once per (cell, direction,
  * batch) into per-direction march records and march those with the ISO kernel, instead of once per ray segment, when a
- * cell is crossed by many rays per direction (a probe in every voxel: hundreds); same routine, same numbers up to the last bits of the record rounding. */
+ * cell is crossed by many rays per direction (a probe in every voxel: hundreds); same routine, same numbers up to the last bits of the record rounding;
+ * "memo_budget_mb" 0 (default: automatic -- half of the free device memory, at most 32 GB in 2D / 40 GB in 3D), n > 0:
+ * the memoised march holds at most n MB of per-direction records at once and takes the spectrum in more groups of
+ * wavelength batches (one batch is the smallest group and is taken even when it exceeds n; J is bit-identical for every
+ * grouping).  A records allocation that fails is retried with half the batches; if one batch does not fit, the solve
+ * evaluates eta, chi in the ray loop as with "memo" 0 (DEX_ERR_OOM only when that happens after the first group);
+ * "memo_fail_allocs" n: fault injection for the tests -- the next n records allocations are treated as failed. */
 dex_status dex_set_tuning(const char* name, int value);
 
 #ifdef __cplusplus

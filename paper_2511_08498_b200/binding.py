@@ -31,7 +31,7 @@ EXPORTS = (
     "dex_mean_intensity", "dex_mean_intensity_host", "dex_mean_intensity_pipelined", "dex_pool_high_water", "dex_trim", "dex_direction_fields",
     "dex_mean_intensity_single_direction", "dex_voigt_profile", "dex_launch_count", "dex_march_timing_enable", "dex_march_timing_read", "dex_march_work_read",
     "dex_set_lanes_per_ray", "dex_get_lanes_per_ray", "dex_measure_fp32_peak", "dex_set_tuning",
-    "dex_brick_slots_static",
+    "dex_brick_slots_static", "dex_last_march_mapping",
 )
 DEX_STATIC_MAX_BRICKS = 1 << 20
 
@@ -114,7 +114,8 @@ def _load():
     L.dex_set_lanes_per_ray.argtypes = [C.c_int]
     L.dex_set_tuning.argtypes = [C.c_char_p, C.c_int]
     L.dex_trim.argtypes = [C.POINTER(C.c_int64)]
-    L.dex_get_lanes_per_ray.argtypes = [C.c_int64, C.c_int, C.POINTER(C.c_int)]
+    L.dex_get_lanes_per_ray.argtypes = [C.c_int64, C.c_int, C.c_int, C.POINTER(C.c_int)]
+    L.dex_last_march_mapping.argtypes = [C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.dex_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]
     return L
 
@@ -166,10 +167,19 @@ def dex_trim() -> int:
     return v.value
 
 
-def dex_get_lanes_per_ray(n_probes: int, n_dirs: int) -> int:
+def dex_get_lanes_per_ray(n_probes: int, n_dirs: int, n_lambda: int = 1) -> int:
+    """Predicted lanes per ray of a whole-spectrum fused-J march (see dex_last_march_mapping for what a march ran with)."""
     v = C.c_int(0)
-    _check(_L.dex_get_lanes_per_ray(int(n_probes), int(n_dirs), C.byref(v)))
+    _check(_L.dex_get_lanes_per_ray(int(n_probes), int(n_dirs), int(n_lambda), C.byref(v)))
     return v.value
+
+
+def dex_last_march_mapping() -> dict:
+    """What the last march launched from this thread ran with: lanes per ray, directions per block of the direction split
+    (0 = not split), wavelength batches per group of the memoised march (0 = not memoised)."""
+    a, b, c = C.c_int(0), C.c_int(0), C.c_int(0)
+    _check(_L.dex_last_march_mapping(C.byref(a), C.byref(b), C.byref(c)))
+    return {"lanes_per_ray": a.value, "dirs_per_block": b.value, "memo_batches_per_group": c.value}
 
 
 def dex_measure_fp32_peak(stream=None):

@@ -20,6 +20,8 @@ std::atomic<int> g_tile_probes{1};
 std::atomic<int> g_voigt_fp32{1};
 std::atomic<int> g_dir_split{-1};
 std::atomic<int> g_memo{-1};
+std::atomic<int> g_memo_budget_mb{0};     // 0 = automatic (memo_group in march.cu)
+std::atomic<int> g_memo_fail_allocs{0};   // fault injection: this many record allocations of the memoised march fail
 std::mutex g_timing_mu;
 struct EvPair { cudaEvent_t a, b; };
 std::vector<EvPair> g_events;
@@ -221,6 +223,12 @@ void dex_count_launch(int n) { g_launches.fetch_add(n); }
 int dex_tuning_voigt_fp32() { return g_voigt_fp32.load(); }
 int dex_tuning_dir_split() { return g_dir_split.load(); }
 int dex_tuning_memo() { return g_memo.load(); }
+int dex_tuning_memo_budget_mb() { return g_memo_budget_mb.load(); }
+bool dex_tuning_memo_fail_alloc() {
+  int n = g_memo_fail_allocs.load();
+  while (n > 0 && !g_memo_fail_allocs.compare_exchange_weak(n, n - 1)) {}
+  return n > 0;
+}
 unsigned long long* dex_line_segment_counter() { return g_timing.load() ? g_d_line_segs : nullptr; }
 
 extern "C" {
@@ -265,9 +273,15 @@ dex_status dex_set_lanes_per_ray(int lanes) {
   return DEX_OK;
 }
 
-dex_status dex_get_lanes_per_ray(int64_t n_probes, int n_dirs, int* lanes) {
+dex_status dex_get_lanes_per_ray(int64_t n_probes, int n_dirs, int n_lambda, int* lanes) {
   if (!lanes) { dex_set_error("NULL lanes"); return DEX_ERR_INVALID_ARG; }
-  *lanes = dex_auto_lanes(lanes_for((long long)n_probes), (long long)n_probes, dex_auto_dir_split((long long)n_probes, n_dirs, 1));
+  *lanes = dex_auto_lanes(lanes_for((long long)n_probes), (long long)n_probes,
+                          dex_auto_dir_split((long long)n_probes, n_dirs, n_lambda < 1 ? 1 : n_lambda));
+  return DEX_OK;
+}
+
+dex_status dex_last_march_mapping(int* lanes_per_ray, int* dirs_per_block, int* memo_batches_per_group) {
+  dex_last_mapping(lanes_per_ray, dirs_per_block, memo_batches_per_group);
   return DEX_OK;
 }
 
@@ -278,6 +292,8 @@ dex_status dex_set_tuning(const char* name, int value) {
   if (!strcmp(name, "voigt_fp32")) { g_voigt_fp32.store(value ? 1 : 0); return DEX_OK; }
   if (!strcmp(name, "dir_split")) { g_dir_split.store(value < 0 ? -1 : value); return DEX_OK; }
   if (!strcmp(name, "memo")) { g_memo.store(value < 0 ? -1 : (value ? 1 : 0)); return DEX_OK; }
+  if (!strcmp(name, "memo_budget_mb")) { g_memo_budget_mb.store(value < 0 ? 0 : value); return DEX_OK; }
+  if (!strcmp(name, "memo_fail_allocs")) { g_memo_fail_allocs.store(value < 0 ? 0 : value); return DEX_OK; }
   dex_set_error("unknown tuning knob");
   return DEX_ERR_INVALID_ARG;
 }

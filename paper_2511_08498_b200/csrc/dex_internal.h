@@ -51,11 +51,15 @@ size_t dex_pool_idle_bytes();      // memory the library's pool holds but no liv
 void dex_count_launch(int n = 1);
 int dex_tuning_voigt_fp32();
 int dex_tuning_memo();    // -1 automatic, 0 never, 1 always: anisotropic provider memoised per direction (march.cu)
-int dex_tuning_dir_split();
+int dex_tuning_memo_budget_mb();   // > 0: cap (MB) on the per-direction records the memoised march holds at once; 0 = automatic
+bool dex_tuning_memo_fail_alloc(); // fault injection ("memo_fail_allocs"): true = treat the next records allocation as failed
+int dex_tuning_dir_split();   // -1 automatic, 0 never, n > 0: n directions per block whenever J is fused
 // automatic mapping of small problems (march.cu): does a fused-J march over n_probes x n_dirs spread its directions over
 // blocks (n_lambda only bounds the temporary I), and how many lanes share a ray (`set` = the caller's knob, 0 = automatic)
 bool dex_auto_dir_split(long long n_probes, int n_dirs, int n_lambda);
-int dex_auto_lanes(int set, long long n_probes, bool dir_split);   // -1 automatic, 0 never, n > 0: n directions per block whenever J is fused
+int dex_auto_lanes(int set, long long n_probes, bool dir_split);   // set: the caller's knob (0 = automatic, else 1/2/4/8 lanes per ray)
+// the mapping the last dex_launch_march of the calling thread ran with (march.cu)
+void dex_last_mapping(int* lanes_per_ray, int* dirs_per_block, int* memo_batches_per_group);
 unsigned long long* dex_line_segment_counter();   // device counter, NULL unless march timing is enabled
 
 // grid_build.cu

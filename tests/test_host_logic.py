@@ -67,6 +67,25 @@ def test_compute_call_without_device_fails_loudly():
         P.dex_build_sparse_grid(2, (64, 64), 16, 1.0)
 
 
+def test_lanes_query_sees_the_wavelength_count():
+    """dex_get_lanes_per_ray is the host-side rule of the launch: a small problem is split over directions (2 lanes per
+    ray) only while its temporary I of n_probes x n_dirs x n_lambda floats stays within 64 Mi floats; a problem of one
+    wave of blocks or more runs one thread per ray.  Before any march the recorded mapping is all zero."""
+    _lib_path()
+    import paper_2511_08498_b200 as P
+    P.dex_set_lanes_per_ray(0)
+    try:
+        assert P.dex_get_lanes_per_ray(4096, 16, 8) == 2
+        assert P.dex_get_lanes_per_ray(4096, 16, 2048) == 8      # 128 Mi floats of I: not split, 8 lanes per ray
+        assert P.dex_get_lanes_per_ray(1 << 20, 16, 8) == 1
+        P.dex_set_lanes_per_ray(4)
+        assert P.dex_get_lanes_per_ray(4096, 16, 8) == 4
+    finally:
+        P.dex_set_lanes_per_ray(0)
+    if not torch.cuda.is_available():
+        assert P.dex_last_march_mapping() == {"lanes_per_ray": 0, "dirs_per_block": 0, "memo_batches_per_group": 0}
+
+
 # ------------------------------------------------------------------------------------------ sharding
 def test_probe_ranges_tile_the_list():
     _lib_path()
